@@ -1,0 +1,325 @@
+// libile: lifecycle and problem definition (host side of the C ABI in include/ile.h).
+#include <stdarg.h>
+#include <stdlib.h>
+#include <vector>
+#include "common.cuh"
+
+int ile_fail(ile_ctx* ctx, int code, const char* fmt, ...) {
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+int ile_scratch(ile_ctx* ctx, size_t bytes, void** out) {
+    if (bytes > ctx->scratch_bytes) {
+        if (ctx->d_scratch) {
+            ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            ILE_CUDA(ctx, cudaFree(ctx->d_scratch));
+            ctx->d_scratch = nullptr;
+            ctx->scratch_bytes = 0;
+        }
+        size_t want = bytes + (bytes >> 2) + 4096;
+        if (cudaMalloc(&ctx->d_scratch, want) != cudaSuccess) {
+            cudaGetLastError();
+            return ile_fail(ctx, ILE_ENOMEM, "scratch allocation of %zu bytes failed", want);
+        }
+        ctx->scratch_bytes = want;
+    }
+    *out = ctx->d_scratch;
+    return ILE_OK;
+}
+
+uint64_t ile_launch_count(ile_ctx* ctx) { return ctx->launches; }
+
+extern "C" const char* ile_version(void) { return "ile-b200 0.1 (sm_100a)"; }
+
+extern "C" int ile_create(ile_ctx** out, int device, void* cuda_stream) {
+    if (!out) return ILE_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return ILE_ECUDA;  // no CUDA device: there is no CPU fallback
+    }
+    ile_ctx* ctx = (ile_ctx*)calloc(1, sizeof(ile_ctx));
+    if (!ctx) return ILE_ENOMEM;
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    if (cudaSetDevice(device) != cudaSuccess) {
+        free(ctx);
+        return ILE_ECUDA;
+    }
+    cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
+    ctx->D_min = 1.0;
+    ctx->D_max = 2.0;
+    *out = ctx;
+    return ILE_OK;
+}
+
+extern "C" int ile_destroy(ile_ctx* ctx) {
+    if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->d_ylm);
+    cudaFree(ctx->d_Qc);
+    cudaFree(ctx->d_Qt);
+    cudaFree(ctx->d_U);
+    cudaFree(ctx->d_V);
+    cudaFree(ctx->d_lnT);
+    cudaFree(ctx->d_scratch);
+    free(ctx);
+    return ILE_OK;
+}
+
+extern "C" const char* ile_last_error(const ile_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+extern "C" int ile_sync(ile_ctx* ctx) {
+    if (!ctx) return ILE_EINVAL;
+    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ILE_CUDA(ctx, cudaGetLastError());
+    return ILE_OK;
+}
+
+extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
+    if (!ctx || variant < 0 || variant > 1) return ile_fail(ctx, ILE_EINVAL, "variant must be 0 or 1");
+    ctx->variant = variant;
+    return ILE_OK;
+}
+
+extern "C" int ile_set_network(ile_ctx* ctx, int K, const double* D, const double* pos_m, double gmst) {
+    if (!ctx) return ILE_EINVAL;
+    if (K < 1 || K > ILE_MAX_K || !D || !pos_m) return ile_fail(ctx, ILE_EINVAL, "set_network: K in 1..%d", ILE_MAX_K);
+    for (int k = 0; k < K; k++)
+        for (int a = 0; a < 3; a++)
+            for (int b = 0; b < 3; b++) {
+                double x = D[k * 9 + a * 3 + b], y = D[k * 9 + b * 3 + a];
+                if (!(fabs(x - y) <= 1e-12 * (fabs(x) + fabs(y) + 1e-300)) && x != y)
+                    return ile_fail(ctx, ILE_EINVAL, "set_network: D[%d] is not symmetric", k);
+            }
+    if (ctx->have_quv && K != ctx->K) return ile_fail(ctx, ILE_ESTATE, "set_network: K differs from the loaded Q/U/V");
+    ctx->K = K;
+    ctx->gmst = gmst;
+    ctx->max_delay = 0.0;
+    for (int k = 0; k < K; k++) {
+        memcpy(ctx->D[k], D + 9 * k, 9 * sizeof(double));
+        memcpy(ctx->pos[k], pos_m + 3 * k, 3 * sizeof(double));
+        double r = sqrt(pos_m[3 * k] * pos_m[3 * k] + pos_m[3 * k + 1] * pos_m[3 * k + 1] + pos_m[3 * k + 2] * pos_m[3 * k + 2]);
+        if (r / ILE_C_LIGHT > ctx->max_delay) ctx->max_delay = r / ILE_C_LIGHT;
+    }
+    ctx->have_net = true;
+    ctx->have_grid = false;  // the range check depends on the delays
+    return ILE_OK;
+}
+
+// exact binomial / factorial in long double (l <= 8: all values < 2^53)
+static long double fact_ld(int n) {
+    long double f = 1.0L;
+    for (int i = 2; i <= n; i++) f *= (long double)i;
+    return f;
+}
+static long double binom_ld(int n, int k) {
+    if (k < 0 || k > n) return 0.0L;
+    return fact_ld(n) / (fact_ld(k) * fact_ld(n - k));
+}
+
+// Eq. (4): coefficient table of -2Y_lm as a polynomial in cos(theta/2), sin(theta/2)
+// (Goldberg et al. 1967 closed form with s = -2).
+extern "C" int ile_set_modes(ile_ctx* ctx, int M, const int* ell, const int* m) {
+    if (!ctx) return ILE_EINVAL;
+    if (M < 1 || M > ILE_MAX_M || !ell || !m) return ile_fail(ctx, ILE_EINVAL, "set_modes: M in 1..%d", ILE_MAX_M);
+    if (ctx->have_quv && M != ctx->M) return ile_fail(ctx, ILE_ESTATE, "set_modes: M differs from the loaded Q/U/V");
+    YlmTable& T = ctx->h_ylm;
+    memset(&T, 0, sizeof(T));
+    T.M = M;
+    const int s = -2;
+    for (int i = 0; i < M; i++) {
+        int l = ell[i], mm = m[i];
+        if (l < 2 || l > ILE_MAX_L || abs(mm) > l) return ile_fail(ctx, ILE_EINVAL, "set_modes: mode %d = (%d,%d) unsupported", i, l, mm);
+        for (int j = 0; j < i; j++)
+            if (ell[j] == l && m[j] == mm) return ile_fail(ctx, ILE_EINVAL, "set_modes: duplicate mode (%d,%d)", l, mm);
+        YlmMode& Y = T.mode[i];
+        Y.m = mm;
+        long double norm = sqrtl(fact_ld(l + mm) * fact_ld(l - mm) * (2 * l + 1) /
+                                 (4.0L * 3.14159265358979323846264338327950288L * fact_ld(l + s) * fact_ld(l - s)));
+        if ((l + mm - s) & 1) norm = -norm;
+        int nt = 0;
+        for (int r = 0; r <= l - s; r++) {
+            int kk = r + s - mm;
+            if (kk < 0 || kk > l + s) continue;
+            long double c = binom_ld(l - s, r) * binom_ld(l + s, kk) * norm;
+            if (r & 1) c = -c;
+            if (nt >= ILE_YLM_MAX_TERMS) return ile_fail(ctx, ILE_EINVAL, "set_modes: too many terms");
+            Y.coef[nt] = (double)c;
+            Y.pc[nt] = 2 * r + s - mm;
+            Y.ps[nt] = 2 * l - 2 * r - s + mm;
+            if (Y.pc[nt] > T.max_pow) T.max_pow = Y.pc[nt];
+            if (Y.ps[nt] > T.max_pow) T.max_pow = Y.ps[nt];
+            nt++;
+        }
+        Y.nterms = nt;
+        if (abs(mm) > T.max_abs_m) T.max_abs_m = abs(mm);
+        ctx->ell[i] = l;
+        ctx->m[i] = mm;
+    }
+    ctx->M = M;
+    if (!ctx->d_ylm) ILE_CUDA(ctx, cudaMalloc(&ctx->d_ylm, sizeof(YlmTable)));
+    ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_ylm, &T, sizeof(YlmTable), cudaMemcpyHostToDevice, ctx->stream));
+    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->have_modes = true;
+    return ILE_OK;
+}
+
+// ---------------------------------------------------------------- Q / U / V
+// Repack Q [K][M][N_Q] complex -> tiled [K][N_Qpad][48]: one stored bin = 24 complex mode
+// slots (zero padded), 8-double groups XOR-swizzled by bin parity so that the DMMA B-fragment
+// LDS.128 of the fused kernel is bank-conflict free.
+__global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restrict__ Qt, int PK, int M, int N_Q, int N_Qpad) {
+    long long total = (long long)PK * N_Qpad * ILE_QT_ROW;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        int col = (int)(idx % ILE_QT_ROW);
+        long long rest = idx / ILE_QT_ROW;
+        int n = (int)(rest % N_Qpad);
+        int pk = (int)(rest / N_Qpad);
+        int r = col ^ ((n & 1) << 3);
+        int mode = r >> 1, part = r & 1;
+        double v = 0.0;
+        if (mode < M && n < N_Q) v = Qc[(((long long)pk * M + mode) * N_Q + n) * 2 + part];
+        Qt[idx] = v;
+    }
+}
+
+extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U,
+                            const double* V, double D_ref, int src_is_device) {
+    if (!ctx) return ILE_EINVAL;
+    if (!ctx->have_net || !ctx->have_modes) return ile_fail(ctx, ILE_ESTATE, "load_quv: set_network and set_modes first");
+    if (P < 1 || N_Q < 4 || !(fs > 0) || !Q || !U || !V || !(D_ref > 0))
+        return ile_fail(ctx, ILE_EINVAL, "load_quv: bad argument");
+    if (ctx->M > ILE_QT_ROW / 2 - 2) return ile_fail(ctx, ILE_EINVAL, "load_quv: at most %d modes", ILE_QT_ROW / 2 - 2);
+    const int K = ctx->K, M = ctx->M;
+    size_t nU = (size_t)P * K * M * M * 2, nQ = (size_t)P * K * M * N_Q * 2;
+    // symmetry check (Eq. 17-18) on the host
+    std::vector<double> hU, hV;
+    const double *pU = U, *pV = V;
+    if (src_is_device) {
+        hU.resize(nU);
+        hV.resize(nU);
+        ILE_CUDA(ctx, cudaMemcpy(hU.data(), U, nU * 8, cudaMemcpyDeviceToHost));
+        ILE_CUDA(ctx, cudaMemcpy(hV.data(), V, nU * 8, cudaMemcpyDeviceToHost));
+        pU = hU.data();
+        pV = hV.data();
+    }
+    for (size_t pk = 0; pk < (size_t)P * K; pk++) {
+        const double* u = pU + pk * M * M * 2;
+        const double* v = pV + pk * M * M * 2;
+        double scale = 0.0;
+        for (int a = 0; a < M * M * 2; a++) scale = fmax(scale, fmax(fabs(u[a]), fabs(v[a])));
+        double tol = 1e-12 * scale;
+        for (int a = 0; a < M; a++)
+            for (int b = 0; b < M; b++) {
+                double ur = u[(a * M + b) * 2], ui = u[(a * M + b) * 2 + 1];
+                double tr = u[(b * M + a) * 2], ti = u[(b * M + a) * 2 + 1];
+                if (fabs(ur - tr) > tol || fabs(ui + ti) > tol)
+                    return ile_fail(ctx, ILE_EINVAL, "load_quv: U[%zu] is not Hermitian at (%d,%d) (Eq. 17)", pk, a, b);
+                double vr = v[(a * M + b) * 2], vi = v[(a * M + b) * 2 + 1];
+                double wr = v[(b * M + a) * 2], wi = v[(b * M + a) * 2 + 1];
+                if (fabs(vr - wr) > tol || fabs(vi - wi) > tol)
+                    return ile_fail(ctx, ILE_EINVAL, "load_quv: V[%zu] is not symmetric at (%d,%d) (Eq. 18)", pk, a, b);
+            }
+    }
+    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_U); cudaFree(ctx->d_V);
+    ctx->d_Qc = ctx->d_Qt = ctx->d_U = ctx->d_V = nullptr;
+    ctx->have_quv = false;
+    int N_Qpad = ((N_Q + 1) & ~1) + 256;
+    size_t nQt = (size_t)P * K * N_Qpad * ILE_QT_ROW;
+    if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qt, nQt * 8) != cudaSuccess ||
+        cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess) {
+        cudaGetLastError();
+        return ile_fail(ctx, ILE_ENOMEM, "load_quv: device allocation failed");
+    }
+    cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_Qc, Q, nQ * 8, kind, ctx->stream));
+    ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_U, U, nU * 8, kind, ctx->stream));
+    ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, V, nU * 8, kind, ctx->stream));
+    repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qt, P * K, M, N_Q, N_Qpad);
+    ILE_LAUNCH_CHECK(ctx);
+    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->P = P; ctx->N_Q = N_Q; ctx->N_Qpad = N_Qpad; ctx->fs = fs; ctx->t_Q0 = t_Q0; ctx->D_ref = D_ref;
+    ctx->have_quv = true;
+    ctx->have_grid = false;
+    return ILE_OK;
+}
+
+extern "C" int ile_set_time_grid(ile_ctx* ctx, double t_lo, double dt, int N_t, int interp) {
+    if (!ctx) return ILE_EINVAL;
+    if (!ctx->have_quv) return ile_fail(ctx, ILE_ESTATE, "set_time_grid: load_quv first");
+    if (N_t < 1 || !(dt > 0) || (interp != 0 && interp != 1)) return ile_fail(ctx, ILE_EINVAL, "set_time_grid: bad argument");
+    double s = dt * ctx->fs;
+    int stride = (int)llrint(s);
+    if (stride < 1 || fabs(s - stride) > 1e-9) return ile_fail(ctx, ILE_EINVAL, "set_time_grid: dt*fs = %.12g is not a positive integer", s);
+    // stored-bin coordinate of the earliest / latest access (G10: a set-up error, never a per-sample branch)
+    double u_min = (t_lo - ctx->max_delay - ctx->t_Q0) * ctx->fs;
+    double u_max = (t_lo + (N_t - 1) * dt + ctx->max_delay - ctx->t_Q0) * ctx->fs;
+    if (u_min < 0.5 || u_max > (double)(ctx->N_Q - 2) - 0.5)
+        return ile_fail(ctx, ILE_ERANGE, "set_time_grid: window [%.3f, %.3f] bins leaves the stored span [0, %d]", u_min, u_max, ctx->N_Q - 1);
+    ctx->t_lo = t_lo; ctx->dt = dt; ctx->N_t = N_t; ctx->interp = interp; ctx->stride = stride;
+    ctx->have_grid = true;
+    return ILE_OK;
+}
+
+extern "C" int ile_set_prior(ile_ctx* ctx, double D_min, double D_max) {
+    if (!ctx) return ILE_EINVAL;
+    if (!(D_min > 0) || !(D_max > D_min)) return ile_fail(ctx, ILE_EINVAL, "set_prior: need 0 < D_min < D_max");
+    ctx->D_min = D_min; ctx->D_max = D_max; ctx->have_prior = true;
+    return ILE_OK;
+}
+
+extern "C" int ile_load_distance_table(ile_ctx* ctx, int nA, int nB, double A_lo, double A_hi, double B_lo, double B_hi,
+                                       const double* lnT) {
+    if (!ctx) return ILE_EINVAL;
+    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (nA == 0) {
+        cudaFree(ctx->d_lnT); ctx->d_lnT = nullptr; ctx->nA = ctx->nB = 0;
+        return ILE_OK;
+    }
+    if (nA < 2 || nB < 2 || !(A_hi > A_lo) || !(B_hi > B_lo) || !lnT) return ile_fail(ctx, ILE_EINVAL, "load_distance_table: bad argument");
+    cudaFree(ctx->d_lnT); ctx->d_lnT = nullptr;
+    if (cudaMalloc(&ctx->d_lnT, (size_t)nA * nB * 8) != cudaSuccess) { cudaGetLastError(); return ile_fail(ctx, ILE_ENOMEM, "table allocation failed"); }
+    ILE_CUDA(ctx, cudaMemcpy(ctx->d_lnT, lnT, (size_t)nA * nB * 8, cudaMemcpyHostToDevice));
+    ctx->nA = nA; ctx->nB = nB; ctx->A_lo = A_lo; ctx->A_hi = A_hi; ctx->B_lo = B_lo; ctx->B_hi = B_hi;
+    return ILE_OK;
+}
+
+int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
+    if (!ctx->have_net || !ctx->have_modes || !ctx->have_quv || !ctx->have_grid)
+        return ile_fail(ctx, ILE_ESTATE, "lnL: network, modes, Q/U/V and time grid must be set first");
+    if (p < 0 || p >= ctx->P) return ile_fail(ctx, ILE_EINVAL, "lnL: intrinsic point %d out of range [0,%d)", p, ctx->P);
+    bool table = ctx->d_lnT != nullptr;
+    if (!((d == 6 && !table) || (d == 5 && table)))
+        return ile_fail(ctx, ILE_EINVAL, "lnL: d = %d does not match the distance-table state (6 without table, 5 with)", d);
+    memset(L, 0, sizeof(*L));
+    const int K = ctx->K, M = ctx->M;
+    L->K = K; L->M = M; L->N_Q = ctx->N_Q; L->N_t = ctx->N_t; L->stride = ctx->stride; L->interp = ctx->interp;
+    L->d = d; L->use_table = table ? 1 : 0; L->N_Qpad = ctx->N_Qpad;
+    L->fs = ctx->fs; L->t_Q0 = ctx->t_Q0; L->t_lo = ctx->t_lo; L->dt = ctx->dt; L->D_ref = ctx->D_ref; L->gmst = ctx->gmst;
+    memcpy(L->D, ctx->D, sizeof(ctx->D));
+    memcpy(L->pos, ctx->pos, sizeof(ctx->pos));
+    const double PI = 3.14159265358979323846;
+    double lo[6] = {0.0, -1.0, 0.0, 0.0, -1.0, ctx->D_min}, hi[6] = {2 * PI, 1.0, PI, 2 * PI, 1.0, ctx->D_max};
+    memcpy(L->lo, lo, sizeof(lo));
+    memcpy(L->hi, hi, sizeof(hi));
+    L->ln_prior_const = -log(2 * PI) - log(2.0) - log(PI) - log(2 * PI) - log(2.0);
+    L->dist_norm = 3.0 / (ctx->D_max * ctx->D_max * ctx->D_max - ctx->D_min * ctx->D_min * ctx->D_min);
+    L->nA = ctx->nA; L->nB = ctx->nB; L->A_lo = ctx->A_lo; L->A_hi = ctx->A_hi; L->B_lo = ctx->B_lo; L->B_hi = ctx->B_hi;
+    L->lnT = ctx->d_lnT;
+    L->Qc = ctx->d_Qc + (size_t)p * K * M * ctx->N_Q * 2;
+    L->Qt = ctx->d_Qt + (size_t)p * K * ctx->N_Qpad * ILE_QT_ROW;
+    L->U = ctx->d_U + (size_t)p * K * M * M * 2;
+    L->V = ctx->d_V + (size_t)p * K * M * M * 2;
+    L->ylm = ctx->d_ylm;
+    return ILE_OK;
+}

@@ -1,0 +1,117 @@
+// Internal declarations shared by the translation units of libile (CUDA, sm_100a only).
+// Nothing here is shared with oracle/ (the CPU oracle is independent numpy code).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <math.h>
+#include "../../include/ile.h"
+
+#define ILE_C_LIGHT 299792458.0
+#define ILE_MAX_L 8
+#define ILE_YLM_MAX_TERMS 12
+#define ILE_QT_ROW 48            // doubles per stored bin in the tiled Q layout (24 complex modes)
+
+// ---------------------------------------------------------------- Ylm term table (device global)
+// -2Y_lm(theta, phi) = e^{i m phi} * sum_t coef[t] * cos(theta/2)^pc[t] * sin(theta/2)^ps[t]
+struct YlmMode {
+    int m;
+    int nterms;
+    int pc[ILE_YLM_MAX_TERMS];
+    int ps[ILE_YLM_MAX_TERMS];
+    double coef[ILE_YLM_MAX_TERMS];
+};
+struct YlmTable {
+    int M;
+    int max_abs_m;
+    int max_pow;
+    int pad;
+    YlmMode mode[ILE_MAX_M];
+};
+
+// ---------------------------------------------------------------- kernel parameter block (by value)
+struct LnlParams {
+    int K, M, N_Q, N_t, stride, interp, d, use_table;
+    int N_Qpad;                   // bins allocated per (p,k) in the tiled layout
+    double fs, t_Q0, t_lo, dt, D_ref, gmst;
+    double D[ILE_MAX_K][9];
+    double pos[ILE_MAX_K][3];
+    double lo[6], hi[6];          // prior box in z
+    double ln_prior_const;        // -ln(2pi) - ln2 - ln(pi) - ln(2pi) - ln2
+    double dist_norm;             // 3 / (D_max^3 - D_min^3)
+    // distance table
+    int nA, nB;
+    double A_lo, A_hi, B_lo, B_hi;
+    const double* lnT;
+    // per intrinsic point data (already offset to point p)
+    const double* Qc;             // [K][M][N_Q][2]
+    const double* Qt;             // [K][N_Qpad][48] tiled + swizzled
+    const double* U;              // [K][M][M][2]
+    const double* V;              // [K][M][M][2]
+    const YlmTable* ylm;
+};
+
+struct ile_ctx {
+    int device;
+    cudaStream_t stream;
+    char err[512];
+    bool have_net, have_modes, have_quv, have_grid, have_prior;
+    int K, M, P, N_Q, N_Qpad;
+    double D[ILE_MAX_K][9], pos[ILE_MAX_K][3], gmst, max_delay;
+    int ell[ILE_MAX_M], m[ILE_MAX_M];
+    YlmTable h_ylm;
+    YlmTable* d_ylm;
+    double fs, t_Q0, D_ref;
+    double *d_Qc, *d_Qt, *d_U, *d_V;
+    double t_lo, dt;
+    int N_t, interp, stride;
+    double D_min, D_max;
+    int nA, nB;
+    double A_lo, A_hi, B_lo, B_hi;
+    double* d_lnT;
+    int variant;
+    int sm_count;
+    // scratch
+    void* d_scratch;
+    size_t scratch_bytes;
+    uint64_t launches;            // kernels launched so far (for bench's gpu_launches)
+};
+
+int ile_fail(ile_ctx* ctx, int code, const char* fmt, ...);
+int ile_scratch(ile_ctx* ctx, size_t bytes, void** out);
+int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* P);
+int ile_launch_lnL_z(ile_ctx* ctx, int p, int N, int d, const double* z, const int* perm, double* lnL,
+                     double* ln_prior);
+int ile_launch_reduce(ile_ctx* ctx, int N, const double* lnw, ile_result* out_dev, int accumulate);
+uint64_t ile_launch_count(ile_ctx* ctx);
+
+#define ILE_CUDA(ctx, call)                                                                   \
+    do {                                                                                      \
+        cudaError_t e__ = (call);                                                             \
+        if (e__ != cudaSuccess)                                                               \
+            return ile_fail((ctx), ILE_ECUDA, "%s failed: %s (%s:%d)", #call,                 \
+                            cudaGetErrorString(e__), __FILE__, __LINE__);                     \
+    } while (0)
+#define ILE_LAUNCH_CHECK(ctx)                                                                 \
+    do {                                                                                      \
+        (ctx)->launches++;                                                                    \
+        cudaError_t e__ = cudaGetLastError();                                                 \
+        if (e__ != cudaSuccess)                                                               \
+            return ile_fail((ctx), ILE_ECUDA, "kernel launch failed: %s (%s:%d)",             \
+                            cudaGetErrorString(e__), __FILE__, __LINE__);                     \
+    } while (0)
+
+// ---------------------------------------------------------------- device helpers
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double neg_inf() { return __longlong_as_double(0xfff0000000000000LL); }
+__device__ __forceinline__ double pos_inf() { return __longlong_as_double(0x7ff0000000000000LL); }

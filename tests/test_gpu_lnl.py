@@ -1,0 +1,158 @@
+"""GPU parity: CUDA path (through the C ABI) vs the oracle, element by element (-m gpu)."""
+import math
+
+import numpy as np
+import pytest
+
+from synth import make_problem
+from synth.workloads import uniform_box_samples
+
+pytestmark = pytest.mark.gpu
+
+
+def _tol(ref):
+    return 1e-9 * np.maximum(1.0, np.abs(ref))      # north_star: per-sample lnL within 1e-9 relative (fp64)
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    return torch
+
+
+def _ile(prob):
+    from paper_2505_11655_b200 import Ile
+    ile = Ile(0)
+    ile.load_problem(prob)
+    return ile
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def test_antenna_and_ylm_parity(torch_mod):
+    from oracle import likelihood as lk
+    torch = torch_mod
+    prob = make_problem(2)
+    ile = _ile(prob)
+    rng = np.random.default_rng(5)
+    N = 4099
+    ra, dec, psi = rng.uniform(0, 2 * math.pi, N), np.arcsin(rng.uniform(-1, 1, N)), rng.uniform(0, math.pi, N)
+    incl, phi = np.arccos(rng.uniform(-1, 1, N)), rng.uniform(0, 2 * math.pi, N)
+    incl[:2] = [0.0, math.pi]
+    Fp, Fx, tau = ile.antenna(_dev(torch, ra), _dev(torch, dec), _dev(torch, psi), prob.K)
+    rFp, rFx, rtau = lk.antenna(prob.D, prob.pos, prob.gmst, ra, dec, psi)
+    np.testing.assert_allclose(Fp.cpu().numpy(), rFp, rtol=0, atol=1e-14)
+    np.testing.assert_allclose(Fx.cpu().numpy(), rFx, rtol=0, atol=1e-14)
+    np.testing.assert_allclose(tau.cpu().numpy(), rtau, rtol=0, atol=1e-17)
+    Y = ile.ylm(_dev(torch, incl), _dev(torch, phi), prob.M).cpu().numpy()
+    rY = lk.ylm(prob.ell, prob.m, incl, phi)
+    np.testing.assert_allclose(Y[..., 0] + 1j * Y[..., 1], rY, rtol=0, atol=2e-15)
+
+
+@pytest.mark.parametrize("cfg,N", [(1, 5000), (2, 1531)])
+def test_lnL_parity_all_entry_points(torch_mod, cfg, N):
+    from oracle import likelihood as lk
+    torch = torch_mod
+    prob = make_problem(cfg)
+    ile = _ile(prob)
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=77 + cfg)
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z)
+    zd = _dev(torch, z)
+    got, lp = ile.lnL_z(0, zd, want_prior=True)                     # fused DMMA kernel (unsorted: multi-round path)
+    got = got.cpu().numpy()
+    assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
+    np.testing.assert_allclose(lp.cpu().numpy(), lk.ln_prior_z(z, prob.D_min, prob.D_max), rtol=1e-14)
+    ile.set_lnL_variant(1)                                          # plain reference kernel
+    got1 = ile.lnL_z(0, zd).cpu().numpy()
+    assert np.all(np.abs(got1 - ref) <= _tol(ref))
+    ang = lk.z_to_angles(z)
+    got2, dump = ile.lnL(0, *[_dev(torch, a) for a in ang], N_t_dump=prob.N_t)
+    assert np.all(np.abs(got2.cpu().numpy() - ref) <= _tol(ref))
+    _, ref_t = lk.lnL_angles(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref,
+                             prob.fs, prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, *[a[:64] for a in ang], return_series=True)
+    d = dump.cpu().numpy()[:64]
+    assert np.all(np.abs(d - ref_t) <= 1e-9 * np.maximum(1.0, np.abs(ref_t)))
+
+
+def test_lnL_localised_samples_single_round(torch_mod):
+    """Samples concentrated on the sky (what the adapted samplers produce): one round per tile."""
+    from oracle import likelihood as lk
+    torch = torch_mod
+    prob = make_problem(3)
+    ile = _ile(prob)
+    N = 2048 + 17
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=5)
+    th = prob.inj[0]["theta0"]
+    z[0] = th["ra"] + 0.01 * (z[0] / (2 * math.pi) - 0.5)
+    z[1] = math.sin(th["dec"]) + 0.01 * z[1]
+    z[:, 7] = [7.0, 0.0, 1.0, 1.0, 0.0, 500.0]                        # one out-of-box sample
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, np.delete(z, 7, axis=1))
+    got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
+    assert got[7] == -np.inf
+    got = np.delete(got, 7)
+    assert ref.max() > 1000.0                                         # loud source: lnL dynamic range
+    assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
+
+
+def test_lnL_nearest_bin_and_table(torch_mod):
+    from oracle import likelihood as lk
+    torch = torch_mod
+    prob = make_problem(5, N=1)
+    ile = _ile(prob)
+    N = 777
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=9)
+    args = (prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+            prob.t_Q0, prob.t_lo, prob.dt, prob.N_t)
+    ref = lk.lnL_z(*args, z, table=prob.table)
+    zd = _dev(torch, z)
+    got = ile.lnL_z(0, zd).cpu().numpy()
+    assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
+    ile.set_time_grid(prob.t_lo, prob.dt, prob.N_t, 0)                # nearest-bin mode
+    ref0 = lk.lnL_z(*args, z, interp=0, table=prob.table)
+    got0 = ile.lnL_z(0, zd).cpu().numpy()
+    assert np.all(np.abs(got0 - ref0) <= _tol(ref0))
+
+
+def test_reduce_parity(torch_mod):
+    from oracle.reduce import reduce_lnw
+    torch = torch_mod
+    prob = make_problem(1)
+    ile = _ile(prob)
+    rng = np.random.default_rng(3)
+    for N in (1, 31, 100003):
+        lnw = rng.normal(0, 30, N) + 4000.0
+        if N > 50:
+            lnw[5] = -np.inf
+            lnw[6] = np.nan
+        ref = reduce_lnw(lnw)
+        got = ile.reduce(_dev(torch, lnw))
+        assert abs(got["ln_integral"] - ref["ln_integral"]) <= 1e-8                 # north_star: log-integral within 1e-8
+        for k in ("n_eff", "n_ess", "rel_variance"):
+            assert abs(got[k] - ref[k]) <= 1e-9 * max(1.0, abs(ref[k]))
+        assert got["n_samples"] == N and got["n_nonfinite"] == ref["n_nonfinite"]
+        assert got["ln_w_max"] == ref["ln_w_max"]
+    got = ile.reduce(_dev(torch, np.full(10, -np.inf)))
+    assert got["ln_integral"] == -np.inf and got["n_eff"] == 0
+
+
+def test_error_paths(torch_mod):
+    from paper_2505_11655_b200 import Ile, IleError
+    prob = make_problem(1)
+    ile = Ile(0)
+    with pytest.raises(IleError):
+        ile.set_time_grid(prob.t_lo, prob.dt, prob.N_t)              # ESTATE: nothing loaded
+    ile.set_network(prob.D, prob.pos, 0.0)
+    ile.set_modes(prob.ell, prob.m)
+    Ubad = prob.U.copy()
+    Ubad[0, 0, 0, 1] += 1e-6
+    with pytest.raises(IleError):
+        ile.load_quv(prob.Q, Ubad, prob.V, prob.fs, prob.t_Q0, prob.D_ref)   # Eq. 17 violated
+    ile.load_quv(prob.Q, prob.U, prob.V, prob.fs, prob.t_Q0, prob.D_ref)
+    with pytest.raises(IleError):
+        ile.set_time_grid(-0.045, prob.dt, prob.N_t)                 # ERANGE: window + delays leave Q
+    with pytest.raises(IleError):
+        ile.set_time_grid(prob.t_lo, 1.5 / prob.fs, 10)              # non-integer stride
