@@ -47,5 +47,7 @@ def iteration(ile, integ, N, g, update=True):
     lnw = np.where(np.isfinite(lnL), lnw, -np.inf)
     res = reduce_lnw(lnw)
     if update:
-        integ.update(z, lnw, ln_ps)
+        # a standalone AV samples uniformly inside its cells, so it follows PAPER.md:265 exactly
+        # (V_{g+1} = V_g N_min / N_live); ln p_s matters only to a portfolio member
+        integ.update(z, lnw, None if integ.kind == "AV" else ln_ps)
     return dict(z=z, ln_ps=ln_ps, lnL=lnL, lnw=lnw, result=res)

@@ -200,3 +200,177 @@ class Ile:
 def result_from_device(buf):
     """uint8 CUDA tensor holding ile_result structs -> numpy structured array (synchronises)."""
     return np.frombuffer(buf.cpu().numpy().tobytes(), dtype=RESULT_DTYPE)
+
+
+def parse_state(blob: bytes):
+    """Decode the blob of ile_integrator_get_state (layout in include/ile.h) into a dict."""
+    buf = memoryview(blob)
+    pos = 0
+
+    def i64(n=1):
+        nonlocal pos
+        a = np.frombuffer(buf, dtype="<i8", count=n, offset=pos)
+        pos += 8 * n
+        return a
+
+    def arr(dtype, *shape):
+        nonlocal pos
+        n = int(np.prod(shape)) if shape else 1
+        a = np.frombuffer(buf, dtype=dtype, count=n, offset=pos).reshape(shape).copy()
+        pos += a.itemsize * n
+        return a
+
+    def member():
+        kind, d = (int(v) for v in i64(2))
+        out = dict(kind=kind, d=d)
+        if kind == KINDS["AC"]:
+            nb = int(i64()[0])
+            out.update(n_bins=nb, H=arr("<u8", d, nb), pi=arr("<f8", d, nb), cdf=arr("<f8", d, nb + 1))
+        elif kind == KINDS["AV"]:
+            n, Cn, N_min = (int(v) for v in i64(3))
+            out.update(n=n, C=Cn, N_min=N_min, L_thr=float(arr("<f8", 1)[0]), keys=arr("<u8", Cn))
+        elif kind == KINDS["GMM"]:
+            Cn = int(i64()[0])
+            out.update(n_comp=Cn, omega=arr("<f8", Cn), mu=arr("<f8", Cn, d), Sigma=arr("<f8", Cn, d, d), L=arr("<f8", Cn, d, d))
+        return out
+
+    kind, d = (int(v) for v in np.frombuffer(buf, dtype="<i8", count=2, offset=0))
+    if kind != KINDS["PORTFOLIO"]:
+        return member()
+    pos = 16
+    Ns = int(i64()[0])
+    out = dict(kind=kind, d=d, n_members=Ns, W=arr("<f8", ILE_MAX_MEMBERS), frozen=arr("<i8", ILE_MAX_MEMBERS),
+               alloc=arr("<i8", ILE_MAX_MEMBERS), members=[])
+    for _ in range(Ns):
+        i64()
+        out["members"].append(member())
+    return out
+
+
+def pack_state(st: dict) -> bytes:
+    """Inverse of parse_state (for ile_integrator_set_state)."""
+    def member(m):
+        parts = [np.array([m["kind"], m["d"]], dtype="<i8").tobytes()]
+        if m["kind"] == KINDS["AC"]:
+            parts += [np.array([m["n_bins"]], dtype="<i8").tobytes(), np.ascontiguousarray(m["H"], dtype="<u8").tobytes(),
+                      np.ascontiguousarray(m["pi"], dtype="<f8").tobytes(), np.ascontiguousarray(m["cdf"], dtype="<f8").tobytes()]
+        elif m["kind"] == KINDS["AV"]:
+            keys = np.ascontiguousarray(m["keys"], dtype="<u8")
+            parts += [np.array([m["n"], len(keys), m.get("N_min", 0)], dtype="<i8").tobytes(),
+                      np.array([m.get("L_thr", -np.inf)], dtype="<f8").tobytes(), keys.tobytes()]
+        elif m["kind"] == KINDS["GMM"]:
+            parts += [np.array([len(m["omega"])], dtype="<i8").tobytes()]
+            parts += [np.ascontiguousarray(m[k], dtype="<f8").tobytes() for k in ("omega", "mu", "Sigma", "L")]
+        return b"".join(parts)
+
+    if st["kind"] != KINDS["PORTFOLIO"]:
+        return member(st)
+    parts = [np.array([st["kind"], st["d"], st["n_members"]], dtype="<i8").tobytes(),
+             np.ascontiguousarray(st["W"], dtype="<f8").tobytes(), np.ascontiguousarray(st["frozen"], dtype="<i8").tobytes(),
+             np.ascontiguousarray(st["alloc"], dtype="<i8").tobytes()]
+    for m in st["members"]:
+        b = member(m)
+        parts += [np.array([len(b)], dtype="<i8").tobytes(), b]
+    return b"".join(parts)
+
+
+class _DevView:
+    """__cuda_array_interface__ holder for a library-owned float64 device buffer."""
+
+    def __init__(self, ptr, shape):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+
+
+class Integrator:
+    """Handle over ile_integrator_* (include/ile.h).  Buffers are torch CUDA float64 tensors."""
+
+    def __init__(self, ile: Ile, kind: str, d: int, lo, hi, seed: int, max_batch: int, n_bins=100, eps=0.1, beta=1.0,
+                 P_thr=0.999, N_min_star=4096, n_gmm=8, members=("AC", "AV", "GMM")):
+        self.ile = ile
+        self.lib = ile.lib
+        self.torch = ile.torch
+        self.kind, self.d = kind, int(d)
+        o = IntegratorOpts()
+        self.ile._ck(self.lib.ile_integrator_opts_default(C.byref(o), C.c_int(KINDS[kind]), C.c_int(d)))
+        for c in range(d):
+            o.lo[c], o.hi[c] = float(lo[c]), float(hi[c])
+        o.seed, o.max_batch = int(seed) & 0xFFFFFFFFFFFFFFFF, int(max_batch)
+        o.n_bins, o.eps, o.beta, o.P_thr, o.N_min_star, o.n_gmm = int(n_bins), float(eps), float(beta), float(P_thr), int(N_min_star), int(n_gmm)
+        if kind == "PORTFOLIO":
+            o.n_members = len(members)
+            for a, k in enumerate(members):
+                o.member_kind[a] = KINDS[k]
+        self.opts = o
+        self.h = C.c_void_p()
+        self.ile._ck(self.lib.ile_integrator_create(ile.ctx, C.byref(o), C.byref(self.h)))
+
+    @classmethod
+    def from_problem(cls, ile: Ile, prob, max_batch=None, kind=None):
+        o = {k: v for k, v in prob.opts.items() if k != "seed"}
+        return cls(ile, kind or prob.kind, prob.d, prob.lo, prob.hi, prob.opts["seed"], max_batch or prob.N, **o)
+
+    def close(self):
+        if self.h:
+            self.lib.ile_integrator_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ck(self, rc):
+        self.ile._ck(rc)
+
+    def reset(self):
+        self._ck(self.lib.ile_integrator_reset(self.h))
+
+    def draw(self, N, it, z=None, ln_ps=None):
+        z = self.ile._empty(self.d, N) if z is None else z
+        ln_ps = self.ile._empty(N) if ln_ps is None else ln_ps
+        self._ck(self.lib.ile_integrator_draw(self.h, C.c_int(N), C.c_uint64(it), _ptr(z), _ptr(ln_ps)))
+        return z, ln_ps
+
+    def ln_pdf(self, z):
+        out = self.ile._empty(z.shape[1])
+        self._ck(self.lib.ile_integrator_ln_pdf(self.h, C.c_int(z.shape[1]), _ptr(z), _ptr(out)))
+        return out
+
+    def update(self, z, lnw, ln_ps=None):
+        self._ck(self.lib.ile_integrator_update(self.h, C.c_int(z.shape[1]), _ptr(z), _ptr(lnw), _ptr(ln_ps)))
+
+    def _results(self, n):
+        return self.torch.zeros(n * C.sizeof(Result), dtype=self.torch.uint8, device=f"cuda:{self.ile.device}")
+
+    def step(self, p, N, it, out=None):
+        """One iteration; returns the device result buffer (decode with result_from_device)."""
+        out = self._results(1) if out is None else out
+        self._ck(self.lib.ile_integrator_step(self.h, C.c_int(p), C.c_int(N), C.c_uint64(it), _ptr(out)))
+        return out
+
+    def run(self, p_first, p_count, n_iter, N, out=None):
+        out = self._results(p_count * n_iter) if out is None else out
+        self._ck(self.lib.ile_integrator_run(self.h, C.c_int(p_first), C.c_int(p_count), C.c_int(n_iter), C.c_int(N), _ptr(out)))
+        return out
+
+    def last_batch(self, N):
+        """Zero-copy torch views of the last batch's z [d,N], ln_ps, lnL, lnw (library-owned memory,
+        valid until the next draw/step)."""
+        ptrs = [C.c_void_p() for _ in range(4)]
+        self._ck(self.lib.ile_integrator_last_batch(self.h, *[C.byref(p) for p in ptrs]))
+        out = []
+        for p, shape in zip(ptrs, ((self.d, N), (N,), (N,), (N,))):
+            out.append(self.torch.as_tensor(_DevView(p.value, shape), device=f"cuda:{self.ile.device}"))
+        return out
+
+    def get_state(self):
+        n = C.c_size_t(0)
+        self._ck(self.lib.ile_integrator_get_state(self.h, None, C.byref(n)))
+        buf = (C.c_ubyte * n.value)()
+        self._ck(self.lib.ile_integrator_get_state(self.h, buf, C.byref(n)))
+        return parse_state(bytes(buf)[:n.value])
+
+    def set_state(self, st):
+        blob = pack_state(st)
+        self._ck(self.lib.ile_integrator_set_state(self.h, blob, C.c_size_t(len(blob))))

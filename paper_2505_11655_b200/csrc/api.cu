@@ -56,6 +56,7 @@ extern "C" int ile_create(ile_ctx** out, int device, void* cuda_stream) {
     cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
     ctx->D_min = 1.0;
     ctx->D_max = 2.0;
+    ctx->sky_sort = 1;
     *out = ctx;
     return ILE_OK;
 }
@@ -85,8 +86,9 @@ extern "C" int ile_sync(ile_ctx* ctx) {
 }
 
 extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
-    if (!ctx || variant < 0 || variant > 1) return ile_fail(ctx, ILE_EINVAL, "variant must be 0 or 1");
-    ctx->variant = variant;
+    if (!ctx || variant < 0 || variant > 2) return ile_fail(ctx, ILE_EINVAL, "variant must be 0, 1 or 2");
+    ctx->variant = variant == 1 ? 1 : 0;
+    ctx->sky_sort = variant == 2 ? 0 : 1;
     return ILE_OK;
 }
 

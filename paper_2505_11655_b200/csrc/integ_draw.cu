@@ -1,0 +1,225 @@
+// libile: integrator draws and sampling-prior densities.
+//   UNIFORM   z = lo + u (hi - lo)
+//   AC        inverse-cdf draw from the per-dimension piecewise-constant marginals
+//   AV        uniform in the union of active cells (reading G21)
+//   GMM       Box-Muller normals through the component's Cholesky factor
+//   PORTFOLIO members draw disjoint index ranges; every sample gets the mixture density
+//             p_s = sum_a W_a p_{s,a}
+// Counter-based generator: Philox4x32-10, counter (sample index, iteration, stream).
+#include "integ.cuh"
+
+#define TWO_PI 6.283185307179586
+
+// ---------------------------------------------------------------- member densities
+__device__ __forceinline__ double ln_pdf_ac(const IntegDev& I, const SamplerDev& S, const double* zz) {
+    double out = 0.0;
+    for (int c = 0; c < I.d; c++) {
+        const long long b = bin_index_dev(zz[c], I.lo[c], I.hi[c], I.nb);
+        const double pdf = __ddiv_rn(__dmul_rn(S.pi[c * I.nb + b], (double)I.nb), __dsub_rn(I.hi[c], I.lo[c]));
+        out = __dadd_rn(out, log(pdf));
+    }
+    return out;
+}
+
+__device__ __forceinline__ double ln_pdf_av(const IntegDev& I, const SamplerDev& S, const double* zz) {
+    const AvState av = *S.av;
+    unsigned long long key = 0, mul = 1;
+    for (int c = 0; c < I.d; c++) {
+        key += (unsigned long long)bin_index_dev(zz[c], I.lo[c], I.hi[c], av.n) * mul;
+        mul *= (unsigned long long)av.n;
+    }
+    long long lo = 0, hi = av.C;          // first position with keys[pos] >= key
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (S.keys[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    return (lo < av.C && S.keys[lo] == key) ? av.ln_ps : neg_inf();
+}
+
+// ln N(z; mu_c, Sigma_c) + ln omega_c for every component; returns the log-sum-exp
+__device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev& S, const double* zz, double* e_out) {
+    const int d = I.d, C = I.n_gmm;
+    const double* omega = S.gmm;
+    const double* mu = omega + C;
+    const double* L = mu + C * d + C * d * d;
+    double e[16];
+    double mx = neg_inf();
+    for (int c = 0; c < C; c++) {
+        const double* Lc = L + c * d * d;
+        double y[ILE_MAX_D];
+        double quad = 0.0, lndet = 0.0;
+        for (int i = 0; i < d; i++) {
+            double s = zz[i] - mu[c * d + i];
+            for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
+            y[i] = s / Lc[i * d + i];
+            quad = quad + y[i] * y[i];
+            lndet = lndet + log(Lc[i * d + i]);
+        }
+        e[c] = -0.5 * quad - lndet - 0.5 * d * log(TWO_PI) + log(omega[c]);
+        mx = fmax(mx, e[c]);
+    }
+    double sum = 0.0;
+    for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
+    if (e_out)
+        for (int c = 0; c < C; c++) e_out[c] = e[c];
+    return mx + log(sum);
+}
+
+__device__ __forceinline__ double member_ln_pdf(const IntegDev& I, int a, const double* zz, bool inbox) {
+    const SamplerDev& S = I.mem[a];
+    switch (S.kind) {
+        case ILE_KIND_UNIFORM: return inbox ? -log(I.V0) : neg_inf();
+        case ILE_KIND_AC: return inbox ? ln_pdf_ac(I, S, zz) : neg_inf();
+        case ILE_KIND_AV: return inbox ? ln_pdf_av(I, S, zz) : neg_inf();
+        case ILE_KIND_GMM: return ln_pdf_gmm(I, S, zz, nullptr);
+    }
+    return neg_inf();
+}
+
+__device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double* zz) {
+    bool inbox = true;
+    for (int c = 0; c < I.d; c++) inbox = inbox && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
+    if (I.n_members == 1) return member_ln_pdf(I, 0, zz, inbox);
+    double e[ILE_MAX_MEMBERS];
+    double mx = neg_inf();
+    for (int a = 0; a < I.n_members; a++) {
+        e[a] = log(I.port->W[a]) + member_ln_pdf(I, a, zz, inbox);
+        mx = fmax(mx, e[a]);
+    }
+    if (!is_finite_d(mx)) return neg_inf();
+    double sum = 0.0;
+    for (int a = 0; a < I.n_members; a++) sum += exp(e[a] - mx);
+    return mx + log(sum);
+}
+
+// ---------------------------------------------------------------- allocation (portfolio, reading G25)
+// N_a = floor(N W_a), remainder to the members in index order.
+__global__ void alloc_kernel(IntegDev I, long long N) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    PortState* P = I.port;
+    long long tot = 0;
+    for (int a = 0; a < I.n_members; a++) {
+        P->alloc[a] = (long long)floor(__dmul_rn((double)N, P->W[a]));
+        tot += P->alloc[a];
+    }
+    long long rem = N - tot;
+    int a = 0;
+    while (rem > 0) {
+        P->alloc[a % I.n_members] += 1;
+        rem--;
+        a++;
+    }
+    long long off = 0;
+    for (int b = 0; b < I.n_members; b++) {
+        P->offset[b] = off;
+        off += P->alloc[b];
+    }
+    P->offset[I.n_members] = off;
+}
+
+// ---------------------------------------------------------------- draw
+__global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned int g, double* __restrict__ z, double* __restrict__ ln_ps) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int a = 0;
+    while (a + 1 < I.n_members && i >= I.port->offset[a + 1]) a++;
+    const SamplerDev& S = I.mem[a];
+    const int d = I.d;
+    double zz[ILE_MAX_D];
+    double u0, u1;
+    philox_pair(I.seed, (unsigned long long)i, g, 0u, &u0, &u1);
+    if (S.kind == ILE_KIND_GMM) {
+        const int C = I.n_gmm;
+        const double* omega = S.gmm;
+        const double* mu = omega + C;
+        const double* L = mu + C * d + C * d * d;
+        int comp = 0;
+        double cw = 0.0;
+        for (int c = 0; c < C; c++) {     // number of cumulative weights <= u0
+            cw = cw + omega[c];
+            if (cw <= u0) comp = c + 1;
+        }
+        if (comp > C - 1) comp = C - 1;
+        double nrm[ILE_MAX_D + 1];
+        const int npair = (d + 1) / 2;
+        for (int p = 0; p < npair; p++) {
+            double ua, ub;
+            philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + p), &ua, &ub);
+            const double r = sqrt(-2.0 * log(1.0 - ua));
+            double sn, cs;
+            sincos(TWO_PI * ub, &sn, &cs);
+            nrm[2 * p] = r * cs;
+            nrm[2 * p + 1] = r * sn;
+        }
+        for (int r = 0; r < d; r++) {
+            double s = mu[comp * d + r];
+            for (int k = 0; k <= r; k++) s = s + L[comp * d * d + r * d + k] * nrm[k];
+            zz[r] = s;
+        }
+    } else {
+        unsigned long long key = 0;
+        long long n = 1;
+        if (S.kind == ILE_KIND_AV) {
+            const AvState av = *S.av;
+            n = av.n;
+            long long cell = (long long)floor(__dmul_rn(u0, (double)av.C));
+            if (cell > av.C - 1) cell = av.C - 1;
+            key = S.keys[cell];
+        }
+        double ua = 0.0, ub = 0.0;
+        for (int c = 0; c < d; c++) {
+            if ((c & 1) == 0) philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + (c >> 1)), &ua, &ub);
+            const double u = (c & 1) ? ub : ua;
+            const double lo = I.lo[c], hi = I.hi[c];
+            double zc;
+            if (S.kind == ILE_KIND_UNIFORM) {
+                zc = __dadd_rn(lo, __dmul_rn(u, __dsub_rn(hi, lo)));
+            } else if (S.kind == ILE_KIND_AC) {
+                const double* cdf = S.cdf + c * (I.nb + 1);
+                const double* pi = S.pi + c * I.nb;
+                int b0 = 0, b1 = I.nb;            // last b in [0, nb) with cdf[b] <= u
+                while (b1 - b0 > 1) {
+                    const int mid = (b0 + b1) >> 1;
+                    if (cdf[mid] <= u) b0 = mid; else b1 = mid;
+                }
+                double r = __ddiv_rn(__dsub_rn(u, cdf[b0]), pi[b0]);
+                r = fmin(r, 1.0 - 0x1.0p-53);
+                const double delta = __ddiv_rn(__dsub_rn(hi, lo), (double)I.nb);
+                zc = __dadd_rn(lo, __dmul_rn(__dadd_rn((double)b0, r), delta));
+            } else {                                // AV
+                const unsigned long long ic = key % (unsigned long long)n;
+                key = key / (unsigned long long)n;
+                const double y = __ddiv_rn(__dadd_rn((double)ic, u), (double)n);
+                zc = __dadd_rn(lo, __dmul_rn(y, __dsub_rn(hi, lo)));
+            }
+            zz[c] = fmin(zc, I.below_hi[c]);
+        }
+    }
+    for (int c = 0; c < d; c++) z[(long long)c * N + i] = zz[c];
+    // a standalone AV draws inside its own cells: p_s is the constant 1 / (v V0)
+    ln_ps[i] = (I.n_members == 1 && S.kind == ILE_KIND_AV) ? S.av->ln_ps : mixture_ln_pdf(I, zz);
+}
+
+__global__ void __launch_bounds__(128) ln_pdf_kernel(IntegDev I, int N, const double* __restrict__ z, double* __restrict__ ln_ps) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double zz[ILE_MAX_D];
+    for (int c = 0; c < I.d; c++) zz[c] = z[(long long)c * N + i];
+    ln_ps[i] = mixture_ln_pdf(I, zz);
+}
+
+int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, double* ln_ps) {
+    ile_ctx* ctx = it->ctx;
+    alloc_kernel<<<1, 32, 0, ctx->stream>>>(it->I, (long long)N);
+    ILE_LAUNCH_CHECK(ctx);
+    draw_kernel<<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, g, z, ln_ps);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}
+
+int integ_launch_ln_pdf(ile_integrator* it, int N, const double* z, double* ln_ps) {
+    ile_ctx* ctx = it->ctx;
+    ln_pdf_kernel<<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, z, ln_ps);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}

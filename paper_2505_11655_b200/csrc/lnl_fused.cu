@@ -11,6 +11,7 @@
 // DESIGN.md section 6 derives the tiling and the roofline.
 #include "common.cuh"
 #include "likelihood_dev.cuh"
+#include "radix_sort.cuh"
 
 #define FT_TS 32          // samples per CTA
 #define FT_THREADS 256
@@ -20,6 +21,47 @@
 #define FT_CAP 15         // largest per-sample offset above the tile base handled in one round
 #define FT_YM 24          // mode slots in the Y tile
 #define FT_REC 16         // doubles per sample record
+
+// ---------------------------------------------------------------- sky sort
+// The fused kernel handles a tile of 32 samples in one round when, for every detector, their
+// first-bin indices n_k = floor(u_k) lie within FT_CAP of the tile minimum.  n_k depends on the
+// sky position only, so samples are ordered by the cell (n_k >> 3)_k of their delays: one key
+// per sample, radix-sorted on the device with the sample index as payload (-> perm).
+#define SKY_CELL_SHIFT 3
+__global__ void __launch_bounds__(256) sky_key_kernel(LnlParams P, int N, const double* __restrict__ z, int n_min, int cell_bits,
+                                                      unsigned long long* __restrict__ key, unsigned int* __restrict__ val, long long* n_dev,
+                                                      int* bits_dev) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) {
+        *n_dev = N;
+        *bits_dev = cell_bits * P.K + 1;
+    }
+    if (i >= N) return;
+    const double ra = z[i], sd = z[(size_t)N + i];
+    bool ok = true;
+    for (int c = 0; c < P.d; c++) {
+        const double v = z[(size_t)c * N + i];
+        ok = ok && (v >= P.lo[c]) && (v < P.hi[c]);
+    }
+    unsigned long long k = 1ull << (cell_bits * P.K);      // out-of-box samples last
+    if (ok) {
+        const double cd = sqrt(fmax((1.0 - sd) * (1.0 + sd), 0.0));
+        double sg, cg;
+        sincos(P.gmst - ra, &sg, &cg);
+        const double n0 = cd * cg, n1 = -cd * sg, n2 = sd;
+        k = 0;
+        for (int kk = 0; kk < P.K; kk++) {
+            const double tau = -(P.pos[kk][0] * n0 + P.pos[kk][1] * n1 + P.pos[kk][2] * n2) / ILE_C_LIGHT;
+            double u = (P.t_lo + tau - P.t_Q0) * P.fs;
+            if (!P.interp) u = floor(u + 0.5);
+            int cell = ((int)floor(u) - n_min) >> SKY_CELL_SHIFT;
+            cell = max(0, min(cell, (1 << cell_bits) - 1));
+            k = (k << cell_bits) | (unsigned long long)cell;
+        }
+    }
+    key[i] = k;
+    val[i] = (unsigned int)i;
+}
 
 // ---------------------------------------------------------------- prep kernel
 // rec[t][0..3]=Re F_k, [4..7]=Im F_k (F = F+ - iFx), [8..11]=u_k (stored-bin coordinate of grid
@@ -363,13 +405,37 @@ int ile_launch_lnL_plain_z(ile_ctx* ctx, const LnlParams& P, int N, const double
 int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* z, const int* perm, double* lnL, double* ln_prior) {
     if (P.K > 3 || 2 * P.M > ILE_QT_ROW) return ile_launch_lnL_plain_z(ctx, P, N, z, lnL, ln_prior);
     const int tiles = (N + FT_TS - 1) / FT_TS;
-    const size_t rec_bytes = (size_t)tiles * FT_TS * FT_REC * sizeof(double);
-    const size_t y_bytes = (size_t)tiles * FT_YM * FT_TS * sizeof(double2);
+    const size_t rec_bytes = ((size_t)tiles * FT_TS * FT_REC * sizeof(double) + 255) / 256 * 256;
+    const size_t y_bytes = ((size_t)tiles * FT_YM * FT_TS * sizeof(double2) + 255) / 256 * 256;
+    const size_t key_bytes = ((size_t)N * 8 + 255) / 256 * 256, val_bytes = ((size_t)N * 4 + 255) / 256 * 256;
+    const size_t sort_bytes = (radix_sort_scratch_bytes(N) + 255) / 256 * 256;
+    const bool sort = perm == nullptr && ctx->sky_sort && N > FT_TS;
     void* scratch = nullptr;
-    int rc = ile_scratch(ctx, rec_bytes + y_bytes + 256, &scratch);
+    int rc = ile_scratch(ctx, rec_bytes + y_bytes + (sort ? 2 * key_bytes + 2 * val_bytes + sort_bytes + 256 : 0), &scratch);
     if (rc) return rc;
-    double* rec = (double*)scratch;
-    double2* yt = (double2*)((char*)scratch + ((rec_bytes + 127) / 128) * 128);
+    char* base = (char*)scratch;
+    double* rec = (double*)base;
+    double2* yt = (double2*)(base + rec_bytes);
+    if (sort) {
+        char* sb = base + rec_bytes + y_bytes;
+        unsigned long long* k0 = (unsigned long long*)sb;
+        unsigned long long* k1 = (unsigned long long*)(sb + key_bytes);
+        unsigned int* v0 = (unsigned int*)(sb + 2 * key_bytes);
+        unsigned int* v1 = (unsigned int*)(sb + 2 * key_bytes + val_bytes);
+        void* hist = sb + 2 * key_bytes + 2 * val_bytes;
+        long long* n_dev = (long long*)(sb + 2 * key_bytes + 2 * val_bytes + sort_bytes);
+        int* bits_dev = (int*)(n_dev + 1);
+        // cells of 2^SKY_CELL_SHIFT stored bins over the range of delays the network allows
+        const int n_min = (int)floor((P.t_lo - ctx->max_delay - P.t_Q0) * P.fs) - 1;
+        const int n_max = (int)floor((P.t_lo + ctx->max_delay - P.t_Q0) * P.fs) + 1;
+        int cell_bits = 1;
+        while ((1 << cell_bits) <= ((n_max - n_min) >> SKY_CELL_SHIFT)) cell_bits++;
+        sky_key_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(P, N, z, n_min, cell_bits, k0, v0, n_dev, bits_dev);
+        ILE_LAUNCH_CHECK(ctx);
+        rc = radix_sort_device(ctx, N, n_dev, bits_dev, (uint64_t*)k0, v0, (uint64_t*)k1, v1, hist, (cell_bits * P.K + 1 + 7) / 8);
+        if (rc) return rc;
+        perm = (const int*)v0;
+    }
     lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, z, perm, rec, yt, ln_prior);
     ILE_LAUNCH_CHECK(ctx);
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;

@@ -1,0 +1,171 @@
+// libile: device-resident stable LSD radix sort (see radix_sort.cuh).  Three kernels per 8-bit
+// pass: per-block digit histogram, one-block exclusive scan of the [digit][block] table, and a
+// stable scatter that ranks keys inside a warp with __match_any_sync.
+#include "radix_sort.cuh"
+
+__device__ __forceinline__ int rs_passes(int bits) { return bits <= 0 ? 0 : (bits + 7) >> 3; }
+
+// which ping-pong buffer holds the data before pass p (inactive passes do not move it)
+__device__ __forceinline__ int rs_src(int p, int npass) { return (p < npass ? p : npass) & 1; }
+
+__global__ void __launch_bounds__(RS_THREADS) rs_hist_kernel(int p, const long long* __restrict__ n_dev, const int* __restrict__ bits_dev,
+                                                             const uint64_t* __restrict__ k0, const uint64_t* __restrict__ k1,
+                                                             uint32_t* __restrict__ hist, int max_blocks) {
+    const int npass = rs_passes(*bits_dev);
+    if (p >= npass) return;
+    const long long n = *n_dev;
+    const long long base = (long long)blockIdx.x * RS_TILE;
+    if (base >= n) return;
+    __shared__ uint32_t sh[256];
+    sh[threadIdx.x] = 0;
+    __syncthreads();
+    const uint64_t* src = rs_src(p, npass) ? k1 : k0;
+    const int shift = 8 * p;
+#pragma unroll 4
+    for (int r = 0; r < RS_TILE / RS_THREADS; r++) {
+        const long long i = base + r * RS_THREADS + threadIdx.x;
+        const bool act = i < n;
+        const int dg = act ? (int)((src[i] >> shift) & 0xffu) : 256;
+        const unsigned m = __match_any_sync(0xffffffffu, dg);
+        if (act && (threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&sh[dg], (uint32_t)__popc(m));
+    }
+    __syncthreads();
+    hist[(size_t)threadIdx.x * max_blocks + blockIdx.x] = sh[threadIdx.x];
+}
+
+// exclusive scan of hist[digit][block], digit-major, over the blocks in use
+__global__ void __launch_bounds__(1024) rs_scan_kernel(int p, const long long* __restrict__ n_dev, const int* __restrict__ bits_dev,
+                                                       uint32_t* __restrict__ hist, int max_blocks) {
+    const int npass = rs_passes(*bits_dev);
+    if (p >= npass) return;
+    const long long n = *n_dev;
+    const int nblocks = (int)((n + RS_TILE - 1) / RS_TILE);
+    __shared__ uint32_t part[1024];
+    const int t = threadIdx.x, dg = t >> 2, qd = t & 3;
+    const int per = (nblocks + 3) >> 2;
+    const int b0 = min(qd * per, nblocks), b1 = min(b0 + per, nblocks);
+    uint32_t s = 0;
+    uint32_t* row = hist + (size_t)dg * max_blocks;
+    for (int b = b0; b < b1; b++) s += row[b];
+    part[t] = s;
+    __syncthreads();
+    // block-wide exclusive scan of part[] (1024 entries, in index order = digit-major order)
+    uint32_t v = s;
+    for (int o = 1; o < 1024; o <<= 1) {
+        uint32_t add = (t >= o) ? part[t - o] : 0;
+        __syncthreads();
+        part[t] += add;
+        __syncthreads();
+    }
+    uint32_t run = part[t] - v;
+    for (int b = b0; b < b1; b++) {
+        uint32_t c = row[b];
+        row[b] = run;
+        run += c;
+    }
+}
+
+template <bool HAS_VAL>
+__global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(int p, const long long* __restrict__ n_dev, const int* __restrict__ bits_dev,
+                                                                uint64_t* __restrict__ k0, uint32_t* __restrict__ v0,
+                                                                uint64_t* __restrict__ k1, uint32_t* __restrict__ v1,
+                                                                const uint32_t* __restrict__ hist, int max_blocks) {
+    const int npass = rs_passes(*bits_dev);
+    if (p >= npass) return;
+    const long long n = *n_dev;
+    const long long base = (long long)blockIdx.x * RS_TILE;
+    if (base >= n) return;
+    __shared__ uint32_t wh[RS_THREADS / 32][257];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int q = threadIdx.x; q < (RS_THREADS / 32) * 257; q += RS_THREADS) (&wh[0][0])[q] = 0;
+    __syncthreads();
+    const bool s = rs_src(p, npass);
+    const uint64_t* ksrc = s ? k1 : k0;
+    uint64_t* kdst = s ? k0 : k1;
+    const uint32_t* vsrc = s ? v1 : v0;
+    uint32_t* vdst = s ? v0 : v1;
+    const int shift = 8 * p;
+    const int ROUNDS = RS_TILE / RS_THREADS;          // rounds per warp; warp w owns keys [w*ROUNDS*32, ...)
+    const long long wbase = base + (long long)w * ROUNDS * 32;
+    // phase A: per-warp digit counts
+    for (int r = 0; r < ROUNDS; r++) {
+        const long long i = wbase + r * 32 + lane;
+        const bool act = i < n;
+        const int dg = act ? (int)((ksrc[i] >> shift) & 0xffu) : 256;
+        const unsigned m = __match_any_sync(0xffffffffu, dg);
+        if (lane == __ffs(m) - 1) wh[w][dg] += (uint32_t)__popc(m);
+        __syncwarp();
+    }
+    __syncthreads();
+    // phase B: turn the counts into start offsets (global base of (digit, block) + earlier warps)
+    {
+        const int dg = threadIdx.x;
+        uint32_t run = hist[(size_t)dg * max_blocks + blockIdx.x];
+        for (int ww = 0; ww < RS_THREADS / 32; ww++) {
+            uint32_t c = wh[ww][dg];
+            wh[ww][dg] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+    // phase C: stable rank and scatter
+    for (int r = 0; r < ROUNDS; r++) {
+        const long long i = wbase + r * 32 + lane;
+        const bool act = i < n;
+        uint64_t key = 0;
+        if (act) key = ksrc[i];
+        const int dg = act ? (int)((key >> shift) & 0xffu) : 256;
+        const unsigned m = __match_any_sync(0xffffffffu, dg);
+        const uint32_t pos = wh[w][dg] + (uint32_t)__popc(m & ((1u << lane) - 1u));
+        __syncwarp();
+        if (lane == __ffs(m) - 1) wh[w][dg] += (uint32_t)__popc(m);
+        __syncwarp();
+        if (act) {
+            kdst[pos] = key;
+            if (HAS_VAL) vdst[pos] = vsrc[i];
+        }
+    }
+}
+
+// result is in buffer (npass & 1): copy back into (k0, v0) when that is buffer 1
+template <bool HAS_VAL>
+__global__ void rs_finish_kernel(const long long* __restrict__ n_dev, const int* __restrict__ bits_dev, uint64_t* __restrict__ k0,
+                                 uint32_t* __restrict__ v0, const uint64_t* __restrict__ k1, const uint32_t* __restrict__ v1, int max_passes) {
+    int npass = rs_passes(*bits_dev);
+    if (npass > max_passes) npass = max_passes;
+    if (!(npass & 1)) return;
+    const long long n = *n_dev;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        k0[i] = k1[i];
+        if (HAS_VAL) v0[i] = v1[i];
+    }
+}
+
+size_t radix_sort_scratch_bytes(int max_n) {
+    size_t blocks = ((size_t)max_n + RS_TILE - 1) / RS_TILE;
+    if (blocks < 1) blocks = 1;
+    return 256 * blocks * sizeof(uint32_t);
+}
+
+int radix_sort_device(ile_ctx* ctx, int max_n, const long long* n_dev, const int* bits_dev, uint64_t* k0, uint32_t* v0, uint64_t* k1,
+                      uint32_t* v1, void* scratch, int max_passes) {
+    if (max_n < 1) return ILE_OK;
+    if (max_passes > RS_MAX_PASSES) max_passes = RS_MAX_PASSES;
+    const int blocks = (max_n + RS_TILE - 1) / RS_TILE;
+    uint32_t* hist = (uint32_t*)scratch;
+    const bool has_val = v0 != nullptr;
+    for (int p = 0; p < max_passes; p++) {
+        rs_hist_kernel<<<blocks, RS_THREADS, 0, ctx->stream>>>(p, n_dev, bits_dev, k0, k1, hist, blocks);
+        ILE_LAUNCH_CHECK(ctx);
+        rs_scan_kernel<<<1, 1024, 0, ctx->stream>>>(p, n_dev, bits_dev, hist, blocks);
+        ILE_LAUNCH_CHECK(ctx);
+        if (has_val) rs_scatter_kernel<true><<<blocks, RS_THREADS, 0, ctx->stream>>>(p, n_dev, bits_dev, k0, v0, k1, v1, hist, blocks);
+        else rs_scatter_kernel<false><<<blocks, RS_THREADS, 0, ctx->stream>>>(p, n_dev, bits_dev, k0, v0, k1, v1, hist, blocks);
+        ILE_LAUNCH_CHECK(ctx);
+    }
+    int g = blocks < ctx->sm_count * 4 ? blocks : ctx->sm_count * 4;
+    if (has_val) rs_finish_kernel<true><<<g, 256, 0, ctx->stream>>>(n_dev, bits_dev, k0, v0, k1, v1, max_passes);
+    else rs_finish_kernel<false><<<g, 256, 0, ctx->stream>>>(n_dev, bits_dev, k0, v0, k1, v1, max_passes);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}
