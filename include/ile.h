@@ -102,6 +102,19 @@ const char *ile_last_error(const ile_ctx *ctx);
 int ile_sync(ile_ctx *ctx); /* waits for the stream; surfaces asynchronous CUDA errors */
 const char *ile_version(void);
 
+/* ------------------------------------------------------------------ measurement
+ * Number of CUDA kernels this context has launched so far. */
+uint64_t ile_kernel_launches(const ile_ctx *ctx);
+/* on != 0: bracket every launch of the fused lnL kernel (the dominant kernel, steps 5-6) with
+ * CUDA events on the context's stream and reset the totals; 0: stop.  ile_kernel_time waits for
+ * the recorded events and returns the summed device time (ms) and the number of launches. */
+int ile_kernel_timing(ile_ctx *ctx, int on);
+int ile_kernel_time(ile_ctx *ctx, double *total_ms, uint64_t *launches);
+/* Register-resident FP64 peak probe with no memory traffic: mode 0 = independent DFMA chains on
+ * the FP64 ALUs, mode 1 = independent DMMA.8x8x4 chains on the FP64 tensor pipe.  Synchronises;
+ * *tflops (host) receives the best of three timed runs. */
+int ile_fp64_peak(ile_ctx *ctx, int mode, double *tflops);
+
 /* ------------------------------------------------------------------ problem definition (host pointers)
  * detector response functions and positions.  D[k] is the 3x3 response tensor
  * (symmetric; only that is checked), pos_m[k] the position in metres in the Earth-fixed frame,

@@ -160,6 +160,30 @@ class Ile:
     def sync(self):
         self._ck(self.lib.ile_sync(self.ctx))
 
+    # ---- measurement helpers (include/ile.h "measurement")
+    def kernel_launches(self) -> int:
+        self.lib.ile_kernel_launches.restype = C.c_uint64
+        return int(self.lib.ile_kernel_launches(self.ctx))
+
+    def kernel_timing(self, on: bool):
+        self._ck(self.lib.ile_kernel_timing(self.ctx, C.c_int(1 if on else 0)))
+
+    def kernel_time(self):
+        """(total device ms, launches) of the fused lnL kernel since kernel_timing(True)."""
+        ms, n = C.c_double(0.0), C.c_uint64(0)
+        self._ck(self.lib.ile_kernel_time(self.ctx, C.byref(ms), C.byref(n)))
+        return ms.value, int(n.value)
+
+    def fp64_peak(self, mode: int) -> float:
+        tf = C.c_double(0.0)
+        self._ck(self.lib.ile_fp64_peak(self.ctx, C.c_int(mode), C.byref(tf)))
+        return tf.value
+
+    def load_quv_ptr(self, P, N_Q, fs, t_Q0, Q_ptr, U_ptr, V_ptr, D_ref):
+        """ile_load_quv from raw host addresses (e.g. pinned torch tensors): no marshalling copies."""
+        self._ck(self.lib.ile_load_quv(self.ctx, C.c_int(P), C.c_int(N_Q), C.c_double(fs), C.c_double(t_Q0), C.c_void_p(Q_ptr),
+                                       C.c_void_p(U_ptr), C.c_void_p(V_ptr), C.c_double(D_ref), C.c_int(0)))
+
     # ---- direct evaluation (torch CUDA float64 tensors)
     def _empty(self, *shape):
         return self.torch.empty(shape, dtype=self.torch.float64, device=f"cuda:{self.device}")

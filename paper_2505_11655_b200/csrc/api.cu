@@ -35,6 +35,54 @@ int ile_scratch(ile_ctx* ctx, size_t bytes, void** out) {
 
 uint64_t ile_launch_count(ile_ctx* ctx) { return ctx->launches; }
 
+extern "C" uint64_t ile_kernel_launches(const ile_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+// ---- device timing of the dominant kernel: cudaEvent pairs recorded on the context's stream
+int ile_timing_begin(ile_ctx* ctx) {
+    if (!ctx->timing_on) return -1;
+    if (ctx->tev_used == ILE_TIMING_SLOTS && ile_timing_drain(ctx) != ILE_OK) return -1;
+    const int slot = ctx->tev_used++;
+    cudaEventRecord(ctx->tev[2 * slot], ctx->stream);
+    return slot;
+}
+void ile_timing_end(ile_ctx* ctx, int slot) {
+    if (slot >= 0) cudaEventRecord(ctx->tev[2 * slot + 1], ctx->stream);
+}
+int ile_timing_drain(ile_ctx* ctx) {
+    if (!ctx->tev) return ILE_OK;
+    for (int s = 0; s < ctx->tev_used; s++) {
+        ILE_CUDA(ctx, cudaEventSynchronize(ctx->tev[2 * s + 1]));
+        float ms = 0.f;
+        ILE_CUDA(ctx, cudaEventElapsedTime(&ms, ctx->tev[2 * s], ctx->tev[2 * s + 1]));
+        ctx->t_ms_total += ms;
+        ctx->t_count++;
+    }
+    ctx->tev_used = 0;
+    return ILE_OK;
+}
+extern "C" int ile_kernel_timing(ile_ctx* ctx, int on) {
+    if (!ctx) return ILE_EINVAL;
+    int rc = ile_timing_drain(ctx);
+    if (rc) return rc;
+    if (on && !ctx->tev) {
+        ctx->tev = (cudaEvent_t*)calloc(2 * ILE_TIMING_SLOTS, sizeof(cudaEvent_t));
+        if (!ctx->tev) return ile_fail(ctx, ILE_ENOMEM, "kernel_timing: out of host memory");
+        for (int s = 0; s < 2 * ILE_TIMING_SLOTS; s++) ILE_CUDA(ctx, cudaEventCreate(&ctx->tev[s]));
+    }
+    ctx->timing_on = on ? 1 : 0;
+    ctx->t_ms_total = 0.0;
+    ctx->t_count = 0;
+    return ILE_OK;
+}
+extern "C" int ile_kernel_time(ile_ctx* ctx, double* total_ms, uint64_t* launches) {
+    if (!ctx) return ILE_EINVAL;
+    int rc = ile_timing_drain(ctx);
+    if (rc) return rc;
+    if (total_ms) *total_ms = ctx->t_ms_total;
+    if (launches) *launches = ctx->t_count;
+    return ILE_OK;
+}
+
 extern "C" const char* ile_version(void) { return "ile-b200 0.1 (sm_100a)"; }
 
 extern "C" int ile_create(ile_ctx** out, int device, void* cuda_stream) {
@@ -72,6 +120,10 @@ extern "C" int ile_destroy(ile_ctx* ctx) {
     cudaFree(ctx->d_V);
     cudaFree(ctx->d_lnT);
     cudaFree(ctx->d_scratch);
+    if (ctx->tev) {
+        for (int s = 0; s < 2 * ILE_TIMING_SLOTS; s++) cudaEventDestroy(ctx->tev[s]);
+        free(ctx->tev);
+    }
     free(ctx);
     return ILE_OK;
 }
@@ -233,15 +285,19 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
             }
     }
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_U); cudaFree(ctx->d_V);
-    ctx->d_Qc = ctx->d_Qt = ctx->d_U = ctx->d_V = nullptr;
-    ctx->have_quv = false;
     int N_Qpad = ((N_Q + 1) & ~1) + 256;
     size_t nQt = (size_t)P * K * N_Qpad * ILE_QT_ROW;
-    if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qt, nQt * 8) != cudaSuccess ||
-        cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess) {
-        cudaGetLastError();
-        return ile_fail(ctx, ILE_ENOMEM, "load_quv: device allocation failed");
+    // same shapes as the resident set (the next intrinsic point of a run): reuse the allocations
+    const bool reuse = ctx->have_quv && ctx->P == P && ctx->N_Q == N_Q && ctx->quv_K == K && ctx->quv_M == M;
+    ctx->have_quv = false;
+    if (!reuse) {
+        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_U); cudaFree(ctx->d_V);
+        ctx->d_Qc = ctx->d_Qt = ctx->d_U = ctx->d_V = nullptr;
+        if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qt, nQt * 8) != cudaSuccess ||
+            cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess) {
+            cudaGetLastError();
+            return ile_fail(ctx, ILE_ENOMEM, "load_quv: device allocation failed");
+        }
     }
     cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_Qc, Q, nQ * 8, kind, ctx->stream));
@@ -250,7 +306,7 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qt, P * K, M, N_Q, N_Qpad);
     ILE_LAUNCH_CHECK(ctx);
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    ctx->P = P; ctx->N_Q = N_Q; ctx->N_Qpad = N_Qpad; ctx->fs = fs; ctx->t_Q0 = t_Q0; ctx->D_ref = D_ref;
+    ctx->P = P; ctx->N_Q = N_Q; ctx->N_Qpad = N_Qpad; ctx->quv_K = K; ctx->quv_M = M; ctx->fs = fs; ctx->t_Q0 = t_Q0; ctx->D_ref = D_ref;
     ctx->have_quv = true;
     ctx->have_grid = false;
     return ILE_OK;

@@ -11,6 +11,7 @@
 #define ILE_C_LIGHT 299792458.0
 #define ILE_MAX_L 8
 #define ILE_YLM_MAX_TERMS 12
+#define ILE_TIMING_SLOTS 256
 #define ILE_QT_ROW 48            // doubles per stored bin in the tiled Q layout (24 complex modes)
 
 // ---------------------------------------------------------------- Ylm term table (device global)
@@ -57,7 +58,7 @@ struct ile_ctx {
     cudaStream_t stream;
     char err[512];
     bool have_net, have_modes, have_quv, have_grid, have_prior;
-    int K, M, P, N_Q, N_Qpad;
+    int K, M, P, N_Q, N_Qpad, quv_K, quv_M;
     double D[ILE_MAX_K][9], pos[ILE_MAX_K][3], gmst, max_delay;
     int ell[ILE_MAX_M], m[ILE_MAX_M];
     YlmTable h_ylm;
@@ -77,6 +78,12 @@ struct ile_ctx {
     void* d_scratch;
     size_t scratch_bytes;
     uint64_t launches;            // kernels launched so far (for bench's gpu_launches)
+    // optional device timing of the fused lnL kernel (ile_kernel_timing): event pairs on the stream
+    int timing_on;
+    cudaEvent_t* tev;             // [2 * ILE_TIMING_SLOTS]
+    int tev_used;
+    double t_ms_total;
+    uint64_t t_count;
 };
 
 int ile_fail(ile_ctx* ctx, int code, const char* fmt, ...);
@@ -86,6 +93,9 @@ int ile_launch_lnL_z(ile_ctx* ctx, int p, int N, int d, const double* z, const i
                      double* ln_prior);
 int ile_launch_reduce(ile_ctx* ctx, int N, const double* lnw, ile_result* out_dev, int accumulate);
 uint64_t ile_launch_count(ile_ctx* ctx);
+int ile_timing_begin(ile_ctx* ctx);            // returns a slot (or -1 when timing is off)
+void ile_timing_end(ile_ctx* ctx, int slot);
+int ile_timing_drain(ile_ctx* ctx);
 
 #define ILE_CUDA(ctx, call)                                                                   \
     do {                                                                                      \

@@ -395,7 +395,9 @@ static int launch_fused_t(ile_ctx* ctx, const LnlParams& P, int N, const double*
         configured = true;
     }
     const int tiles = (N + FT_TS - 1) / FT_TS;
+    const int slot = ile_timing_begin(ctx);
     lnl_fused_kernel<NPAIR, SINGLE><<<tiles, FT_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL);
+    ile_timing_end(ctx, slot);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }

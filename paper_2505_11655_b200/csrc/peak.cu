@@ -1,0 +1,76 @@
+// libile: FP64 peak probes ("the build must measure the real FP64 FMA peak with a
+// register-resident FMA-chain micro-benchmark").  Two kernels with no memory traffic: independent
+// DFMA chains on the FP64 ALUs, and independent DMMA.8x8x4 chains on the FP64 tensor pipe.  The
+// roofline of the fused lnL kernel is quoted against the larger of the two measured rates.
+#include "common.cuh"
+
+#define PK_CHAINS 8
+
+__global__ void __launch_bounds__(256) dfma_chain_kernel(int iters, double seed, double* out) {
+    double a[PK_CHAINS];
+#pragma unroll
+    for (int c = 0; c < PK_CHAINS; c++) a[c] = seed + c + threadIdx.x * 1e-9;
+    const double m = 1.0 - 1e-9, b = 1e-9;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int r = 0; r < 8; r++)
+#pragma unroll
+            for (int c = 0; c < PK_CHAINS; c++) a[c] = fma(a[c], m, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < PK_CHAINS; c++) s += a[c];
+    if (s == 12345.678) out[blockIdx.x * blockDim.x + threadIdx.x] = s;   // never true: keeps the chain live
+}
+
+__global__ void __launch_bounds__(256) dmma_chain_kernel(int iters, double seed, double* out) {
+    double d0[PK_CHAINS], d1[PK_CHAINS];
+#pragma unroll
+    for (int c = 0; c < PK_CHAINS; c++) { d0[c] = seed + c; d1[c] = seed - c; }
+    const double a = 1e-9 * (threadIdx.x & 3), b = 1.0 + 1e-9 * (threadIdx.x >> 2);
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int r = 0; r < 4; r++)
+#pragma unroll
+            for (int c = 0; c < PK_CHAINS; c++)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(d0[c]), "+d"(d1[c]) : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < PK_CHAINS; c++) s += d0[c] + d1[c];
+    if (s == 12345.678) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+// mode 0: DFMA chains (2 flop per thread-instruction); mode 1: DMMA m8n8k4 (512 flop per warp-
+// instruction).  Runs on the context's stream, synchronises, returns TFLOP/s of the best of 3 runs.
+extern "C" int ile_fp64_peak(ile_ctx* ctx, int mode, double* tflops) {
+    if (!ctx) return ILE_EINVAL;
+    if (!tflops || mode < 0 || mode > 1) return ile_fail(ctx, ILE_EINVAL, "fp64_peak: mode 0 (DFMA) or 1 (DMMA)");
+    const int blocks = ctx->sm_count * 8, threads = 256, iters = mode == 0 ? 4096 : 2048;
+    void* scratch = nullptr;
+    int rc = ile_scratch(ctx, (size_t)blocks * threads * 8, &scratch);
+    if (rc) return rc;
+    cudaEvent_t e0, e1;
+    ILE_CUDA(ctx, cudaEventCreate(&e0));
+    ILE_CUDA(ctx, cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int rep = 0; rep < 4; rep++) {
+        ILE_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+        if (mode == 0) dfma_chain_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, 1.0, (double*)scratch);
+        else dmma_chain_kernel<<<blocks, threads, 0, ctx->stream>>>(iters, 1.0, (double*)scratch);
+        ILE_LAUNCH_CHECK(ctx);
+        ILE_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+        ILE_CUDA(ctx, cudaEventSynchronize(e1));
+        float ms = 0.f;
+        ILE_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        const double flop = mode == 0 ? (double)blocks * threads * iters * 8.0 * PK_CHAINS * 2.0
+                                      : (double)blocks * (threads / 32) * iters * 4.0 * PK_CHAINS * 512.0;
+        const double tf = flop / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *tflops = best;
+    return ILE_OK;
+}
