@@ -138,9 +138,10 @@ extern "C" int ile_sync(ile_ctx* ctx) {
 }
 
 extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
-    if (!ctx || variant < 0 || variant > 2) return ile_fail(ctx, ILE_EINVAL, "variant must be 0, 1 or 2");
+    if (!ctx || variant < 0 || variant > 3) return ile_fail(ctx, ILE_EINVAL, "variant must be 0..3");
     ctx->variant = variant == 1 ? 1 : 0;
     ctx->sky_sort = variant == 2 ? 0 : 1;
+    ctx->fused_gen1 = variant == 3 ? 1 : 0;
     return ILE_OK;
 }
 

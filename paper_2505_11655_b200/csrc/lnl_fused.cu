@@ -67,10 +67,9 @@ __global__ void __launch_bounds__(256) sky_key_kernel(LnlParams P, int N, const 
 // rec[t][0..3]=Re F_k, [4..7]=Im F_k (F = F+ - iFx), [8..11]=u_k (stored-bin coordinate of grid
 // time 0 at detector k), [12]=x, [13]=B, [14]=valid, [15]=ln prior.
 // ytile[t/32][m][t%32] = (Re, Im) Y_m, zero for m >= M.
-__global__ void __launch_bounds__(128) lnl_prep_kernel(LnlParams P, int N, const double* __restrict__ z, const int* __restrict__ perm,
+__global__ void __launch_bounds__(128) lnl_prep_kernel(LnlParams P, int N, int Npad, const double* __restrict__ z, const int* __restrict__ perm,
                                                        double* __restrict__ rec, double2* __restrict__ ytile, double* __restrict__ ln_prior) {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
-    int Npad = (N + FT_TS - 1) / FT_TS * FT_TS;
     if (t >= Npad) return;
     double2* yt = ytile + (size_t)(t / FT_TS) * FT_YM * FT_TS + (t % FT_TS);
     double* r = rec + (size_t)t * FT_REC;
@@ -403,10 +402,11 @@ static int launch_fused_t(ile_ctx* ctx, const LnlParams& P, int N, const double*
 }
 
 int ile_launch_lnL_plain_z(ile_ctx* ctx, const LnlParams& P, int N, const double* z, double* lnL, double* ln_prior);
+int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL);
 
 int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* z, const int* perm, double* lnL, double* ln_prior) {
     if (P.K > 3 || 2 * P.M > ILE_QT_ROW) return ile_launch_lnL_plain_z(ctx, P, N, z, lnL, ln_prior);
-    const int tiles = (N + FT_TS - 1) / FT_TS;
+    const int tiles = (N + 63) / 64 * 2;                       // 32-sample sub-tiles, padded to whole 64-sample tiles
     const size_t rec_bytes = ((size_t)tiles * FT_TS * FT_REC * sizeof(double) + 255) / 256 * 256;
     const size_t y_bytes = ((size_t)tiles * FT_YM * FT_TS * sizeof(double2) + 255) / 256 * 256;
     const size_t key_bytes = ((size_t)N * 8 + 255) / 256 * 256, val_bytes = ((size_t)N * 4 + 255) / 256 * 256;
@@ -438,8 +438,9 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         if (rc) return rc;
         perm = (const int*)v0;
     }
-    lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, z, perm, rec, yt, ln_prior);
+    lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
     ILE_LAUNCH_CHECK(ctx);
+    if (!ctx->fused_gen1) return ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL);
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
     if (np == 5 && rem >= 1 && rem <= 4) return launch_fused_t<5, true>(ctx, P, N, rec, yt, perm, lnL);
     if (np == 1 && rem >= 1 && rem <= 4) return launch_fused_t<1, true>(ctx, P, N, rec, yt, perm, lnL);
