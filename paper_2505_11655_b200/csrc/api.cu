@@ -105,6 +105,7 @@ extern "C" int ile_create(ile_ctx** out, int device, void* cuda_stream) {
     ctx->D_min = 1.0;
     ctx->D_max = 2.0;
     ctx->sky_sort = 1;
+    ctx->fused_rb = 4;
     *out = ctx;
     return ILE_OK;
 }
@@ -138,7 +139,8 @@ extern "C" int ile_sync(ile_ctx* ctx) {
 }
 
 extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
-    if (!ctx || variant < 0 || variant > 3) return ile_fail(ctx, ILE_EINVAL, "variant must be 0..3");
+    if (!ctx || variant < 0 || variant > 4) return ile_fail(ctx, ILE_EINVAL, "variant must be 0..4");
+    ctx->fused_rb = variant == 4 ? 8 : 4;
     ctx->variant = variant == 1 ? 1 : 0;
     ctx->sky_sort = variant == 2 ? 0 : 1;
     ctx->fused_gen1 = variant == 3 ? 1 : 0;

@@ -440,7 +440,10 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
     }
     lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
     ILE_LAUNCH_CHECK(ctx);
-    if (!ctx->fused_gen1) return ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL);
+    if (!ctx->fused_gen1) {
+        rc = ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL);
+        if (rc != 1) return rc;                              // 1: shape not instantiated -> first generation
+    }
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
     if (np == 5 && rem >= 1 && rem <= 4) return launch_fused_t<5, true>(ctx, P, N, rec, yt, perm, lnL);
     if (np == 1 && rem >= 1 && rem <= 4) return launch_fused_t<1, true>(ctx, P, N, rec, yt, perm, lnL);

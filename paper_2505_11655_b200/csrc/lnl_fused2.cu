@@ -15,7 +15,6 @@
 #include "common.cuh"
 #include "likelihood_dev.cuh"
 
-#define F2_TS 64
 #define F2_THREADS 256
 #define F2_WARPS 8
 #define F2_RING 80        // S ring length in stored bins
@@ -26,15 +25,17 @@
 #define F2_REC 16
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
 
+// RB = row blocks of 8 samples per CTA: 8 (64 samples, one CTA per SM) or 4 (32 samples, two per SM)
+template <int K, int RB>
 struct Fused2Smem {
-    double S[3][F2_TS][F2_SROW];             // 135,168 B
-    double2 A[3][F2_NP][8][32];              //  73,728 B  [k][k-step pair][row block][lane]
-    double rec[F2_TS][F2_REC];               //   8,192 B
-    double w1[3][F2_TS];                     // interpolation fraction f
-    int n[3][F2_TS];
+    double S[K][8 * RB][F2_SROW];            // S_k[sample][ring bin]
+    double2 A[K][F2_NP][RB][32];             // coefficient fragments [k][k-step pair][row block][lane]
+    double rec[8 * RB][F2_REC];
+    double w1[K][8 * RB];                    // interpolation fraction f
+    int n[K][8 * RB];
     int base[4];
-    int part[F2_TS];
-    int done[F2_TS];
+    int part[8 * RB];
+    int done[8 * RB];
     int n_part, n_left;
 };
 
@@ -65,26 +66,31 @@ __device__ __forceinline__ double exp_small(double d) {
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
 }
 
-template <int NPAIR, bool SINGLE, bool TABLE>
-__global__ void __launch_bounds__(F2_THREADS, 1)
+
+template <int K, int RB, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+__global__ void __launch_bounds__(F2_THREADS, (RB == 4 ? 2 : 1))
 lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const double2* __restrict__ ytile, const int* __restrict__ perm,
                   double* __restrict__ lnL) {
+    constexpr int TS = 8 * RB;        // samples per CTA
+    constexpr int SPW = RB;           // sample rows per warp in the epilogue
+    constexpr int NPT = NPAIR + (SINGLE ? 1 : 0);
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    Fused2Smem& sm = *reinterpret_cast<Fused2Smem*>(smem_raw);
+    Fused2Smem<K, RB>& sm = *reinterpret_cast<Fused2Smem<K, RB>*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int tile = blockIdx.x;
-    const int K = P.K, stride = P.stride, N_t = P.N_t;
+    const int stride = STRIDE1 ? 1 : P.stride, N_t = P.N_t;
     const int c = lane & 3, rq = lane >> 2;
 
     // ---- stage the tile's records
     {
-        const double* src = rec + (size_t)tile * F2_TS * F2_REC;
-        for (int q = tid; q < F2_TS * F2_REC; q += F2_THREADS) (&sm.rec[0][0])[q] = src[q];
+        const double* src = rec + (size_t)tile * TS * F2_REC;
+        for (int q = tid; q < TS * F2_REC; q += F2_THREADS) (&sm.rec[0][0])[q] = src[q];
     }
     __syncthreads();
-    if (tid < F2_TS) {
+    if (tid < TS) {
         const bool valid = sm.rec[tid][14] != 0.0;
         sm.done[tid] = valid ? 0 : 1;
+#pragma unroll
         for (int k = 0; k < K; k++) {
             const double u = sm.rec[tid][8 + k];
             const double fl = floor(u);
@@ -92,89 +98,96 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
             sm.w1[k][tid] = u - fl;
         }
         if (!valid) {
-            const int t = tile * F2_TS + tid;
+            const int t = tile * TS + tid;
             if (t < N) lnL[perm ? perm[t] : t] = neg_inf();
         }
     }
     // ---- coefficient fragments: A[k][p][rb][lane] = x (Re, Im)(F_k Y_m), sample 8 rb + lane/4,
     //      mode m = 4 p + lane%4; the trailing half k-step (SINGLE) holds Re or Im of mode
     //      4 NPAIR + (lane%4)/2 in .x
-    {
-        const int NPT = NPAIR + (SINGLE ? 1 : 0);
-        for (int q = tid; q < K * NPT * 8 * 32; q += F2_THREADS) {
-            const int ln = q & 31, rb = (q >> 5) & 7, p = (q >> 8) % NPT, k = (q >> 8) / NPT;
-            const int s = 8 * rb + (ln >> 2), cc = ln & 3;
-            const double x = sm.rec[s][12], fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
-            const double2* yt = ytile + ((size_t)(2 * tile + (s >> 5)) * F2_YM) * 32 + (s & 31);
-            double2 a;
-            if (p < NPAIR) {
-                const double2 y = yt[(4 * p + cc) * 32];
-                a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
-            } else {
-                const double2 y = yt[(4 * NPAIR + (cc >> 1)) * 32];
-                a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
-            }
-            sm.A[k][p][rb][ln] = a;
+    for (int q = tid; q < K * NPT * RB * 32; q += F2_THREADS) {
+        const int ln = q & 31, rb = (q >> 5) & (RB - 1), pk = q / (32 * RB), p = pk % NPT, k = pk / NPT;
+        const int s = 8 * rb + (ln >> 2), cc = ln & 3;
+        const int t = tile * TS + s;
+        const double x = sm.rec[s][12], fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
+        const double2* yt = ytile + ((size_t)(t >> 5) * F2_YM) * 32 + (t & 31);
+        double2 a;
+        if (p < NPAIR) {
+            const double2 y = yt[(4 * p + cc) * 32];
+            a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
+        } else {
+            const double2 y = yt[(4 * NPAIR + (cc >> 1)) * 32];
+            a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
         }
+        sm.A[k][p][rb][ln] = a;
     }
 
     for (;;) {   // rounds: normally one; more only when the tile's delay spread exceeds F2_CAP
         __syncthreads();
         if (tid < 32) {
-            int base[3];
-            bool q0, q1;
-            const int dn0 = sm.done[lane], dn1 = sm.done[lane + 32];
+            constexpr int NS = TS / 32;       // samples per lane
+            int base[K];
+            int dn[NS];
+            bool qq[NS];
+#pragma unroll
+            for (int h = 0; h < NS; h++) dn[h] = sm.done[lane + 32 * h];
+#pragma unroll
             for (int k = 0; k < K; k++) {
-                int v = min(dn0 ? 0x7fffffff : sm.n[k][lane], dn1 ? 0x7fffffff : sm.n[k][lane + 32]);
+                int v = 0x7fffffff;
+#pragma unroll
+                for (int h = 0; h < NS; h++) v = min(v, dn[h] ? 0x7fffffff : sm.n[k][lane + 32 * h]);
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, o));
                 base[k] = v & ~1;
             }
-            q0 = !dn0;
-            q1 = !dn1;
-            for (int k = 0; k < K; k++) {
-                q0 = q0 && (sm.n[k][lane] - base[k] <= F2_CAP);
-                q1 = q1 && (sm.n[k][lane + 32] - base[k] <= F2_CAP);
+            unsigned any_q = 0, left = 0;
+            int first_left = -1;
+#pragma unroll
+            for (int h = 0; h < NS; h++) {
+                qq[h] = !dn[h];
+#pragma unroll
+                for (int k = 0; k < K; k++) qq[h] = qq[h] && (sm.n[k][lane + 32 * h] - base[k] <= F2_CAP);
+                any_q |= __ballot_sync(0xffffffffu, qq[h]);
+                const unsigned l = __ballot_sync(0xffffffffu, !dn[h]);
+                if (l && first_left < 0) first_left = 32 * h + __ffs(l) - 1;
+                left |= l;
             }
-            unsigned m0 = __ballot_sync(0xffffffffu, q0), m1 = __ballot_sync(0xffffffffu, q1);
-            const unsigned l0 = __ballot_sync(0xffffffffu, !dn0), l1 = __ballot_sync(0xffffffffu, !dn1);
-            if ((l0 | l1) != 0 && (m0 | m1) == 0) {   // pivot on the first unfinished sample: always progresses
-                const int piv = l0 ? __ffs(l0) - 1 : 32 + __ffs(l1) - 1;
-                for (int k = 0; k < K; k++) base[k] = sm.n[k][piv] & ~1;
-                q0 = !dn0;
-                q1 = !dn1;
-                for (int k = 0; k < K; k++) {
-                    q0 = q0 && (sm.n[k][lane] >= base[k]) && (sm.n[k][lane] - base[k] <= F2_CAP);
-                    q1 = q1 && (sm.n[k][lane + 32] >= base[k]) && (sm.n[k][lane + 32] - base[k] <= F2_CAP);
+            if (left != 0 && any_q == 0) {   // pivot on the first unfinished sample: always progresses
+#pragma unroll
+                for (int k = 0; k < K; k++) base[k] = sm.n[k][first_left] & ~1;
+#pragma unroll
+                for (int h = 0; h < NS; h++) {
+                    qq[h] = !dn[h];
+#pragma unroll
+                    for (int k = 0; k < K; k++)
+                        qq[h] = qq[h] && (sm.n[k][lane + 32 * h] >= base[k]) && (sm.n[k][lane + 32 * h] - base[k] <= F2_CAP);
                 }
-                m0 = __ballot_sync(0xffffffffu, q0);
-                m1 = __ballot_sync(0xffffffffu, q1);
             }
-            sm.part[lane] = q0 ? 1 : 0;
-            sm.part[lane + 32] = q1 ? 1 : 0;
+#pragma unroll
+            for (int h = 0; h < NS; h++) sm.part[lane + 32 * h] = qq[h] ? 1 : 0;
             if (lane == 0) {
+#pragma unroll
                 for (int k = 0; k < K; k++) sm.base[k] = base[k];
-                sm.n_part = __popc(m0) + __popc(m1);
-                sm.n_left = __popc(l0) + __popc(l1);
+                sm.n_left = left ? 1 : 0;
             }
         }
         __syncthreads();
         if (sm.n_left == 0) break;
 
-        // per-sample epilogue state of this warp's 8 rows: reference m (warp-uniform), lane-partial sum
-        double run_m[8], run_s[8];
+        // per-sample epilogue state of this warp's rows: reference m (warp-uniform), lane-partial sum
+        double run_m[SPW], run_s[SPW];
 #pragma unroll
-        for (int q = 0; q < 8; q++) { run_m[q] = -1.0e300; run_s[q] = 0.0; }
+        for (int q = 0; q < SPW; q++) { run_m[q] = -1.0e300; run_s[q] = 0.0; }
 
         const int last_bin = stride * (N_t - 1) + 1 + F2_CAP;   // highest stored bin (relative to base) any sample reads
         int c_lo = 0, j0 = 0;
         int ntiles = min(F2_RING / 8, (last_bin + 1 - c_lo + 7) / 8);
-        for (int phase = 0;; phase++) {
+        for (;;) {
             const int c_hi = c_lo + ntiles * 8;
             int j1 = (c_hi - 1 - F2_CAP - 1) / stride + 1;      // outputs whose reads are all below c_hi
             if (j1 > N_t) j1 = N_t;
 
-            // ---------------- contraction: unit = (k, 8 bins) x 64 samples, 8 DMMA chains per warp
+            // ---------------- contraction: unit = (k, 8 bins) x TS samples, RB DMMA chains per warp
             {
                 const int nunits = K * ntiles;
                 double2 bn[NPAIR];
@@ -197,13 +210,13 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                     for (int p = 0; p < NPAIR; p++) b[p] = bn[p];
                     const double bsc = bs;
                     if (u + F2_WARPS < nunits) load_b(u + F2_WARPS);
-                    double d[8][2];
+                    double d[RB][2];
 #pragma unroll
-                    for (int rb = 0; rb < 8; rb++) d[rb][0] = d[rb][1] = 0.0;
+                    for (int rb = 0; rb < RB; rb++) d[rb][0] = d[rb][1] = 0.0;
 #pragma unroll
                     for (int p = 0; p < NPAIR; p++) {
 #pragma unroll
-                        for (int rb = 0; rb < 8; rb++) {
+                        for (int rb = 0; rb < RB; rb++) {
                             const double2 a = sm.A[k][p][rb][lane];
                             dmma2(d[rb][0], d[rb][1], a.x, b[p].x);
                             dmma2(d[rb][0], d[rb][1], a.y, b[p].y);
@@ -211,55 +224,70 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                     }
                     if (SINGLE) {
 #pragma unroll
-                        for (int rb = 0; rb < 8; rb++) {
-                            const double a = sm.A[k][NPAIR][rb][lane].x;
-                            dmma2(d[rb][0], d[rb][1], a, bsc);
-                        }
+                        for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], sm.A[k][NPAIR][rb][lane].x, bsc);
                     }
                     const int col = (c_lo + 8 * t) % F2_RING + 2 * c;
 #pragma unroll
-                    for (int rb = 0; rb < 8; rb++)
+                    for (int rb = 0; rb < RB; rb++)
                         *reinterpret_cast<double2*>(&sm.S[k][8 * rb + rq][col]) = make_double2(d[rb][0], d[rb][1]);
                 }
             }
             __syncthreads();   // S complete for bins < c_hi
 
-            // ---------------- epilogue: shift + interpolate + sum detectors + streaming log-sum-exp
+            // ---------------- epilogue: shift + interpolate + sum detectors + streaming log-sum-exp.
+            // Four sample rows in flight per warp (independent dependency chains); rows that do not
+            // take part in this round are computed on clamped offsets and discarded.
 #pragma unroll
-            for (int q = 0; q < 8; q++) {
-                const int s = 8 * w + q;
-                if (!sm.part[s]) continue;
-                const double Bq = sm.rec[s][13], x = sm.rec[s][12];
-                const double cB = TABLE ? 0.0 : x * x * Bq;
-                double f1[3], f0[3];
-                int off[3];
-                for (int k = 0; k < K; k++) {
-                    f1[k] = sm.w1[k][s];
-                    f0[k] = 1.0 - f1[k];
-                    off[k] = sm.n[k][s] - sm.base[k];
+            for (int g0 = 0; g0 < SPW; g0 += 4) {
+                double f1[4][K], f0[4][K], cB[4], Bq[4];
+                int c0[4][K];
+                const double* Srow[4];
+#pragma unroll
+                for (int i = 0; i < 4; i++) {
+                    const int s = SPW * w + g0 + i;
+                    const double x = sm.rec[s][12];
+                    Bq[i] = sm.rec[s][13];
+                    cB[i] = TABLE ? 0.0 : x * x * Bq[i];
+                    Srow[i] = &sm.S[0][s][0];
+#pragma unroll
+                    for (int k = 0; k < K; k++) {
+                        f1[i][k] = sm.w1[k][s];
+                        f0[i][k] = 1.0 - f1[i][k];
+                        const int off = min(max(sm.n[k][s] - sm.base[k], 0), F2_CAP);
+                        c0[i][k] = (off + stride * j0) % F2_RING;
+                    }
                 }
                 for (int jb = j0; jb < j1; jb += 32) {
-                    const int jj = jb + lane;
-                    double v = neg_inf();
-                    if (jj < j1) {
-                        double A = -cB;
+                    const int jl = jb - j0 + lane;
+                    const bool act = jb + lane < j1;
+                    double v[4];
+#pragma unroll
+                    for (int i = 0; i < 4; i++) {
+                        double A = -cB[i];
+#pragma unroll
                         for (int k = 0; k < K; k++) {
-                            const int b0 = off[k] + stride * jj;
-                            const int r0 = b0 % F2_RING;
+                            int r0 = c0[i][k] + stride * jl;
+                            if (STRIDE1) { if (r0 >= F2_RING) r0 -= F2_RING; }
+                            else r0 %= F2_RING;
                             const int r1 = (r0 + 1 == F2_RING) ? 0 : r0 + 1;
-                            A = fma(f0[k], sm.S[k][s][r0], A);
-                            A = fma(f1[k], sm.S[k][s][r1], A);
+                            const double* row = Srow[i] + k * (TS * F2_SROW);
+                            A = fma(f0[i][k], row[r0], A);
+                            A = fma(f1[i][k], row[r1], A);
                         }
-                        v = TABLE ? table_lookup(P, A, Bq) : A;
+                        if (TABLE) A = table_lookup(P, A, Bq[i]);
+                        v[i] = act ? A : neg_inf();
                     }
-                    double dl = v - run_m[q];
-                    if (__any_sync(0xffffffffu, dl > 30.0)) {      // raise the reference (rare)
-                        const double mx = warp_max(v);
-                        run_s[q] *= exp(run_m[q] - mx);
-                        run_m[q] = mx;
-                        dl = v - mx;
+#pragma unroll
+                    for (int i = 0; i < 4; i++) {
+                        double dl = v[i] - run_m[g0 + i];
+                        if (__any_sync(0xffffffffu, dl > 30.0)) {      // raise the reference (rare)
+                            const double mx = warp_max(v[i]);
+                            run_s[g0 + i] *= exp(run_m[g0 + i] - mx);
+                            run_m[g0 + i] = mx;
+                            dl = v[i] - mx;
+                        }
+                        if (dl > -40.0) run_s[g0 + i] += exp_small(dl);
                     }
-                    if (dl > -40.0) run_s[q] += exp_small(dl);
                 }
             }
             if (j1 >= N_t) break;
@@ -270,12 +298,11 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
         }
         // ---------------- finalise this round's samples
 #pragma unroll
-        for (int q = 0; q < 8; q++) {
-            const int s = 8 * w + q;
-            if (!sm.part[s]) continue;
+        for (int q = 0; q < SPW; q++) {
+            const int s = SPW * w + q;
             const double tot = warp_sum(run_s[q]);
-            if (lane == 0) {
-                const int t = tile * F2_TS + s;
+            if (lane == 0 && sm.part[s]) {
+                const int t = tile * TS + s;
                 if (t < N) lnL[perm ? perm[t] : t] = run_m[q] + log(tot) - log((double)N_t);
                 sm.done[s] = 1;
             }
@@ -283,29 +310,39 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
     }
 }
 
-template <int NPAIR, bool SINGLE, bool TABLE>
+template <int K, int RB, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
 static int launch_fused2_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
     static bool configured = false;
-    const int smem = (int)sizeof(Fused2Smem);
+    const int smem = (int)sizeof(Fused2Smem<K, RB>);
     if (!configured) {
-        ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused2_kernel<NPAIR, SINGLE, TABLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused2_kernel<K, RB, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         configured = true;
     }
-    const int tiles = (N + F2_TS - 1) / F2_TS;
+    const int tiles = (N + 8 * RB - 1) / (8 * RB);
     const int slot = ile_timing_begin(ctx);
-    lnl_fused2_kernel<NPAIR, SINGLE, TABLE><<<tiles, F2_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL);
+    lnl_fused2_kernel<K, RB, NPAIR, SINGLE, TABLE, STRIDE1><<<tiles, F2_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL);
     ile_timing_end(ctx, slot);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }
 
-// rec / yt as written by lnl_prep_kernel for ceil(N/64)*64 padded samples
+template <int K, int RB, int NPAIR, bool SINGLE>
+static int launch_fused2_k(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
+    const bool tb = P.use_table != 0, s1 = P.stride == 1;
+    if (tb) return s1 ? launch_fused2_t<K, RB, NPAIR, SINGLE, true, true>(ctx, P, N, rec, yt, perm, lnL)
+                      : launch_fused2_t<K, RB, NPAIR, SINGLE, true, false>(ctx, P, N, rec, yt, perm, lnL);
+    return s1 ? launch_fused2_t<K, RB, NPAIR, SINGLE, false, true>(ctx, P, N, rec, yt, perm, lnL)
+              : launch_fused2_t<K, RB, NPAIR, SINGLE, false, false>(ctx, P, N, rec, yt, perm, lnL);
+}
+
+// rec / yt as written by lnl_prep_kernel for ceil(N/64)*64 padded samples.  Returns 1 when the
+// shape has no instantiation (the caller falls back to the first-generation kernel).
 int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
-    const bool tb = P.use_table != 0;
-    if (np == 5 && rem >= 1 && rem <= 4)
-        return tb ? launch_fused2_t<5, true, true>(ctx, P, N, rec, yt, perm, lnL) : launch_fused2_t<5, true, false>(ctx, P, N, rec, yt, perm, lnL);
-    if (np == 1 && rem >= 1 && rem <= 4)
-        return tb ? launch_fused2_t<1, true, true>(ctx, P, N, rec, yt, perm, lnL) : launch_fused2_t<1, true, false>(ctx, P, N, rec, yt, perm, lnL);
-    return tb ? launch_fused2_t<6, false, true>(ctx, P, N, rec, yt, perm, lnL) : launch_fused2_t<6, false, false>(ctx, P, N, rec, yt, perm, lnL);
+    const int rb = ctx->fused_rb == 8 ? 8 : 4;
+    if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4)
+        return rb == 4 ? launch_fused2_k<3, 4, 5, true>(ctx, P, N, rec, yt, perm, lnL) : launch_fused2_k<3, 8, 5, true>(ctx, P, N, rec, yt, perm, lnL);
+    if (P.K == 2 && np == 1 && rem >= 1 && rem <= 4)
+        return rb == 4 ? launch_fused2_k<2, 4, 1, true>(ctx, P, N, rec, yt, perm, lnL) : launch_fused2_k<2, 8, 1, true>(ctx, P, N, rec, yt, perm, lnL);
+    return 1;
 }
