@@ -23,6 +23,9 @@
 #define F2_CAP 15         // largest per-sample offset above the tile base handled in one round
 #define F2_YM 24          // mode slots in the prep kernel's Y tile (32-sample sub-tiles)
 #define F2_REC 16
+#ifndef F2_G
+#define F2_G 4
+#endif
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
 
 // RB = row blocks of 8 samples per CTA: 8 (64 samples, one CTA per SM) or 4 (32 samples, two per SM)
@@ -37,13 +40,16 @@ struct Fused2Smem {
     int part[8 * RB];
     int done[8 * RB];
     int n_part, n_left;
+    double2 ew[8 * RB][K];                   // epilogue constants per sample: (1 - f_k, f_k)
+    double2 ec[8 * RB];                      // (x^2 B, B)
+    int eoff[8 * RB][4];                     // n_k - base_k, clamped to [0, F2_CAP]
 };
 
 __device__ __forceinline__ void dmma2(double& d0, double& d1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-// exp(d) for d in (-40, 31]: k = rint(d log2 e) by the magic-number add, r = d - k ln2,
+// exp(d) for d in (-690, 31]: k = rint(d log2 e) by the magic-number add, r = d - k ln2,
 // degree-10 Taylor polynomial (|r| <= 0.3466: truncation < 2.3e-13 relative), scaled by 2^k through
 // the exponent field.  13 FP64 instructions; the tolerance budget is DESIGN.md section 6.
 __device__ __forceinline__ double exp_small(double d) {
@@ -74,6 +80,7 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
     constexpr int TS = 8 * RB;        // samples per CTA
     constexpr int SPW = RB;           // sample rows per warp in the epilogue
     constexpr int NPT = NPAIR + (SINGLE ? 1 : 0);
+    constexpr int G = F2_G < SPW ? F2_G : SPW;   // sample rows in flight per warp in the epilogue
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Fused2Smem<K, RB>& sm = *reinterpret_cast<Fused2Smem<K, RB>*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -168,12 +175,30 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
             if (lane == 0) {
 #pragma unroll
                 for (int k = 0; k < K; k++) sm.base[k] = base[k];
-                sm.n_left = left ? 1 : 0;
+                sm.n_left = __popc(left);
             }
+            unsigned np_ = 0;
+#pragma unroll
+            for (int h = 0; h < NS; h++) np_ += __popc(__ballot_sync(0xffffffffu, qq[h]));
+            if (lane == 0) sm.n_part = (int)np_;
         }
         __syncthreads();
         if (sm.n_left == 0) break;
+        const bool last_round = sm.n_part == sm.n_left;   // every unfinished sample takes part: no re-check needed
 
+        // epilogue constants of this warp's own rows (written and read by the same warp)
+        if (lane < SPW) {
+            const int s = SPW * w + lane;
+            const double x = sm.rec[s][12], Bs = sm.rec[s][13];
+            sm.ec[s] = make_double2(TABLE ? 0.0 : x * x * Bs, Bs);
+#pragma unroll
+            for (int k = 0; k < K; k++) {
+                const double f = sm.w1[k][s];
+                sm.ew[s][k] = make_double2(1.0 - f, f);
+                sm.eoff[s][k] = min(max(sm.n[k][s] - sm.base[k], 0), F2_CAP);
+            }
+        }
+        __syncwarp();
         // per-sample epilogue state of this warp's rows: reference m (warp-uniform), lane-partial sum
         double run_m[SPW], run_s[SPW];
 #pragma unroll
@@ -187,106 +212,156 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
             int j1 = (c_hi - 1 - F2_CAP - 1) / stride + 1;      // outputs whose reads are all below c_hi
             if (j1 > N_t) j1 = N_t;
 
-            // ---------------- contraction: unit = (k, 8 bins) x TS samples, RB DMMA chains per warp
+            // ---------------- contraction: unit = (k, 8 bins) x TS samples, RB DMMA chains per warp.
+            // Q fragments of the next unit are loaded into the other register set while this one
+            // is multiplied (two units per trip: no register copies).
             {
                 const int nunits = K * ntiles;
-                double2 bn[NPAIR];
-                double bs = 0.0;
-                auto load_b = [&](int u) {
-                    const int k = u / ntiles, t = u - k * ntiles;
+                auto unit_kt = [&](int u, int& k, int& t) {
+                    k = (u >= ntiles ? 1 : 0) + (u >= 2 * ntiles ? 1 : 0);
+                    t = u - k * ntiles;
+                };
+                auto load_b = [&](int u, double2 (&b)[NPAIR], double& bs) {
+                    int k, t;
+                    unit_kt(u, k, t);
                     const int row = sm.base[k] + c_lo + 8 * t + rq;
                     const int swz = (row & 1) << 3;
                     const double* qrow = P.Qt + ((size_t)k * P.N_Qpad + row) * ILE_QT_ROW;
 #pragma unroll
-                    for (int p = 0; p < NPAIR; p++) bn[p] = __ldg(reinterpret_cast<const double2*>(qrow + ((8 * p + 2 * c) ^ swz)));
+                    for (int p = 0; p < NPAIR; p++) b[p] = __ldg(reinterpret_cast<const double2*>(qrow + ((8 * p + 2 * c) ^ swz)));
                     if (SINGLE) bs = __ldg(qrow + ((8 * NPAIR + c) ^ swz));
                 };
-                int u = w;
-                if (u < nunits) load_b(u);
-                for (; u < nunits; u += F2_WARPS) {
-                    const int k = u / ntiles, t = u - k * ntiles;
-                    double2 b[NPAIR];
+                auto compute = [&](int u, const double2 (&b)[NPAIR], const double bs) {
+                    int k, t;
+                    unit_kt(u, k, t);
+                    // two accumulators per row block (the .x and .y halves of each k-step pair):
+                    // 2 RB independent DMMA chains per warp
+                    double d[RB][2], e[RB][2];
 #pragma unroll
-                    for (int p = 0; p < NPAIR; p++) b[p] = bn[p];
-                    const double bsc = bs;
-                    if (u + F2_WARPS < nunits) load_b(u + F2_WARPS);
-                    double d[RB][2];
-#pragma unroll
-                    for (int rb = 0; rb < RB; rb++) d[rb][0] = d[rb][1] = 0.0;
+                    for (int rb = 0; rb < RB; rb++) d[rb][0] = d[rb][1] = e[rb][0] = e[rb][1] = 0.0;
+                    const double2* Ak = &sm.A[k][0][0][lane];
 #pragma unroll
                     for (int p = 0; p < NPAIR; p++) {
+                        double2 a[RB];
 #pragma unroll
-                        for (int rb = 0; rb < RB; rb++) {
-                            const double2 a = sm.A[k][p][rb][lane];
-                            dmma2(d[rb][0], d[rb][1], a.x, b[p].x);
-                            dmma2(d[rb][0], d[rb][1], a.y, b[p].y);
-                        }
+                        for (int rb = 0; rb < RB; rb++) a[rb] = Ak[(p * RB + rb) * 32];
+#pragma unroll
+                        for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], a[rb].x, b[p].x);
+#pragma unroll
+                        for (int rb = 0; rb < RB; rb++) dmma2(e[rb][0], e[rb][1], a[rb].y, b[p].y);
                     }
                     if (SINGLE) {
 #pragma unroll
-                        for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], sm.A[k][NPAIR][rb][lane].x, bsc);
+                        for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs);
                     }
-                    const int col = (c_lo + 8 * t) % F2_RING + 2 * c;
 #pragma unroll
-                    for (int rb = 0; rb < RB; rb++)
-                        *reinterpret_cast<double2*>(&sm.S[k][8 * rb + rq][col]) = make_double2(d[rb][0], d[rb][1]);
+                    for (int rb = 0; rb < RB; rb++) { d[rb][0] += e[rb][0]; d[rb][1] += e[rb][1]; }
+                    int cr = c_lo + 8 * t;
+                    cr -= (cr / F2_RING) * F2_RING;
+                    double* srow = &sm.S[k][rq][cr + 2 * c];
+#pragma unroll
+                    for (int rb = 0; rb < RB; rb++) *reinterpret_cast<double2*>(srow + rb * 8 * F2_SROW) = make_double2(d[rb][0], d[rb][1]);
+                    if (cr == 0 && c == 0) {      // ring column F2_RING mirrors column 0: the epilogue reads [r], [r+1] unwrapped
+#pragma unroll
+                        for (int rb = 0; rb < RB; rb++) srow[rb * 8 * F2_SROW + F2_RING] = d[rb][0];
+                    }
+                };
+                double2 b0[NPAIR], b1[NPAIR];
+                double s0 = 0.0, s1 = 0.0;
+#ifdef F2_DBG_NOMMA
+                int u = nunits;
+#else
+                int u = w;
+#endif
+                if (u < nunits) load_b(u, b0, s0);
+                while (u < nunits) {
+                    if (u + F2_WARPS < nunits) load_b(u + F2_WARPS, b1, s1);
+                    compute(u, b0, s0);
+                    u += F2_WARPS;
+                    if (u >= nunits) break;
+                    if (u + F2_WARPS < nunits) load_b(u + F2_WARPS, b0, s0);
+                    compute(u, b1, s1);
+                    u += F2_WARPS;
                 }
             }
             __syncthreads();   // S complete for bins < c_hi
 
             // ---------------- epilogue: shift + interpolate + sum detectors + streaming log-sum-exp.
-            // Four sample rows in flight per warp (independent dependency chains); rows that do not
+            // G sample rows in flight per warp (independent dependency chains); rows that do not
             // take part in this round are computed on clamped offsets and discarded.
+            {
+                int j0m = stride * j0;
+                j0m -= (j0m / F2_RING) * F2_RING;
 #pragma unroll
-            for (int g0 = 0; g0 < SPW; g0 += 4) {
-                double f1[4][K], f0[4][K], cB[4], Bq[4];
-                int c0[4][K];
-                const double* Srow[4];
+                for (int g0 = 0; g0 < SPW; g0 += G) {
+                    double2 wk[G][K], cb[G];
+                    int r[G][K];                   // ring column of this lane's first tap
+                    const double* Srow[G];
 #pragma unroll
-                for (int i = 0; i < 4; i++) {
-                    const int s = SPW * w + g0 + i;
-                    const double x = sm.rec[s][12];
-                    Bq[i] = sm.rec[s][13];
-                    cB[i] = TABLE ? 0.0 : x * x * Bq[i];
-                    Srow[i] = &sm.S[0][s][0];
-#pragma unroll
-                    for (int k = 0; k < K; k++) {
-                        f1[i][k] = sm.w1[k][s];
-                        f0[i][k] = 1.0 - f1[i][k];
-                        const int off = min(max(sm.n[k][s] - sm.base[k], 0), F2_CAP);
-                        c0[i][k] = (off + stride * j0) % F2_RING;
-                    }
-                }
-                for (int jb = j0; jb < j1; jb += 32) {
-                    const int jl = jb - j0 + lane;
-                    const bool act = jb + lane < j1;
-                    double v[4];
-#pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        double A = -cB[i];
+                    for (int i = 0; i < G; i++) {
+                        const int s = SPW * w + g0 + i;
+                        cb[i] = sm.ec[s];
+                        Srow[i] = &sm.S[0][s][0];
+                        const int4 o4 = *reinterpret_cast<const int4*>(&sm.eoff[s][0]);
+                        const int off[4] = {o4.x, o4.y, o4.z, o4.w};
 #pragma unroll
                         for (int k = 0; k < K; k++) {
-                            int r0 = c0[i][k] + stride * jl;
-                            if (STRIDE1) { if (r0 >= F2_RING) r0 -= F2_RING; }
-                            else r0 %= F2_RING;
-                            const int r1 = (r0 + 1 == F2_RING) ? 0 : r0 + 1;
-                            const double* row = Srow[i] + k * (TS * F2_SROW);
-                            A = fma(f0[i][k], row[r0], A);
-                            A = fma(f1[i][k], row[r1], A);
+                            wk[i][k] = sm.ew[s][k];
+                            int rr = off[k] + j0m;
+                            if (rr >= F2_RING) rr -= F2_RING;
+                            if (STRIDE1) {
+                                rr += lane;
+                                if (rr >= F2_RING) rr -= F2_RING;
+                            }
+                            r[i][k] = rr;
                         }
-                        if (TABLE) A = table_lookup(P, A, Bq[i]);
-                        v[i] = act ? A : neg_inf();
                     }
+#ifdef F2_DBG_NOEPI
+                    for (int jb = j0; jb < j0; jb += 32) {
+#else
+                    for (int jb = j0; jb < j1; jb += 32) {
+#endif
+                        const bool act = jb + lane < j1;
+                        double v[G];
 #pragma unroll
-                    for (int i = 0; i < 4; i++) {
-                        double dl = v[i] - run_m[g0 + i];
-                        if (__any_sync(0xffffffffu, dl > 30.0)) {      // raise the reference (rare)
-                            const double mx = warp_max(v[i]);
-                            run_s[g0 + i] *= exp(run_m[g0 + i] - mx);
-                            run_m[g0 + i] = mx;
-                            dl = v[i] - mx;
+                        for (int i = 0; i < G; i++) {
+                            double A = -cb[i].x;
+#pragma unroll
+                            for (int k = 0; k < K; k++) {
+                                int r0;
+                                if (STRIDE1) {
+                                    r0 = r[i][k];
+                                    const int nx = r0 + 32;
+                                    r[i][k] = nx >= F2_RING ? nx - F2_RING : nx;
+                                } else {
+                                    r0 = (r[i][k] + stride * (jb - j0 + lane)) % F2_RING;
+                                }
+                                const double* row = Srow[i] + k * (TS * F2_SROW) + r0;
+                                A = fma(wk[i][k].x, row[0], A);
+                                A = fma(wk[i][k].y, row[1], A);
+                            }
+                            if (TABLE) A = table_lookup(P, A, cb[i].y);
+                            v[i] = act ? A : neg_inf();
                         }
-                        if (dl > -40.0) run_s[g0 + i] += exp_small(dl);
+#pragma unroll
+                        for (int i = 0; i < G; i++) {
+                            double dl = v[i] - run_m[g0 + i];
+                            if (__any_sync(0xffffffffu, dl > 30.0)) {      // raise the reference (rare)
+                                // new reference >= max_lane v, found on the ordered high words with
+                                // one REDUX; it need not be the exact maximum
+                                const int h = __double2hiint(v[i]);
+                                const int key = __reduce_max_sync(0xffffffffu, h ^ ((h >> 31) & 0x7fffffff));
+                                const int hm = key ^ ((key >> 31) & 0x7fffffff);
+                                const double mx = __hiloint2double(hm, hm < 0 ? 0 : -1);
+                                const double dm = run_m[g0 + i] - mx;
+                                // the running sum may hold terms up to e^30 above its reference: rescale it
+                                // exactly (exp_small is valid down to the underflow of 2^k)
+                                run_s[g0 + i] = dm > -690.0 ? run_s[g0 + i] * exp_small(dm) : 0.0;
+                                run_m[g0 + i] = mx;
+                                dl = v[i] - mx;
+                            }
+                            if (dl > -40.0) run_s[g0 + i] += exp_small(dl);
+                        }
                     }
                 }
             }
@@ -307,6 +382,7 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                 sm.done[s] = 1;
             }
         }
+        if (last_round) break;
     }
 }
 
