@@ -1,15 +1,16 @@
-// libile: fused lnL kernel, second generation.  Design notes in DESIGN.md
-// section 6; the measurements behind it (profiles/r1_pipes.md): on sm_100a a dependent DMMA.8x8x4
-// issues every ~150 cycles while the pipe accepts one every 16, and DFMA shares that FP64 datapath.
-// Hence: >= 8 independent accumulator chains per warp in the contraction, and an epilogue with as
-// few FP64 instructions per (sample, time bin) as the arithmetic allows.
+// libile: fused lnL kernel.  Design notes in DESIGN.md section 6; the
+// measurements behind it are in profiles/r1_pipes.md: on sm_100a a dependent DMMA.8x8x4 issues
+// every ~150 cycles while the pipe accepts one every 16, and DFMA shares that FP64 datapath.
+// Hence: 8 independent accumulator chains per warp in the contraction, and an epilogue that is
+// branch-free straight-line code over 8 independent (sample, 32-bin) groups with as few FP64
+// instructions per (sample, time bin) as the arithmetic allows.
 //
-//   one CTA = 64 samples (delay-cell sorted), 8 warps, one CTA per SM
+//   one CTA = 32 samples (delay-cell sorted), 8 warps, two CTAs per SM
 //   contraction   S_k[s][n] = sum_r coef_k[s][r] Q_k[r][n]  (coef = x Re/Im(F_k Y_m), K-dim 2M):
-//                 unit = (detector k, 8 stored bins) x all 64 samples = 8 independent DMMA chains;
-//                 A fragments (coef) from shared memory in fragment order, B fragments (Q) straight
-//                 from global/L2 into registers, prefetched one unit ahead; D -> S ring in smem
-//   epilogue      one warp per sample row, lanes along time: per-sample delay shift + linear
+//                 unit = (detector k, 8 stored bins) x 32 samples; A fragments (coef) from shared
+//                 memory in fragment order, B fragments (Q) straight from global/L2 into registers,
+//                 loaded one unit ahead; D -> S ring in shared memory
+//   epilogue      one warp per 4 sample rows, lanes along time: per-sample delay shift + linear
 //                 interpolation (2 FMA per detector), ln L(t_j) = A_j - x^2 B, streaming log-sum-exp
 //                 with a lazily raised reference and a 13-instruction exp
 #include "common.cuh"
@@ -17,32 +18,32 @@
 
 #define F2_THREADS 256
 #define F2_WARPS 8
-#define F2_RING 80        // S ring length in stored bins
+#define F2_TS 32          // samples per CTA
+#define F2_RB 4           // row blocks of 8 samples
+#define F2_SPW 4          // sample rows per warp in the epilogue
+#define F2_RING 80        // S ring length in stored bins (+ column F2_RING mirroring column 0)
 #define F2_SROW 88        // S row stride (== 8 mod 16: conflict-free 128-bit fragment stores)
 #define F2_NEW 64         // new stored bins per phase (phase 0: F2_RING)
 #define F2_CAP 15         // largest per-sample offset above the tile base handled in one round
 #define F2_YM 24          // mode slots in the prep kernel's Y tile (32-sample sub-tiles)
 #define F2_REC 16
-#ifndef F2_G
-#define F2_G 4
-#endif
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
+#define F2_NG 2           // 32-bin groups per phase (at most 64 outputs per phase)
 
-// RB = row blocks of 8 samples per CTA: 8 (64 samples, one CTA per SM) or 4 (32 samples, two per SM)
-template <int K, int RB>
+template <int K>
 struct Fused2Smem {
-    double S[K][8 * RB][F2_SROW];            // S_k[sample][ring bin]
-    double2 A[K][F2_NP][RB][32];             // coefficient fragments [k][k-step pair][row block][lane]
-    double rec[8 * RB][F2_REC];
-    double w1[K][8 * RB];                    // interpolation fraction f
-    int n[K][8 * RB];
+    double S[K][F2_TS][F2_SROW];             // S_k[sample][ring bin]
+    double2 A[K][F2_NP][F2_RB][32];          // coefficient fragments [k][k-step pair][row block][lane]
+    double rec[F2_TS][F2_REC];
+    double w1[K][F2_TS];                     // interpolation fraction f
+    double2 ew[F2_TS][K];                    // epilogue constants per sample: (1 - f_k, f_k)
+    double2 ec[F2_TS];                       // (x^2 B, B)
+    int eoff[F2_TS][4];                      // n_k - base_k, clamped to [0, F2_CAP]
+    int n[K][F2_TS];
     int base[4];
-    int part[8 * RB];
-    int done[8 * RB];
+    int part[F2_TS];
+    int done[F2_TS];
     int n_part, n_left;
-    double2 ew[8 * RB][K];                   // epilogue constants per sample: (1 - f_k, f_k)
-    double2 ec[8 * RB];                      // (x^2 B, B)
-    int eoff[8 * RB][4];                     // n_k - base_k, clamped to [0, F2_CAP]
 };
 
 __device__ __forceinline__ void dmma2(double& d0, double& d1, double a, double b) {
@@ -72,37 +73,98 @@ __device__ __forceinline__ double exp_small(double d) {
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
 }
 
+#ifdef F2_TIMERS
+__device__ unsigned long long f2_timers[8];
+#define F2_T(i) do { const long long t__ = clock64(); if (lane == 0) atomicAdd(&f2_timers[i], (unsigned long long)(t__ - tmark)); tmark = t__; } while (0)
+#else
+#define F2_T(i)
+#endif
 
-template <int K, int RB, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
-__global__ void __launch_bounds__(F2_THREADS, (RB == 4 ? 2 : 1))
+// general round set-up (warp 0): tile base = even floor of the per-detector minimum first bin over
+// the unfinished samples; a sample takes part when all its offsets are within F2_CAP; when none
+// does, pivot on the first unfinished sample so that every round makes progress
+template <int K>
+__device__ __forceinline__ void round_setup(Fused2Smem<K>& sm, int lane) {
+    int base[K];
+    const int dn = sm.done[lane];
+#pragma unroll
+    for (int k = 0; k < K; k++) {
+        int v = dn ? 0x7fffffff : sm.n[k][lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, o));
+        base[k] = v & ~1;
+    }
+    bool q = !dn;
+#pragma unroll
+    for (int k = 0; k < K; k++) q = q && (sm.n[k][lane] - base[k] <= F2_CAP);
+    unsigned mq = __ballot_sync(0xffffffffu, q);
+    const unsigned left = __ballot_sync(0xffffffffu, !dn);
+    if (left != 0 && mq == 0) {
+        const int piv = __ffs(left) - 1;
+#pragma unroll
+        for (int k = 0; k < K; k++) base[k] = sm.n[k][piv] & ~1;
+        q = !dn;
+#pragma unroll
+        for (int k = 0; k < K; k++) q = q && (sm.n[k][lane] >= base[k]) && (sm.n[k][lane] - base[k] <= F2_CAP);
+        mq = __ballot_sync(0xffffffffu, q);
+    }
+    sm.part[lane] = q ? 1 : 0;
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < K; k++) sm.base[k] = base[k];
+        sm.n_part = __popc(mq);
+        sm.n_left = __popc(left);
+    }
+}
+
+// epilogue constants of sample s for the current tile base
+template <int K, bool TABLE>
+__device__ __forceinline__ void sample_consts(Fused2Smem<K>& sm, int s) {
+    const double x = sm.rec[s][12], Bs = sm.rec[s][13];
+    sm.ec[s] = make_double2(TABLE ? 0.0 : x * x * Bs, Bs);
+#pragma unroll
+    for (int k = 0; k < K; k++) {
+        const double f = sm.w1[k][s];
+        sm.ew[s][k] = make_double2(1.0 - f, f);
+        sm.eoff[s][k] = min(max(sm.n[k][s] - sm.base[k], 0), F2_CAP);
+    }
+}
+
+template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+__global__ void __launch_bounds__(F2_THREADS, 2)
 lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const double2* __restrict__ ytile, const int* __restrict__ perm,
                   double* __restrict__ lnL) {
-    constexpr int TS = 8 * RB;        // samples per CTA
-    constexpr int SPW = RB;           // sample rows per warp in the epilogue
+    constexpr int RB = F2_RB, TS = F2_TS, SPW = F2_SPW, NG = F2_NG;
     constexpr int NPT = NPAIR + (SINGLE ? 1 : 0);
-    constexpr int G = F2_G < SPW ? F2_G : SPW;   // sample rows in flight per warp in the epilogue
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    Fused2Smem<K, RB>& sm = *reinterpret_cast<Fused2Smem<K, RB>*>(smem_raw);
+    Fused2Smem<K>& sm = *reinterpret_cast<Fused2Smem<K>*>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int tile = blockIdx.x;
     const int stride = STRIDE1 ? 1 : P.stride, N_t = P.N_t;
     const int c = lane & 3, rq = lane >> 2;
+#ifdef F2_TIMERS
+    long long tmark = clock64();
+#endif
 
-    // ---- stage the tile's records
+    // ---- stage the tile's records; tile base by shared-memory atomicMin
     {
         const double* src = rec + (size_t)tile * TS * F2_REC;
         for (int q = tid; q < TS * F2_REC; q += F2_THREADS) (&sm.rec[0][0])[q] = src[q];
+        if (tid < 4) sm.base[tid] = 0x7ffffffe;
     }
     __syncthreads();
+    bool valid = false;
     if (tid < TS) {
-        const bool valid = sm.rec[tid][14] != 0.0;
+        valid = sm.rec[tid][14] != 0.0;
         sm.done[tid] = valid ? 0 : 1;
 #pragma unroll
         for (int k = 0; k < K; k++) {
             const double u = sm.rec[tid][8 + k];
             const double fl = floor(u);
-            sm.n[k][tid] = (int)fl;
+            const int nk = (int)fl;
+            sm.n[k][tid] = nk;
             sm.w1[k][tid] = u - fl;
+            if (valid) atomicMin(&sm.base[k], nk & ~1);
         }
         if (!valid) {
             const int t = tile * TS + tid;
@@ -111,94 +173,61 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
     }
     // ---- coefficient fragments: A[k][p][rb][lane] = x (Re, Im)(F_k Y_m), sample 8 rb + lane/4,
     //      mode m = 4 p + lane%4; the trailing half k-step (SINGLE) holds Re or Im of mode
-    //      4 NPAIR + (lane%4)/2 in .x
-    for (int q = tid; q < K * NPT * RB * 32; q += F2_THREADS) {
-        const int ln = q & 31, rb = (q >> 5) & (RB - 1), pk = q / (32 * RB), p = pk % NPT, k = pk / NPT;
-        const int s = 8 * rb + (ln >> 2), cc = ln & 3;
-        const int t = tile * TS + s;
-        const double x = sm.rec[s][12], fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
-        const double2* yt = ytile + ((size_t)(t >> 5) * F2_YM) * 32 + (t & 31);
-        double2 a;
-        if (p < NPAIR) {
-            const double2 y = yt[(4 * p + cc) * 32];
-            a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
-        } else {
-            const double2 y = yt[(4 * NPAIR + (cc >> 1)) * 32];
-            a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
+    //      4 NPAIR + (lane%4)/2 in .x.  Fully unrolled: all of a thread's Y loads are in flight at once.
+    {
+        constexpr int NA = K * NPT * RB * 32;
+        constexpr int IT = (NA + F2_THREADS - 1) / F2_THREADS;
+        double2 yv[IT];
+#pragma unroll
+        for (int it = 0; it < IT; it++) {
+            const int q = tid + it * F2_THREADS;
+            const int ln = q & 31, rb = (q >> 5) & (RB - 1), pk = q / (32 * RB), p = pk % NPT;
+            const int s = 8 * rb + (ln >> 2), cc = ln & 3;
+            const int t = tile * TS + s;
+            const int m = p < NPAIR ? 4 * p + cc : 4 * NPAIR + (cc >> 1);
+            yv[it] = make_double2(0.0, 0.0);
+            if (q < NA) yv[it] = ytile[((size_t)(t >> 5) * F2_YM + m) * 32 + (t & 31)];
         }
-        sm.A[k][p][rb][ln] = a;
+#pragma unroll
+        for (int it = 0; it < IT; it++) {
+            const int q = tid + it * F2_THREADS;
+            const int ln = q & 31, rb = (q >> 5) & (RB - 1), pk = q / (32 * RB), p = pk % NPT, k = pk / NPT;
+            const int s = 8 * rb + (ln >> 2), cc = ln & 3;
+            const double x = sm.rec[s][12], fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
+            const double2 y = yv[it];
+            double2 a;
+            if (p < NPAIR) a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
+            else a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
+            if (q < NA) sm.A[k][p][rb][ln] = a;
+        }
     }
+    const int n_valid = __syncthreads_count(valid);      // also publishes n, w1, base, A
+    if (n_valid == 0) return;
+    // ---- round 0: who fits within F2_CAP of the base (normally everybody)
+    bool part0 = false;
+    if (tid < TS) {
+        part0 = valid;
+#pragma unroll
+        for (int k = 0; k < K; k++) part0 = part0 && (sm.n[k][tid] - sm.base[k] <= F2_CAP);
+        sm.part[tid] = part0 ? 1 : 0;
+        sample_consts<K, TABLE>(sm, tid);
+    }
+    const int n_part0 = __syncthreads_count(part0);
+    bool last_round = n_part0 == n_valid;
+    bool need_setup = n_part0 == 0;                       // nobody fits: the general set-up pivots
+    F2_T(0);
 
-    for (;;) {   // rounds: normally one; more only when the tile's delay spread exceeds F2_CAP
-        __syncthreads();
-        if (tid < 32) {
-            constexpr int NS = TS / 32;       // samples per lane
-            int base[K];
-            int dn[NS];
-            bool qq[NS];
-#pragma unroll
-            for (int h = 0; h < NS; h++) dn[h] = sm.done[lane + 32 * h];
-#pragma unroll
-            for (int k = 0; k < K; k++) {
-                int v = 0x7fffffff;
-#pragma unroll
-                for (int h = 0; h < NS; h++) v = min(v, dn[h] ? 0x7fffffff : sm.n[k][lane + 32 * h]);
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, o));
-                base[k] = v & ~1;
-            }
-            unsigned any_q = 0, left = 0;
-            int first_left = -1;
-#pragma unroll
-            for (int h = 0; h < NS; h++) {
-                qq[h] = !dn[h];
-#pragma unroll
-                for (int k = 0; k < K; k++) qq[h] = qq[h] && (sm.n[k][lane + 32 * h] - base[k] <= F2_CAP);
-                any_q |= __ballot_sync(0xffffffffu, qq[h]);
-                const unsigned l = __ballot_sync(0xffffffffu, !dn[h]);
-                if (l && first_left < 0) first_left = 32 * h + __ffs(l) - 1;
-                left |= l;
-            }
-            if (left != 0 && any_q == 0) {   // pivot on the first unfinished sample: always progresses
-#pragma unroll
-                for (int k = 0; k < K; k++) base[k] = sm.n[k][first_left] & ~1;
-#pragma unroll
-                for (int h = 0; h < NS; h++) {
-                    qq[h] = !dn[h];
-#pragma unroll
-                    for (int k = 0; k < K; k++)
-                        qq[h] = qq[h] && (sm.n[k][lane + 32 * h] >= base[k]) && (sm.n[k][lane + 32 * h] - base[k] <= F2_CAP);
-                }
-            }
-#pragma unroll
-            for (int h = 0; h < NS; h++) sm.part[lane + 32 * h] = qq[h] ? 1 : 0;
-            if (lane == 0) {
-#pragma unroll
-                for (int k = 0; k < K; k++) sm.base[k] = base[k];
-                sm.n_left = __popc(left);
-            }
-            unsigned np_ = 0;
-#pragma unroll
-            for (int h = 0; h < NS; h++) np_ += __popc(__ballot_sync(0xffffffffu, qq[h]));
-            if (lane == 0) sm.n_part = (int)np_;
+    for (int round = 0;; round++) {   // rounds: normally one; more only when the tile's delay spread exceeds F2_CAP
+        if (round > 0 || need_setup) {
+            __syncthreads();
+            if (tid < 32) round_setup<K>(sm, lane);
+            __syncthreads();
+            if (sm.n_left == 0) break;
+            last_round = sm.n_part == sm.n_left;
+            if (tid < TS) sample_consts<K, TABLE>(sm, tid);
+            __syncthreads();
+            need_setup = false;
         }
-        __syncthreads();
-        if (sm.n_left == 0) break;
-        const bool last_round = sm.n_part == sm.n_left;   // every unfinished sample takes part: no re-check needed
-
-        // epilogue constants of this warp's own rows (written and read by the same warp)
-        if (lane < SPW) {
-            const int s = SPW * w + lane;
-            const double x = sm.rec[s][12], Bs = sm.rec[s][13];
-            sm.ec[s] = make_double2(TABLE ? 0.0 : x * x * Bs, Bs);
-#pragma unroll
-            for (int k = 0; k < K; k++) {
-                const double f = sm.w1[k][s];
-                sm.ew[s][k] = make_double2(1.0 - f, f);
-                sm.eoff[s][k] = min(max(sm.n[k][s] - sm.base[k], 0), F2_CAP);
-            }
-        }
-        __syncwarp();
         // per-sample epilogue state of this warp's rows: reference m (warp-uniform), lane-partial sum
         double run_m[SPW], run_s[SPW];
 #pragma unroll
@@ -211,10 +240,9 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
             const int c_hi = c_lo + ntiles * 8;
             int j1 = (c_hi - 1 - F2_CAP - 1) / stride + 1;      // outputs whose reads are all below c_hi
             if (j1 > N_t) j1 = N_t;
-
-            // ---------------- contraction: unit = (k, 8 bins) x TS samples, RB DMMA chains per warp.
-            // Q fragments of the next unit are loaded into the other register set while this one
-            // is multiplied (two units per trip: no register copies).
+            F2_T(1);
+            // ---------------- contraction: unit = (k, 8 bins) x 32 samples.  Q fragments of the next
+            // unit are loaded into the other register set while this one is multiplied.
             {
                 const int nunits = K * ntiles;
                 auto unit_kt = [&](int u, int& k, int& t) {
@@ -268,11 +296,7 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                 };
                 double2 b0[NPAIR], b1[NPAIR];
                 double s0 = 0.0, s1 = 0.0;
-#ifdef F2_DBG_NOMMA
-                int u = nunits;
-#else
                 int u = w;
-#endif
                 if (u < nunits) load_b(u, b0, s0);
                 while (u < nunits) {
                     if (u + F2_WARPS < nunits) load_b(u + F2_WARPS, b1, s1);
@@ -284,141 +308,162 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                     u += F2_WARPS;
                 }
             }
+            F2_T(2);
             __syncthreads();   // S complete for bins < c_hi
-
-            // ---------------- epilogue: shift + interpolate + sum detectors + streaming log-sum-exp.
-            // G sample rows in flight per warp (independent dependency chains); rows that do not
-            // take part in this round are computed on clamped offsets and discarded.
+            F2_T(3);
+            // ---------------- epilogue: shift + interpolate + sum detectors, then a streaming
+            // log-sum-exp.  Straight-line code over SPW x NG independent (sample row, 32-bin group)
+            // chains; rows that do not take part in this round run on clamped offsets and are discarded.
             {
                 int j0m = stride * j0;
                 j0m -= (j0m / F2_RING) * F2_RING;
+                double v[SPW][NG];
 #pragma unroll
-                for (int g0 = 0; g0 < SPW; g0 += G) {
-                    double2 wk[G][K], cb[G];
-                    int r[G][K];                   // ring column of this lane's first tap
-                    const double* Srow[G];
+                for (int i = 0; i < SPW; i++) {
+                    const int s = SPW * w + i;
+                    const double2 cb = sm.ec[s];
+                    const int4 o4 = *reinterpret_cast<const int4*>(&sm.eoff[s][0]);
+                    const int off[4] = {o4.x, o4.y, o4.z, o4.w};
+                    double2 wk[K];
+                    int r[K];
 #pragma unroll
-                    for (int i = 0; i < G; i++) {
-                        const int s = SPW * w + g0 + i;
-                        cb[i] = sm.ec[s];
-                        Srow[i] = &sm.S[0][s][0];
-                        const int4 o4 = *reinterpret_cast<const int4*>(&sm.eoff[s][0]);
-                        const int off[4] = {o4.x, o4.y, o4.z, o4.w};
+                    for (int k = 0; k < K; k++) {
+                        wk[k] = sm.ew[s][k];
+                        int rr = off[k] + j0m;
+                        if (rr >= F2_RING) rr -= F2_RING;
+                        if (STRIDE1) {
+                            rr += lane;
+                            if (rr >= F2_RING) rr -= F2_RING;
+                        }
+                        r[k] = rr;
+                    }
+                    const double* Srow = &sm.S[0][s][0];
+#pragma unroll
+                    for (int gi = 0; gi < NG; gi++) {
+                        const int jl = 32 * gi + lane;
+                        double A = -cb.x;
 #pragma unroll
                         for (int k = 0; k < K; k++) {
-                            wk[i][k] = sm.ew[s][k];
-                            int rr = off[k] + j0m;
-                            if (rr >= F2_RING) rr -= F2_RING;
+                            int r0;
                             if (STRIDE1) {
-                                rr += lane;
-                                if (rr >= F2_RING) rr -= F2_RING;
+                                r0 = r[k] + 32 * gi;
+                                if (r0 >= F2_RING) r0 -= F2_RING;
+                            } else {
+                                r0 = (r[k] + stride * jl) % F2_RING;
                             }
-                            r[i][k] = rr;
+                            const double* row = Srow + k * (TS * F2_SROW) + r0;
+                            A = fma(wk[k].x, row[0], A);
+                            A = fma(wk[k].y, row[1], A);
                         }
+                        if (TABLE) A = table_lookup(P, A, cb.y);
+                        v[i][gi] = (j0 + jl < j1) ? A : neg_inf();
                     }
-#ifdef F2_DBG_NOEPI
-                    for (int jb = j0; jb < j0; jb += 32) {
-#else
-                    for (int jb = j0; jb < j1; jb += 32) {
-#endif
-                        const bool act = jb + lane < j1;
-                        double v[G];
+                }
+                // raise the references where a new value is more than e^30 above (rare)
+                bool need = false;
 #pragma unroll
-                        for (int i = 0; i < G; i++) {
-                            double A = -cb[i].x;
+                for (int i = 0; i < SPW; i++)
 #pragma unroll
-                            for (int k = 0; k < K; k++) {
-                                int r0;
-                                if (STRIDE1) {
-                                    r0 = r[i][k];
-                                    const int nx = r0 + 32;
-                                    r[i][k] = nx >= F2_RING ? nx - F2_RING : nx;
-                                } else {
-                                    r0 = (r[i][k] + stride * (jb - j0 + lane)) % F2_RING;
-                                }
-                                const double* row = Srow[i] + k * (TS * F2_SROW) + r0;
-                                A = fma(wk[i][k].x, row[0], A);
-                                A = fma(wk[i][k].y, row[1], A);
-                            }
-                            if (TABLE) A = table_lookup(P, A, cb[i].y);
-                            v[i] = act ? A : neg_inf();
-                        }
+                    for (int gi = 0; gi < NG; gi++) need = need || (v[i][gi] - run_m[i] > 30.0);
+                if (__any_sync(0xffffffffu, need)) {
 #pragma unroll
-                        for (int i = 0; i < G; i++) {
-                            double dl = v[i] - run_m[g0 + i];
-                            if (__any_sync(0xffffffffu, dl > 30.0)) {      // raise the reference (rare)
-                                // new reference >= max_lane v, found on the ordered high words with
-                                // one REDUX; it need not be the exact maximum
-                                const int h = __double2hiint(v[i]);
-                                const int key = __reduce_max_sync(0xffffffffu, h ^ ((h >> 31) & 0x7fffffff));
-                                const int hm = key ^ ((key >> 31) & 0x7fffffff);
-                                const double mx = __hiloint2double(hm, hm < 0 ? 0 : -1);
-                                const double dm = run_m[g0 + i] - mx;
-                                // the running sum may hold terms up to e^30 above its reference: rescale it
-                                // exactly (exp_small is valid down to the underflow of 2^k)
-                                run_s[g0 + i] = dm > -690.0 ? run_s[g0 + i] * exp_small(dm) : 0.0;
-                                run_m[g0 + i] = mx;
-                                dl = v[i] - mx;
-                            }
-                            if (dl > -40.0) run_s[g0 + i] += exp_small(dl);
+                    for (int i = 0; i < SPW; i++) {
+                        double vm = v[i][0];
+#pragma unroll
+                        for (int gi = 1; gi < NG; gi++) vm = fmax(vm, v[i][gi]);
+                        if (__any_sync(0xffffffffu, vm - run_m[i] > 30.0)) {
+                            // new reference >= max over lanes, found on the ordered high words with
+                            // one REDUX; it need not be the exact maximum
+                            const int h = __double2hiint(vm);
+                            const int key = __reduce_max_sync(0xffffffffu, h ^ ((h >> 31) & 0x7fffffff));
+                            const int hm = key ^ ((key >> 31) & 0x7fffffff);
+                            const double mx = __hiloint2double(hm, hm < 0 ? 0 : -1);
+                            const double dm = run_m[i] - mx;
+                            // the running sum may hold terms up to e^30 above its reference: rescale exactly
+                            run_s[i] = dm > -690.0 ? run_s[i] * exp_small(dm) : 0.0;
+                            run_m[i] = mx;
                         }
                     }
                 }
+#pragma unroll
+                for (int i = 0; i < SPW; i++)
+#pragma unroll
+                    for (int gi = 0; gi < NG; gi++) {
+                        const double dl = v[i][gi] - run_m[i];
+                        const double e = exp_small(fmax(dl, -45.0));
+                        run_s[i] += dl > -40.0 ? e : 0.0;       // terms below e^-40 of the reference are dropped
+                    }
             }
+            F2_T(4);
             if (j1 >= N_t) break;
             j0 = j1;
             c_lo = c_hi;
             ntiles = min(F2_NEW / 8, (last_bin + 1 - c_lo + 7) / 8);
             __syncthreads();   // ring reads done before the next phase overwrites old bins
+            F2_T(5);
         }
-        // ---------------- finalise this round's samples
+        // ---------------- finalise this round's samples: lane q < SPW writes sample row q
+        {
+            double my_m = run_m[0], my_t = warp_sum(run_s[0]);
 #pragma unroll
-        for (int q = 0; q < SPW; q++) {
-            const int s = SPW * w + q;
-            const double tot = warp_sum(run_s[q]);
-            if (lane == 0 && sm.part[s]) {
-                const int t = tile * TS + s;
-                if (t < N) lnL[perm ? perm[t] : t] = run_m[q] + log(tot) - log((double)N_t);
-                sm.done[s] = 1;
+            for (int q = 1; q < SPW; q++) {
+                const double t = warp_sum(run_s[q]);
+                if (lane == q) { my_m = run_m[q]; my_t = t; }
+            }
+            if (lane < SPW) {
+                const int s = SPW * w + lane;
+                if (sm.part[s]) {
+                    const int t = tile * TS + s;
+                    if (t < N) lnL[perm ? perm[t] : t] = my_m + log(my_t) - log((double)N_t);
+                    sm.done[s] = 1;
+                }
             }
         }
+        F2_T(6);
         if (last_round) break;
     }
 }
 
-template <int K, int RB, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
 static int launch_fused2_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
     static bool configured = false;
-    const int smem = (int)sizeof(Fused2Smem<K, RB>);
+    const int smem = (int)sizeof(Fused2Smem<K>);
     if (!configured) {
-        ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused2_kernel<K, RB, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         configured = true;
     }
-    const int tiles = (N + 8 * RB - 1) / (8 * RB);
+    const int tiles = (N + F2_TS - 1) / F2_TS;
     const int slot = ile_timing_begin(ctx);
-    lnl_fused2_kernel<K, RB, NPAIR, SINGLE, TABLE, STRIDE1><<<tiles, F2_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL);
+    lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1><<<tiles, F2_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL);
     ile_timing_end(ctx, slot);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }
 
-template <int K, int RB, int NPAIR, bool SINGLE>
+template <int K, int NPAIR, bool SINGLE>
 static int launch_fused2_k(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
     const bool tb = P.use_table != 0, s1 = P.stride == 1;
-    if (tb) return s1 ? launch_fused2_t<K, RB, NPAIR, SINGLE, true, true>(ctx, P, N, rec, yt, perm, lnL)
-                      : launch_fused2_t<K, RB, NPAIR, SINGLE, true, false>(ctx, P, N, rec, yt, perm, lnL);
-    return s1 ? launch_fused2_t<K, RB, NPAIR, SINGLE, false, true>(ctx, P, N, rec, yt, perm, lnL)
-              : launch_fused2_t<K, RB, NPAIR, SINGLE, false, false>(ctx, P, N, rec, yt, perm, lnL);
+    if (tb) return s1 ? launch_fused2_t<K, NPAIR, SINGLE, true, true>(ctx, P, N, rec, yt, perm, lnL)
+                      : launch_fused2_t<K, NPAIR, SINGLE, true, false>(ctx, P, N, rec, yt, perm, lnL);
+    return s1 ? launch_fused2_t<K, NPAIR, SINGLE, false, true>(ctx, P, N, rec, yt, perm, lnL)
+              : launch_fused2_t<K, NPAIR, SINGLE, false, false>(ctx, P, N, rec, yt, perm, lnL);
 }
 
 // rec / yt as written by lnl_prep_kernel for ceil(N/64)*64 padded samples.  Returns 1 when the
 // shape has no instantiation (the caller falls back to the first-generation kernel).
 int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
-    const int rb = ctx->fused_rb == 8 ? 8 : 4;
-    if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4)
-        return rb == 4 ? launch_fused2_k<3, 4, 5, true>(ctx, P, N, rec, yt, perm, lnL) : launch_fused2_k<3, 8, 5, true>(ctx, P, N, rec, yt, perm, lnL);
-    if (P.K == 2 && np == 1 && rem >= 1 && rem <= 4)
-        return rb == 4 ? launch_fused2_k<2, 4, 1, true>(ctx, P, N, rec, yt, perm, lnL) : launch_fused2_k<2, 8, 1, true>(ctx, P, N, rec, yt, perm, lnL);
+    if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4) return launch_fused2_k<3, 5, true>(ctx, P, N, rec, yt, perm, lnL);
+    if (P.K == 2 && np == 1 && rem >= 1 && rem <= 4) return launch_fused2_k<2, 1, true>(ctx, P, N, rec, yt, perm, lnL);
     return 1;
 }
+
+#ifdef F2_TIMERS
+extern "C" int ile_dbg_timers(unsigned long long* out8) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out8, f2_timers, sizeof(f2_timers));
+    unsigned long long z[8] = {0};
+    cudaMemcpyToSymbol(f2_timers, z, sizeof(z));
+    return 0;
+}
+#endif
