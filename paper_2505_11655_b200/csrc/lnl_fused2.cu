@@ -359,19 +359,24 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                         v[i][gi] = (j0 + jl < j1) ? A : neg_inf();
                     }
                 }
-                // raise the references where a new value is more than e^30 above (rare)
+                // raise the references where a new value is more than e^30 above (rare).  The range
+                // tests compare the high words as integers (ALU pipe): the FP64 pipe is the bottleneck.
+                double dl[SPW][NG];
                 bool need = false;
 #pragma unroll
                 for (int i = 0; i < SPW; i++)
 #pragma unroll
-                    for (int gi = 0; gi < NG; gi++) need = need || (v[i][gi] - run_m[i] > 30.0);
+                    for (int gi = 0; gi < NG; gi++) {
+                        dl[i][gi] = v[i][gi] - run_m[i];
+                        need = need || (__double2hiint(dl[i][gi]) >= 0x403E0000);          // dl >= 30
+                    }
                 if (__any_sync(0xffffffffu, need)) {
 #pragma unroll
                     for (int i = 0; i < SPW; i++) {
                         double vm = v[i][0];
 #pragma unroll
                         for (int gi = 1; gi < NG; gi++) vm = fmax(vm, v[i][gi]);
-                        if (__any_sync(0xffffffffu, vm - run_m[i] > 30.0)) {
+                        if (__any_sync(0xffffffffu, vm - run_m[i] >= 30.0)) {
                             // new reference >= max over lanes, found on the ordered high words with
                             // one REDUX; it need not be the exact maximum
                             const int h = __double2hiint(vm);
@@ -382,6 +387,8 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                             // the running sum may hold terms up to e^30 above its reference: rescale exactly
                             run_s[i] = dm > -690.0 ? run_s[i] * exp_small(dm) : 0.0;
                             run_m[i] = mx;
+#pragma unroll
+                            for (int gi = 0; gi < NG; gi++) dl[i][gi] = v[i][gi] - mx;
                         }
                     }
                 }
@@ -389,9 +396,11 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
                 for (int i = 0; i < SPW; i++)
 #pragma unroll
                     for (int gi = 0; gi < NG; gi++) {
-                        const double dl = v[i][gi] - run_m[i];
-                        const double e = exp_small(fmax(dl, -45.0));
-                        run_s[i] += dl > -40.0 ? e : 0.0;       // terms below e^-40 of the reference are dropped
+                        // terms below e^-40 of the reference are dropped: dl <= -40 <=> high word >= 0xC0440000
+                        const bool keep = (unsigned)__double2hiint(dl[i][gi]) < 0xC0440000u;
+                        const double da = __hiloint2double(keep ? __double2hiint(dl[i][gi]) : (int)0xC0440000, keep ? __double2loint(dl[i][gi]) : 0);
+                        const double e = exp_small(da);
+                        run_s[i] += __hiloint2double(keep ? __double2hiint(e) : 0, keep ? __double2loint(e) : 0);
                     }
             }
             F2_T(4);
