@@ -119,6 +119,8 @@ extern "C" int ile_destroy(ile_ctx* ctx) {
     cudaFree(ctx->d_Qt);
     cudaFree(ctx->d_U);
     cudaFree(ctx->d_V);
+    cudaFree(ctx->d_UVp);
+    cudaFree(ctx->d_pairs);
     cudaFree(ctx->d_lnT);
     cudaFree(ctx->d_scratch);
     if (ctx->tev) {
@@ -144,6 +146,7 @@ extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
     ctx->variant = variant == 1 ? 1 : 0;
     ctx->sky_sort = variant == 2 ? 0 : 1;
     ctx->fused_gen1 = variant == 3 ? 1 : 0;
+    ctx->prep_gen1 = (variant == 3 || variant == 4) ? 1 : 0;
     return ILE_OK;
 }
 
@@ -223,6 +226,16 @@ extern "C" int ile_set_modes(ile_ctx* ctx, int M, const int* ell, const int* m) 
         ctx->m[i] = mm;
     }
     ctx->M = M;
+    {   // pair list of the upper triangle, row by row
+        std::vector<int2> pr;
+        for (int a = 0; a < M; a++)
+            for (int b = a; b < M; b++) pr.push_back(make_int2(a, b));
+        cudaFree(ctx->d_pairs);
+        ctx->d_pairs = nullptr;
+        ctx->n_pairs = (int)pr.size();
+        ILE_CUDA(ctx, cudaMalloc(&ctx->d_pairs, pr.size() * sizeof(int2)));
+        ILE_CUDA(ctx, cudaMemcpy(ctx->d_pairs, pr.data(), pr.size() * sizeof(int2), cudaMemcpyHostToDevice));
+    }
     if (!ctx->d_ylm) ILE_CUDA(ctx, cudaMalloc(&ctx->d_ylm, sizeof(YlmTable)));
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_ylm, &T, sizeof(YlmTable), cudaMemcpyHostToDevice, ctx->stream));
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -246,6 +259,21 @@ __global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restric
         double v = 0.0;
         if (mode < M && n < N_Q) v = Qc[(((long long)pk * M + mode) * N_Q + n) * 2 + part];
         Qt[idx] = v;
+    }
+}
+
+__global__ void pack_uv_kernel(const double* __restrict__ U, const double* __restrict__ V, const int2* __restrict__ pairs, double* __restrict__ UVp,
+                               int P, int K, int M, int n_pairs) {
+    const long long total = (long long)P * n_pairs * K;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        const int k = (int)(idx % K);
+        const int pr = (int)((idx / K) % n_pairs);
+        const int p = (int)(idx / ((long long)K * n_pairs));
+        const int2 ab = pairs[pr];
+        const double w = ab.x == ab.y ? 1.0 : 2.0;
+        const size_t src = ((((size_t)p * K + k) * M + ab.x) * M + ab.y) * 2;
+        double* o = UVp + (size_t)idx * 4;
+        o[0] = w * U[src]; o[1] = w * U[src + 1]; o[2] = w * V[src]; o[3] = w * V[src + 1];
     }
 }
 
@@ -294,10 +322,11 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     const bool reuse = ctx->have_quv && ctx->P == P && ctx->N_Q == N_Q && ctx->quv_K == K && ctx->quv_M == M;
     ctx->have_quv = false;
     if (!reuse) {
-        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_U); cudaFree(ctx->d_V);
-        ctx->d_Qc = ctx->d_Qt = ctx->d_U = ctx->d_V = nullptr;
+        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_U); cudaFree(ctx->d_V); cudaFree(ctx->d_UVp);
+        ctx->d_Qc = ctx->d_Qt = ctx->d_U = ctx->d_V = ctx->d_UVp = nullptr;
         if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qt, nQt * 8) != cudaSuccess ||
-            cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess) {
+            cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess ||
+            cudaMalloc(&ctx->d_UVp, (size_t)P * ctx->n_pairs * K * 4 * 8) != cudaSuccess) {
             cudaGetLastError();
             return ile_fail(ctx, ILE_ENOMEM, "load_quv: device allocation failed");
         }
@@ -307,6 +336,8 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_U, U, nU * 8, kind, ctx->stream));
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, V, nU * 8, kind, ctx->stream));
     repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qt, P * K, M, N_Q, N_Qpad);
+    ILE_LAUNCH_CHECK(ctx);
+    pack_uv_kernel<<<ctx->sm_count * 2, 256, 0, ctx->stream>>>(ctx->d_U, ctx->d_V, ctx->d_pairs, ctx->d_UVp, P, K, M, ctx->n_pairs);
     ILE_LAUNCH_CHECK(ctx);
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->P = P; ctx->N_Q = N_Q; ctx->N_Qpad = N_Qpad; ctx->quv_K = K; ctx->quv_M = M; ctx->fs = fs; ctx->t_Q0 = t_Q0; ctx->D_ref = D_ref;
@@ -382,5 +413,8 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
     L->U = ctx->d_U + (size_t)p * K * M * M * 2;
     L->V = ctx->d_V + (size_t)p * K * M * M * 2;
     L->ylm = ctx->d_ylm;
+    L->pairs = ctx->d_pairs;
+    L->n_pairs = ctx->n_pairs;
+    L->UVp = ctx->d_UVp + (size_t)p * ctx->n_pairs * K * 4;
     return ILE_OK;
 }

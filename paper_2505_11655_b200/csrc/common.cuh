@@ -51,6 +51,11 @@ struct LnlParams {
     const double* U;              // [K][M][M][2]
     const double* V;              // [K][M][M][2]
     const YlmTable* ylm;
+    // upper-triangle pair list (a <= b) and the matching packed matrices, Eq. 17-18:
+    // UVp[pair][k] = w (Re U_ab, Im U_ab, Re V_ab, Im V_ab), w = 1 on the diagonal and 2 off it
+    const int2* pairs;
+    int n_pairs;
+    const double* UVp;
 };
 
 struct ile_ctx {
@@ -64,7 +69,9 @@ struct ile_ctx {
     YlmTable h_ylm;
     YlmTable* d_ylm;
     double fs, t_Q0, D_ref;
-    double *d_Qc, *d_Qt, *d_U, *d_V;
+    double *d_Qc, *d_Qt, *d_U, *d_V, *d_UVp;
+    int2* d_pairs;
+    int n_pairs;
     double t_lo, dt;
     int N_t, interp, stride;
     double D_min, D_max;
@@ -73,6 +80,7 @@ struct ile_ctx {
     double* d_lnT;
     int variant;
     int fused_rb;                 // row blocks of 8 samples per CTA of the fused kernel: 4 (default, two CTAs per SM) or 8
+    int prep_gen1;                // 1: one-thread-per-sample prep kernel (A/B timing)
     int fused_gen1;               // 1: first-generation fused kernel (kept for A/B timing)
     int sky_sort;                 // 1 (default): order samples by delay cell before the fused kernel
     int sm_count;

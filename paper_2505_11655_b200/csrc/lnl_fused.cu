@@ -132,6 +132,55 @@ __global__ void __launch_bounds__(128) lnl_prep_kernel(LnlParams P, int N, int N
     r[15] = 0.0;
 }
 
+// ---------------------------------------------------------------- prep kernel without the quadratic term
+// Steps 1-3 only (antenna, delays, harmonics, x, ln prior): one thread per sample, Y_m stored
+// straight into the tile (no per-thread arrays).  The U/V quadratic term B (step 4) is computed by
+// the fused kernel's prologue, where 8 threads share each sample.  rec[13] = 0 here.
+__global__ void __launch_bounds__(128) lnl_prep3_kernel(LnlParams P, int N, int Npad, const double* __restrict__ z, const int* __restrict__ perm,
+                                                        double* __restrict__ rec, double2* __restrict__ ytile, double* __restrict__ ln_prior) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= Npad) return;
+    double2* yt = ytile + (size_t)(t / FT_TS) * FT_YM * FT_TS + (t % FT_TS);
+    double* r = rec + (size_t)t * FT_REC;
+    bool valid = false;
+    SampleIn s;
+    if (t < N) {
+        const int i = perm ? perm[t] : t;
+        s = sample_from_z(P, z, N, i);
+        valid = s.valid;
+        if (ln_prior) ln_prior[i] = valid ? ln_prior_dev(P, s) : neg_inf();
+    }
+    if (!valid) {
+        for (int m = 0; m < FT_YM; m++) yt[m * FT_TS] = make_double2(0.0, 0.0);
+        for (int q = 0; q < FT_REC; q += 2) *reinterpret_cast<double2*>(r + q) = make_double2(0.0, 0.0);
+        return;
+    }
+    double Fp[ILE_MAX_K], Fx[ILE_MAX_K], tau[ILE_MAX_K];
+    antenna_dev(P, s, Fp, Fx, tau);
+    ylm_dev(P.ylm, s.ch, s.sh, -s.phi_ref, [&](int m, double yr, double yi) { yt[m * FT_TS] = make_double2(yr, yi); });
+    for (int m = P.M; m < FT_YM; m++) yt[m * FT_TS] = make_double2(0.0, 0.0);
+    double u[ILE_MAX_K];
+#pragma unroll
+    for (int k = 0; k < ILE_MAX_K; k++) {
+        u[k] = 0.0;
+        if (k < P.K) {
+            u[k] = (P.t_lo + tau[k] - P.t_Q0) * P.fs;
+            if (!P.interp) u[k] = floor(u[k] + 0.5);
+        } else {
+            Fp[k] = Fx[k] = 0.0;
+        }
+    }
+    double2* r2 = reinterpret_cast<double2*>(r);
+    r2[0] = make_double2(Fp[0], Fp[1]);
+    r2[1] = make_double2(Fp[2], Fp[3]);
+    r2[2] = make_double2(-Fx[0], -Fx[1]);
+    r2[3] = make_double2(-Fx[2], -Fx[3]);
+    r2[4] = make_double2(u[0], u[1]);
+    r2[5] = make_double2(u[2], u[3]);
+    r2[6] = make_double2(P.use_table ? 1.0 : P.D_ref / s.dist, 0.0);
+    r2[7] = make_double2(1.0, 0.0);
+}
+
 // ---------------------------------------------------------------- PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -402,7 +451,7 @@ static int launch_fused_t(ile_ctx* ctx, const LnlParams& P, int N, const double*
 }
 
 int ile_launch_lnL_plain_z(ile_ctx* ctx, const LnlParams& P, int N, const double* z, double* lnL, double* ln_prior);
-int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL);
+int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad);
 
 int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* z, const int* perm, double* lnL, double* ln_prior) {
     if (P.K > 3 || 2 * P.M > ILE_QT_ROW) return ile_launch_lnL_plain_z(ctx, P, N, z, lnL, ln_prior);
@@ -438,10 +487,16 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         if (rc) return rc;
         perm = (const int*)v0;
     }
-    lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
+    // the second-generation fused kernel computes the quadratic term itself (prologue)
+    const int n2_ = 2 * P.M, np_ = n2_ / 8, rem_ = n2_ % 8;
+    const bool gen2 = !ctx->fused_gen1 && rem_ >= 1 && rem_ <= 4 && ((P.K == 3 && np_ == 5) || (P.K == 2 && np_ == 1));
+    if (gen2 && !ctx->prep_gen1)
+        lnl_prep3_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
+    else
+        lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
     ILE_LAUNCH_CHECK(ctx);
     if (!ctx->fused_gen1) {
-        rc = ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL);
+        rc = ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL, gen2 && !ctx->prep_gen1);
         if (rc != 1) return rc;                              // 1: shape not instantiated -> first generation
     }
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;

@@ -6,6 +6,9 @@
 // instructions per (sample, time bin) as the arithmetic allows.
 //
 //   one CTA = 32 samples (delay-cell sorted), 8 warps, two CTAs per SM
+//   prologue      step 4, the U/V quadratic term B: the tile's harmonics and the packed upper-triangle
+//                 matrices are staged in the (still idle) S ring; warp w sums pairs w, w + 8, ...
+//                 for all 32 samples; then the coefficient fragments are built
 //   contraction   S_k[s][n] = sum_r coef_k[s][r] Q_k[r][n]  (coef = x Re/Im(F_k Y_m), K-dim 2M):
 //                 unit = (detector k, 8 stored bins) x 32 samples; A fragments (coef) from shared
 //                 memory in fragment order, B fragments (Q) straight from global/L2 into registers,
@@ -28,6 +31,7 @@
 #define F2_YM 24          // mode slots in the prep kernel's Y tile (32-sample sub-tiles)
 #define F2_REC 16
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
+#define F2_UVMAX (300 * 3 * 2)   // packed U/V entries staged in shared memory (M <= 24: 300 pairs)
 #define F2_NG 2           // 32-bin groups per phase (at most 64 outputs per phase)
 
 template <int K>
@@ -132,8 +136,8 @@ __device__ __forceinline__ void sample_consts(Fused2Smem<K>& sm, int s) {
 
 template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
 __global__ void __launch_bounds__(F2_THREADS, 2)
-lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const double2* __restrict__ ytile, const int* __restrict__ perm,
-                  double* __restrict__ lnL) {
+lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, const double2* __restrict__ ytile,
+                  const int* __restrict__ perm, double* __restrict__ lnL) {
     constexpr int RB = F2_RB, TS = F2_TS, SPW = F2_SPW, NG = F2_NG;
     constexpr int NPT = NPAIR + (SINGLE ? 1 : 0);
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -142,6 +146,9 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
     const int tile = blockIdx.x;
     const int stride = STRIDE1 ? 1 : P.stride, N_t = P.N_t;
     const int c = lane & 3, rq = lane >> 2;
+    double2* ysm = reinterpret_cast<double2*>(&sm.S[0][0][0]);              // [F2_YM][32] during the prologue
+    double* qpart = reinterpret_cast<double*>(ysm + F2_YM * 32);            // [8 warps][3 K][32] partial quadratic sums
+    double2* uvsm = reinterpret_cast<double2*>(qpart + F2_WARPS * 3 * K * 32); // packed U/V, up to F2_UVMAX entries
 #ifdef F2_TIMERS
     long long tmark = clock64();
 #endif
@@ -151,6 +158,15 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
         const double* src = rec + (size_t)tile * TS * F2_REC;
         for (int q = tid; q < TS * F2_REC; q += F2_THREADS) (&sm.rec[0][0])[q] = src[q];
         if (tid < 4) sm.base[tid] = 0x7ffffffe;
+        // the tile's harmonics Y[m][s] (12 KB) are staged in the S ring, which is idle until phase 0
+        const double2* ysrc = ytile + (size_t)tile * F2_YM * 32;
+        for (int q = tid; q < F2_YM * 32; q += F2_THREADS) ysm[q] = ysrc[q];
+        // ... and so are the packed U/V matrices of this intrinsic point (16 B per pair, detector and matrix)
+        if (quad) {
+            const double2* usrc = reinterpret_cast<const double2*>(P.UVp);
+            const int nuv = min(P.n_pairs * K * 2, F2_UVMAX);
+            for (int q = tid; q < nuv; q += F2_THREADS) uvsm[q] = __ldg(usrc + q);
+        }
     }
     __syncthreads();
     bool valid = false;
@@ -177,28 +193,59 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
     {
         constexpr int NA = K * NPT * RB * 32;
         constexpr int IT = (NA + F2_THREADS - 1) / F2_THREADS;
-        double2 yv[IT];
-#pragma unroll
-        for (int it = 0; it < IT; it++) {
-            const int q = tid + it * F2_THREADS;
-            const int ln = q & 31, rb = (q >> 5) & (RB - 1), pk = q / (32 * RB), p = pk % NPT;
-            const int s = 8 * rb + (ln >> 2), cc = ln & 3;
-            const int t = tile * TS + s;
-            const int m = p < NPAIR ? 4 * p + cc : 4 * NPAIR + (cc >> 1);
-            yv[it] = make_double2(0.0, 0.0);
-            if (q < NA) yv[it] = ytile[((size_t)(t >> 5) * F2_YM + m) * 32 + (t & 31)];
-        }
 #pragma unroll
         for (int it = 0; it < IT; it++) {
             const int q = tid + it * F2_THREADS;
             const int ln = q & 31, rb = (q >> 5) & (RB - 1), pk = q / (32 * RB), p = pk % NPT, k = pk / NPT;
             const int s = 8 * rb + (ln >> 2), cc = ln & 3;
-            const double x = sm.rec[s][12], fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
-            const double2 y = yv[it];
-            double2 a;
-            if (p < NPAIR) a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
-            else a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
-            if (q < NA) sm.A[k][p][rb][ln] = a;
+            const int m = p < NPAIR ? 4 * p + cc : 4 * NPAIR + (cc >> 1);
+            if (q < NA) {
+                const double x = sm.rec[s][12], fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
+                const double2 y = ysm[m * 32 + s];
+                double2 a;
+                if (p < NPAIR) a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
+                else a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
+                sm.A[k][p][rb][ln] = a;
+            }
+        }
+    }
+    // ---- step 4, the U/V quadratic term (Eq. 7 with the Eq. 17-18 symmetries): warp w sums the
+    //      upper-triangle pairs w, w + 8, ... for all 32 samples (lane = sample; the packed matrix
+    //      entries are warp-uniform loads); partial sums meet in shared memory
+    if (quad) {
+        double uu[K], vr[K], vi[K];
+#pragma unroll
+        for (int k = 0; k < K; k++) uu[k] = vr[k] = vi[k] = 0.0;
+        // pair (a, b), a <= b, number pq of the row-by-row upper triangle: advanced arithmetically,
+        // so that the matrix loads of several iterations are independent and overlap
+        const int M = P.M;
+        int a = 0, b = w;
+        while (b >= M && a < M) { a++; b = b - M + a; }
+        const int npq = (P.n_pairs - w + F2_WARPS - 1) / F2_WARPS;
+#pragma unroll 4
+        for (int it = 0; it < npq; it++) {
+            const int pq = w + it * F2_WARPS;
+            const double2* uv = uvsm + pq * K * 2;
+            double2 u[K], v[K];
+#pragma unroll
+            for (int k = 0; k < K; k++) { u[k] = uv[2 * k]; v[k] = uv[2 * k + 1]; }
+            const double2 ya = ysm[a * 32 + lane], yb = ysm[b * 32 + lane];
+            const double t1 = ya.x * yb.x, t2 = ya.y * yb.y, t3 = ya.x * yb.y, t4 = ya.y * yb.x;
+            const double pr = t1 + t2, pi = t3 - t4, qr = t1 - t2, qi = t3 + t4;   // conj(y_a) y_b, y_a y_b
+#pragma unroll
+            for (int k = 0; k < K; k++) {
+                uu[k] += u[k].x * pr - u[k].y * pi;
+                vr[k] += v[k].x * qr - v[k].y * qi;
+                vi[k] += v[k].x * qi + v[k].y * qr;
+            }
+            b += F2_WARPS;
+            while (b >= M && a < M) { a++; b = b - M + a; }
+        }
+#pragma unroll
+        for (int k = 0; k < K; k++) {
+            qpart[(w * 3 * K + 3 * k + 0) * 32 + lane] = uu[k];
+            qpart[(w * 3 * K + 3 * k + 1) * 32 + lane] = vr[k];
+            qpart[(w * 3 * K + 3 * k + 2) * 32 + lane] = vi[k];
         }
     }
     const int n_valid = __syncthreads_count(valid);      // also publishes n, w1, base, A
@@ -210,6 +257,22 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
 #pragma unroll
         for (int k = 0; k < K; k++) part0 = part0 && (sm.n[k][tid] - sm.base[k] <= F2_CAP);
         sm.part[tid] = part0 ? 1 : 0;
+        if (quad) {
+            double B = 0.0;
+#pragma unroll
+            for (int k = 0; k < K; k++) {
+                double uu = 0.0, vr = 0.0, vi = 0.0;
+#pragma unroll
+                for (int ww = 0; ww < F2_WARPS; ww++) {
+                    uu += qpart[(ww * 3 * K + 3 * k + 0) * 32 + tid];
+                    vr += qpart[(ww * 3 * K + 3 * k + 1) * 32 + tid];
+                    vi += qpart[(ww * 3 * K + 3 * k + 2) * 32 + tid];
+                }
+                const double fr = sm.rec[tid][k], fi = sm.rec[tid][4 + k];
+                B += (fr * fr + fi * fi) * uu + ((fr * fr - fi * fi) * vr - 2.0 * fr * fi * vi);
+            }
+            sm.rec[tid][13] = 0.25 * B;
+        }
         sample_consts<K, TABLE>(sm, tid);
     }
     const int n_part0 = __syncthreads_count(part0);
@@ -434,7 +497,7 @@ lnl_fused2_kernel(LnlParams P, int N, const double* __restrict__ rec, const doub
 }
 
 template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
-static int launch_fused2_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
+static int launch_fused2_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
     static bool configured = false;
     const int smem = (int)sizeof(Fused2Smem<K>);
     if (!configured) {
@@ -443,27 +506,28 @@ static int launch_fused2_t(ile_ctx* ctx, const LnlParams& P, int N, const double
     }
     const int tiles = (N + F2_TS - 1) / F2_TS;
     const int slot = ile_timing_begin(ctx);
-    lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1><<<tiles, F2_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL);
+    lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1><<<tiles, F2_THREADS, smem, ctx->stream>>>(P, N, quad ? 1 : 0, rec, yt, perm, lnL);
     ile_timing_end(ctx, slot);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }
 
 template <int K, int NPAIR, bool SINGLE>
-static int launch_fused2_k(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
+static int launch_fused2_k(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
     const bool tb = P.use_table != 0, s1 = P.stride == 1;
-    if (tb) return s1 ? launch_fused2_t<K, NPAIR, SINGLE, true, true>(ctx, P, N, rec, yt, perm, lnL)
-                      : launch_fused2_t<K, NPAIR, SINGLE, true, false>(ctx, P, N, rec, yt, perm, lnL);
-    return s1 ? launch_fused2_t<K, NPAIR, SINGLE, false, true>(ctx, P, N, rec, yt, perm, lnL)
-              : launch_fused2_t<K, NPAIR, SINGLE, false, false>(ctx, P, N, rec, yt, perm, lnL);
+    if (tb) return s1 ? launch_fused2_t<K, NPAIR, SINGLE, true, true>(ctx, P, N, rec, yt, perm, lnL, quad)
+                      : launch_fused2_t<K, NPAIR, SINGLE, true, false>(ctx, P, N, rec, yt, perm, lnL, quad);
+    return s1 ? launch_fused2_t<K, NPAIR, SINGLE, false, true>(ctx, P, N, rec, yt, perm, lnL, quad)
+              : launch_fused2_t<K, NPAIR, SINGLE, false, false>(ctx, P, N, rec, yt, perm, lnL, quad);
 }
 
-// rec / yt as written by lnl_prep_kernel for ceil(N/64)*64 padded samples.  Returns 1 when the
+// rec / yt as written by lnl_prep_kernel (quad = false) or lnl_prep3_kernel (quad = true: the
+// quadratic term is computed here) for ceil(N/64)*64 padded samples.  Returns 1 when the
 // shape has no instantiation (the caller falls back to the first-generation kernel).
-int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL) {
+int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
-    if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4) return launch_fused2_k<3, 5, true>(ctx, P, N, rec, yt, perm, lnL);
-    if (P.K == 2 && np == 1 && rem >= 1 && rem <= 4) return launch_fused2_k<2, 1, true>(ctx, P, N, rec, yt, perm, lnL);
+    if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4) return launch_fused2_k<3, 5, true>(ctx, P, N, rec, yt, perm, lnL, quad);
+    if (P.K == 2 && np == 1 && rem >= 1 && rem <= 4) return launch_fused2_k<2, 1, true>(ctx, P, N, rec, yt, perm, lnL, quad);
     return 1;
 }
 
