@@ -14,8 +14,8 @@ counted as samples x time bins.
 `e2e`     the same step through the C ABI from HOST buffers: every step loads that intrinsic
           point's Q/U/V from pinned host memory (ile_load_quv: host -> device copy + repack), runs
           the iteration and reads the ile_result struct back to the host.
-`roofline` the fused lnL kernel (steps 5-6): algorithmic flop (264 per sample-bin, DESIGN.md
-          section 7) / its device time, timed live with CUDA events on the launching stream,
+`roofline` the fused lnL kernel (steps 4-6): algorithmic flop (289.4 per sample-bin, DESIGN.md
+          section 6) / its device time, timed live with CUDA events on the launching stream,
           against the FP64 peak measured in the same process by the library's register-resident
           DFMA / DMMA chain probes (bound "alu": the path is FP64-arithmetic bound, not HBM bound).
 `cpu_baseline` the oracle (oracle/, numpy fp64, as it stands) on the host cores, one AC iteration
@@ -43,7 +43,15 @@ if ROOT not in sys.path:
 METRIC = "extrinsic lnL evals/s (samples x time bins)"
 UNIT = "sample-bins/s"
 CFG = 2
-FLOP_PER_UNIT = 264.0          # 2 K (2M + 2) flop per sample-bin at K = 3, M = 21
+
+
+def flop_per_unit(K, M, N_t):
+    """Algorithmic flop of the fused kernel per (sample, time bin): contraction +
+    interpolation 2 K (2M + 2), plus the U/V quadratic term (K 6 M(M+1)/2 FMA + 8 M(M+1)/2 flop per
+    sample) spread over the N_t bins.  264 + 25.4 = 289.4 at K = 3, M = 21, N_t = 400."""
+    pairs = M * (M + 1) // 2
+    return 2.0 * K * (2 * M + 2) + (2.0 * K * 6 * pairs + 8.0 * pairs) / N_t
+
 ORACLE_SAMPLE_N = 1 << 14
 
 
@@ -231,7 +239,8 @@ def run_ours(args):
         value = world * units_per_step * args.steps / (ms * 1e-3)
         e2e_value = world * units_per_step * args.steps / (e2e_ms * 1e-3)
         k_avg_ms = k_ms / max(k_n, 1)
-        achieved = FLOP_PER_UNIT * units_per_step / (k_avg_ms * 1e-3) / 1e12
+        fpu = flop_per_unit(prob.K, prob.M, prob.N_t)
+        achieved = fpu * units_per_step / (k_avg_ms * 1e-3) / 1e12
         peak = max(peak_dfma, peak_dmma)
         # oracle on the host cores (rank 0, N = 1 only), bounded sample
         cpu = None
@@ -247,10 +256,10 @@ def run_ours(args):
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches),
             "clocks": clk,
-            "roofline": {"bound": "alu", "kernel": "lnl_fused_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "roofline": {"bound": "alu", "kernel": "lnl_fused2_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": None, "kernel_ms": k_avg_ms, "kernel_launches": int(k_n),
                          "kernel_share_of_step": k_ms / ms, "peak_source": "measured in-process: max(DFMA chain, DMMA chain)",
-                         "peak_dfma": peak_dfma, "peak_dmma": peak_dmma, "flop_per_unit": FLOP_PER_UNIT},
+                         "peak_dfma": peak_dfma, "peak_dmma": peak_dmma, "flop_per_unit": fpu},
             "cpu_baseline": cpu,
             "check": {"ln_integral_last": float(last["ln_integral"]), "n_eff_last": float(last["n_eff"]),
                       "samples_per_s": value / prob.N_t},
@@ -263,7 +272,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -30,10 +30,10 @@ __global__ void __launch_bounds__(RS_THREADS) rs_hist_kernel(int p, const long l
         if (act && (threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&sh[dg], (uint32_t)__popc(m));
     }
     __syncthreads();
-    hist[(size_t)threadIdx.x * max_blocks + blockIdx.x] = sh[threadIdx.x];
+    hist[(size_t)blockIdx.x * 256 + threadIdx.x] = sh[threadIdx.x];      // [block][digit]: coalesced
 }
 
-// exclusive scan of hist[digit][block], digit-major, over the blocks in use
+// exclusive scan of the counts in (digit, block) order; stored as hist[block][digit]
 __global__ void __launch_bounds__(1024) rs_scan_kernel(int p, const long long* __restrict__ n_dev, const int* __restrict__ bits_dev,
                                                        uint32_t* __restrict__ hist, int max_blocks) {
     const int npass = rs_passes(*bits_dev);
@@ -41,26 +41,27 @@ __global__ void __launch_bounds__(1024) rs_scan_kernel(int p, const long long* _
     const long long n = *n_dev;
     const int nblocks = (int)((n + RS_TILE - 1) / RS_TILE);
     __shared__ uint32_t part[1024];
-    const int t = threadIdx.x, dg = t >> 2, qd = t & 3;
+    // thread (qd, dg): digit dg, quarter qd of the blocks; consecutive threads read consecutive digits
+    const int t = threadIdx.x, dg = t & 255, qd = t >> 8;
     const int per = (nblocks + 3) >> 2;
     const int b0 = min(qd * per, nblocks), b1 = min(b0 + per, nblocks);
     uint32_t s = 0;
-    uint32_t* row = hist + (size_t)dg * max_blocks;
-    for (int b = b0; b < b1; b++) s += row[b];
-    part[t] = s;
+#pragma unroll 8
+    for (int b = b0; b < b1; b++) s += hist[(size_t)b * 256 + dg];
+    part[dg * 4 + qd] = s;                       // digit-major order of the scan
     __syncthreads();
-    // block-wide exclusive scan of part[] (1024 entries, in index order = digit-major order)
-    uint32_t v = s;
+    // block-wide exclusive scan of part[] (1024 entries)
+    const int o_idx = dg * 4 + qd;
     for (int o = 1; o < 1024; o <<= 1) {
         uint32_t add = (t >= o) ? part[t - o] : 0;
         __syncthreads();
         part[t] += add;
         __syncthreads();
     }
-    uint32_t run = part[t] - v;
+    uint32_t run = part[o_idx] - s;
     for (int b = b0; b < b1; b++) {
-        uint32_t c = row[b];
-        row[b] = run;
+        uint32_t c = hist[(size_t)b * 256 + dg];
+        hist[(size_t)b * 256 + dg] = run;
         run += c;
     }
 }
@@ -100,7 +101,7 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(int p, const lon
     // phase B: turn the counts into start offsets (global base of (digit, block) + earlier warps)
     {
         const int dg = threadIdx.x;
-        uint32_t run = hist[(size_t)dg * max_blocks + blockIdx.x];
+        uint32_t run = hist[(size_t)blockIdx.x * 256 + dg];
         for (int ww = 0; ww < RS_THREADS / 32; ww++) {
             uint32_t c = wh[ww][dg];
             wh[ww][dg] = run;
