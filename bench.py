@@ -127,7 +127,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n = 1 << 12
+    n = 1 << 11
     rate, sec, cores, prob = oracle_rate(n, steps=args.steps, warmup=min(args.warmup, 1))
     sample = f"config {CFG} shapes (K=3, M=21, N_t={prob.N_t}, AC), {n} samples per step instead of {1 << 20}"
     print(json.dumps({
@@ -146,6 +146,21 @@ def _config_dict(prob, N):
 
 
 # ------------------------------------------------------------------------------- our arm
+def max_over_ranks(values, world, device):
+    """Every multi-GPU number is the maximum over ranks of the per-rank device time."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def aggregate_value(units_per_step_per_rank, steps, world, ms):
+    """Whole-job throughput: replicas do not communicate, every rank processes its own units."""
+    return world * units_per_step_per_rank * steps / (ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -230,14 +245,11 @@ def run_ours(args):
     barrier()
     e2e_s = time.perf_counter() - t0
 
-    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = float(t[0]), float(t[1])
+    ms, e2e_ms = max_over_ranks([ms, e2e_s * 1e3], world, dev)
 
     if rank == 0:
-        value = world * units_per_step * args.steps / (ms * 1e-3)
-        e2e_value = world * units_per_step * args.steps / (e2e_ms * 1e-3)
+        value = aggregate_value(units_per_step, args.steps, world, ms)
+        e2e_value = aggregate_value(units_per_step, args.steps, world, e2e_ms)
         k_avg_ms = k_ms / max(k_n, 1)
         fpu = flop_per_unit(prob.K, prob.M, prob.N_t)
         achieved = fpu * units_per_step / (k_avg_ms * 1e-3) / 1e12
