@@ -53,6 +53,7 @@ def flop_per_unit(K, M, N_t):
     return 2.0 * K * (2 * M + 2) + (2.0 * K * 6 * pairs + 8.0 * pairs) / N_t
 
 ORACLE_SAMPLE_N = 1 << 14
+NCU_TRAFFIC_BYTES = 550.80e6 + 15.23e6   # profiles/r1_fused_kernel.md (algorithmic: 512 B in + 8 B out per sample = 545 MB)
 
 
 # ------------------------------------------------------------------------------- clocks
@@ -269,7 +270,8 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": clk,
             "roofline": {"bound": "alu", "kernel": "lnl_fused2_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": None, "kernel_ms": k_avg_ms, "kernel_launches": int(k_n),
+                         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES,
+                         "traffic_note": "dram bytes read+written per launch of this kernel, ncu --set full, profiles/r1_fused_kernel.md", "kernel_ms": k_avg_ms, "kernel_launches": int(k_n),
                          "kernel_share_of_step": k_ms / ms, "peak_source": "measured in-process: max(DFMA chain, DMMA chain)",
                          "peak_dfma": peak_dfma, "peak_dmma": peak_dmma, "flop_per_unit": fpu},
             "cpu_baseline": cpu,

@@ -1,0 +1,106 @@
+"""Full BASELINE.json sizes in the launch configuration bench.py times (-m gpu): the oracle cannot
+evaluate 2^20..2^22 samples, so per-sample lnL is checked on a seeded subset of the batch the
+device drew itself, and the reductions through properties that hold at any size."""
+import numpy as np
+import pytest
+
+from synth import make_problem
+
+pytestmark = pytest.mark.gpu
+
+
+def _tol(ref):
+    return 1e-9 * np.maximum(1.0, np.abs(ref))
+
+
+@pytest.mark.parametrize("cfg,P,n_iter", [(2, 1, 3), (3, 1, 3), (4, 3, 1), (5, 1, 3)])
+def test_full_batch_sampled_parity(cfg, P, n_iter):
+    import torch
+    from paper_2505_11655_b200 import Ile, Integrator, result_from_device
+    from oracle.ile import IleProblem
+    from oracle.reduce import reduce_lnw
+    prob = make_problem(cfg, P=P)
+    N = prob.N                                           # 2^20, 2^22, 2^18, 2^21
+    ile = Ile(0)
+    ile.load_problem(prob)
+    g = Integrator.from_problem(ile, prob, max_batch=N)
+    rng = np.random.default_rng(100 + cfg)
+    for p in range(P):
+        g.reset()
+        op = IleProblem(prob, p)
+        for it in range(n_iter):
+            res = result_from_device(g.step(p, N, it))[0]
+            z, lp, lnL, lnw = g.last_batch(N)
+            idx = np.sort(rng.choice(N, size=192, replace=False))
+            tidx = torch.from_numpy(idx).cuda()
+            zs = z[:, tidx].cpu().numpy()
+            got = lnL[tidx].cpu().numpy()
+            ref = op.lnL_z(zs)
+            fin = np.isfinite(ref)
+            assert np.array_equal(fin, np.isfinite(got))
+            assert np.all(np.abs(got[fin] - ref[fin]) <= _tol(ref[fin])), np.abs(got[fin] - ref[fin]).max()
+            # ln w of the sampled entries, then the reduction of the device's own ln w in fp64 on the host
+            lw = lnw.cpu().numpy()
+            ref_w = np.where(fin, ref + op.ln_prior(zs) - lp[tidx].cpu().numpy(), -np.inf)
+            assert np.all(np.abs(lw[idx][fin] - ref_w[fin]) <= 2e-9 * np.maximum(1.0, np.abs(ref_w[fin])))
+            red = reduce_lnw(lw)                         # oracle reduction on the full device batch
+            assert abs(res["ln_integral"] - red["ln_integral"]) <= 1e-8
+            assert abs(res["n_eff"] - red["n_eff"]) <= 1e-7 * max(1.0, red["n_eff"])
+            assert abs(res["n_ess"] - red["n_ess"]) <= 1e-7 * max(1.0, red["n_ess"])
+            assert 1.0 - 1e-9 <= res["n_eff"] <= res["n_ess"] * (1 + 1e-12) <= N * (1 + 1e-12)
+            assert res["n_samples"] == N and res["cum_n_samples"] == N * (it + 1)
+    if prob.kind == "AV":
+        assert res["n_bins"] > 1 and 1 <= res["n_cells"] <= N and res["N_min"] >= 4096
+        keys = g.get_state()["keys"]
+        assert np.all(np.diff(keys.astype(np.int64)) > 0)          # sorted, unique
+    if prob.kind == "PORTFOLIO":
+        st = g.get_state()
+        assert abs(st["W"][:3].sum() - 1.0) < 1e-12 and st["alloc"][:3].sum() == N
+
+
+@pytest.mark.parametrize("N", [1, 31, 33, 64, 97])
+def test_ragged_and_tiny_batches(N):
+    import torch
+    from paper_2505_11655_b200 import Ile
+    from oracle import likelihood as lk
+    from synth.workloads import uniform_box_samples
+    prob = make_problem(2, P=1)
+    ile = Ile(0)
+    ile.load_problem(prob)
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=N)
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z)
+    got = ile.lnL_z(0, torch.from_numpy(z).cuda()).cpu().numpy()
+    assert np.all(np.abs(got - ref) <= _tol(ref))
+
+
+def test_all_samples_outside_the_box_and_empty_batch():
+    import torch
+    from paper_2505_11655_b200 import Ile
+    prob = make_problem(1)
+    ile = Ile(0)
+    ile.load_problem(prob)
+    z = np.tile(np.array([[7.0], [0.0], [1.0], [1.0], [0.0], [500.0]]), (1, 70))     # RA outside [0, 2 pi)
+    got, lp = ile.lnL_z(0, torch.from_numpy(z).cuda(), want_prior=True)
+    assert torch.all(got == -float("inf")) and torch.all(lp == -float("inf"))
+    red = ile.reduce(got)
+    assert red["ln_integral"] == -np.inf and red["n_eff"] == 0 and red["n_samples"] == 70
+    empty = torch.empty((6, 0), dtype=torch.float64, device="cuda")
+    assert ile.lnL_z(0, empty).numel() == 0
+
+
+def test_delay_spread_beyond_one_round():
+    """Unsorted samples all over the sky in one tile force the multi-round path (variant 2)."""
+    import torch
+    from paper_2505_11655_b200 import Ile
+    from oracle import likelihood as lk
+    from synth.workloads import uniform_box_samples
+    prob = make_problem(3, P=1)
+    ile = Ile(0)
+    ile.load_problem(prob)
+    ile.set_lnL_variant(2)
+    z = uniform_box_samples(prob.lo, prob.hi, 257, seed=4)
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z)
+    got = ile.lnL_z(0, torch.from_numpy(z).cuda()).cpu().numpy()
+    assert np.all(np.abs(got - ref) <= _tol(ref))
