@@ -141,7 +141,8 @@ extern "C" int ile_sync(ile_ctx* ctx) {
 }
 
 extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
-    if (!ctx || variant < 0 || variant > 4) return ile_fail(ctx, ILE_EINVAL, "variant must be 0..4");
+    if (!ctx || variant < 0 || variant > 5) return ile_fail(ctx, ILE_EINVAL, "variant must be 0..5");
+    ctx->fused_gen3 = variant == 5 ? 1 : 0;
     ctx->fused_rb = variant == 4 ? 8 : 4;
     ctx->variant = variant == 1 ? 1 : 0;
     ctx->sky_sort = variant == 2 ? 0 : 1;

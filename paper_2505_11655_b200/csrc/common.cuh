@@ -80,6 +80,7 @@ struct ile_ctx {
     double* d_lnT;
     int variant;
     int fused_rb;                 // row blocks of 8 samples per CTA of the fused kernel: 4 (default, two CTAs per SM) or 8
+    int fused_gen3;               // 1: warp-specialised persistent fused kernel
     int prep_gen1;                // 1: one-thread-per-sample prep kernel (A/B timing)
     int fused_gen1;               // 1: first-generation fused kernel (kept for A/B timing)
     int sky_sort;                 // 1 (default): order samples by delay cell before the fused kernel

@@ -452,6 +452,7 @@ static int launch_fused_t(ile_ctx* ctx, const LnlParams& P, int N, const double*
 
 int ile_launch_lnL_plain_z(ile_ctx* ctx, const LnlParams& P, int N, const double* z, double* lnL, double* ln_prior);
 int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad);
+int ile_launch_fused3(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad);
 
 int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* z, const int* perm, double* lnL, double* ln_prior) {
     if (P.K > 3 || 2 * P.M > ILE_QT_ROW) return ile_launch_lnL_plain_z(ctx, P, N, z, lnL, ln_prior);
@@ -496,7 +497,8 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
     ILE_LAUNCH_CHECK(ctx);
     if (!ctx->fused_gen1) {
-        rc = ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL, gen2 && !ctx->prep_gen1);
+        rc = ctx->fused_gen3 ? ile_launch_fused3(ctx, P, N, rec, yt, perm, lnL, gen2 && !ctx->prep_gen1)
+                             : ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL, gen2 && !ctx->prep_gen1);
         if (rc != 1) return rc;                              // 1: shape not instantiated -> first generation
     }
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;

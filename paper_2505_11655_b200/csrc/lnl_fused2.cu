@@ -134,16 +134,48 @@ __device__ __forceinline__ void sample_consts(Fused2Smem<K>& sm, int s) {
     }
 }
 
-template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
-__global__ void __launch_bounds__(F2_THREADS, 2)
-lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, const double2* __restrict__ ytile,
-                  const int* __restrict__ perm, double* __restrict__ lnL) {
+// ---------------------------------------------------------------- synchronisation policies
+// MODE 0: the tile is processed by a whole CTA (256 threads) that also does its own contraction.
+// MODE 1: the tile is processed by one 8-warp epilogue group of a warp-specialised persistent CTA;
+//         the contraction is done by the CTA's dedicated warps (lnl_fused3_kernel), handed over
+//         through a command block and two named barriers per slot.
+#define F3_MW 4                       // contraction warps (warpgroup 0)
+#ifndef F3_MREGS
+#define F3_MREGS 224                  // registers per thread of the contraction warps after setmaxnreg
+#endif
+#ifndef F3_EREGS
+#define F3_EREGS 64                   // ... and of the epilogue warps
+#endif
+#define F3_THREADS (128 + 2 * F2_THREADS)
+enum { F3_BAR_GROUP = 1, F3_BAR_FULL = 3, F3_BAR_EMPTY = 5 };   // + slot
+struct F3Cmd {
+    int go;                           // 0: this slot's group has no more tiles
+    int c_lo, ntiles;                 // ring bins [c_lo, c_lo + 8 ntiles) are to be computed
+    int base[3];                      // tile base bin per detector
+    int pad[2];
+};
+__device__ __forceinline__ void named_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void named_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+template <int MODE>
+__device__ __forceinline__ void tile_sync(int slot) {
+    if (MODE == 0) __syncthreads();
+    else named_sync(F3_BAR_GROUP + slot, F2_THREADS);
+}
+template <int MODE>
+__device__ __forceinline__ int tile_count(int slot, bool pred) {
+    if (MODE == 0) return __syncthreads_count(pred);
+    int r;
+    asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n bar.red.popc.u32 %0, %1, %2, p;\n}" : "=r"(r) : "r"(F3_BAR_GROUP + slot), "r"(F2_THREADS), "r"((int)pred) : "memory");
+    return r;
+}
+
+template <int MODE, int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+__device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const int slot, const int tid, const int tile, const LnlParams& P,
+                                          const int N, const int quad, const double* __restrict__ rec, const double2* __restrict__ ytile,
+                                          const int* __restrict__ perm, double* __restrict__ lnL) {
     constexpr int RB = F2_RB, TS = F2_TS, SPW = F2_SPW, NG = F2_NG;
     constexpr int NPT = NPAIR + (SINGLE ? 1 : 0);
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    Fused2Smem<K>& sm = *reinterpret_cast<Fused2Smem<K>*>(smem_raw);
-    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int tile = blockIdx.x;
+    const int lane = tid & 31, w = tid >> 5;
     const int stride = STRIDE1 ? 1 : P.stride, N_t = P.N_t;
     const int c = lane & 3, rq = lane >> 2;
     double2* ysm = reinterpret_cast<double2*>(&sm.S[0][0][0]);              // [F2_YM][32] during the prologue
@@ -168,7 +200,7 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
             for (int q = tid; q < nuv; q += F2_THREADS) uvsm[q] = __ldg(usrc + q);
         }
     }
-    __syncthreads();
+    tile_sync<MODE>(slot);
     bool valid = false;
     if (tid < TS) {
         valid = sm.rec[tid][14] != 0.0;
@@ -248,7 +280,7 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
             qpart[(w * 3 * K + 3 * k + 2) * 32 + lane] = vi[k];
         }
     }
-    const int n_valid = __syncthreads_count(valid);      // also publishes n, w1, base, A
+    const int n_valid = tile_count<MODE>(slot, valid);      // also publishes n, w1, base, A
     if (n_valid == 0) return;
     // ---- round 0: who fits within F2_CAP of the base (normally everybody)
     bool part0 = false;
@@ -275,20 +307,20 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
         }
         sample_consts<K, TABLE>(sm, tid);
     }
-    const int n_part0 = __syncthreads_count(part0);
+    const int n_part0 = tile_count<MODE>(slot, part0);
     bool last_round = n_part0 == n_valid;
     bool need_setup = n_part0 == 0;                       // nobody fits: the general set-up pivots
     F2_T(0);
 
     for (int round = 0;; round++) {   // rounds: normally one; more only when the tile's delay spread exceeds F2_CAP
         if (round > 0 || need_setup) {
-            __syncthreads();
+            tile_sync<MODE>(slot);
             if (tid < 32) round_setup<K>(sm, lane);
-            __syncthreads();
+            tile_sync<MODE>(slot);
             if (sm.n_left == 0) break;
             last_round = sm.n_part == sm.n_left;
             if (tid < TS) sample_consts<K, TABLE>(sm, tid);
-            __syncthreads();
+            tile_sync<MODE>(slot);
             need_setup = false;
         }
         // per-sample epilogue state of this warp's rows: reference m (warp-uniform), lane-partial sum
@@ -304,75 +336,90 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
             int j1 = (c_hi - 1 - F2_CAP - 1) / stride + 1;      // outputs whose reads are all below c_hi
             if (j1 > N_t) j1 = N_t;
             F2_T(1);
-            // ---------------- contraction: unit = (k, 8 bins) x 32 samples.  Q fragments of the next
-            // unit are loaded into the other register set while this one is multiplied.
-            {
-                const int nunits = K * ntiles;
-                auto unit_kt = [&](int u, int& k, int& t) {
-                    k = (u >= ntiles ? 1 : 0) + (u >= 2 * ntiles ? 1 : 0);
-                    t = u - k * ntiles;
-                };
-                auto load_b = [&](int u, double2 (&b)[NPAIR], double& bs) {
-                    int k, t;
-                    unit_kt(u, k, t);
-                    const int row = sm.base[k] + c_lo + 8 * t + rq;
-                    const int swz = (row & 1) << 3;
-                    const double* qrow = P.Qt + ((size_t)k * P.N_Qpad + row) * ILE_QT_ROW;
+            if (MODE == 1) {
+                // ---------------- hand the phase to the contraction warps and wait for S
+                if (tid == 0) {
+                    cmd->c_lo = c_lo;
+                    cmd->ntiles = ntiles;
 #pragma unroll
-                    for (int p = 0; p < NPAIR; p++) b[p] = __ldg(reinterpret_cast<const double2*>(qrow + ((8 * p + 2 * c) ^ swz)));
-                    if (SINGLE) bs = __ldg(qrow + ((8 * NPAIR + c) ^ swz));
-                };
-                auto compute = [&](int u, const double2 (&b)[NPAIR], const double bs) {
-                    int k, t;
-                    unit_kt(u, k, t);
-                    // two accumulators per row block (the .x and .y halves of each k-step pair):
-                    // 2 RB independent DMMA chains per warp
-                    double d[RB][2], e[RB][2];
-#pragma unroll
-                    for (int rb = 0; rb < RB; rb++) d[rb][0] = d[rb][1] = e[rb][0] = e[rb][1] = 0.0;
-                    const double2* Ak = &sm.A[k][0][0][lane];
-#pragma unroll
-                    for (int p = 0; p < NPAIR; p++) {
-                        double2 a[RB];
-#pragma unroll
-                        for (int rb = 0; rb < RB; rb++) a[rb] = Ak[(p * RB + rb) * 32];
-#pragma unroll
-                        for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], a[rb].x, b[p].x);
-#pragma unroll
-                        for (int rb = 0; rb < RB; rb++) dmma2(e[rb][0], e[rb][1], a[rb].y, b[p].y);
-                    }
-                    if (SINGLE) {
-#pragma unroll
-                        for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs);
-                    }
-#pragma unroll
-                    for (int rb = 0; rb < RB; rb++) { d[rb][0] += e[rb][0]; d[rb][1] += e[rb][1]; }
-                    int cr = c_lo + 8 * t;
-                    cr -= (cr / F2_RING) * F2_RING;
-                    double* srow = &sm.S[k][rq][cr + 2 * c];
-#pragma unroll
-                    for (int rb = 0; rb < RB; rb++) *reinterpret_cast<double2*>(srow + rb * 8 * F2_SROW) = make_double2(d[rb][0], d[rb][1]);
-                    if (cr == 0 && c == 0) {      // ring column F2_RING mirrors column 0: the epilogue reads [r], [r+1] unwrapped
-#pragma unroll
-                        for (int rb = 0; rb < RB; rb++) srow[rb * 8 * F2_SROW + F2_RING] = d[rb][0];
-                    }
-                };
-                double2 b0[NPAIR], b1[NPAIR];
-                double s0 = 0.0, s1 = 0.0;
-                int u = w;
-                if (u < nunits) load_b(u, b0, s0);
-                while (u < nunits) {
-                    if (u + F2_WARPS < nunits) load_b(u + F2_WARPS, b1, s1);
-                    compute(u, b0, s0);
-                    u += F2_WARPS;
-                    if (u >= nunits) break;
-                    if (u + F2_WARPS < nunits) load_b(u + F2_WARPS, b0, s0);
-                    compute(u, b1, s1);
-                    u += F2_WARPS;
+                    for (int k = 0; k < K; k++) cmd->base[k] = sm.base[k];
+                    cmd->go = 1;
                 }
-            }
+                __threadfence_block();
+                named_arrive(F3_BAR_EMPTY + slot, 128 + F2_THREADS);   // previous ring reads done, command valid
+                named_sync(F3_BAR_FULL + slot, 128 + F2_THREADS);      // S complete for bins < c_hi
+            } else {
+            // ---------------- contraction: unit = (k, 8 bins) x 32 samples.  Q fragments of the next
+                // unit are loaded into the other register set while this one is multiplied.
+                {
+                    const int nunits = K * ntiles;
+                    auto unit_kt = [&](int u, int& k, int& t) {
+                        k = (u >= ntiles ? 1 : 0) + (u >= 2 * ntiles ? 1 : 0);
+                        t = u - k * ntiles;
+                    };
+                    auto load_b = [&](int u, double2 (&b)[NPAIR], double& bs) {
+                        int k, t;
+                        unit_kt(u, k, t);
+                        const int row = sm.base[k] + c_lo + 8 * t + rq;
+                        const int swz = (row & 1) << 3;
+                        const double* qrow = P.Qt + ((size_t)k * P.N_Qpad + row) * ILE_QT_ROW;
+#pragma unroll
+                        for (int p = 0; p < NPAIR; p++) b[p] = __ldg(reinterpret_cast<const double2*>(qrow + ((8 * p + 2 * c) ^ swz)));
+                        if (SINGLE) bs = __ldg(qrow + ((8 * NPAIR + c) ^ swz));
+                    };
+                    auto compute = [&](int u, const double2 (&b)[NPAIR], const double bs) {
+                        int k, t;
+                        unit_kt(u, k, t);
+                        // two accumulators per row block (the .x and .y halves of each k-step pair):
+                        // 2 RB independent DMMA chains per warp
+                        double d[RB][2], e[RB][2];
+#pragma unroll
+                        for (int rb = 0; rb < RB; rb++) d[rb][0] = d[rb][1] = e[rb][0] = e[rb][1] = 0.0;
+                        const double2* Ak = &sm.A[k][0][0][lane];
+#pragma unroll
+                        for (int p = 0; p < NPAIR; p++) {
+                            const double2 bp = b[p];
+                            double2 a[RB];
+#pragma unroll
+                            for (int rb = 0; rb < RB; rb++) a[rb] = Ak[(p * RB + rb) * 32];
+#pragma unroll
+                            for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], a[rb].x, bp.x);
+#pragma unroll
+                            for (int rb = 0; rb < RB; rb++) dmma2(e[rb][0], e[rb][1], a[rb].y, bp.y);
+                        }
+                        if (SINGLE) {
+#pragma unroll
+                            for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs);
+                        }
+#pragma unroll
+                        for (int rb = 0; rb < RB; rb++) { d[rb][0] += e[rb][0]; d[rb][1] += e[rb][1]; }
+                        int cr = c_lo + 8 * t;
+                        cr -= (cr / F2_RING) * F2_RING;
+                        double* srow = &sm.S[k][rq][cr + 2 * c];
+#pragma unroll
+                        for (int rb = 0; rb < RB; rb++) *reinterpret_cast<double2*>(srow + rb * 8 * F2_SROW) = make_double2(d[rb][0], d[rb][1]);
+                        if (cr == 0 && c == 0) {      // ring column F2_RING mirrors column 0: the epilogue reads [r], [r+1] unwrapped
+#pragma unroll
+                            for (int rb = 0; rb < RB; rb++) srow[rb * 8 * F2_SROW + F2_RING] = d[rb][0];
+                        }
+                    };
+                    double2 b0[NPAIR], b1[NPAIR];
+                    double s0 = 0.0, s1 = 0.0;
+                    int u = w;
+                    if (u < nunits) load_b(u, b0, s0);
+                    while (u < nunits) {
+                        if (u + F2_WARPS < nunits) load_b(u + F2_WARPS, b1, s1);
+                        compute(u, b0, s0);
+                        u += F2_WARPS;
+                        if (u >= nunits) break;
+                        if (u + F2_WARPS < nunits) load_b(u + F2_WARPS, b0, s0);
+                        compute(u, b1, s1);
+                        u += F2_WARPS;
+                    }
+                }
+    }
             F2_T(2);
-            __syncthreads();   // S complete for bins < c_hi
+            if (MODE == 0) tile_sync<MODE>(slot);   // S complete for bins < c_hi
             F2_T(3);
             // ---------------- epilogue: shift + interpolate + sum detectors, then a streaming
             // log-sum-exp.  Straight-line code over SPW x NG independent (sample row, 32-bin group)
@@ -471,7 +518,7 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
             j0 = j1;
             c_lo = c_hi;
             ntiles = min(F2_NEW / 8, (last_bin + 1 - c_lo + 7) / 8);
-            __syncthreads();   // ring reads done before the next phase overwrites old bins
+            if (MODE == 0) tile_sync<MODE>(slot);   // ring reads done before the next phase overwrites old bins (MODE 1: the EMPTY barrier)
             F2_T(5);
         }
         // ---------------- finalise this round's samples: lane q < SPW writes sample row q
@@ -494,6 +541,16 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
         F2_T(6);
         if (last_round) break;
     }
+}
+
+
+template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+__global__ void __launch_bounds__(F2_THREADS, 2)
+lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, const double2* __restrict__ ytile,
+                  const int* __restrict__ perm, double* __restrict__ lnL) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Fused2Smem<K>& sm = *reinterpret_cast<Fused2Smem<K>*>(smem_raw);
+    tile_body<0, K, NPAIR, SINGLE, TABLE, STRIDE1>(sm, nullptr, 0, threadIdx.x, blockIdx.x, P, N, quad, rec, ytile, perm, lnL);
 }
 
 template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
@@ -540,3 +597,213 @@ extern "C" int ile_dbg_timers(unsigned long long* out8) {
     return 0;
 }
 #endif
+
+// ================================================================ warp-specialised persistent kernel
+// One CTA per SM: warpgroup 0 = 4 contraction warps (one per SM sub-partition) with a large
+// register budget (setmaxnreg), warpgroups 1-4 = two epilogue groups of 8 warps, each working on
+// its own 32-sample tile ("slot") with tile_body<1>.  The contraction warps alternate between the
+// two slots, so the FP64 pipe is fed while either group is in its epilogue or prologue.
+template <int K>
+struct Fused3Smem {
+    Fused2Smem<K> slot[2];
+    F3Cmd cmd[2];
+};
+
+// contraction of one phase of one slot by the 4 contraction warps: warp mw takes the 8-bin tiles
+// t = mw, mw + 4, ... of every detector, two tiles of the same detector at a time (they share the
+// A fragments): 16 independent DMMA chains per warp
+template <int K, int NPAIR, bool SINGLE>
+__device__ __forceinline__ void contract_phase(Fused2Smem<K>& sm, const LnlParams& P, const int c_lo, const int ntiles, const int* base,
+                                               const int mw, const int lane) {
+    constexpr int RB = F2_RB;
+    const int c = lane & 3, rq = lane >> 2;
+    const int nper = ntiles > mw ? (ntiles - mw + 7) / 8 : 0;       // items per detector for this warp
+    const int nitems = K * nper;
+    auto item_kt = [&](int j, int& k, int& t0, int& nu) {
+        k = nper == 2 ? (j >> 1) : j;
+        t0 = mw + 8 * (nper == 2 ? (j & 1) : 0);
+        nu = (t0 + 4 < ntiles) ? 2 : 1;
+    };
+    auto load_b = [&](int j, double2 (&b)[2][NPAIR], double (&bs)[2]) {
+        int k, t0, nu;
+        item_kt(j, k, t0, nu);
+#pragma unroll
+        for (int u = 0; u < 2; u++) {
+            if (u < nu) {
+                const int row = base[k] + c_lo + 8 * (t0 + 4 * u) + rq;
+                const int swz = (row & 1) << 3;
+                const double* qrow = P.Qt + ((size_t)k * P.N_Qpad + row) * ILE_QT_ROW;
+#pragma unroll
+                for (int p = 0; p < NPAIR; p++) b[u][p] = __ldg(reinterpret_cast<const double2*>(qrow + ((8 * p + 2 * c) ^ swz)));
+                if (SINGLE) bs[u] = __ldg(qrow + ((8 * NPAIR + c) ^ swz));
+            }
+        }
+    };
+    auto store_unit = [&](int k, int t, const double (&d)[RB][2]) {
+        int cr = c_lo + 8 * t;
+        cr -= (cr / F2_RING) * F2_RING;
+        double* srow = &sm.S[k][rq][cr + 2 * c];
+#pragma unroll
+        for (int rb = 0; rb < RB; rb++) *reinterpret_cast<double2*>(srow + rb * 8 * F2_SROW) = make_double2(d[rb][0], d[rb][1]);
+        if (cr == 0 && c == 0) {
+#pragma unroll
+            for (int rb = 0; rb < RB; rb++) srow[rb * 8 * F2_SROW + F2_RING] = d[rb][0];
+        }
+    };
+    auto compute = [&](int j, const double2 (&b)[2][NPAIR], const double (&bs)[2]) {
+        int k, t0, nu;
+        item_kt(j, k, t0, nu);
+        const double2* Ak = &sm.A[k][0][0][lane];
+        if (nu == 2) {
+            double d[2][RB][2], e[2][RB][2];
+#pragma unroll
+            for (int u = 0; u < 2; u++)
+#pragma unroll
+                for (int rb = 0; rb < RB; rb++) d[u][rb][0] = d[u][rb][1] = e[u][rb][0] = e[u][rb][1] = 0.0;
+#pragma unroll
+            for (int p = 0; p < NPAIR; p++) {
+                const double2 bp[2] = {b[0][p], b[1][p]};
+                double2 a[RB];
+#pragma unroll
+                for (int rb = 0; rb < RB; rb++) a[rb] = Ak[(p * RB + rb) * 32];
+#pragma unroll
+                for (int u = 0; u < 2; u++)
+#pragma unroll
+                    for (int rb = 0; rb < RB; rb++) dmma2(d[u][rb][0], d[u][rb][1], a[rb].x, bp[u].x);
+#pragma unroll
+                for (int u = 0; u < 2; u++)
+#pragma unroll
+                    for (int rb = 0; rb < RB; rb++) dmma2(e[u][rb][0], e[u][rb][1], a[rb].y, bp[u].y);
+            }
+            if (SINGLE) {
+#pragma unroll
+                for (int u = 0; u < 2; u++)
+#pragma unroll
+                    for (int rb = 0; rb < RB; rb++) dmma2(d[u][rb][0], d[u][rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs[u]);
+            }
+#pragma unroll
+            for (int u = 0; u < 2; u++) {
+#pragma unroll
+                for (int rb = 0; rb < RB; rb++) { d[u][rb][0] += e[u][rb][0]; d[u][rb][1] += e[u][rb][1]; }
+                store_unit(k, t0 + 4 * u, d[u]);
+            }
+        } else {
+            double d[RB][2], e[RB][2];
+#pragma unroll
+            for (int rb = 0; rb < RB; rb++) d[rb][0] = d[rb][1] = e[rb][0] = e[rb][1] = 0.0;
+#pragma unroll
+            for (int p = 0; p < NPAIR; p++) {
+                const double2 bp = b[0][p];
+                double2 a[RB];
+#pragma unroll
+                for (int rb = 0; rb < RB; rb++) a[rb] = Ak[(p * RB + rb) * 32];
+#pragma unroll
+                for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], a[rb].x, bp.x);
+#pragma unroll
+                for (int rb = 0; rb < RB; rb++) dmma2(e[rb][0], e[rb][1], a[rb].y, bp.y);
+            }
+            if (SINGLE) {
+#pragma unroll
+                for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs[0]);
+            }
+#pragma unroll
+            for (int rb = 0; rb < RB; rb++) { d[rb][0] += e[rb][0]; d[rb][1] += e[rb][1]; }
+            store_unit(k, t0, d);
+        }
+    };
+    double2 bA[2][NPAIR], bB[2][NPAIR];
+    double sA[2] = {0.0, 0.0}, sB[2] = {0.0, 0.0};
+    int j = 0;
+    if (j < nitems) load_b(j, bA, sA);
+    while (j < nitems) {
+        if (j + 1 < nitems) load_b(j + 1, bB, sB);
+        compute(j, bA, sA);
+        j++;
+        if (j >= nitems) break;
+        if (j + 1 < nitems) load_b(j + 1, bA, sA);
+        compute(j, bB, sB);
+        j++;
+    }
+}
+
+template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+__global__ void __launch_bounds__(F3_THREADS, 1)
+lnl_fused3_kernel(LnlParams P, int N, int ntiles_total, int quad, const double* __restrict__ rec, const double2* __restrict__ ytile,
+                  const int* __restrict__ perm, double* __restrict__ lnL) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    Fused3Smem<K>& cta = *reinterpret_cast<Fused3Smem<K>*>(smem_raw);
+    const int wg = threadIdx.x >> 7;
+    if (wg == 0) {
+        // ---------------- contraction warps
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(F3_MREGS));
+        const int mw = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        int alive = 3, slot = 0;
+        while (alive) {
+            if (alive & (1 << slot)) {
+#ifdef F2_TIMERS
+                long long tmark = clock64();
+#endif
+                named_sync(F3_BAR_EMPTY + slot, 128 + F2_THREADS);
+                F2_T(7);
+                const volatile F3Cmd* cm = &cta.cmd[slot];
+                if (!cm->go) {
+                    alive &= ~(1 << slot);
+                } else {
+                    int base[3];
+#pragma unroll
+                    for (int k = 0; k < K; k++) base[k] = cm->base[k];
+                    contract_phase<K, NPAIR, SINGLE>(cta.slot[slot], P, cm->c_lo, cm->ntiles, base, mw, lane);
+                    __threadfence_block();
+                    named_arrive(F3_BAR_FULL + slot, 128 + F2_THREADS);
+                }
+            }
+            slot ^= 1;
+        }
+    } else {
+        // ---------------- epilogue groups: slot 0 = warpgroups 1-2, slot 1 = warpgroups 3-4
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(F3_EREGS));
+        const int slot = (wg - 1) >> 1;
+        const int tid = threadIdx.x - 128 - slot * F2_THREADS;
+        for (int tile = 2 * blockIdx.x + slot; tile < ntiles_total; tile += 2 * gridDim.x) {
+            named_sync(F3_BAR_GROUP + slot, F2_THREADS);   // the previous tile's finalisation is done with this slot's memory
+            tile_body<1, K, NPAIR, SINGLE, TABLE, STRIDE1>(cta.slot[slot], &cta.cmd[slot], slot, tid, tile, P, N, quad, rec, ytile, perm, lnL);
+        }
+        if (tid == 0) cta.cmd[slot].go = 0;
+        __threadfence_block();
+        named_arrive(F3_BAR_EMPTY + slot, 128 + F2_THREADS);
+    }
+}
+
+template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+static int launch_fused3_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
+    static bool configured = false;
+    const int smem = (int)sizeof(Fused3Smem<K>);
+    if (!configured) {
+        ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused3_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        configured = true;
+    }
+    const int tiles = (N + F2_TS - 1) / F2_TS;
+    int grid = (tiles + 1) / 2;
+    if (grid > ctx->sm_count) grid = ctx->sm_count;
+    const int slot = ile_timing_begin(ctx);
+    lnl_fused3_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1><<<grid, F3_THREADS, smem, ctx->stream>>>(P, N, tiles, quad ? 1 : 0, rec, yt, perm, lnL);
+    ile_timing_end(ctx, slot);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}
+
+template <int K, int NPAIR, bool SINGLE>
+static int launch_fused3_k(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
+    const bool tb = P.use_table != 0, s1 = P.stride == 1;
+    if (tb) return s1 ? launch_fused3_t<K, NPAIR, SINGLE, true, true>(ctx, P, N, rec, yt, perm, lnL, quad)
+                      : launch_fused3_t<K, NPAIR, SINGLE, true, false>(ctx, P, N, rec, yt, perm, lnL, quad);
+    return s1 ? launch_fused3_t<K, NPAIR, SINGLE, false, true>(ctx, P, N, rec, yt, perm, lnL, quad)
+              : launch_fused3_t<K, NPAIR, SINGLE, false, false>(ctx, P, N, rec, yt, perm, lnL, quad);
+}
+
+int ile_launch_fused3(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
+    const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
+    if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4) return launch_fused3_k<3, 5, true>(ctx, P, N, rec, yt, perm, lnL, quad);
+    if (P.K == 2 && np == 1 && rem >= 1 && rem <= 4) return launch_fused3_k<2, 1, true>(ctx, P, N, rec, yt, perm, lnL, quad);
+    return 1;
+}
