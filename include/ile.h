@@ -158,7 +158,8 @@ int ile_lnL(ile_ctx *ctx, int p, int N, const double *ra, const double *dec, con
  * (optional) receives ln p(z).  ile_set_lnL_variant: 0 = default (samples ordered by delay cell
  * on the device, then the fused DMMA kernel), 1 = plain one-thread-per-sample kernel (in-library
  * cross-check), 2 = fused kernel without the delay-cell ordering, 3 = first-generation fused kernel,
- * 4 = default fused kernel behind the one-thread-per-sample preparation kernel. */
+ * 4 = default fused kernel behind the one-thread-per-sample preparation kernel (which then also
+ * computes the quadratic term), 5 = warp-specialised persistent fused kernel (experimental, slower). */
 int ile_lnL_z(ile_ctx *ctx, int p, int N, int d, const double *z /*[d][N]*/, double *lnL /*[N]*/,
               double *ln_prior /*[N] or NULL*/);
 int ile_set_lnL_variant(ile_ctx *ctx, int variant);

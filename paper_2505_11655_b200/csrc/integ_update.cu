@@ -495,41 +495,70 @@ __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g
     return mx;
 }
 
-__global__ void __launch_bounds__(256) gmm_accum_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ lnw,
-                                                        const UpdScratch* __restrict__ us, double* __restrict__ part) {
+// E step: a[c][i] = responsibility of component c for sample i times its importance weight
+// (0 for samples outside the box or with a non-finite weight); one evaluation of the mixture per sample
+__global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ lnw,
+                                                       const UpdScratch* __restrict__ us, double* __restrict__ aw) {
     if (us->abort || us->n_valid == 0) return;
-    const int d = I.d, C = I.n_gmm, comp = blockIdx.y;
-    const int nacc = 1 + d + d * (d + 1) / 2;
+    const int d = I.d, C = I.n_gmm;
     const double* g = I.mem[a].gmm;
-    const double* mu = g + C + comp * d;
     const double m = double_from_ord(us->m_ord);
-    double acc[GMM_NACC_MAX];
-    for (int q = 0; q < GMM_NACC_MAX; q++) acc[q] = 0.0;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         const double w = lnw[i];
-        if (!is_finite_d(w) || !in_box_dev(I, z, N, i)) continue;
+        const bool ok = is_finite_d(w) && in_box_dev(I, z, N, i);
         double zz[ILE_MAX_D], e[16];
         for (int c = 0; c < d; c++) zz[c] = z[(long long)c * N + i];
-        const double mx = ln_comp_all(I, g, zz, e);
-        double sum = 0.0;
-        for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
-        const double aw = exp(e[comp] - mx) / sum * exp(w - m);
-        acc[0] += aw;
-        int q = 1 + d;
-        for (int r = 0; r < d; r++) {
-            const double dr = zz[r] - mu[r];
-            acc[1 + r] += aw * dr;
-            for (int s = 0; s <= r; s++) acc[q++] += aw * dr * (zz[s] - mu[s]);
+        double mx = 0.0, sum = 1.0;
+        if (ok) {
+            mx = ln_comp_all(I, g, zz, e);
+            sum = 0.0;
+            for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
+        }
+        const double wt = ok ? exp(w - m) : 0.0;
+        for (int c = 0; c < C; c++) aw[(long long)c * N + i] = ok ? exp(e[c] - mx) / sum * wt : 0.0;
+    }
+}
+
+// M-step moments of component blockIdx.y about its old mean: s0, s1[D], s2[D(D+1)/2] (registers)
+template <int D>
+__global__ void __launch_bounds__(256) gmm_moments_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ aw,
+                                                          const UpdScratch* __restrict__ us, double* __restrict__ part) {
+    if (us->abort || us->n_valid == 0) return;
+    constexpr int NACC = 1 + D + D * (D + 1) / 2;
+    const int C = I.n_gmm, comp = blockIdx.y;
+    const double* mu = I.mem[a].gmm + C + comp * D;
+    double mu_r[D];
+#pragma unroll
+    for (int r = 0; r < D; r++) mu_r[r] = mu[r];
+    double acc[NACC];
+#pragma unroll
+    for (int q = 0; q < NACC; q++) acc[q] = 0.0;
+    const double* awc = aw + (long long)comp * N;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        const double wgt = awc[i];
+        if (wgt == 0.0) continue;
+        double dz[D];
+#pragma unroll
+        for (int r = 0; r < D; r++) dz[r] = z[(long long)r * N + i] - mu_r[r];
+        acc[0] += wgt;
+        int q = 1 + D;
+#pragma unroll
+        for (int r = 0; r < D; r++) {
+            const double t = wgt * dz[r];
+            acc[1 + r] += t;
+#pragma unroll
+            for (int s2 = 0; s2 <= r; s2++) acc[q++] += t * dz[s2];
         }
     }
     __shared__ double sh[8][GMM_NACC_MAX];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (int q = 0; q < nacc; q++) {
+#pragma unroll
+    for (int q = 0; q < NACC; q++) {
         const double v = warp_sum(acc[q]);
         if (lane == 0) sh[w][q] = v;
     }
     __syncthreads();
-    if (threadIdx.x < nacc) {
+    if (threadIdx.x < NACC) {
         double v = 0.0;
         for (int ww = 0; ww < 8; ww++) v += sh[ww][threadIdx.x];
         part[((size_t)comp * gridDim.x + blockIdx.x) * GMM_NACC_MAX + threadIdx.x] = v;
@@ -556,11 +585,18 @@ __global__ void gmm_finish_kernel(IntegDev I, int a, const UpdScratch* __restric
     double* Sigma = mu + C * d;
     double* L = Sigma + C * d * d;
     __shared__ double s0s[16];
+    __shared__ double tot_sh[16][GMM_NACC_MAX];
+    // thread (component, accumulator) sums its column of the per-block partials in block order
+    for (int e = threadIdx.x; e < C * nacc; e += blockDim.x) {
+        const int cc = e / nacc, q = e - cc * nacc;
+        double v = 0.0;
+        for (int b = 0; b < blocks; b++) v += part[((size_t)cc * blocks + b) * GMM_NACC_MAX + q];
+        tot_sh[cc][q] = v;
+    }
+    __syncthreads();
     double acc[GMM_NACC_MAX];
     if (c < C) {
-        for (int q = 0; q < nacc; q++) acc[q] = 0.0;
-        for (int b = 0; b < blocks; b++)
-            for (int q = 0; q < nacc; q++) acc[q] += part[((size_t)c * blocks + b) * GMM_NACC_MAX + q];
+        for (int q = 0; q < nacc; q++) acc[q] = tot_sh[c][q];
         s0s[c] = acc[0];
     }
     __syncthreads();
@@ -731,10 +767,16 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
             ILE_LAUNCH_CHECK(ctx);
             mask_max_kernel<<<grid, 256, 0, st>>>(I, N, z, lnw, nullptr, MASK_BOX, it->us);
             ILE_LAUNCH_CHECK(ctx);
-            dim3 g(it->gmm_blocks, I.n_gmm);
-            gmm_accum_kernel<<<g, 256, 0, st>>>(I, a, N, z, lnw, it->us, it->gmm_part);
+            gmm_resp_kernel<<<grid, 256, 0, st>>>(I, a, N, z, lnw, it->us, it->gmm_aw);
             ILE_LAUNCH_CHECK(ctx);
-            gmm_finish_kernel<<<1, 32, 0, st>>>(I, a, it->us, it->gmm_part, it->gmm_blocks);
+            dim3 g(it->gmm_blocks, I.n_gmm);
+            switch (I.d) {
+#define GMM_CASE(D) case D: gmm_moments_kernel<D><<<g, 256, 0, st>>>(I, a, N, z, it->gmm_aw, it->us, it->gmm_part); break;
+                GMM_CASE(1) GMM_CASE(2) GMM_CASE(3) GMM_CASE(4) GMM_CASE(5) GMM_CASE(6) GMM_CASE(7) GMM_CASE(8)
+#undef GMM_CASE
+            }
+            ILE_LAUNCH_CHECK(ctx);
+            gmm_finish_kernel<<<1, 256, 0, st>>>(I, a, it->us, it->gmm_part, it->gmm_blocks);
             ILE_LAUNCH_CHECK(ctx);
             return ILE_OK;
         }
