@@ -529,6 +529,7 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     const unsigned char* r = (const unsigned char*)buf;
     const unsigned char* end = r + bytes;
+    bool dry = true;                       // first pass validates the whole blob, second pass writes
     auto get_i64 = [&](long long* v) -> bool {
         if (r + 8 > end) return false;
         memcpy(v, r, 8);
@@ -537,7 +538,7 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
     };
     auto get_dev = [&](void* dst, size_t n) -> bool {
         if (r + n > end) return false;
-        if (n && cudaMemcpy(dst, r, n, cudaMemcpyHostToDevice) != cudaSuccess) return false;
+        if (!dry && n && cudaMemcpy(dst, r, n, cudaMemcpyHostToDevice) != cudaSuccess) return false;
         r += n;
         return true;
     };
@@ -558,10 +559,12 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
             memcpy(&s.L_thr, r, 8);
             r += 8;
             if (s.n < 1 || s.n > I.n_max || s.C < 1 || s.C > it->cap) return false;
-            if (cudaMemcpy(S.av, &s, sizeof(s), cudaMemcpyHostToDevice) != cudaSuccess) return false;
+            if (!dry && cudaMemcpy(S.av, &s, sizeof(s), cudaMemcpyHostToDevice) != cudaSuccess) return false;
             if (!get_dev(S.keys, (size_t)s.C * 8)) return false;
-            av_refresh_kernel<<<1, 32, 0, ctx->stream>>>(I, a);
-            ctx->launches++;
+            if (!dry) {
+                av_refresh_kernel<<<1, 32, 0, ctx->stream>>>(I, a);
+                ctx->launches++;
+            }
             return true;
         }
         if (S.kind == ILE_KIND_GMM) {
@@ -572,6 +575,9 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
         return true;
     };
     bool ok = true;
+  for (int pass = 0; pass < 2 && ok; pass++) {
+    dry = pass == 0;
+    r = (const unsigned char*)buf;
     if (I.kind == ILE_KIND_PORTFOLIO) {
         long long kind, d, Ns;
         ok = get_i64(&kind) && get_i64(&d) && get_i64(&Ns) && kind == ILE_KIND_PORTFOLIO && d == I.d && Ns == I.n_members;
@@ -587,7 +593,7 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
             long long off = 0;
             for (int a = 0; a < I.n_members; a++) { P.offset[a] = off; off += P.alloc[a]; }
             P.offset[I.n_members] = off;
-            ok = cudaMemcpy(I.port, &P, sizeof(P), cudaMemcpyHostToDevice) == cudaSuccess;
+            ok = dry || cudaMemcpy(I.port, &P, sizeof(P), cudaMemcpyHostToDevice) == cudaSuccess;
         }
         for (int a = 0; a < I.n_members && ok; a++) {
             long long nb;
@@ -596,6 +602,8 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
     } else {
         ok = get_member(0);
     }
+    if (ok && r != end) ok = false;        // trailing bytes: not a blob of this integrator
+  }
     if (!ok) {
         cudaGetLastError();
         return ile_fail(ctx, ILE_EINVAL, "integrator_set_state: blob does not match this integrator (kind, d, sizes) or is truncated");
