@@ -201,6 +201,16 @@ int ile_integrator_last_batch(ile_integrator *it, const double **z, const double
 int ile_integrator_get_state(ile_integrator *it, void *buf, size_t *bytes);
 int ile_integrator_set_state(ile_integrator *it, const void *buf, size_t bytes);
 
+/* ------------------------------------------------------------------ fair draws
+ * "fairly drawing some (fixed) number of extrinsic parameters from the
+ * underlying ILE Monte Carlo integral weighted samples".  M draws with replacement from N samples
+ * with log-weights lnw (device): probability of sample i = w_i / sum w.  mode 0 = systematic
+ * resampling (one uniform, equally spaced positions: every count within 1 of M w_i / sum w),
+ * 1 = independent draws.  Uniforms: Philox counter (0 or j, iter), key = seed.  idx (device,
+ * int64 [M]) receives the drawn sample indices, -1 everywhere if no weight is positive.  Exact:
+ * fixed-point weights rint(exp(ln w - max) 2^40) and integer prefix sums. */
+int ile_fair_draw(ile_ctx *ctx, int N, const double *lnw, int M, uint64_t seed, uint64_t iter, int mode, int64_t *idx);
+
 #ifdef __cplusplus
 }
 #endif

@@ -215,6 +215,13 @@ class Ile:
         self._ck(self.lib.ile_lnL_z(self.ctx, C.c_int(p), C.c_int(N), C.c_int(d), _ptr(z), _ptr(out), _ptr(lp)))
         return (out, lp) if want_prior else out
 
+    def fair_draw(self, lnw, M, seed, it, mode="systematic"):
+        """ile_fair_draw: int64 CUDA tensor [M] of sample indices drawn with probability w / sum w."""
+        idx = self.torch.empty(M, dtype=self.torch.int64, device=f"cuda:{self.device}")
+        self._ck(self.lib.ile_fair_draw(self.ctx, C.c_int(lnw.numel()), _ptr(lnw), C.c_int(M), C.c_uint64(int(seed) & 0xFFFFFFFFFFFFFFFF),
+                                        C.c_uint64(it), C.c_int(0 if mode == "systematic" else 1), _ptr(idx)))
+        return idx
+
     def reduce(self, lnw):
         res = self.torch.zeros(C.sizeof(Result), dtype=self.torch.uint8, device=f"cuda:{self.device}")
         self._ck(self.lib.ile_reduce(self.ctx, C.c_int(lnw.numel()), _ptr(lnw), _ptr(res)))

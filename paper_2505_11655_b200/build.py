@@ -20,7 +20,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "--expt-extended-lambda"]
 EXTRA = os.environ.get("ILE_NVCC_EXTRA", "").split()      # e.g. -DF2_G=2 for kernel experiments
-PER_FILE = {"integ_draw.cu": ["-fmad=false"], "integ_update.cu": ["-fmad=false"], "integ_api.cu": ["-fmad=false"]}
+PER_FILE = {"integ_draw.cu": ["-fmad=false"], "integ_update.cu": ["-fmad=false"], "integ_api.cu": ["-fmad=false"], "fairdraw.cu": ["-fmad=false"]}
 
 
 def sources():
