@@ -201,6 +201,25 @@ int ile_integrator_last_batch(ile_integrator *it, const double **z, const double
 int ile_integrator_get_state(ile_integrator *it, void *buf, size_t *bytes);
 int ile_integrator_set_state(ile_integrator *it, const void *buf, size_t bytes);
 
+/* ------------------------------------------------------------------ built-in test integrands
+ * The paper's integrator test problems evaluated on the device, so that a whole AC / AV / portfolio
+ * loop runs with no host round-trip on something with a known integral:
+ *   ILE_F_GAUSSIAN_MIX  ln f = ln sum_c exp(ln_amp_c - |z - c_c|^2 / (2 sigma_c^2)), n_comp <= 4
+ *                       (Fig. 6: two components, sigma = sqrt 2, centres (+-4, 0, 0));
+ *                       par = per component { centre[ILE_MAX_D], sigma, ln_amp }
+ *   ILE_F_ROSENBROCK    ln f = -sum_i [ (a - z_i)^2 + b (z_{i+1} - z_i^2)^2 ] / T (Fig. 3);
+ *                       par = { a, b, T }
+ * The integral is over the integrator's box with unit prior density: ln w = ln f - ln p_s. */
+enum { ILE_F_GAUSSIAN_MIX = 0, ILE_F_ROSENBROCK = 1 };
+typedef struct {
+    int32_t kind, n_comp;
+    double par[4 * (ILE_MAX_D + 2)];
+} ile_integrand;
+/* One iteration on integrand *f (host struct, copied): draw, ln f, reduce into *out_dev, update.
+ * Works for any d in 1..ILE_MAX_D; needs no loaded problem.  ln f of the batch is left in the
+ * lnL buffer of ile_integrator_last_batch. */
+int ile_integrator_step_integrand(ile_integrator *it, const ile_integrand *f, int N, uint64_t iter, ile_result *out_dev);
+
 /* ------------------------------------------------------------------ fair draws
  * "fairly drawing some (fixed) number of extrinsic parameters from the
  * underlying ILE Monte Carlo integral weighted samples".  M draws with replacement from N samples

@@ -41,6 +41,29 @@ RESULT_DTYPE = np.dtype([("ln_integral", "f8"), ("rel_variance", "f8"), ("n_eff"
 assert RESULT_DTYPE.itemsize == C.sizeof(Result)
 
 
+class Integrand(C.Structure):
+    """ile_integrand (include/ile.h): built-in test integrands."""
+    _fields_ = [("kind", C.c_int32), ("n_comp", C.c_int32), ("par", C.c_double * (4 * (ILE_MAX_D + 2)))]
+
+    @classmethod
+    def gaussian_mix(cls, centers, sigmas, ln_amps):
+        f = cls()
+        f.kind, f.n_comp = 0, len(sigmas)
+        for c, (ctr, sg, la) in enumerate(zip(centers, sigmas, ln_amps)):
+            for k, v in enumerate(ctr):
+                f.par[c * (ILE_MAX_D + 2) + k] = float(v)
+            f.par[c * (ILE_MAX_D + 2) + ILE_MAX_D] = float(sg)
+            f.par[c * (ILE_MAX_D + 2) + ILE_MAX_D + 1] = float(la)
+        return f
+
+    @classmethod
+    def rosenbrock(cls, a=1.0, b=100.0, T=1.0):
+        f = cls()
+        f.kind, f.n_comp = 1, 0
+        f.par[0], f.par[1], f.par[2] = float(a), float(b), float(T)
+        return f
+
+
 class IntegratorOpts(C.Structure):
     _fields_ = [("kind", C.c_int32), ("d", C.c_int32), ("lo", C.c_double * ILE_MAX_D), ("hi", C.c_double * ILE_MAX_D),
                 ("seed", C.c_uint64), ("max_batch", C.c_int64), ("n_bins", C.c_int32), ("pad0", C.c_int32), ("eps", C.c_double),
@@ -378,6 +401,12 @@ class Integrator:
         """One iteration; returns the device result buffer (decode with result_from_device)."""
         out = self._results(1) if out is None else out
         self._ck(self.lib.ile_integrator_step(self.h, C.c_int(p), C.c_int(N), C.c_uint64(it), _ptr(out)))
+        return out
+
+    def step_integrand(self, f, N, it, out=None):
+        """One iteration on a built-in test integrand (Integrand.gaussian_mix / .rosenbrock)."""
+        out = self._results(1) if out is None else out
+        self._ck(self.lib.ile_integrator_step_integrand(self.h, C.byref(f), C.c_int(N), C.c_uint64(it), _ptr(out)))
         return out
 
     def run(self, p_first, p_count, n_iter, N, out=None):

@@ -402,6 +402,76 @@ static int step_internal(ile_integrator* it, int p, int N, uint64_t iter, ile_re
     return ILE_OK;
 }
 
+// ---------------------------------------------------------------- built-in test integrands
+__global__ void __launch_bounds__(256) integrand_kernel(IntegDev I, ile_integrand F, int N, const double* __restrict__ z,
+                                                        const double* __restrict__ ln_ps, double* __restrict__ lnf, double* __restrict__ lnw) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int d = I.d;
+    double zz[ILE_MAX_D];
+    bool inbox = true;
+    for (int c = 0; c < d; c++) {
+        zz[c] = z[(long long)c * N + i];
+        inbox = inbox && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
+    }
+    double v = neg_inf();
+    if (inbox) {
+        if (F.kind == ILE_F_GAUSSIAN_MIX) {
+            double e[4], mx = neg_inf();
+            for (int c = 0; c < F.n_comp; c++) {
+                const double* pc = F.par + c * (ILE_MAX_D + 2);
+                double r2 = 0.0;
+                for (int k = 0; k < d; k++) r2 = r2 + (zz[k] - pc[k]) * (zz[k] - pc[k]);
+                const double sg = pc[ILE_MAX_D];
+                e[c] = pc[ILE_MAX_D + 1] - 0.5 * r2 / (sg * sg);
+                mx = fmax(mx, e[c]);
+            }
+            double sum = 0.0;
+            for (int c = 0; c < F.n_comp; c++) sum += exp(e[c] - mx);
+            v = mx + log(sum);
+        } else {
+            const double a = F.par[0], b = F.par[1], T = F.par[2];
+            double sacc = 0.0;
+            for (int k = 0; k + 1 < d; k++) {
+                const double t1 = a - zz[k], t2 = zz[k + 1] - zz[k] * zz[k];
+                sacc = sacc + t1 * t1 + b * (t2 * t2);
+            }
+            v = -sacc / T;
+        }
+    }
+    lnf[i] = v;
+    lnw[i] = is_finite_d(v) ? v - ln_ps[i] : neg_inf();
+}
+
+extern "C" int ile_integrator_step_integrand(ile_integrator* it, const ile_integrand* f, int N, uint64_t iter, ile_result* out_dev) {
+    if (!it) return ILE_EINVAL;
+    ile_ctx* ctx = it->ctx;
+    int rc = check_N(it, N, "integrator_step_integrand");
+    if (rc) return rc;
+    if (!f || f->kind < 0 || f->kind > ILE_F_ROSENBROCK || (f->kind == ILE_F_GAUSSIAN_MIX && (f->n_comp < 1 || f->n_comp > 4)))
+        return ile_fail(ctx, ILE_EINVAL, "integrator_step_integrand: unknown integrand or n_comp outside 1..4");
+    if (f->kind == ILE_F_ROSENBROCK && (it->I.d < 2 || !(f->par[2] > 0.0)))
+        return ile_fail(ctx, ILE_EINVAL, "integrator_step_integrand: Rosenbrock needs d >= 2 and T > 0");
+    const IntegDev& I = it->I;
+    rc = integ_launch_draw(it, N, (unsigned int)iter, it->z, it->ln_ps);
+    if (rc) return rc;
+    it->drew = true;
+    it->last_N = N;
+    integrand_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(I, *f, N, it->z, it->ln_ps, it->lnL, it->lnw);
+    ILE_LAUNCH_CHECK(ctx);
+    rc = ile_launch_reduce(ctx, N, it->lnw, it->res, 1);
+    if (rc) return rc;
+    annotate_kernel<<<1, 32, 0, ctx->stream>>>(I, it->res, 1);
+    ILE_LAUNCH_CHECK(ctx);
+    const double* lp = (I.n_members == 1 && I.mem[0].kind == ILE_KIND_AV) ? nullptr : it->ln_ps;
+    rc = integ_launch_update(it, N, it->z, it->lnw, lp);
+    if (rc) return rc;
+    annotate_kernel<<<1, 32, 0, ctx->stream>>>(I, it->res, 0);
+    ILE_LAUNCH_CHECK(ctx);
+    if (out_dev) ILE_CUDA(ctx, cudaMemcpyAsync(out_dev, it->res, sizeof(ile_result), cudaMemcpyDeviceToDevice, ctx->stream));
+    return ILE_OK;
+}
+
 extern "C" int ile_integrator_step(ile_integrator* it, int p, int N, uint64_t iter, ile_result* out_dev) {
     if (!it) return ILE_EINVAL;
     int rc = check_N(it, N, "integrator_step");
