@@ -129,6 +129,16 @@ int ile_set_modes(ile_ctx *ctx, int M, const int *ell, const int *m);
 int ile_load_quv(ile_ctx *ctx, int P, int N_Q, double fs, double t_Q0,
                  const double *Q /*[P][K][M][N_Q][2]*/, const double *U /*[P][K][M][M][2]*/,
                  const double *V /*[P][K][M][M][2]*/, double D_ref, int src_is_device);
+/* SURVEY 8(f) #1; the same Q, U, V computed on the device from
+ * frequency-domain inputs (device pointers, numpy FFT bin order f_j = j df, j <= N_f/2, else
+ * (j - N_f) df): h [P][M][N_f][2] mode spectra, d [K][N_f][2] data spectra, S [K][N_f/2+1]
+ * one-sided PSDs over |f|; <a|b>_k = 2 sum_{|f| > f_low} df a*(f) b(f) / S_k(|f|).  fs = N_f df;
+ * the stored window is t_n = t_Q0 + n / fs, n < N_Q (t_Q0 fs must be an integer).  Installs the
+ * result like ile_load_quv (synchronises).  ile_get_quv copies point p back to host arrays in
+ * ile_load_quv's layout (any of Q, U, V may be NULL). */
+int ile_precompute_quv(ile_ctx *ctx, int P, int N_f, double df, double f_low, const double *h, const double *d,
+                       const double *S, double t_Q0, int N_Q, double D_ref);
+int ile_get_quv(ile_ctx *ctx, int p, double *Q, double *U, double *V);
 /* Geocentric time grid t_j = t_lo + j dt, j < N_t, marginalised with a uniform prior
  * (PAPER.md:94, 547).  dt * fs must be a positive integer (native-spaced grid).  interp: 1 =
  * linear interpolation of Q between stored bins, 0 = nearest bin.  ILE_ERANGE unless

@@ -154,6 +154,19 @@ class Ile:
         self._ck(self.lib.ile_load_quv(self.ctx, C.c_int(Q.shape[0]), C.c_int(Q.shape[3]), C.c_double(fs), C.c_double(t_Q0),
                                        pQ, pU, pV, C.c_double(D_ref), C.c_int(0)))
 
+    def precompute_quv(self, h, d, S, df, f_low, t_Q0, N_Q, D_ref):
+        """ile_precompute_quv from CUDA tensors: h [P,M,N_f] complex128, d [K,N_f] complex128, S [K,N_f/2+1] float64."""
+        P, M, N_f = h.shape
+        self._ck(self.lib.ile_precompute_quv(self.ctx, C.c_int(P), C.c_int(N_f), C.c_double(df), C.c_double(f_low), _ptr(h), _ptr(d), _ptr(S),
+                                             C.c_double(t_Q0), C.c_int(N_Q), C.c_double(D_ref)))
+
+    def get_quv(self, p, K, M, N_Q):
+        Q = np.empty((K, M, N_Q), dtype=np.complex128)
+        U = np.empty((K, M, M), dtype=np.complex128)
+        V = np.empty((K, M, M), dtype=np.complex128)
+        self._ck(self.lib.ile_get_quv(self.ctx, C.c_int(p), Q.ctypes.data_as(C.c_void_p), U.ctypes.data_as(C.c_void_p), V.ctypes.data_as(C.c_void_p)))
+        return Q, U, V
+
     def set_time_grid(self, t_lo, dt, N_t, interp=1):
         self._ck(self.lib.ile_set_time_grid(self.ctx, C.c_double(t_lo), C.c_double(dt), C.c_int(N_t), C.c_int(interp)))
 

@@ -1,0 +1,163 @@
+// libile: the inner products Q, U, V of Eq. (6a-c) on the device (PAPER.md:78-87,
+// 337-345: "GPU-optimized ... overlaps for U, V, Q" is the paper's own wish).
+//   w_k[j]      = 2 df / S_k(|f_j|) for |f_j| > f_low, else 0            (numpy FFT bin order)
+//   U_k[a][b]   = sum_j w_k[j] conj(h_a[j]) h_b[j]                        (6b)
+//   V_k[a][b]   = sum_j w_k[j] h_a[-j] h_b[j]                             (6c)
+//   Q_k[a][n]   = sum_j w_k[j] conj(h_a[j]) d_k[j] exp(2 pi i j (n + n0) / N_f)   (6a), t_n = (n0 + n) / fs
+// First version: plain FP64 kernels that follow the definition (one block per matrix entry; one
+// thread per output time with the twiddle advanced by complex rotation and re-seeded from an exact
+// table every 32 bins).  The result is installed through ile_load_quv (symmetry check, repack).
+#include "common.cuh"
+
+#define PC_THREADS 256
+#define PC_RESEED 32
+
+__global__ void pc_weight_kernel(int K, int N_f, double df, double f_low, const double* __restrict__ S, double* __restrict__ w) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
+    if (j >= N_f) return;
+    const int ja = j <= N_f / 2 ? j : N_f - j;
+    const double f = (double)ja * df;
+    w[(size_t)k * N_f + j] = f > f_low ? 2.0 * df / S[(size_t)k * (N_f / 2 + 1) + ja] : 0.0;
+}
+
+__global__ void pc_twiddle_kernel(int N_f, double2* __restrict__ W) {
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= N_f) return;
+    double s, c;
+    sincospi(2.0 * (double)m / (double)N_f, &s, &c);
+    W[m] = make_double2(c, s);
+}
+
+// grid (M*M, K, P): U and V entry (a, b) of detector k, point p
+__global__ void __launch_bounds__(PC_THREADS) pc_uv_kernel(int M, int N_f, const double2* __restrict__ h, const double* __restrict__ w,
+                                                           double2* __restrict__ U, double2* __restrict__ V) {
+    const int a = blockIdx.x / M, b = blockIdx.x % M, k = blockIdx.y, p = blockIdx.z, K = gridDim.y;
+    const double2* ha = h + ((size_t)p * M + a) * N_f;
+    const double2* hb = h + ((size_t)p * M + b) * N_f;
+    const double* wk = w + (size_t)k * N_f;
+    double ur = 0.0, ui = 0.0, vr = 0.0, vi = 0.0;
+    for (int j = threadIdx.x; j < N_f; j += PC_THREADS) {
+        const double wj = wk[j];
+        if (wj == 0.0) continue;
+        const double2 x = ha[j], y = hb[j], xm = ha[j == 0 ? 0 : N_f - j];
+        ur += wj * (x.x * y.x + x.y * y.y);           // conj(x) y
+        ui += wj * (x.x * y.y - x.y * y.x);
+        vr += wj * (xm.x * y.x - xm.y * y.y);         // x(-f) y
+        vi += wj * (xm.x * y.y + xm.y * y.x);
+    }
+    __shared__ double sh[4][PC_THREADS / 32];
+    ur = warp_sum(ur); ui = warp_sum(ui); vr = warp_sum(vr); vi = warp_sum(vi);
+    if ((threadIdx.x & 31) == 0) {
+        const int wi = threadIdx.x >> 5;
+        sh[0][wi] = ur; sh[1][wi] = ui; sh[2][wi] = vr; sh[3][wi] = vi;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int q = 0; q < PC_THREADS / 32; q++)
+            for (int e = 0; e < 4; e++) t[e] += sh[e][q];
+        const size_t o = (((size_t)p * K + k) * M + a) * M + b;
+        U[o] = make_double2(t[0], t[1]);
+        V[o] = make_double2(t[2], t[3]);
+    }
+}
+
+// x_{k,a}[j] = w_k[j] conj(h_a[j]) d_k[j]  (shared by all output times)
+__global__ void pc_prod_kernel(int M, int K, int N_f, const double2* __restrict__ h, const double2* __restrict__ d, const double* __restrict__ w,
+                               double2* __restrict__ x) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, ka = blockIdx.y, p = blockIdx.z;
+    if (j >= N_f) return;
+    const int k = ka / M, a = ka % M;
+    const double wj = w[(size_t)k * N_f + j];
+    const double2 hh = h[((size_t)p * M + a) * N_f + j], dd = d[(size_t)k * N_f + j];
+    x[((size_t)p * K * M + ka) * N_f + j] = make_double2(wj * (hh.x * dd.x + hh.y * dd.y), wj * (hh.x * dd.y - hh.y * dd.x));
+}
+
+// grid (ceil(N_Q / 128), K*M, P): thread = output time n; Q[n] = sum_j x[j] W^{j (n + n0)}
+__global__ void __launch_bounds__(128) pc_q_kernel(int N_f, int N_Q, int n0, const double2* __restrict__ x, const double2* __restrict__ W,
+                                                   const double* __restrict__ w, int M, double2* __restrict__ Q) {
+    __shared__ double2 xs[PC_RESEED * 8];
+    const int n = blockIdx.x * 128 + threadIdx.x, ka = blockIdx.y, p = blockIdx.z, KM = gridDim.y;
+    const double2* xp = x + ((size_t)p * KM + ka) * N_f;
+    long long step = ((long long)n + n0) % N_f;
+    if (step < 0) step += N_f;
+    const double2 rot = W[step];
+    double qr = 0.0, qi = 0.0;
+    for (int j0 = 0; j0 < N_f; j0 += PC_RESEED * 8) {
+        __syncthreads();
+        for (int q = threadIdx.x; q < PC_RESEED * 8; q += 128) xs[q] = j0 + q < N_f ? xp[j0 + q] : make_double2(0.0, 0.0);
+        __syncthreads();
+#pragma unroll 1
+        for (int g = 0; g < 8; g++) {
+            const int jb = j0 + g * PC_RESEED;
+            if (jb >= N_f) break;
+            double2 tw = W[(int)(((long long)jb * step) % N_f)];       // exact re-seed
+#pragma unroll
+            for (int q = 0; q < PC_RESEED; q++) {
+                const double2 v = xs[g * PC_RESEED + q];
+                qr += v.x * tw.x - v.y * tw.y;
+                qi += v.x * tw.y + v.y * tw.x;
+                const double tr = tw.x * rot.x - tw.y * rot.y;
+                tw.y = tw.x * rot.y + tw.y * rot.x;
+                tw.x = tr;
+            }
+        }
+    }
+    if (n < N_Q) Q[((size_t)p * KM + ka) * N_Q + n] = make_double2(qr, qi);
+}
+
+// Eq. (6a-c) for P intrinsic points from frequency-domain inputs (device pointers, numpy FFT bin
+// order): h [P][M][N_f][2] mode spectra, d [K][N_f][2] data spectra, S [K][N_f/2+1] one-sided PSDs
+// over |f|.  fs = N_f df; the stored window starts at t_Q0 (t_Q0 fs must be an integer) and has N_Q
+// bins.  The result replaces the context's Q/U/V exactly as ile_load_quv would.
+extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, double f_low, const double* h, const double* d, const double* S,
+                                  double t_Q0, int N_Q, double D_ref) {
+    if (!ctx) return ILE_EINVAL;
+    if (!ctx->have_net || !ctx->have_modes) return ile_fail(ctx, ILE_ESTATE, "precompute_quv: set_network and set_modes first");
+    if (P < 1 || N_f < 8 || (N_f & 1) || !(df > 0) || !h || !d || !S || N_Q < 4 || N_Q > N_f || !(D_ref > 0))
+        return ile_fail(ctx, ILE_EINVAL, "precompute_quv: bad argument");
+    const double fs = (double)N_f * df;
+    const double n0d = t_Q0 * fs;
+    const long long n0 = llrint(n0d);
+    if (fabs(n0d - (double)n0) > 1e-6) return ile_fail(ctx, ILE_EINVAL, "precompute_quv: t_Q0 * fs = %.9g is not an integer", n0d);
+    const int K = ctx->K, M = ctx->M;
+    const size_t nQ = (size_t)P * K * M * N_Q, nU = (size_t)P * K * M * M, nX = (size_t)P * K * M * N_f;
+    double *w = nullptr;
+    double2 *W = nullptr, *x = nullptr, *Q = nullptr, *U = nullptr, *V = nullptr;
+    auto cleanup = [&]() { cudaFree(w); cudaFree(W); cudaFree(x); cudaFree(Q); cudaFree(U); cudaFree(V); };
+    if (cudaMalloc(&w, (size_t)K * N_f * 8) != cudaSuccess || cudaMalloc(&W, (size_t)N_f * 16) != cudaSuccess ||
+        cudaMalloc(&x, nX * 16) != cudaSuccess || cudaMalloc(&Q, nQ * 16) != cudaSuccess || cudaMalloc(&U, nU * 16) != cudaSuccess ||
+        cudaMalloc(&V, nU * 16) != cudaSuccess) {
+        cudaGetLastError();
+        cleanup();
+        return ile_fail(ctx, ILE_ENOMEM, "precompute_quv: device allocation failed");
+    }
+    cudaStream_t st = ctx->stream;
+    pc_weight_kernel<<<dim3((N_f + 255) / 256, K), 256, 0, st>>>(K, N_f, df, f_low, S, w);
+    pc_twiddle_kernel<<<(N_f + 255) / 256, 256, 0, st>>>(N_f, W);
+    pc_uv_kernel<<<dim3(M * M, K, P), PC_THREADS, 0, st>>>(M, N_f, (const double2*)h, w, U, V);
+    pc_prod_kernel<<<dim3((N_f + 255) / 256, K * M, P), 256, 0, st>>>(M, K, N_f, (const double2*)h, (const double2*)d, w, x);
+    pc_q_kernel<<<dim3((N_Q + 127) / 128, K * M, P), 128, 0, st>>>(N_f, N_Q, (int)n0, x, W, w, M, Q);
+    ctx->launches += 5;
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        cleanup();
+        return ile_fail(ctx, ILE_ECUDA, "precompute_quv: %s", cudaGetErrorString(e));
+    }
+    const int rc = ile_load_quv(ctx, P, N_Q, fs, (double)n0 / fs, (const double*)Q, (const double*)U, (const double*)V, D_ref, 1);
+    cleanup();
+    return rc;
+}
+
+// Copies the resident Q/U/V of intrinsic point p to host arrays (caller layout of ile_load_quv).
+extern "C" int ile_get_quv(ile_ctx* ctx, int p, double* Q, double* U, double* V) {
+    if (!ctx) return ILE_EINVAL;
+    if (!ctx->have_quv) return ile_fail(ctx, ILE_ESTATE, "get_quv: nothing loaded");
+    if (p < 0 || p >= ctx->P) return ile_fail(ctx, ILE_EINVAL, "get_quv: point out of range");
+    const size_t nQ = (size_t)ctx->K * ctx->M * ctx->N_Q * 2, nU = (size_t)ctx->K * ctx->M * ctx->M * 2;
+    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (Q) ILE_CUDA(ctx, cudaMemcpy(Q, ctx->d_Qc + (size_t)p * nQ, nQ * 8, cudaMemcpyDeviceToHost));
+    if (U) ILE_CUDA(ctx, cudaMemcpy(U, ctx->d_U + (size_t)p * nU, nU * 8, cudaMemcpyDeviceToHost));
+    if (V) ILE_CUDA(ctx, cudaMemcpy(V, ctx->d_V + (size_t)p * nU, nU * 8, cudaMemcpyDeviceToHost));
+    return ILE_OK;
+}
