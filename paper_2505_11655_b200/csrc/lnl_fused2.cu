@@ -48,6 +48,7 @@ struct Fused2Smem {
     int part[F2_TS];
     int done[F2_TS];
     int n_part, n_left;
+    double etab[64];                         // 2^(j/64), the table of exp_tab
 };
 
 __device__ __forceinline__ void dmma2(double& d0, double& d1, double a, double b) {
@@ -75,6 +76,43 @@ __device__ __forceinline__ double exp_small(double d) {
     p = fma(p, r, 1.0);
     p = fma(p, r, 1.0);
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// 2^(j/64), j = 0..63, correctly rounded
+__device__ const double f2_exp2_tab[64] = {
+    0x1.0000000000000p+0, 0x1.02c9a3e778061p+0, 0x1.059b0d3158574p+0, 0x1.0874518759bc8p+0,
+    0x1.0b5586cf9890fp+0, 0x1.0e3ec32d3d1a2p+0, 0x1.11301d0125b51p+0, 0x1.1429aaea92de0p+0,
+    0x1.172b83c7d517bp+0, 0x1.1a35beb6fcb75p+0, 0x1.1d4873168b9aap+0, 0x1.2063b88628cd6p+0,
+    0x1.2387a6e756238p+0, 0x1.26b4565e27cddp+0, 0x1.29e9df51fdee1p+0, 0x1.2d285a6e4030bp+0,
+    0x1.306fe0a31b715p+0, 0x1.33c08b26416ffp+0, 0x1.371a7373aa9cbp+0, 0x1.3a7db34e59ff7p+0,
+    0x1.3dea64c123422p+0, 0x1.4160a21f72e2ap+0, 0x1.44e086061892dp+0, 0x1.486a2b5c13cd0p+0,
+    0x1.4bfdad5362a27p+0, 0x1.4f9b2769d2ca7p+0, 0x1.5342b569d4f82p+0, 0x1.56f4736b527dap+0,
+    0x1.5ab07dd485429p+0, 0x1.5e76f15ad2148p+0, 0x1.6247eb03a5585p+0, 0x1.6623882552225p+0,
+    0x1.6a09e667f3bcdp+0, 0x1.6dfb23c651a2fp+0, 0x1.71f75e8ec5f74p+0, 0x1.75feb564267c9p+0,
+    0x1.7a11473eb0187p+0, 0x1.7e2f336cf4e62p+0, 0x1.82589994cce13p+0, 0x1.868d99b4492edp+0,
+    0x1.8ace5422aa0dbp+0, 0x1.8f1ae99157736p+0, 0x1.93737b0cdc5e5p+0, 0x1.97d829fde4e50p+0,
+    0x1.9c49182a3f090p+0, 0x1.a0c667b5de565p+0, 0x1.a5503b23e255dp+0, 0x1.a9e6b5579fdbfp+0,
+    0x1.ae89f995ad3adp+0, 0x1.b33a2b84f15fbp+0, 0x1.b7f76f2fb5e47p+0, 0x1.bcc1e904bc1d2p+0,
+    0x1.c199bdd85529cp+0, 0x1.c67f12e57d14bp+0, 0x1.cb720dcef9069p+0, 0x1.d072d4a07897cp+0,
+    0x1.d5818dcfba487p+0, 0x1.da9e603db3285p+0, 0x1.dfc97337b9b5fp+0, 0x1.e502ee78b3ff6p+0,
+    0x1.ea4afa2a490dap+0, 0x1.efa1bee615a27p+0, 0x1.f50765b6e4540p+0, 0x1.fa7c1819e90d8p+0,
+};
+
+// exp(d) for d in [-40, 31] in 8 FP64 instructions: k = rint(64 d / ln2) by the magic-number add,
+// r = d - k ln2/64 (|r| <= 0.00542; the rounding of ln2/64 costs < 3e-15 for |d| <= 40),
+// exp(d) = 2^(k >> 6) tab[k & 63] (1 + r (1 + r/2 + r^2/6 + r^3/24)): truncation r^5/120 < 4e-14 relative.
+// tab = the shared-memory copy of f2_exp2_tab.
+__device__ __forceinline__ double exp_tab(double d, const double* __restrict__ tab) {
+    const double t = fma(d, 0x1.71547652b82fep+6, 6755399441055744.0);
+    const int k = __double2loint(t);
+    const double kf = t - 6755399441055744.0;
+    const double r = fma(kf, -0x1.62e42fefa39efp-7, d);
+    const double T = tab[k & 63];
+    double p = fma(r, 1.0 / 24.0, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    const double e = fma(T * r, p, T);
+    return __hiloint2double(__double2hiint(e) + ((k >> 6) << 20), __double2loint(e));
 }
 
 #ifdef F2_TIMERS
@@ -190,6 +228,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         const double* src = rec + (size_t)tile * TS * F2_REC;
         for (int q = tid; q < TS * F2_REC; q += F2_THREADS) (&sm.rec[0][0])[q] = src[q];
         if (tid < 4) sm.base[tid] = 0x7ffffffe;
+        if (tid >= 64 && tid < 128) sm.etab[tid - 64] = f2_exp2_tab[tid - 64];
         // the tile's harmonics Y[m][s] (12 KB) are staged in the S ring, which is idle until phase 0
         const double2* ysrc = ytile + (size_t)tile * F2_YM * 32;
         for (int q = tid; q < F2_YM * 32; q += F2_THREADS) ysm[q] = ysrc[q];
@@ -509,7 +548,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                         // terms below e^-40 of the reference are dropped: dl <= -40 <=> high word >= 0xC0440000
                         const bool keep = (unsigned)__double2hiint(dl[i][gi]) < 0xC0440000u;
                         const double da = __hiloint2double(keep ? __double2hiint(dl[i][gi]) : (int)0xC0440000, keep ? __double2loint(dl[i][gi]) : 0);
-                        const double e = exp_small(da);
+                        const double e = exp_tab(da, sm.etab);
                         run_s[i] += __hiloint2double(keep ? __double2hiint(e) : 0, keep ? __double2loint(e) : 0);
                     }
             }

@@ -4,9 +4,10 @@
 //   U_k[a][b]   = sum_j w_k[j] conj(h_a[j]) h_b[j]                        (6b)
 //   V_k[a][b]   = sum_j w_k[j] h_a[-j] h_b[j]                             (6c)
 //   Q_k[a][n]   = sum_j w_k[j] conj(h_a[j]) d_k[j] exp(2 pi i j (n + n0) / N_f)   (6a), t_n = (n0 + n) / fs
-// First version: plain FP64 kernels that follow the definition (one block per matrix entry; one
-// thread per output time with the twiddle advanced by complex rotation and re-seeded from an exact
-// table every 32 bins).  The result is installed through ile_load_quv (symmetry check, repack).
+// U, V: one block per matrix entry, by the definition.  Q: for power-of-two N_f <= 2^18 a four-step
+// inverse FFT (column DFTs in registers, row FFTs in shared memory, only the stored window written);
+// otherwise the definition (one thread per output time, twiddle advanced by complex rotation and
+// re-seeded from an exact table every 32 bins).  Installed through ile_load_quv (symmetry check, repack).
 #include "common.cuh"
 
 #define PC_THREADS 256
@@ -106,6 +107,79 @@ __global__ void __launch_bounds__(128) pc_q_kernel(int N_f, int N_Q, int n0, con
     if (n < N_Q) Q[((size_t)p * KM + ka) * N_Q + n] = make_double2(qr, qi);
 }
 
+// ---------------------------------------------------------------- power-of-two N_f: four-step inverse FFT
+// N_f = N1 N2, j = j1 + N1 j2, n = n1 N2 + n2:
+//   W_N^{jn} = W_N1^{j1 n1} W_N^{j1 n2} W_N2^{j2 n2}
+// pc_fft_cols: thread = (series, j1): x[j1 + N1 j2] = w conj(h) d formed on the fly (coalesced over j1), the
+//   N2-point DFT over j2 by its definition, times the twiddle W_N^{j1 n2}           -> B[series][n2][j1]
+// pc_fft_rows: CTA = (n2, series): N1-point radix-2 decimation-in-frequency FFT in shared memory (natural
+//   order in, bit-reversed out), then only the outputs n = n1 N2 + n2 that fall in the stored window
+//   [n0, n0 + N_Q) are written.  Every twiddle is an exact entry of the sincospi table W.
+template <int N2>
+__global__ void __launch_bounds__(256) pc_fft_cols_kernel(int M, int K, int N_f, int N1, const double2* __restrict__ h,
+                                                          const double2* __restrict__ d, const double* __restrict__ w,
+                                                          const double2* __restrict__ W, double2* __restrict__ B) {
+    __shared__ double2 w2[N2];
+    const int j1 = blockIdx.x * 256 + threadIdx.x, ka = blockIdx.y, p = blockIdx.z;
+    const int k = ka / M, a = ka % M;
+    if (threadIdx.x < N2) w2[threadIdx.x] = W[(size_t)threadIdx.x * (N_f / N2)];
+    __syncthreads();
+    if (j1 >= N1) return;
+    double2 x[N2];
+#pragma unroll
+    for (int j2 = 0; j2 < N2; j2++) {
+        const int j = j1 + N1 * j2;
+        const double wj = w[(size_t)k * N_f + j];
+        const double2 hh = h[((size_t)p * M + a) * N_f + j], dd = d[(size_t)k * N_f + j];
+        x[j2] = make_double2(wj * (hh.x * dd.x + hh.y * dd.y), wj * (hh.x * dd.y - hh.y * dd.x));
+    }
+    double2* Bp = B + ((size_t)p * K * M + ka) * N_f;
+#pragma unroll 1
+    for (int n2 = 0; n2 < N2; n2++) {
+        double sr = 0.0, si = 0.0;
+#pragma unroll
+        for (int j2 = 0; j2 < N2; j2++) {
+            const double2 t = w2[(j2 * n2) & (N2 - 1)];
+            sr += x[j2].x * t.x - x[j2].y * t.y;
+            si += x[j2].x * t.y + x[j2].y * t.x;
+        }
+        const double2 t = W[(j1 * n2) & (N_f - 1)];
+        Bp[(size_t)n2 * N1 + j1] = make_double2(sr * t.x - si * t.y, sr * t.y + si * t.x);
+    }
+}
+
+__global__ void __launch_bounds__(256) pc_fft_rows_kernel(int N_f, int N1, int log2N1, int N2, int N_Q, int n0m, const double2* __restrict__ B,
+                                                          const double2* __restrict__ W, double2* __restrict__ Q) {
+    extern __shared__ double2 sm[];
+    const int n2 = blockIdx.x, s = blockIdx.y;
+    const double2* Bp = B + ((size_t)s * N2 + n2) * N1;
+    for (int i = threadIdx.x; i < N1; i += 256) sm[i] = Bp[i];
+    __syncthreads();
+    for (int half = N1 >> 1, tstride = N_f / N1; half >= 1; half >>= 1, tstride <<= 1) {
+        for (int t = threadIdx.x; t < (N1 >> 1); t += 256) {
+            const int pos = t & (half - 1), i = ((t - pos) << 1) + pos, j = i + half;
+            const double2 u = sm[i], v = sm[j], tw = W[(size_t)pos * tstride];
+            const double dr = u.x - v.x, di = u.y - v.y;
+            sm[i] = make_double2(u.x + v.x, u.y + v.y);
+            sm[j] = make_double2(dr * tw.x - di * tw.y, dr * tw.y + di * tw.x);
+        }
+        __syncthreads();
+    }
+    // window bins t with (n0m + t) mod N2 == n2
+    int t0 = (n2 - n0m) % N2;
+    if (t0 < 0) t0 += N2;
+    for (int t = t0 + threadIdx.x * N2; t < N_Q; t += 256 * N2) {
+        const int n = (n0m + t) & (N_f - 1), n1 = n / N2;
+        Q[(size_t)s * N_Q + t] = sm[__brev((unsigned)n1) >> (32 - log2N1)];
+    }
+}
+
+template <int N2>
+static void launch_fft_cols(int P, int M, int K, int N_f, int N1, const double2* h, const double2* d, const double* w, const double2* W, double2* B,
+                            cudaStream_t st) {
+    pc_fft_cols_kernel<N2><<<dim3((N1 + 255) / 256, K * M, P), 256, 0, st>>>(M, K, N_f, N1, h, d, w, W, B);
+}
+
 // Eq. (6a-c) for P intrinsic points from frequency-domain inputs (device pointers, numpy FFT bin
 // order): h [P][M][N_f][2] mode spectra, d [K][N_f][2] data spectra, S [K][N_f/2+1] one-sided PSDs
 // over |f|.  fs = N_f df; the stored window starts at t_Q0 (t_Q0 fs must be an integer) and has N_Q
@@ -136,8 +210,28 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     pc_weight_kernel<<<dim3((N_f + 255) / 256, K), 256, 0, st>>>(K, N_f, df, f_low, S, w);
     pc_twiddle_kernel<<<(N_f + 255) / 256, 256, 0, st>>>(N_f, W);
     pc_uv_kernel<<<dim3(M * M, K, P), PC_THREADS, 0, st>>>(M, N_f, (const double2*)h, w, U, V);
-    pc_prod_kernel<<<dim3((N_f + 255) / 256, K * M, P), 256, 0, st>>>(M, K, N_f, (const double2*)h, (const double2*)d, w, x);
-    pc_q_kernel<<<dim3((N_Q + 127) / 128, K * M, P), 128, 0, st>>>(N_f, N_Q, (int)n0, x, W, w, M, Q);
+    if ((N_f & (N_f - 1)) == 0 && N_f <= (1 << 18)) {                       // four-step FFT; x serves as B
+        const int N1 = N_f <= 4096 ? N_f : (N_f <= 4096 * 32 ? 4096 : 8192), N2 = N_f / N1;
+        int log2N1 = 0;
+        while ((1 << log2N1) < N1) log2N1++;
+        const double2 *hh = (const double2*)h, *dd = (const double2*)d;
+        switch (N2) {
+            case 1: launch_fft_cols<1>(P, M, K, N_f, N1, hh, dd, w, W, x, st); break;
+            case 2: launch_fft_cols<2>(P, M, K, N_f, N1, hh, dd, w, W, x, st); break;
+            case 4: launch_fft_cols<4>(P, M, K, N_f, N1, hh, dd, w, W, x, st); break;
+            case 8: launch_fft_cols<8>(P, M, K, N_f, N1, hh, dd, w, W, x, st); break;
+            case 16: launch_fft_cols<16>(P, M, K, N_f, N1, hh, dd, w, W, x, st); break;
+            default: launch_fft_cols<32>(P, M, K, N_f, N1, hh, dd, w, W, x, st); break;
+        }
+        const size_t smem = (size_t)N1 * sizeof(double2);
+        cudaFuncSetAttribute(pc_fft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        long long n0m = n0 % N_f;
+        if (n0m < 0) n0m += N_f;
+        pc_fft_rows_kernel<<<dim3(N2, P * K * M), 256, smem, st>>>(N_f, N1, log2N1, N2, N_Q, (int)n0m, x, W, Q);
+    } else {
+        pc_prod_kernel<<<dim3((N_f + 255) / 256, K * M, P), 256, 0, st>>>(M, K, N_f, (const double2*)h, (const double2*)d, w, x);
+        pc_q_kernel<<<dim3((N_Q + 127) / 128, K * M, P), 128, 0, st>>>(N_f, N_Q, (int)n0, x, W, w, M, Q);
+    }
     ctx->launches += 5;
     cudaError_t e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) {
