@@ -407,6 +407,7 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
     memcpy(L->hi, hi, sizeof(hi));
     L->ln_prior_const = -log(2 * PI) - log(2.0) - log(PI) - log(2 * PI) - log(2.0);
     L->dist_norm = 3.0 / (ctx->D_max * ctx->D_max * ctx->D_max - ctx->D_min * ctx->D_min * ctx->D_min);
+    L->ln_Nt = log((double)ctx->N_t);
     L->nA = ctx->nA; L->nB = ctx->nB; L->A_lo = ctx->A_lo; L->A_hi = ctx->A_hi; L->B_lo = ctx->B_lo; L->B_hi = ctx->B_hi;
     L->lnT = ctx->d_lnT;
     L->Qc = ctx->d_Qc + (size_t)p * K * M * ctx->N_Q * 2;

@@ -41,6 +41,7 @@ struct LnlParams {
     double lo[6], hi[6];          // prior box in z
     double ln_prior_const;        // -ln(2pi) - ln2 - ln(pi) - ln(2pi) - ln2
     double dist_norm;             // 3 / (D_max^3 - D_min^3)
+    double ln_Nt;                 // ln N_t (time-marginalisation normaliser)
     // distance table
     int nA, nB;
     double A_lo, A_hi, B_lo, B_hi;

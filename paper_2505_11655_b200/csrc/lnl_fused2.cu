@@ -115,8 +115,12 @@ __device__ __forceinline__ double exp_tab(double d, const double* __restrict__ t
     return __hiloint2double(__double2hiint(e) + ((k >> 6) << 20), __double2loint(e));
 }
 
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+
 #ifdef F2_TIMERS
-__device__ unsigned long long f2_timers[8];
+__device__ unsigned long long f2_timers[16];
 #define F2_T(i) do { const long long t__ = clock64(); if (lane == 0) atomicAdd(&f2_timers[i], (unsigned long long)(t__ - tmark)); tmark = t__; } while (0)
 #else
 #define F2_T(i)
@@ -225,21 +229,28 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
 
     // ---- stage the tile's records; tile base by shared-memory atomicMin
     {
-        const double* src = rec + (size_t)tile * TS * F2_REC;
-        for (int q = tid; q < TS * F2_REC; q += F2_THREADS) (&sm.rec[0][0])[q] = src[q];
-        if (tid < 4) sm.base[tid] = 0x7ffffffe;
-        if (tid >= 64 && tid < 128) sm.etab[tid - 64] = f2_exp2_tab[tid - 64];
+        // all copies are 16-byte cp.async: every load of the tile is in flight at once and the
+        // prologue pays one memory round trip (a load/store loop pays one per iteration)
+        const double2* src = reinterpret_cast<const double2*>(rec + (size_t)tile * TS * F2_REC);
+        double2* rdst = reinterpret_cast<double2*>(&sm.rec[0][0]);
+        for (int q = tid; q < TS * F2_REC / 2; q += F2_THREADS) cp_async16(rdst + q, src + q);
         // the tile's harmonics Y[m][s] (12 KB) are staged in the S ring, which is idle until phase 0
         const double2* ysrc = ytile + (size_t)tile * F2_YM * 32;
-        for (int q = tid; q < F2_YM * 32; q += F2_THREADS) ysm[q] = ysrc[q];
+#pragma unroll
+        for (int q = tid; q < F2_YM * 32; q += F2_THREADS) cp_async16(ysm + q, ysrc + q);
         // ... and so are the packed U/V matrices of this intrinsic point (16 B per pair, detector and matrix)
         if (quad) {
             const double2* usrc = reinterpret_cast<const double2*>(P.UVp);
             const int nuv = min(P.n_pairs * K * 2, F2_UVMAX);
-            for (int q = tid; q < nuv; q += F2_THREADS) uvsm[q] = __ldg(usrc + q);
+            for (int q = tid; q < nuv; q += F2_THREADS) cp_async16(uvsm + q, usrc + q);
         }
+        if (tid < 4) sm.base[tid] = 0x7ffffffe;
+        if (tid >= 64 && tid < 128) sm.etab[tid - 64] = f2_exp2_tab[tid - 64];
+        asm volatile("cp.async.commit_group;\n cp.async.wait_group 0;" ::: "memory");
     }
+    F2_T(8);
     tile_sync<MODE>(slot);
+    F2_T(9);
     bool valid = false;
     if (tid < TS) {
         valid = sm.rec[tid][14] != 0.0;
@@ -280,6 +291,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             }
         }
     }
+    F2_T(10);
     // ---- step 4, the U/V quadratic term (Eq. 7 with the Eq. 17-18 symmetries): warp w sums the
     //      upper-triangle pairs w, w + 8, ... for all 32 samples (lane = sample; the packed matrix
     //      entries are warp-uniform loads); partial sums meet in shared memory
@@ -319,7 +331,9 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             qpart[(w * 3 * K + 3 * k + 2) * 32 + lane] = vi[k];
         }
     }
+    F2_T(11);
     const int n_valid = tile_count<MODE>(slot, valid);      // also publishes n, w1, base, A
+    F2_T(12);
     if (n_valid == 0) return;
     // ---- round 0: who fits within F2_CAP of the base (normally everybody)
     bool part0 = false;
@@ -346,6 +360,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         }
         sample_consts<K, TABLE>(sm, tid);
     }
+    F2_T(13);
     const int n_part0 = tile_count<MODE>(slot, part0);
     bool last_round = n_part0 == n_valid;
     bool need_setup = n_part0 == 0;                       // nobody fits: the general set-up pivots
@@ -572,7 +587,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                 const int s = SPW * w + lane;
                 if (sm.part[s]) {
                     const int t = tile * TS + s;
-                    if (t < N) lnL[perm ? perm[t] : t] = my_m + log(my_t) - log((double)N_t);
+                    if (t < N) lnL[perm ? perm[t] : t] = my_m + log(my_t) - P.ln_Nt;
                     sm.done[s] = 1;
                 }
             }
@@ -628,10 +643,10 @@ int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec
 }
 
 #ifdef F2_TIMERS
-extern "C" int ile_dbg_timers(unsigned long long* out8) {
+extern "C" int ile_dbg_timers(unsigned long long* out16) {
     cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out8, f2_timers, sizeof(f2_timers));
-    unsigned long long z[8] = {0};
+    cudaMemcpyFromSymbol(out16, f2_timers, sizeof(f2_timers));
+    unsigned long long z[16] = {0};
     cudaMemcpyToSymbol(f2_timers, z, sizeof(z));
     return 0;
 }
