@@ -30,6 +30,7 @@
 #define F2_CAP 15         // largest per-sample offset above the tile base handled in one round
 #define F2_YM 24          // mode slots in the prep kernel's Y tile (32-sample sub-tiles)
 #define F2_REC 16
+#define F2_RECS 17         // record row stride in shared memory (odd: lane = sample reads are conflict-free)
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
 #define F2_UVMAX (300 * 3 * 2)   // packed U/V entries staged in shared memory (M <= 24: 300 pairs)
 #define F2_NG 2           // 32-bin groups per phase (at most 64 outputs per phase)
@@ -38,7 +39,7 @@ template <int K>
 struct Fused2Smem {
     double S[K][F2_TS][F2_SROW];             // S_k[sample][ring bin]
     double2 A[K][F2_NP][F2_RB][32];          // coefficient fragments [k][k-step pair][row block][lane]
-    double rec[F2_TS][F2_REC];
+    double rec[F2_TS][F2_RECS];
     double w1[K][F2_TS];                     // interpolation fraction f
     double2 ew[F2_TS][K];                    // epilogue constants per sample: (1 - f_k, f_k)
     double2 ec[F2_TS];                       // (x^2 B, B)
@@ -115,6 +116,9 @@ __device__ __forceinline__ double exp_tab(double d, const double* __restrict__ t
     return __hiloint2double(__double2hiint(e) + ((k >> 6) << 20), __double2loint(e));
 }
 
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
 }
@@ -231,9 +235,8 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
     {
         // all copies are 16-byte cp.async: every load of the tile is in flight at once and the
         // prologue pays one memory round trip (a load/store loop pays one per iteration)
-        const double2* src = reinterpret_cast<const double2*>(rec + (size_t)tile * TS * F2_REC);
-        double2* rdst = reinterpret_cast<double2*>(&sm.rec[0][0]);
-        for (int q = tid; q < TS * F2_REC / 2; q += F2_THREADS) cp_async16(rdst + q, src + q);
+        const double* src = rec + (size_t)tile * TS * F2_REC;
+        for (int q = tid; q < TS * F2_REC; q += F2_THREADS) cp_async8(&sm.rec[q / F2_REC][q % F2_REC], src + q);
         // the tile's harmonics Y[m][s] (12 KB) are staged in the S ring, which is idle until phase 0
         const double2* ysrc = ytile + (size_t)tile * F2_YM * 32;
 #pragma unroll
@@ -273,21 +276,23 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
     //      mode m = 4 p + lane%4; the trailing half k-step (SINGLE) holds Re or Im of mode
     //      4 NPAIR + (lane%4)/2 in .x.  Fully unrolled: all of a thread's Y loads are in flight at once.
     {
-        constexpr int NA = K * NPT * RB * 32;
-        constexpr int IT = (NA + F2_THREADS - 1) / F2_THREADS;
+        // warp w: row block w % 4, k-step pairs w / 4, w / 4 + 2, ...; the sample's record entries are
+        // loaded once per detector (record rows are 17 doubles apart: conflict-free)
+        static_assert(F2_WARPS == 2 * RB, "fragment builder: 8 warps = 4 row blocks x 2");
+        const int rb = w & (RB - 1), h = w >> 2;
+        const int s = 8 * rb + (lane >> 2), cc = lane & 3;
+        const double x = sm.rec[s][12];
 #pragma unroll
-        for (int it = 0; it < IT; it++) {
-            const int q = tid + it * F2_THREADS;
-            const int ln = q & 31, rb = (q >> 5) & (RB - 1), pk = q / (32 * RB), p = pk % NPT, k = pk / NPT;
-            const int s = 8 * rb + (ln >> 2), cc = ln & 3;
-            const int m = p < NPAIR ? 4 * p + cc : 4 * NPAIR + (cc >> 1);
-            if (q < NA) {
-                const double x = sm.rec[s][12], fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
+        for (int k = 0; k < K; k++) {
+            const double fr = x * sm.rec[s][k], fi = x * sm.rec[s][4 + k];
+#pragma unroll
+            for (int p = h; p < NPT; p += 2) {
+                const int m = p < NPAIR ? 4 * p + cc : 4 * NPAIR + (cc >> 1);
                 const double2 y = ysm[m * 32 + s];
                 double2 a;
                 if (p < NPAIR) a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
                 else a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
-                sm.A[k][p][rb][ln] = a;
+                sm.A[k][p][rb][lane] = a;
             }
         }
     }
@@ -299,30 +304,39 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         double uu[K], vr[K], vi[K];
 #pragma unroll
         for (int k = 0; k < K; k++) uu[k] = vr[k] = vi[k] = 0.0;
-        // pair (a, b), a <= b, number pq of the row-by-row upper triangle: advanced arithmetically,
-        // so that the matrix loads of several iterations are independent and overlap
-        const int M = P.M;
-        int a = 0, b = w;
-        while (b >= M && a < M) { a++; b = b - M + a; }
-        const int npq = (P.n_pairs - w + F2_WARPS - 1) / F2_WARPS;
-#pragma unroll 4
-        for (int it = 0; it < npq; it++) {
-            const int pq = w + it * F2_WARPS;
+        // warp w takes the contiguous run [w npw, (w + 1) npw) of the row-by-row upper triangle
+        // (pairs (a, b), a <= b): y_a stays in registers along a row, so a pair costs one
+        // harmonic load and the warp-uniform matrix loads (the loop is shared-memory-bound otherwise)
+        const int M = P.M, npw = (P.n_pairs + F2_WARPS - 1) / F2_WARPS;
+        int pq = w * npw;
+        const int pq_end = min(pq + npw, P.n_pairs);
+        int a = 0, b = pq;
+        while (a < M && b >= M - a) { b -= M - a; a++; }
+        b += a;
+        while (pq < pq_end) {
+            const double2 ya = ysm[a * 32 + lane];
+            const int cnt = min(M - b, pq_end - pq);
             const double2* uv = uvsm + pq * K * 2;
-            double2 u[K], v[K];
+            const double2* yrow = ysm + b * 32 + lane;
+#pragma unroll 4
+            for (int i = 0; i < cnt; i++) {
+                double2 u[K], v[K];
 #pragma unroll
-            for (int k = 0; k < K; k++) { u[k] = uv[2 * k]; v[k] = uv[2 * k + 1]; }
-            const double2 ya = ysm[a * 32 + lane], yb = ysm[b * 32 + lane];
-            const double t1 = ya.x * yb.x, t2 = ya.y * yb.y, t3 = ya.x * yb.y, t4 = ya.y * yb.x;
-            const double pr = t1 + t2, pi = t3 - t4, qr = t1 - t2, qi = t3 + t4;   // conj(y_a) y_b, y_a y_b
+                for (int k = 0; k < K; k++) { u[k] = uv[i * K * 2 + 2 * k]; v[k] = uv[i * K * 2 + 2 * k + 1]; }
+                const double2 yb = yrow[i * 32];
+                // conj(y_a) y_b = (pr, pi), y_a y_b = (qr, qi): 6 FP64 instructions, then 6 FMAs per detector
+                const double t2 = ya.y * yb.y, t4 = ya.y * yb.x;
+                const double pr = fma(ya.x, yb.x, t2), qr = fma(ya.x, yb.x, -t2), pi = fma(ya.x, yb.y, -t4), qi = fma(ya.x, yb.y, t4);
 #pragma unroll
-            for (int k = 0; k < K; k++) {
-                uu[k] += u[k].x * pr - u[k].y * pi;
-                vr[k] += v[k].x * qr - v[k].y * qi;
-                vi[k] += v[k].x * qi + v[k].y * qr;
+                for (int k = 0; k < K; k++) {
+                    uu[k] = fma(-u[k].y, pi, fma(u[k].x, pr, uu[k]));
+                    vr[k] = fma(-v[k].y, qi, fma(v[k].x, qr, vr[k]));
+                    vi[k] = fma(v[k].y, qr, fma(v[k].x, qi, vi[k]));
+                }
             }
-            b += F2_WARPS;
-            while (b >= M && a < M) { a++; b = b - M + a; }
+            pq += cnt;
+            a++;
+            b = a;
         }
 #pragma unroll
         for (int k = 0; k < K; k++) {
