@@ -29,6 +29,7 @@
 #define F2_NEW 64         // new stored bins per phase (phase 0: F2_RING)
 #define F2_CAP 15         // largest per-sample offset above the tile base handled in one round
 #define F2_YM 24          // mode slots in the prep kernel's Y tile (32-sample sub-tiles)
+#define F2_YS 34          // row stride of the staged Y tile in shared memory (conflict-free fragment-builder reads)
 #define F2_REC 16
 #define F2_RECS 17         // record row stride in shared memory (odd: lane = sample reads are conflict-free)
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
@@ -38,7 +39,7 @@
 template <int K>
 struct Fused2Smem {
     double S[K][F2_TS][F2_SROW];             // S_k[sample][ring bin]
-    double2 A[K][F2_NP][F2_RB][32];          // coefficient fragments [k][k-step pair][row block][lane]
+    double2 A[K][F2_NP][F2_RB][32];          // coefficient fragments [k][k-step pair][row block][lane]; the half k-step: [row block pair][lane]
     double rec[F2_TS][F2_RECS];
     double w1[K][F2_TS];                     // interpolation fraction f
     double2 ew[F2_TS][K];                    // epilogue constants per sample: (1 - f_k, f_k)
@@ -224,8 +225,8 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
     const int lane = tid & 31, w = tid >> 5;
     const int stride = STRIDE1 ? 1 : P.stride, N_t = P.N_t;
     const int c = lane & 3, rq = lane >> 2;
-    double2* ysm = reinterpret_cast<double2*>(&sm.S[0][0][0]);              // [F2_YM][32] during the prologue
-    double* qpart = reinterpret_cast<double*>(ysm + F2_YM * 32);            // [8 warps][3 K][32] partial quadratic sums
+    double2* ysm = reinterpret_cast<double2*>(&sm.S[0][0][0]);              // [F2_YM][F2_YS] during the prologue
+    double* qpart = reinterpret_cast<double*>(ysm + F2_YM * F2_YS);            // [8 warps][3 K][32] partial quadratic sums
     double2* uvsm = reinterpret_cast<double2*>(qpart + F2_WARPS * 3 * K * 32); // packed U/V, up to F2_UVMAX entries
 #ifdef F2_TIMERS
     long long tmark = clock64();
@@ -240,7 +241,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         // the tile's harmonics Y[m][s] (12 KB) are staged in the S ring, which is idle until phase 0
         const double2* ysrc = ytile + (size_t)tile * F2_YM * 32;
 #pragma unroll
-        for (int q = tid; q < F2_YM * 32; q += F2_THREADS) cp_async16(ysm + q, ysrc + q);
+        for (int q = tid; q < F2_YM * 32; q += F2_THREADS) cp_async16(ysm + (q >> 5) * F2_YS + (q & 31), ysrc + q);
         // ... and so are the packed U/V matrices of this intrinsic point (16 B per pair, detector and matrix)
         if (quad) {
             const double2* usrc = reinterpret_cast<const double2*>(P.UVp);
@@ -288,11 +289,11 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
 #pragma unroll
             for (int p = h; p < NPT; p += 2) {
                 const int m = p < NPAIR ? 4 * p + cc : 4 * NPAIR + (cc >> 1);
-                const double2 y = ysm[m * 32 + s];
-                double2 a;
-                if (p < NPAIR) a = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
-                else a = make_double2((cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y, 0.0);
-                sm.A[k][p][rb][lane] = a;
+                const double2 y = ysm[m * F2_YS + s];
+                if (p < NPAIR) sm.A[k][p][rb][lane] = make_double2(fr * y.x - fi * y.y, fr * y.y + fi * y.x);
+                else   // the half k-step: row blocks (0, 1) and (2, 3) share a double2, two 128-bit loads per unit
+                    reinterpret_cast<double*>(&sm.A[k][NPAIR][0][0])[((rb >> 1) * 32 + lane) * 2 + (rb & 1)] =
+                        (cc & 1) ? fr * y.y + fi * y.x : fr * y.x - fi * y.y;
             }
         }
     }
@@ -314,16 +315,16 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         while (a < M && b >= M - a) { b -= M - a; a++; }
         b += a;
         while (pq < pq_end) {
-            const double2 ya = ysm[a * 32 + lane];
+            const double2 ya = ysm[a * F2_YS + lane];
             const int cnt = min(M - b, pq_end - pq);
             const double2* uv = uvsm + pq * K * 2;
-            const double2* yrow = ysm + b * 32 + lane;
+            const double2* yrow = ysm + b * F2_YS + lane;
 #pragma unroll 4
             for (int i = 0; i < cnt; i++) {
                 double2 u[K], v[K];
 #pragma unroll
                 for (int k = 0; k < K; k++) { u[k] = uv[i * K * 2 + 2 * k]; v[k] = uv[i * K * 2 + 2 * k + 1]; }
-                const double2 yb = yrow[i * 32];
+                const double2 yb = yrow[i * F2_YS];
                 // conj(y_a) y_b = (pr, pi), y_a y_b = (qr, qi): 6 FP64 instructions, then 6 FMAs per detector
                 const double t2 = ya.y * yb.y, t4 = ya.y * yb.x;
                 const double pr = fma(ya.x, yb.x, t2), qr = fma(ya.x, yb.x, -t2), pi = fma(ya.x, yb.y, -t4), qi = fma(ya.x, yb.y, t4);
@@ -457,7 +458,11 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                         }
                         if (SINGLE) {
 #pragma unroll
-                            for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs);
+                            for (int rb = 0; rb < RB; rb += 2) {
+                                const double2 as = Ak[(NPAIR * RB + (rb >> 1)) * 32];
+                                dmma2(d[rb][0], d[rb][1], as.x, bs);
+                                dmma2(d[rb + 1][0], d[rb + 1][1], as.y, bs);
+                            }
                         }
 #pragma unroll
                         for (int rb = 0; rb < RB; rb++) { d[rb][0] += e[rb][0]; d[rb][1] += e[rb][1]; }
@@ -747,7 +752,11 @@ __device__ __forceinline__ void contract_phase(Fused2Smem<K>& sm, const LnlParam
 #pragma unroll
                 for (int u = 0; u < 2; u++)
 #pragma unroll
-                    for (int rb = 0; rb < RB; rb++) dmma2(d[u][rb][0], d[u][rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs[u]);
+                    for (int rb = 0; rb < RB; rb += 2) {
+                        const double2 as = Ak[(NPAIR * RB + (rb >> 1)) * 32];
+                        dmma2(d[u][rb][0], d[u][rb][1], as.x, bs[u]);
+                        dmma2(d[u][rb + 1][0], d[u][rb + 1][1], as.y, bs[u]);
+                    }
             }
 #pragma unroll
             for (int u = 0; u < 2; u++) {
@@ -772,7 +781,11 @@ __device__ __forceinline__ void contract_phase(Fused2Smem<K>& sm, const LnlParam
             }
             if (SINGLE) {
 #pragma unroll
-                for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], Ak[(NPAIR * RB + rb) * 32].x, bs[0]);
+                for (int rb = 0; rb < RB; rb += 2) {
+                    const double2 as = Ak[(NPAIR * RB + (rb >> 1)) * 32];
+                    dmma2(d[rb][0], d[rb][1], as.x, bs[0]);
+                    dmma2(d[rb + 1][0], d[rb + 1][1], as.y, bs[0]);
+                }
             }
 #pragma unroll
             for (int rb = 0; rb < RB; rb++) { d[rb][0] += e[rb][0]; d[rb][1] += e[rb][1]; }
