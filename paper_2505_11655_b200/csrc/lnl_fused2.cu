@@ -500,7 +500,16 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             {
                 int j0m = stride * j0;
                 j0m -= (j0m / F2_RING) * F2_RING;
+                const int jl0 = j0m + lane;                       // STRIDE1: ring bin of this lane's first output, before the sample offset
+                bool inr[NG];                                     // output j0 + 32 gi + lane exists
+#pragma unroll
+                for (int gi = 0; gi < NG; gi++) inr[gi] = j0 + 32 * gi + lane < j1;
+                // v: the values; (dh, dlo): high and low words of v - reference, the high word of a
+                // missing output set to that of -inf.  All range logic runs on the high words in the
+                // integer pipe: the FP64 pipe and the issue slots are what this loop is short of.
                 double v[SPW][NG];
+                int dh[SPW][NG], dlo[SPW][NG];
+                bool need = false;
 #pragma unroll
                 for (int i = 0; i < SPW; i++) {
                     const int s = SPW * w + i;
@@ -512,53 +521,47 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
 #pragma unroll
                     for (int k = 0; k < K; k++) {
                         wk[k] = sm.ew[s][k];
-                        int rr = off[k] + j0m;
-                        if (rr >= F2_RING) rr -= F2_RING;
                         if (STRIDE1) {
-                            rr += lane;
+                            const unsigned rr = off[k] + jl0;                      // < 15 + 80 + 31: one wrap
+                            r[k] = (int)min(rr, rr - F2_RING);
+                        } else {
+                            int rr = off[k] + j0m;
                             if (rr >= F2_RING) rr -= F2_RING;
+                            r[k] = rr;
                         }
-                        r[k] = rr;
                     }
                     const double* Srow = &sm.S[0][s][0];
 #pragma unroll
                     for (int gi = 0; gi < NG; gi++) {
-                        const int jl = 32 * gi + lane;
                         double A = -cb.x;
 #pragma unroll
                         for (int k = 0; k < K; k++) {
                             int r0;
                             if (STRIDE1) {
-                                r0 = r[k] + 32 * gi;
-                                if (r0 >= F2_RING) r0 -= F2_RING;
+                                const unsigned rr = r[k] + 32 * gi;                // < 80 + 32: one wrap
+                                r0 = gi == 0 ? r[k] : (int)min(rr, rr - F2_RING);
                             } else {
-                                r0 = (r[k] + stride * jl) % F2_RING;
+                                r0 = (r[k] + stride * (32 * gi + lane)) % F2_RING;
                             }
                             const double* row = Srow + k * (TS * F2_SROW) + r0;
                             A = fma(wk[k].x, row[0], A);
                             A = fma(wk[k].y, row[1], A);
                         }
                         if (TABLE) A = table_lookup(P, A, cb.y);
-                        v[i][gi] = (j0 + jl < j1) ? A : neg_inf();
+                        v[i][gi] = A;
+                        const double dl = A - run_m[i];
+                        dh[i][gi] = inr[gi] ? __double2hiint(dl) : (int)0xFFF00000;
+                        dlo[i][gi] = __double2loint(dl);
+                        need = need || (dh[i][gi] >= 0x403E0000);                  // dl >= 30 (or NaN)
                     }
                 }
-                // raise the references where a new value is more than e^30 above (rare).  The range
-                // tests compare the high words as integers (ALU pipe): the FP64 pipe is the bottleneck.
-                double dl[SPW][NG];
-                bool need = false;
-#pragma unroll
-                for (int i = 0; i < SPW; i++)
-#pragma unroll
-                    for (int gi = 0; gi < NG; gi++) {
-                        dl[i][gi] = v[i][gi] - run_m[i];
-                        need = need || (__double2hiint(dl[i][gi]) >= 0x403E0000);          // dl >= 30
-                    }
+                // raise the references where a new value is more than e^30 above (rare)
                 if (__any_sync(0xffffffffu, need)) {
 #pragma unroll
                     for (int i = 0; i < SPW; i++) {
-                        double vm = v[i][0];
+                        double vm = neg_inf();
 #pragma unroll
-                        for (int gi = 1; gi < NG; gi++) vm = fmax(vm, v[i][gi]);
+                        for (int gi = 0; gi < NG; gi++) vm = fmax(vm, inr[gi] ? v[i][gi] : neg_inf());
                         if (__any_sync(0xffffffffu, vm - run_m[i] >= 30.0)) {
                             // new reference >= max over lanes, found on the ordered high words with
                             // one REDUX; it need not be the exact maximum
@@ -571,7 +574,11 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                             run_s[i] = dm > -690.0 ? run_s[i] * exp_small(dm) : 0.0;
                             run_m[i] = mx;
 #pragma unroll
-                            for (int gi = 0; gi < NG; gi++) dl[i][gi] = v[i][gi] - mx;
+                            for (int gi = 0; gi < NG; gi++) {
+                                const double dl = v[i][gi] - mx;
+                                dh[i][gi] = inr[gi] ? __double2hiint(dl) : (int)0xFFF00000;
+                                dlo[i][gi] = __double2loint(dl);
+                            }
                         }
                     }
                 }
@@ -579,11 +586,11 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                 for (int i = 0; i < SPW; i++)
 #pragma unroll
                     for (int gi = 0; gi < NG; gi++) {
-                        // terms below e^-40 of the reference are dropped: dl <= -40 <=> high word >= 0xC0440000
-                        const bool keep = (unsigned)__double2hiint(dl[i][gi]) < 0xC0440000u;
-                        const double da = __hiloint2double(keep ? __double2hiint(dl[i][gi]) : (int)0xC0440000, keep ? __double2loint(dl[i][gi]) : 0);
-                        const double e = exp_tab(da, sm.etab);
-                        run_s[i] += __hiloint2double(keep ? __double2hiint(e) : 0, keep ? __double2loint(e) : 0);
+                        // terms below e^-40 of the reference (and missing outputs) are clamped to e^-40:
+                        // dl <= -40 <=> high word >= 0xC0440000 as unsigned; one integer min.  The
+                        // (N_t + 64) e^-40 < 3e-15 this adds to a sum >= 1 is in the tolerance budget.
+                        const unsigned hc = min((unsigned)dh[i][gi], 0xC0440000u);
+                        run_s[i] += exp_tab(__hiloint2double((int)hc, dlo[i][gi]), sm.etab);
                     }
             }
             F2_T(4);
