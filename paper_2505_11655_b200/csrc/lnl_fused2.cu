@@ -51,6 +51,8 @@ struct Fused2Smem {
     int done[F2_TS];
     int n_part, n_left;
     double etab[64];                         // 2^(j/64), the table of exp_tab
+    int cap;                                 // largest offset above the base among this round's samples
+    int pad_;
 };
 
 __device__ __forceinline__ void dmma2(double& d0, double& d1, double a, double b) {
@@ -165,6 +167,7 @@ __device__ __forceinline__ void round_setup(Fused2Smem<K>& sm, int lane) {
         for (int k = 0; k < K; k++) sm.base[k] = base[k];
         sm.n_part = __popc(mq);
         sm.n_left = __popc(left);
+        sm.cap = 0;
     }
 }
 
@@ -177,7 +180,9 @@ __device__ __forceinline__ void sample_consts(Fused2Smem<K>& sm, int s) {
     for (int k = 0; k < K; k++) {
         const double f = sm.w1[k][s];
         sm.ew[s][k] = make_double2(1.0 - f, f);
-        sm.eoff[s][k] = min(max(sm.n[k][s] - sm.base[k], 0), F2_CAP);
+        const int o = min(max(sm.n[k][s] - sm.base[k], 0), F2_CAP);
+        sm.eoff[s][k] = o;
+        if (sm.part[s]) atomicMax(&sm.cap, o);
     }
 }
 
@@ -249,6 +254,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             for (int q = tid; q < nuv; q += F2_THREADS) cp_async16(uvsm + q, usrc + q);
         }
         if (tid < 4) sm.base[tid] = 0x7ffffffe;
+        if (tid == 4) sm.cap = 0;
         if (tid >= 64 && tid < 128) sm.etab[tid - 64] = f2_exp2_tab[tid - 64];
         asm volatile("cp.async.commit_group;\n cp.async.wait_group 0;" ::: "memory");
     }
@@ -397,13 +403,16 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
 #pragma unroll
         for (int q = 0; q < SPW; q++) { run_m[q] = -1.0e300; run_s[q] = 0.0; }
 
-        const int last_bin = stride * (N_t - 1) + 1 + F2_CAP;   // highest stored bin (relative to base) any sample reads
+        // cap: the largest offset of a sample of this round above the base (<= F2_CAP; small after the sort);
+        // the last bins of the window are only computed as far as some sample reads them
+        const int cap = STRIDE1 ? sm.cap : F2_CAP;
+        const int last_bin = stride * (N_t - 1) + 1 + cap;      // highest stored bin (relative to base) any sample reads
         int c_lo = 0, j0 = 0;
         int ntiles = min(F2_RING / 8, (last_bin + 1 - c_lo + 7) / 8);
         for (;;) {
             const int c_hi = c_lo + ntiles * 8;
-            int j1 = (c_hi - 1 - F2_CAP - 1) / stride + 1;      // outputs whose reads are all below c_hi
-            if (j1 > N_t) j1 = N_t;
+            int j1 = (c_hi - 1 - cap - 1) / stride + 1;         // outputs whose reads are all below c_hi ...
+            j1 = min(min(j1, j0 + 32 * NG), N_t);               // ... as many as one epilogue pass takes
             F2_T(1);
             if (MODE == 1) {
                 // ---------------- hand the phase to the contraction warps and wait for S
