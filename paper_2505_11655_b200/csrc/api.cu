@@ -117,6 +117,7 @@ extern "C" int ile_destroy(ile_ctx* ctx) {
     cudaFree(ctx->d_ylm);
     cudaFree(ctx->d_Qc);
     cudaFree(ctx->d_Qt);
+    cudaFree(ctx->d_Qf);
     cudaFree(ctx->d_U);
     cudaFree(ctx->d_V);
     cudaFree(ctx->d_UVp);
@@ -248,7 +249,10 @@ extern "C" int ile_set_modes(ile_ctx* ctx, int M, const int* ell, const int* m) 
 // Repack Q [K][M][N_Q] complex -> tiled [K][N_Qpad][48]: one stored bin = 24 complex mode
 // slots (zero padded), 8-double groups XOR-swizzled by bin parity so that the DMMA B-fragment
 // LDS.128 of the fused kernel is bank-conflict free.
-__global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restrict__ Qt, int PK, int M, int N_Q, int N_Qpad) {
+// Qf holds the same values fragment-major, [N_Qpad/2 bin pairs][6 k-step pairs][2 bins][8 columns]:
+// the 8 bins x 4 lanes x 16 bytes of one DMMA B-fragment load are four whole 128-byte lines.
+__global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restrict__ Qt, double* __restrict__ Qf, int PK, int M, int N_Q,
+                                int N_Qpad) {
     long long total = (long long)PK * N_Qpad * ILE_QT_ROW;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
         int col = (int)(idx % ILE_QT_ROW);
@@ -260,6 +264,7 @@ __global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restric
         double v = 0.0;
         if (mode < M && n < N_Q) v = Qc[(((long long)pk * M + mode) * N_Q + n) * 2 + part];
         Qt[idx] = v;
+        Qf[(((long long)pk * N_Qpad + n) >> 1) * (2 * ILE_QT_ROW) + (r >> 3) * 16 + (n & 1) * 8 + (r & 7)] = v;
     }
 }
 
@@ -323,9 +328,9 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     const bool reuse = ctx->have_quv && ctx->P == P && ctx->N_Q == N_Q && ctx->quv_K == K && ctx->quv_M == M;
     ctx->have_quv = false;
     if (!reuse) {
-        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_U); cudaFree(ctx->d_V); cudaFree(ctx->d_UVp);
-        ctx->d_Qc = ctx->d_Qt = ctx->d_U = ctx->d_V = ctx->d_UVp = nullptr;
-        if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qt, nQt * 8) != cudaSuccess ||
+        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_Qf); cudaFree(ctx->d_U); cudaFree(ctx->d_V); cudaFree(ctx->d_UVp);
+        ctx->d_Qc = ctx->d_Qt = ctx->d_Qf = ctx->d_U = ctx->d_V = ctx->d_UVp = nullptr;
+        if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qt, nQt * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qf, nQt * 8) != cudaSuccess ||
             cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess ||
             cudaMalloc(&ctx->d_UVp, (size_t)P * ctx->n_pairs * K * 4 * 8) != cudaSuccess) {
             cudaGetLastError();
@@ -336,7 +341,7 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_Qc, Q, nQ * 8, kind, ctx->stream));
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_U, U, nU * 8, kind, ctx->stream));
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, V, nU * 8, kind, ctx->stream));
-    repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qt, P * K, M, N_Q, N_Qpad);
+    repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qt, ctx->d_Qf, P * K, M, N_Q, N_Qpad);
     ILE_LAUNCH_CHECK(ctx);
     pack_uv_kernel<<<ctx->sm_count * 2, 256, 0, ctx->stream>>>(ctx->d_U, ctx->d_V, ctx->d_pairs, ctx->d_UVp, P, K, M, ctx->n_pairs);
     ILE_LAUNCH_CHECK(ctx);
@@ -412,6 +417,7 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
     L->lnT = ctx->d_lnT;
     L->Qc = ctx->d_Qc + (size_t)p * K * M * ctx->N_Q * 2;
     L->Qt = ctx->d_Qt + (size_t)p * K * ctx->N_Qpad * ILE_QT_ROW;
+    L->Qf = ctx->d_Qf + (size_t)p * K * ctx->N_Qpad * ILE_QT_ROW;
     L->U = ctx->d_U + (size_t)p * K * M * M * 2;
     L->V = ctx->d_V + (size_t)p * K * M * M * 2;
     L->ylm = ctx->d_ylm;

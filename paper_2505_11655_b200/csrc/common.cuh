@@ -49,6 +49,7 @@ struct LnlParams {
     // per intrinsic point data (already offset to point p)
     const double* Qc;             // [K][M][N_Q][2]
     const double* Qt;             // [K][N_Qpad][48] tiled + swizzled
+    const double* Qf;             // [K][N_Qpad/2][6][2][8] fragment-major: one 128-byte line per (bin pair, k-step pair)
     const double* U;              // [K][M][M][2]
     const double* V;              // [K][M][M][2]
     const YlmTable* ylm;
@@ -70,7 +71,7 @@ struct ile_ctx {
     YlmTable h_ylm;
     YlmTable* d_ylm;
     double fs, t_Q0, D_ref;
-    double *d_Qc, *d_Qt, *d_U, *d_V, *d_UVp;
+    double *d_Qc, *d_Qt, *d_Qf, *d_U, *d_V, *d_UVp;
     int2* d_pairs;
     int n_pairs;
     double t_lo, dt;

@@ -439,11 +439,11 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                         int k, t;
                         unit_kt(u, k, t);
                         const int row = sm.base[k] + c_lo + 8 * t + rq;
-                        const int swz = (row & 1) << 3;
-                        const double* qrow = P.Qt + ((size_t)k * P.N_Qpad + row) * ILE_QT_ROW;
+                        // fragment-major Q: bin pair block of 96 doubles, 16 per k-step pair, 8 per bin
+                        const double* qrow = P.Qf + (((size_t)k * P.N_Qpad + row) >> 1) * (2 * ILE_QT_ROW) + (row & 1) * 8;
 #pragma unroll
-                        for (int p = 0; p < NPAIR; p++) b[p] = __ldg(reinterpret_cast<const double2*>(qrow + ((8 * p + 2 * c) ^ swz)));
-                        if (SINGLE) bs = __ldg(qrow + ((8 * NPAIR + c) ^ swz));
+                        for (int p = 0; p < NPAIR; p++) b[p] = __ldg(reinterpret_cast<const double2*>(qrow + 16 * p + 2 * c));
+                        if (SINGLE) bs = __ldg(qrow + 16 * NPAIR + c);
                     };
                     auto compute = [&](int u, const double2 (&b)[NPAIR], const double bs) {
                         int k, t;
@@ -645,7 +645,11 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
 template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
 static int launch_fused2_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
     static bool configured = false;
+#ifdef F2_SMEM_PAD
+    const int smem = (int)sizeof(Fused2Smem<K>) + F2_SMEM_PAD;      // experiment: force one CTA per SM
+#else
     const int smem = (int)sizeof(Fused2Smem<K>);
+#endif
     if (!configured) {
         ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         configured = true;
@@ -720,11 +724,10 @@ __device__ __forceinline__ void contract_phase(Fused2Smem<K>& sm, const LnlParam
         for (int u = 0; u < 2; u++) {
             if (u < nu) {
                 const int row = base[k] + c_lo + 8 * (t0 + 4 * u) + rq;
-                const int swz = (row & 1) << 3;
-                const double* qrow = P.Qt + ((size_t)k * P.N_Qpad + row) * ILE_QT_ROW;
+                const double* qrow = P.Qf + (((size_t)k * P.N_Qpad + row) >> 1) * (2 * ILE_QT_ROW) + (row & 1) * 8;
 #pragma unroll
-                for (int p = 0; p < NPAIR; p++) b[u][p] = __ldg(reinterpret_cast<const double2*>(qrow + ((8 * p + 2 * c) ^ swz)));
-                if (SINGLE) bs[u] = __ldg(qrow + ((8 * NPAIR + c) ^ swz));
+                for (int p = 0; p < NPAIR; p++) b[u][p] = __ldg(reinterpret_cast<const double2*>(qrow + 16 * p + 2 * c));
+                if (SINGLE) bs[u] = __ldg(qrow + 16 * NPAIR + c);
             }
         }
     };
