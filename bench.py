@@ -283,6 +283,35 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_precompute(args):
+    """Side measurement: ile_precompute_quv on P = 16 intrinsic points, K = 3, M = 21, N_f = 32768,
+    N_Q = 1024 stored bins, device-resident spectra; one JSON line, not the headline metric."""
+    import torch
+    from paper_2505_11655_b200 import Ile
+    from synth import make_modes, make_network
+    from synth.spectra import make_spectra
+    P, K, N_f, N_Q, fs = 16, 3, 32768, 1024, 4096.0
+    ell, m = make_modes(4)
+    D, pos = make_network(K, np.random.Generator(np.random.Philox(99)))
+    h, d, S, df = make_spectra(K, ell, m, N_f, fs, seed=1, P=1)
+    ile = Ile(0)
+    ile.set_network(D, pos, 0.0)
+    ile.set_modes(ell, m)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    hd, dd, Sd = dev(np.repeat(h, P, axis=0)), dev(d), dev(S)
+    call = lambda: ile.precompute_quv(hd, dd, Sd, df, 20.0, -(N_Q // 2) / fs, N_Q, 500.0)
+    for _ in range(max(args.warmup, 1)):
+        call()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        call()                                               # returns after the tables are installed (synchronous)
+    ms = (time.perf_counter() - t0) * 1e3 / args.steps
+    print(json.dumps({"metric": "Q/U/V precompute (Eq. 6a-c)", "value": P / (ms * 1e-3), "unit": "intrinsic points/s", "ms_per_step": ms,
+                      "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": f"P={P} points, K={K}, M={len(ell)}, N_f={N_f}, N_Q={N_Q}, spectra resident in HBM"}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -290,8 +319,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precompute", action="store_true", help="time the Q/U/V precompute instead of the hot path (side measurement)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.precompute:
+        run_precompute(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

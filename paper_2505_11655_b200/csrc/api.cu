@@ -118,6 +118,7 @@ extern "C" int ile_destroy(ile_ctx* ctx) {
     cudaFree(ctx->d_Qc);
     cudaFree(ctx->d_Qt);
     cudaFree(ctx->d_Qf);
+    cudaFree(ctx->pc_buf);
     cudaFree(ctx->d_U);
     cudaFree(ctx->d_V);
     cudaFree(ctx->d_UVp);

@@ -81,6 +81,8 @@ struct ile_ctx {
     double A_lo, A_hi, B_lo, B_hi;
     double* d_lnT;
     int variant;
+    void* pc_buf;                 // scratch of ile_precompute_quv (grow-only, freed at destroy)
+    size_t pc_bytes;
     int fused_rb;                 // row blocks of 8 samples per CTA of the fused kernel: 4 (default, two CTAs per SM) or 8
     int fused_gen3;               // 1: warp-specialised persistent fused kernel
     int prep_gen1;                // 1: one-thread-per-sample prep kernel (A/B timing)

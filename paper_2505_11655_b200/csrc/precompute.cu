@@ -4,7 +4,7 @@
 //   U_k[a][b]   = sum_j w_k[j] conj(h_a[j]) h_b[j]                        (6b)
 //   V_k[a][b]   = sum_j w_k[j] h_a[-j] h_b[j]                             (6c)
 //   Q_k[a][n]   = sum_j w_k[j] conj(h_a[j]) d_k[j] exp(2 pi i j (n + n0) / N_f)   (6a), t_n = (n0 + n) / fs
-// U, V: one block per matrix entry, by the definition.  Q: for power-of-two N_f <= 2^18 a four-step
+// U, V: upper triangle, frequency slices staged in shared memory, deterministic two-stage sum.  Q: for power-of-two N_f <= 2^18 a four-step
 // inverse FFT (column DFTs in registers, row FFTs in shared memory, only the stored window written);
 // otherwise the definition (one thread per output time, twiddle advanced by complex rotation and
 // re-seeded from an exact table every 32 bins).  Installed through ile_load_quv (symmetry check, repack).
@@ -29,37 +29,79 @@ __global__ void pc_twiddle_kernel(int N_f, double2* __restrict__ W) {
     W[m] = make_double2(c, s);
 }
 
-// grid (M*M, K, P): U and V entry (a, b) of detector k, point p
-__global__ void __launch_bounds__(PC_THREADS) pc_uv_kernel(int M, int N_f, const double2* __restrict__ h, const double* __restrict__ w,
-                                                           double2* __restrict__ U, double2* __restrict__ V) {
-    const int a = blockIdx.x / M, b = blockIdx.x % M, k = blockIdx.y, p = blockIdx.z, K = gridDim.y;
-    const double2* ha = h + ((size_t)p * M + a) * N_f;
-    const double2* hb = h + ((size_t)p * M + b) * N_f;
-    const double* wk = w + (size_t)k * N_f;
-    double ur = 0.0, ui = 0.0, vr = 0.0, vi = 0.0;
-    for (int j = threadIdx.x; j < N_f; j += PC_THREADS) {
-        const double wj = wk[j];
-        if (wj == 0.0) continue;
-        const double2 x = ha[j], y = hb[j], xm = ha[j == 0 ? 0 : N_f - j];
-        ur += wj * (x.x * y.x + x.y * y.y);           // conj(x) y
-        ui += wj * (x.x * y.y - x.y * y.x);
-        vr += wj * (xm.x * y.x - xm.y * y.y);         // x(-f) y
-        vi += wj * (xm.x * y.y + xm.y * y.x);
+// U and V, upper triangle.  Block (slice, p): frequency slice of point p in chunks of PC_CH bins staged in
+// shared memory (h_m[j] and h_m[-j] for all modes, w_k[j]); thread = pair (a <= b), 4 K running sums;
+// per-block partial sums go to part[p][slice][pair][k][4] and are added in slice order by pc_uv_finish_kernel
+// (deterministic), which also fills the lower triangle by Eq. 17-18.
+#define PC_CH 32
+__global__ void __launch_bounds__(PC_THREADS) pc_uv_kernel(int M, int K, int N_f, int n_pairs, int chunks_per_block, const int2* __restrict__ pairs,
+                                                           const double2* __restrict__ h, const double* __restrict__ w, double* __restrict__ part) {
+    __shared__ double2 hs[ILE_MAX_M][PC_CH + 1], hm[ILE_MAX_M][PC_CH + 1];
+    __shared__ double ws[ILE_MAX_K][PC_CH];
+    const int p = blockIdx.y, tid = threadIdx.x;
+    const double2* hp = h + (size_t)p * M * N_f;
+    const bool act = tid < n_pairs;
+    const int2 ab = act ? pairs[tid] : make_int2(0, 0);
+    double acc[ILE_MAX_K][4];
+#pragma unroll
+    for (int k = 0; k < ILE_MAX_K; k++) acc[k][0] = acc[k][1] = acc[k][2] = acc[k][3] = 0.0;
+    for (int cc = 0; cc < chunks_per_block; cc++) {
+        const int j0 = (blockIdx.x * chunks_per_block + cc) * PC_CH;
+        if (j0 >= N_f) break;
+        __syncthreads();                                              // the previous chunk is consumed
+        for (int q = tid; q < K * PC_CH; q += PC_THREADS) {
+            const int k = q / PC_CH, jj = q % PC_CH;
+            ws[k][jj] = j0 + jj < N_f ? w[(size_t)k * N_f + j0 + jj] : 0.0;
+        }
+        // chunks outside the band carry no weight
+        if (!__syncthreads_or(tid < K * PC_CH && ws[tid / PC_CH][tid % PC_CH] != 0.0)) continue;
+        for (int q = tid; q < M * PC_CH; q += PC_THREADS) {
+            const int m = q / PC_CH, jj = q % PC_CH, j = j0 + jj;
+            const bool in = j < N_f;
+            hs[m][jj] = in ? hp[(size_t)m * N_f + j] : make_double2(0.0, 0.0);
+            hm[m][jj] = in ? hp[(size_t)m * N_f + (j == 0 ? 0 : N_f - j)] : make_double2(0.0, 0.0);
+        }
+        __syncthreads();
+        if (act) {
+#pragma unroll 4
+            for (int jj = 0; jj < PC_CH; jj++) {
+                const double2 x = hs[ab.x][jj], y = hs[ab.y][jj], xm = hm[ab.x][jj];
+                const double cr = x.x * y.x + x.y * y.y, ci = x.x * y.y - x.y * y.x;          // conj(x) y
+                const double vr = xm.x * y.x - xm.y * y.y, vi = xm.x * y.y + xm.y * y.x;      // x(-f) y
+#pragma unroll
+                for (int k = 0; k < ILE_MAX_K; k++)
+                    if (k < K) {
+                        const double wj = ws[k][jj];
+                        acc[k][0] += wj * cr; acc[k][1] += wj * ci; acc[k][2] += wj * vr; acc[k][3] += wj * vi;
+                    }
+            }
+        }
     }
-    __shared__ double sh[4][PC_THREADS / 32];
-    ur = warp_sum(ur); ui = warp_sum(ui); vr = warp_sum(vr); vi = warp_sum(vi);
-    if ((threadIdx.x & 31) == 0) {
-        const int wi = threadIdx.x >> 5;
-        sh[0][wi] = ur; sh[1][wi] = ui; sh[2][wi] = vr; sh[3][wi] = vi;
+    if (act) {
+        double* o = part + ((((size_t)p * gridDim.x + blockIdx.x) * n_pairs + tid) * K) * 4;
+        for (int k = 0; k < K; k++) {
+            o[4 * k + 0] = acc[k][0]; o[4 * k + 1] = acc[k][1]; o[4 * k + 2] = acc[k][2]; o[4 * k + 3] = acc[k][3];
+        }
     }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double t[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int q = 0; q < PC_THREADS / 32; q++)
-            for (int e = 0; e < 4; e++) t[e] += sh[e][q];
-        const size_t o = (((size_t)p * K + k) * M + a) * M + b;
-        U[o] = make_double2(t[0], t[1]);
-        V[o] = make_double2(t[2], t[3]);
+}
+
+__global__ void pc_uv_finish_kernel(int P, int M, int K, int n_pairs, int slices, const int2* __restrict__ pairs, const double* __restrict__ part,
+                                    double2* __restrict__ U, double2* __restrict__ V) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= P * n_pairs * K) return;
+    const int k = idx % K, pr = (idx / K) % n_pairs, p = idx / (K * n_pairs);
+    double t[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int sl = 0; sl < slices; sl++) {
+        const double* o = part + ((((size_t)p * slices + sl) * n_pairs + pr) * K + k) * 4;
+        for (int e = 0; e < 4; e++) t[e] += o[e];
+    }
+    const int2 ab = pairs[pr];
+    const size_t base = ((size_t)p * K + k) * M * M;
+    U[base + ab.x * M + ab.y] = make_double2(t[0], t[1]);
+    V[base + ab.x * M + ab.y] = make_double2(t[2], t[3]);
+    if (ab.x != ab.y) {
+        U[base + ab.y * M + ab.x] = make_double2(t[0], -t[1]);      // U Hermitian (Eq. 17)
+        V[base + ab.y * M + ab.x] = make_double2(t[2], t[3]);       // V symmetric (Eq. 18)
     }
 }
 
@@ -112,7 +154,7 @@ __global__ void __launch_bounds__(128) pc_q_kernel(int N_f, int N_Q, int n0, con
 //   W_N^{jn} = W_N1^{j1 n1} W_N^{j1 n2} W_N2^{j2 n2}
 // pc_fft_cols: thread = (series, j1): x[j1 + N1 j2] = w conj(h) d formed on the fly (coalesced over j1), the
 //   N2-point DFT over j2 by its definition, times the twiddle W_N^{j1 n2}           -> B[series][n2][j1]
-// pc_fft_rows: CTA = (n2, series): N1-point radix-2 decimation-in-frequency FFT in shared memory (natural
+// pc_fft_rows: CTA = (n2, series): N1-point decimation-in-frequency FFT in shared memory, two radix-2 stages per pass (natural
 //   order in, bit-reversed out), then only the outputs n = n1 N2 + n2 that fall in the stored window
 //   [n0, n0 + N_Q) are written.  Every twiddle is an exact entry of the sincospi table W.
 template <int N2>
@@ -155,13 +197,35 @@ __global__ void __launch_bounds__(256) pc_fft_rows_kernel(int N_f, int N1, int l
     const double2* Bp = B + ((size_t)s * N2 + n2) * N1;
     for (int i = threadIdx.x; i < N1; i += 256) sm[i] = Bp[i];
     __syncthreads();
-    for (int half = N1 >> 1, tstride = N_f / N1; half >= 1; half >>= 1, tstride <<= 1) {
+    // two radix-2 stages per pass (halves H and H/2 on the elements p, p + H/2, p + H, p + 3H/2):
+    // W_2H^(p + H/2) = i W_2H^p, so a pass needs two table twiddles; a last single stage if log2 N1 is odd
+    int H = N1 >> 1, ts = N_f / N1, stages = log2N1;
+    while (stages >= 2) {
+        const int q = H >> 1;
+        for (int t = threadIdx.x; t < (N1 >> 2); t += 256) {
+            const int pos = t & (q - 1), i0 = ((t - pos) << 2) + pos;
+            const double2 x0 = sm[i0], x1 = sm[i0 + q], x2 = sm[i0 + 2 * q], x3 = sm[i0 + 3 * q];
+            const double2 w1 = W[(size_t)pos * ts], w2 = W[(size_t)pos * 2 * ts];
+            const double2 y0 = make_double2(x0.x + x2.x, x0.y + x2.y), y1 = make_double2(x1.x + x3.x, x1.y + x3.y);
+            const double ar = x0.x - x2.x, ai = x0.y - x2.y, br = x1.x - x3.x, bi = x1.y - x3.y;
+            const double2 y2 = make_double2(ar * w1.x - ai * w1.y, ar * w1.y + ai * w1.x);
+            const double2 y3 = make_double2(-(br * w1.y + bi * w1.x), br * w1.x - bi * w1.y);      // (x1 - x3) i w1
+            const double cr = y0.x - y1.x, ci = y0.y - y1.y, dr = y2.x - y3.x, di = y2.y - y3.y;
+            sm[i0] = make_double2(y0.x + y1.x, y0.y + y1.y);
+            sm[i0 + q] = make_double2(cr * w2.x - ci * w2.y, cr * w2.y + ci * w2.x);
+            sm[i0 + 2 * q] = make_double2(y2.x + y3.x, y2.y + y3.y);
+            sm[i0 + 3 * q] = make_double2(dr * w2.x - di * w2.y, dr * w2.y + di * w2.x);
+        }
+        __syncthreads();
+        H >>= 2;
+        ts <<= 2;
+        stages -= 2;
+    }
+    if (stages == 1) {                                   // H == 1: last butterflies, twiddle 1
         for (int t = threadIdx.x; t < (N1 >> 1); t += 256) {
-            const int pos = t & (half - 1), i = ((t - pos) << 1) + pos, j = i + half;
-            const double2 u = sm[i], v = sm[j], tw = W[(size_t)pos * tstride];
-            const double dr = u.x - v.x, di = u.y - v.y;
-            sm[i] = make_double2(u.x + v.x, u.y + v.y);
-            sm[j] = make_double2(dr * tw.x - di * tw.y, dr * tw.y + di * tw.x);
+            const double2 u = sm[2 * t], v = sm[2 * t + 1];
+            sm[2 * t] = make_double2(u.x + v.x, u.y + v.y);
+            sm[2 * t + 1] = make_double2(u.x - v.x, u.y - v.y);
         }
         __syncthreads();
     }
@@ -194,22 +258,41 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     const double n0d = t_Q0 * fs;
     const long long n0 = llrint(n0d);
     if (fabs(n0d - (double)n0) > 1e-6) return ile_fail(ctx, ILE_EINVAL, "precompute_quv: t_Q0 * fs = %.9g is not an integer", n0d);
-    const int K = ctx->K, M = ctx->M;
+    const int K = ctx->K, M = ctx->M, n_pairs = ctx->n_pairs;
+    if (n_pairs > PC_THREADS || K * PC_CH > PC_THREADS) return ile_fail(ctx, ILE_EINVAL, "precompute_quv: at most 22 modes");
     const size_t nQ = (size_t)P * K * M * N_Q, nU = (size_t)P * K * M * M, nX = (size_t)P * K * M * N_f;
-    double *w = nullptr;
-    double2 *W = nullptr, *x = nullptr, *Q = nullptr, *U = nullptr, *V = nullptr;
-    auto cleanup = [&]() { cudaFree(w); cudaFree(W); cudaFree(x); cudaFree(Q); cudaFree(U); cudaFree(V); };
-    if (cudaMalloc(&w, (size_t)K * N_f * 8) != cudaSuccess || cudaMalloc(&W, (size_t)N_f * 16) != cudaSuccess ||
-        cudaMalloc(&x, nX * 16) != cudaSuccess || cudaMalloc(&Q, nQ * 16) != cudaSuccess || cudaMalloc(&U, nU * 16) != cudaSuccess ||
-        cudaMalloc(&V, nU * 16) != cudaSuccess) {
-        cudaGetLastError();
-        cleanup();
-        return ile_fail(ctx, ILE_ENOMEM, "precompute_quv: device allocation failed");
+    // frequency slices per point: enough blocks for two waves, at least one chunk each
+    const int chunks = (N_f + PC_CH - 1) / PC_CH;
+    int slices = (2 * ctx->sm_count + P - 1) / P;
+    if (slices > chunks) slices = chunks;
+    const int cpb = (chunks + slices - 1) / slices;
+    slices = (chunks + cpb - 1) / cpb;
+    const size_t nPart = (size_t)P * slices * n_pairs * K * 4;
+    // one grow-only scratch allocation: w | W | x | Q | U | V | part  (256-byte aligned pieces)
+    auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t o_w = 0, o_W = o_w + al((size_t)K * N_f * 8), o_x = o_W + al((size_t)N_f * 16), o_Q = o_x + al(nX * 16),
+                 o_U = o_Q + al(nQ * 16), o_V = o_U + al(nU * 16), o_p = o_V + al(nU * 16), total = o_p + al(nPart * 8);
+    if (total > ctx->pc_bytes) {
+        cudaStreamSynchronize(ctx->stream);
+        cudaFree(ctx->pc_buf);
+        ctx->pc_buf = nullptr;
+        ctx->pc_bytes = 0;
+        if (cudaMalloc(&ctx->pc_buf, total) != cudaSuccess) {
+            cudaGetLastError();
+            return ile_fail(ctx, ILE_ENOMEM, "precompute_quv: device allocation of %zu bytes failed", total);
+        }
+        ctx->pc_bytes = total;
     }
+    char* buf = (char*)ctx->pc_buf;
+    double* w = (double*)(buf + o_w);
+    double2 *W = (double2*)(buf + o_W), *x = (double2*)(buf + o_x), *Q = (double2*)(buf + o_Q), *U = (double2*)(buf + o_U),
+            *V = (double2*)(buf + o_V);
+    double* part = (double*)(buf + o_p);
     cudaStream_t st = ctx->stream;
     pc_weight_kernel<<<dim3((N_f + 255) / 256, K), 256, 0, st>>>(K, N_f, df, f_low, S, w);
     pc_twiddle_kernel<<<(N_f + 255) / 256, 256, 0, st>>>(N_f, W);
-    pc_uv_kernel<<<dim3(M * M, K, P), PC_THREADS, 0, st>>>(M, N_f, (const double2*)h, w, U, V);
+    pc_uv_kernel<<<dim3(slices, P), PC_THREADS, 0, st>>>(M, K, N_f, n_pairs, cpb, ctx->d_pairs, (const double2*)h, w, part);
+    pc_uv_finish_kernel<<<(P * n_pairs * K + 255) / 256, 256, 0, st>>>(P, M, K, n_pairs, slices, ctx->d_pairs, part, U, V);
     if ((N_f & (N_f - 1)) == 0 && N_f <= (1 << 18)) {                       // four-step FFT; x serves as B
         const int N1 = N_f <= 4096 ? N_f : (N_f <= 4096 * 32 ? 4096 : 8192), N2 = N_f / N1;
         int log2N1 = 0;
@@ -232,15 +315,10 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
         pc_prod_kernel<<<dim3((N_f + 255) / 256, K * M, P), 256, 0, st>>>(M, K, N_f, (const double2*)h, (const double2*)d, w, x);
         pc_q_kernel<<<dim3((N_Q + 127) / 128, K * M, P), 128, 0, st>>>(N_f, N_Q, (int)n0, x, W, w, M, Q);
     }
-    ctx->launches += 5;
-    cudaError_t e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) {
-        cleanup();
-        return ile_fail(ctx, ILE_ECUDA, "precompute_quv: %s", cudaGetErrorString(e));
-    }
-    const int rc = ile_load_quv(ctx, P, N_Q, fs, (double)n0 / fs, (const double*)Q, (const double*)U, (const double*)V, D_ref, 1);
-    cleanup();
-    return rc;
+    ctx->launches += 6;
+    ILE_LAUNCH_CHECK(ctx);
+    ILE_CUDA(ctx, cudaStreamSynchronize(st));          // ile_load_quv reads U and V back for its symmetry check
+    return ile_load_quv(ctx, P, N_Q, fs, (double)n0 / fs, (const double*)Q, (const double*)U, (const double*)V, D_ref, 1);
 }
 
 // Copies the resident Q/U/V of intrinsic point p to host arrays (caller layout of ile_load_quv).
