@@ -134,8 +134,11 @@ int ile_load_quv(ile_ctx *ctx, int P, int N_Q, double fs, double t_Q0,
  * (j - N_f) df): h [P][M][N_f][2] mode spectra, d [K][N_f][2] data spectra, S [K][N_f/2+1]
  * one-sided PSDs over |f|; <a|b>_k = 2 sum_{|f| > f_low} df a*(f) b(f) / S_k(|f|).  fs = N_f df;
  * the stored window is t_n = t_Q0 + n / fs, n < N_Q (t_Q0 fs must be an integer).  Installs the
- * result like ile_load_quv (synchronises).  ile_get_quv copies point p back to host arrays in
- * ile_load_quv's layout (any of Q, U, V may be NULL). */
+ * result like ile_load_quv (synchronises).  The inputs stay the caller's; scratch is one grow-only
+ * device allocation owned by the context (freed by ile_destroy).  Errors: ILE_ESTATE before
+ * set_network/set_modes, ILE_EINVAL for bad sizes, N_Q > N_f, t_Q0 off the sample grid or more
+ * than 22 modes, ILE_ENOMEM, ILE_ECUDA; the resident Q/U/V are untouched on error.
+ * ile_get_quv copies point p back to host arrays in ile_load_quv's layout (any of Q, U, V may be NULL). */
 int ile_precompute_quv(ile_ctx *ctx, int P, int N_f, double df, double f_low, const double *h, const double *d,
                        const double *S, double t_Q0, int N_Q, double D_ref);
 int ile_get_quv(ile_ctx *ctx, int p, double *Q, double *U, double *V);
