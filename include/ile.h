@@ -137,7 +137,7 @@ int ile_load_quv(ile_ctx *ctx, int P, int N_Q, double fs, double t_Q0,
  * result like ile_load_quv (synchronises).  The inputs stay the caller's; scratch is one grow-only
  * device allocation owned by the context (freed by ile_destroy).  Errors: ILE_ESTATE before
  * set_network/set_modes, ILE_EINVAL for bad sizes, N_Q > N_f, t_Q0 off the sample grid or more
- * than 22 modes, ILE_ENOMEM, ILE_ECUDA; the resident Q/U/V are untouched on error.
+ * than 22 modes (the resident Q/U/V stay as they were), ILE_ENOMEM, ILE_ECUDA.
  * ile_get_quv copies point p back to host arrays in ile_load_quv's layout (any of Q, U, V may be NULL). */
 int ile_precompute_quv(ile_ctx *ctx, int P, int N_f, double df, double f_low, const double *h, const double *d,
                        const double *S, double t_Q0, int N_Q, double D_ref);
