@@ -156,3 +156,23 @@ def test_error_paths(torch_mod):
         ile.set_time_grid(-0.045, prob.dt, prob.N_t)                 # ERANGE: window + delays leave Q
     with pytest.raises(IleError):
         ile.set_time_grid(prob.t_lo, 1.5 / prob.fs, 10)              # non-integer stride
+
+
+@pytest.mark.parametrize("N_t,stride", [(1, 1), (7, 1), (63, 1), (64, 1), (65, 1), (129, 1), (333, 1), (50, 2), (131, 3)])
+def test_time_grid_shapes(torch_mod, N_t, stride):
+    """Window lengths around the 64-output phases of the fused kernel (one phase, exactly full, one bin over, a
+    short tail) and time steps of 2 and 3 stored bins, on the l <= 4 three-detector problem."""
+    from oracle import likelihood as lk
+    torch = torch_mod
+    prob = make_problem(2)
+    ile = _ile(prob)
+    dt = stride / prob.fs
+    t_lo = -0.5 * (N_t - 1) * dt
+    t_lo = round(t_lo * prob.fs) / prob.fs                              # on the stored grid
+    ile.set_time_grid(t_lo, dt, N_t, 1)
+    N = 32 * 9 + 5
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=100 + N_t)
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, t_lo, dt, N_t, z)
+    got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
+    assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
