@@ -36,8 +36,23 @@ __device__ __forceinline__ double ln_pdf_av(const IntegDev& I, const SamplerDev&
     return (lo < av.C && S.keys[lo] == key) ? av.ln_ps : neg_inf();
 }
 
+// Per-component constants of a GMM member, computed once per block into shared memory instead of once per
+// sample: gc[c] = sum_i ln L_c[i][i] (same order as the per-sample loop had), gc[16 + c] = ln omega_c.
+// The densities below are bit-identical to evaluating these logarithms in place.
+#define GMM_GC 32
+__device__ __forceinline__ void gmm_consts(const IntegDev& I, const double* g, double* gc, int t, int nt) {
+    const int d = I.d, C = I.n_gmm;
+    const double* L = g + C + C * d + C * d * d;
+    for (int c = t; c < C; c += nt) {
+        double lndet = 0.0;
+        for (int i = 0; i < d; i++) lndet = lndet + log(L[c * d * d + i * d + i]);
+        gc[c] = lndet;
+        gc[16 + c] = log(g[c]);
+    }
+}
+
 // ln N(z; mu_c, Sigma_c) + ln omega_c for every component; returns the log-sum-exp
-__device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev& S, const double* zz, double* e_out) {
+__device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev& S, const double* zz, double* e_out, const double* gc) {
     const int d = I.d, C = I.n_gmm;
     const double* omega = S.gmm;
     const double* mu = omega + C;
@@ -47,15 +62,14 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
     for (int c = 0; c < C; c++) {
         const double* Lc = L + c * d * d;
         double y[ILE_MAX_D];
-        double quad = 0.0, lndet = 0.0;
+        double quad = 0.0;
         for (int i = 0; i < d; i++) {
             double s = zz[i] - mu[c * d + i];
             for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
             y[i] = s / Lc[i * d + i];
             quad = quad + y[i] * y[i];
-            lndet = lndet + log(Lc[i * d + i]);
         }
-        e[c] = -0.5 * quad - lndet - 0.5 * d * log(TWO_PI) + log(omega[c]);
+        e[c] = -0.5 * quad - gc[c] - 0.5 * d * log(TWO_PI) + gc[16 + c];
         mx = fmax(mx, e[c]);
     }
     double sum = 0.0;
@@ -65,25 +79,25 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
     return mx + log(sum);
 }
 
-__device__ __forceinline__ double member_ln_pdf(const IntegDev& I, int a, const double* zz, bool inbox) {
+__device__ __forceinline__ double member_ln_pdf(const IntegDev& I, int a, const double* zz, bool inbox, const double* gc_all) {
     const SamplerDev& S = I.mem[a];
     switch (S.kind) {
         case ILE_KIND_UNIFORM: return inbox ? -log(I.V0) : neg_inf();
         case ILE_KIND_AC: return inbox ? ln_pdf_ac(I, S, zz) : neg_inf();
         case ILE_KIND_AV: return inbox ? ln_pdf_av(I, S, zz) : neg_inf();
-        case ILE_KIND_GMM: return ln_pdf_gmm(I, S, zz, nullptr);
+        case ILE_KIND_GMM: return ln_pdf_gmm(I, S, zz, nullptr, gc_all + a * GMM_GC);
     }
     return neg_inf();
 }
 
-__device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double* zz) {
+__device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double* zz, const double* gc_all) {
     bool inbox = true;
     for (int c = 0; c < I.d; c++) inbox = inbox && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
-    if (I.n_members == 1) return member_ln_pdf(I, 0, zz, inbox);
+    if (I.n_members == 1) return member_ln_pdf(I, 0, zz, inbox, gc_all);
     double e[ILE_MAX_MEMBERS];
     double mx = neg_inf();
     for (int a = 0; a < I.n_members; a++) {
-        e[a] = log(I.port->W[a]) + member_ln_pdf(I, a, zz, inbox);
+        e[a] = gc_all[ILE_MAX_MEMBERS * GMM_GC + a] + member_ln_pdf(I, a, zz, inbox, gc_all);
         mx = fmax(mx, e[a]);
     }
     if (!is_finite_d(mx)) return neg_inf();
@@ -118,7 +132,21 @@ __global__ void alloc_kernel(IntegDev I, long long N) {
 }
 
 // ---------------------------------------------------------------- draw
+// every GMM member's per-component constants and the members' ln W_a, once per block
+__device__ __forceinline__ void block_gmm_consts(const IntegDev& I, double* gc_all) {
+    bool any = I.n_members > 1;
+    if (I.n_members > 1 && threadIdx.x < I.n_members) gc_all[ILE_MAX_MEMBERS * GMM_GC + threadIdx.x] = log(I.port->W[threadIdx.x]);   // ln W_a
+    for (int a = 0; a < I.n_members; a++)
+        if (I.mem[a].kind == ILE_KIND_GMM) {
+            gmm_consts(I, I.mem[a].gmm, gc_all + a * GMM_GC, threadIdx.x, blockDim.x);
+            any = true;
+        }
+    if (any) __syncthreads();
+}
+
 __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned int g, double* __restrict__ z, double* __restrict__ ln_ps) {
+    __shared__ double gc_all[ILE_MAX_MEMBERS * GMM_GC + ILE_MAX_MEMBERS];
+    block_gmm_consts(I, gc_all);
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= N) return;
     int a = 0;
@@ -197,15 +225,17 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
     }
     for (int c = 0; c < d; c++) z[(long long)c * N + i] = zz[c];
     // a standalone AV draws inside its own cells: p_s is the constant 1 / (v V0)
-    ln_ps[i] = (I.n_members == 1 && S.kind == ILE_KIND_AV) ? S.av->ln_ps : mixture_ln_pdf(I, zz);
+    ln_ps[i] = (I.n_members == 1 && S.kind == ILE_KIND_AV) ? S.av->ln_ps : mixture_ln_pdf(I, zz, gc_all);
 }
 
 __global__ void __launch_bounds__(128) ln_pdf_kernel(IntegDev I, int N, const double* __restrict__ z, double* __restrict__ ln_ps) {
+    __shared__ double gc_all[ILE_MAX_MEMBERS * GMM_GC + ILE_MAX_MEMBERS];
+    block_gmm_consts(I, gc_all);
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= N) return;
     double zz[ILE_MAX_D];
     for (int c = 0; c < I.d; c++) zz[c] = z[(long long)c * N + i];
-    ln_ps[i] = mixture_ln_pdf(I, zz);
+    ln_ps[i] = mixture_ln_pdf(I, zz, gc_all);
 }
 
 int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, double* ln_ps) {

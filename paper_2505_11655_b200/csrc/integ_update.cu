@@ -472,7 +472,9 @@ __global__ void av_commit_kernel(IntegDev I, int a, UpdScratch* us) {
 // ---------------------------------------------------------------- GMM (one weighted EM step)
 #define GMM_NACC 36                                         // 1 + d + d(d+1)/2 at d = 7; d = 8 needs 45
 #define GMM_NACC_MAX 48
-__device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g, const double* zz, double* e) {
+// gc: per-component constants in shared memory (gc[c] = sum_i ln L_c[i][i], gc[16 + c] = ln omega_c), computed
+// once per block; bit-identical to evaluating the logarithms per sample
+__device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g, const double* zz, double* e, const double* gc) {
     const int d = I.d, C = I.n_gmm;
     const double* omega = g;
     const double* mu = omega + C;
@@ -481,15 +483,14 @@ __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g
     for (int c = 0; c < C; c++) {
         const double* Lc = L + c * d * d;
         double y[ILE_MAX_D];
-        double quad = 0.0, lndet = 0.0;
+        double quad = 0.0;
         for (int i = 0; i < d; i++) {
             double s = zz[i] - mu[c * d + i];
             for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
             y[i] = s / Lc[i * d + i];
             quad = quad + y[i] * y[i];
-            lndet = lndet + log(Lc[i * d + i]);
         }
-        e[c] = -0.5 * quad - lndet - 0.5 * d * log(6.283185307179586) + log(omega[c]);
+        e[c] = -0.5 * quad - gc[c] - 0.5 * d * log(6.283185307179586) + gc[16 + c];
         mx = fmax(mx, e[c]);
     }
     return mx;
@@ -502,6 +503,15 @@ __global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N,
     if (us->abort || us->n_valid == 0) return;
     const int d = I.d, C = I.n_gmm;
     const double* g = I.mem[a].gmm;
+    __shared__ double gc[32];
+    if (threadIdx.x < C) {
+        const double* L = g + C + C * d + C * d * d;
+        double lndet = 0.0;
+        for (int i = 0; i < d; i++) lndet = lndet + log(L[threadIdx.x * d * d + i * d + i]);
+        gc[threadIdx.x] = lndet;
+        gc[16 + threadIdx.x] = log(g[threadIdx.x]);
+    }
+    __syncthreads();
     const double m = double_from_ord(us->m_ord);
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         const double w = lnw[i];
@@ -510,7 +520,7 @@ __global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N,
         for (int c = 0; c < d; c++) zz[c] = z[(long long)c * N + i];
         double mx = 0.0, sum = 1.0;
         if (ok) {
-            mx = ln_comp_all(I, g, zz, e);
+            mx = ln_comp_all(I, g, zz, e, gc);
             sum = 0.0;
             for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
         }
