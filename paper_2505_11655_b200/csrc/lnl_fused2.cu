@@ -173,9 +173,17 @@ __device__ __forceinline__ void round_setup(Fused2Smem<K>& sm, int lane) {
 
 // epilogue constants of sample s for the current tile base
 template <int K, bool TABLE>
-__device__ __forceinline__ void sample_consts(Fused2Smem<K>& sm, int s) {
+__device__ __forceinline__ void sample_consts(Fused2Smem<K>& sm, const LnlParams& P, int s) {
     const double x = sm.rec[s][12], Bs = sm.rec[s][13];
-    sm.ec[s] = make_double2(TABLE ? 0.0 : x * x * Bs, Bs);
+    if (TABLE) {
+        // distance table (G28): the B coordinate is per sample: row index and fraction of the clamped bilinear lookup
+        double b = (Bs - P.B_lo) / (P.B_hi - P.B_lo) * (double)(P.nB - 1);
+        b = fmin(fmax(b, 0.0), (double)(P.nB - 1));
+        const int ib = min((int)floor(b), P.nB - 2);
+        sm.ec[s] = make_double2(b - ib, (double)ib);
+    } else {
+        sm.ec[s] = make_double2(x * x * Bs, Bs);
+    }
 #pragma unroll
     for (int k = 0; k < K; k++) {
         const double f = sm.w1[k][s];
@@ -230,6 +238,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
     const int lane = tid & 31, w = tid >> 5;
     const int stride = STRIDE1 ? 1 : P.stride, N_t = P.N_t;
     const int c = lane & 3, rq = lane >> 2;
+    const double tabA_s = TABLE ? (double)(P.nA - 1) / (P.A_hi - P.A_lo) : 0.0, tabA_o = -P.A_lo * tabA_s;   // column coordinate of the distance table
     double2* ysm = reinterpret_cast<double2*>(&sm.S[0][0][0]);              // [F2_YM][F2_YS] during the prologue
     double* qpart = reinterpret_cast<double*>(ysm + F2_YM * F2_YS);            // [8 warps][3 K][32] partial quadratic sums
     double2* uvsm = reinterpret_cast<double2*>(qpart + F2_WARPS * 3 * K * 32); // packed U/V, up to F2_UVMAX entries
@@ -379,7 +388,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             }
             sm.rec[tid][13] = 0.25 * B;
         }
-        sample_consts<K, TABLE>(sm, tid);
+        sample_consts<K, TABLE>(sm, P, tid);
     }
     F2_T(13);
     const int n_part0 = tile_count<MODE>(slot, part0);
@@ -394,7 +403,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             tile_sync<MODE>(slot);
             if (sm.n_left == 0) break;
             last_round = sm.n_part == sm.n_left;
-            if (tid < TS) sample_consts<K, TABLE>(sm, tid);
+            if (tid < TS) sample_consts<K, TABLE>(sm, P, tid);
             tile_sync<MODE>(slot);
             need_setup = false;
         }
@@ -542,7 +551,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                     const double* Srow = &sm.S[0][s][0];
 #pragma unroll
                     for (int gi = 0; gi < NG; gi++) {
-                        double A = -cb.x;
+                        double A = TABLE ? 0.0 : -cb.x;
 #pragma unroll
                         for (int k = 0; k < K; k++) {
                             int r0;
@@ -556,7 +565,18 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                             A = fma(wk[k].x, row[0], A);
                             A = fma(wk[k].y, row[1], A);
                         }
-                        if (TABLE) A = table_lookup(P, A, cb.y);
+                        if (TABLE) {
+                            // lnT(A, B), bilinear and clamped: the row (cb.y) and its fraction (cb.x) are the sample's,
+                            // the column coordinate one FMA (no division per bin), each lerp a subtraction and an FMA
+                            double a = fma(A, tabA_s, tabA_o);
+                            a = fmin(fmax(a, 0.0), (double)(P.nA - 1));
+                            const int ia = min((int)a, P.nA - 2);
+                            const double fa = a - (double)ia;
+                            const double* T0 = P.lnT + (size_t)(int)cb.y * P.nA + ia;
+                            const double t00 = __ldg(T0), t01 = __ldg(T0 + 1), t10 = __ldg(T0 + P.nA), t11 = __ldg(T0 + P.nA + 1);
+                            const double t0 = fma(fa, t01 - t00, t00), t1 = fma(fa, t11 - t10, t10);
+                            A = fma(cb.x, t1 - t0, t0);
+                        }
                         v[i][gi] = A;
                         const double dl = A - run_m[i];
                         dh[i][gi] = inr[gi] ? __double2hiint(dl) : (int)0xFFF00000;
