@@ -229,6 +229,8 @@ extern "C" int ile_set_modes(ile_ctx* ctx, int M, const int* ell, const int* m) 
         ctx->m[i] = mm;
     }
     ctx->M = M;
+    ctx->ylm_max_pow = T.max_pow;
+    ctx->ylm_max_abs_m = T.max_abs_m;
     {   // pair list of the upper triangle, row by row
         std::vector<int2> pr;
         for (int a = 0; a < M; a++)

@@ -81,6 +81,7 @@ struct ile_ctx {
     double A_lo, A_hi, B_lo, B_hi;
     double* d_lnT;
     int variant;
+    int ylm_max_pow, ylm_max_abs_m;   // sizes of the harmonics' power and phase tables (shared-memory scratch of the prep kernel)
     void* pc_buf;                 // scratch of ile_precompute_quv (grow-only, freed at destroy)
     size_t pc_bytes;
     int fused_rb;                 // row blocks of 8 samples per CTA of the fused kernel: 4 (default, two CTAs per SM) or 8

@@ -62,7 +62,9 @@ __device__ __forceinline__ void antenna_dev(const LnlParams& P, const SampleIn& 
     double n[3] = {cd * cg, -cd * sg, sd};
     double X[3] = {-cp * sg - sp * cg * sd, -cp * cg + sp * sg * sd, sp * cd};
     double Y[3] = {sp * sg - cp * cg * sd, sp * cg + cp * sg * sd, cp * cd};
-    for (int k = 0; k < P.K; k++) {
+#pragma unroll
+    for (int k = 0; k < ILE_MAX_K; k++) {
+        if (k >= P.K) break;
         double fp = 0.0, fx = 0.0;
 #pragma unroll
         for (int a = 0; a < 3; a++)
@@ -102,6 +104,44 @@ __device__ __forceinline__ void ylm_dev(const YlmTable* __restrict__ T, double c
         int m = Y.m;
         int am = m < 0 ? -m : m;
         double c = cm[am], s = m < 0 ? -sm[am] : sm[am];
+        store(i, acc * c, acc * s);
+    }
+}
+
+// The same with the power and phase tables in shared memory, scr[q * stride + thread] (they are indexed by the
+// mode table at run time: as per-thread arrays they live in local memory, i.e. in L2/DRAM at 2^20 threads).
+// scr holds 2 (max_pow + 1) + 2 (max_abs_m + 1) doubles per thread.
+template <typename Store>
+__device__ __forceinline__ void ylm_dev_smem(const YlmTable* __restrict__ T, double ch, double sh, double phi, double* scr, int stride, Store store) {
+    const int mp = T->max_pow, mm = T->max_abs_m;
+    double* pc = scr;
+    double* ps = pc + (mp + 1) * stride;
+    double* cm = ps + (mp + 1) * stride;
+    double* sm = cm + (mm + 1) * stride;
+    double a = 1.0, b = 1.0;
+    pc[0] = 1.0;
+    ps[0] = 1.0;
+    for (int q = 1; q <= mp; q++) {
+        a *= ch;
+        b *= sh;
+        pc[q * stride] = a;
+        ps[q * stride] = b;
+    }
+    cm[0] = 1.0;
+    sm[0] = 0.0;
+    for (int q = 1; q <= mm; q++) {
+        double sq, cq;
+        sincos((double)q * phi, &sq, &cq);
+        cm[q * stride] = cq;
+        sm[q * stride] = sq;
+    }
+    const int M = T->M;
+    for (int i = 0; i < M; i++) {
+        const YlmMode& Y = T->mode[i];
+        double acc = 0.0;
+        for (int t = 0; t < Y.nterms; t++) acc += Y.coef[t] * pc[Y.pc[t] * stride] * ps[Y.ps[t] * stride];
+        const int m = Y.m, am = m < 0 ? -m : m;
+        const double c = cm[am * stride], s = m < 0 ? -sm[am * stride] : sm[am * stride];
         store(i, acc * c, acc * s);
     }
 }

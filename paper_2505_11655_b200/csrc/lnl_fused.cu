@@ -136,8 +136,19 @@ __global__ void __launch_bounds__(128) lnl_prep_kernel(LnlParams P, int N, int N
 // Steps 1-3 only (antenna, delays, harmonics, x, ln prior): one thread per sample, Y_m stored
 // straight into the tile (no per-thread arrays).  The U/V quadratic term B (step 4) is computed by
 // the fused kernel's prologue, where 8 threads share each sample.  rec[13] = 0 here.
-__global__ void __launch_bounds__(128) lnl_prep3_kernel(LnlParams P, int N, int Npad, const double* __restrict__ z, const int* __restrict__ perm,
-                                                        double* __restrict__ rec, double2* __restrict__ ytile, double* __restrict__ ln_prior) {
+__global__ void __launch_bounds__(128) lnl_prep3_kernel(LnlParams P, int N, int Npad, int scr_doubles, const double* __restrict__ z,
+                                                        const int* __restrict__ perm, double* __restrict__ rec, double2* __restrict__ ytile,
+                                                        double* __restrict__ ln_prior) {
+    // shared memory: the harmonics' per-thread power and phase tables, then a copy of the mode table
+    extern __shared__ __align__(16) double prep_scr[];
+    YlmTable* tab = reinterpret_cast<YlmTable*>(prep_scr + scr_doubles);
+    {
+        const int4* src = reinterpret_cast<const int4*>(P.ylm);
+        int4* dst = reinterpret_cast<int4*>(tab);
+        const int n16 = (int)((offsetof(YlmTable, mode) + (size_t)P.M * sizeof(YlmMode) + 15) / 16);
+        for (int q = threadIdx.x; q < n16; q += blockDim.x) dst[q] = src[q];
+    }
+    __syncthreads();
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= Npad) return;
     double2* yt = ytile + (size_t)(t / FT_TS) * FT_YM * FT_TS + (t % FT_TS);
@@ -157,7 +168,7 @@ __global__ void __launch_bounds__(128) lnl_prep3_kernel(LnlParams P, int N, int 
     }
     double Fp[ILE_MAX_K], Fx[ILE_MAX_K], tau[ILE_MAX_K];
     antenna_dev(P, s, Fp, Fx, tau);
-    ylm_dev(P.ylm, s.ch, s.sh, -s.phi_ref, [&](int m, double yr, double yi) { yt[m * FT_TS] = make_double2(yr, yi); });
+    ylm_dev_smem(tab, s.ch, s.sh, -s.phi_ref, prep_scr + threadIdx.x, blockDim.x, [&](int m, double yr, double yi) { yt[m * FT_TS] = make_double2(yr, yi); });
     for (int m = P.M; m < FT_YM; m++) yt[m * FT_TS] = make_double2(0.0, 0.0);
     double u[ILE_MAX_K];
 #pragma unroll
@@ -491,10 +502,15 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
     // the second-generation fused kernel computes the quadratic term itself (prologue)
     const int n2_ = 2 * P.M, np_ = n2_ / 8, rem_ = n2_ % 8;
     const bool gen2 = !ctx->fused_gen1 && rem_ >= 1 && rem_ <= 4 && ((P.K == 3 && np_ == 5) || (P.K == 2 && np_ == 1));
-    if (gen2 && !ctx->prep_gen1)
-        lnl_prep3_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
-    else
+    if (gen2 && !ctx->prep_gen1) {
+        // shared-memory scratch of the harmonics: (2 (max_pow + 1) + 2 (max_abs_m + 1)) doubles per thread
+        // ... and a copy of the mode table
+        const int scr_d = (2 * (ctx->ylm_max_pow + 1) + 2 * (ctx->ylm_max_abs_m + 1)) * 128;
+        const size_t scr = (size_t)scr_d * sizeof(double) + sizeof(YlmTable) + 16;
+        lnl_prep3_kernel<<<(tiles * FT_TS + 127) / 128, 128, scr, ctx->stream>>>(P, N, tiles * FT_TS, scr_d, z, perm, rec, yt, ln_prior);
+    } else {
         lnl_prep_kernel<<<(tiles * FT_TS + 127) / 128, 128, 0, ctx->stream>>>(P, N, tiles * FT_TS, z, perm, rec, yt, ln_prior);
+    }
     ILE_LAUNCH_CHECK(ctx);
     if (!ctx->fused_gen1) {
         rc = ctx->fused_gen3 ? ile_launch_fused3(ctx, P, N, rec, yt, perm, lnL, gen2 && !ctx->prep_gen1)
