@@ -241,7 +241,8 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
     const double tabA_s = TABLE ? (double)(P.nA - 1) / (P.A_hi - P.A_lo) : 0.0, tabA_o = -P.A_lo * tabA_s;   // column coordinate of the distance table
     double2* ysm = reinterpret_cast<double2*>(&sm.S[0][0][0]);              // [F2_YM][F2_YS] during the prologue
     double* qpart = reinterpret_cast<double*>(ysm + F2_YM * F2_YS);            // [8 warps][3 K][32] partial quadratic sums
-    double2* uvsm = reinterpret_cast<double2*>(qpart + F2_WARPS * 3 * K * 32); // packed U/V, up to F2_UVMAX entries
+    double* qred = qpart + F2_WARPS * 3 * K * 32;                           // [3 K][32] their sums
+    double2* uvsm = reinterpret_cast<double2*>(qred + 3 * K * 32);          // packed U/V, up to F2_UVMAX entries
 #ifdef F2_TIMERS
     long long tmark = clock64();
 #endif
@@ -365,6 +366,21 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
     const int n_valid = tile_count<MODE>(slot, valid);      // also publishes n, w1, base, A
     F2_T(12);
     if (n_valid == 0) return;
+    // the 8 partial sums of each of the 3 K quadratic-form components are added by all warps (8 components
+    // at a time): left to warp 0 alone it is a serial chain of ~100 FP64 instructions queueing behind the
+    // other CTA's DMMAs while 7 warps wait at the next barrier
+    if (quad) {
+        for (int v = w; v < 3 * K; v += F2_WARPS) {
+            double t[F2_WARPS];
+#pragma unroll
+            for (int ww = 0; ww < F2_WARPS; ww++) t[ww] = qpart[(ww * 3 * K + v) * 32 + lane];
+            double acc = t[0];
+#pragma unroll
+            for (int ww = 1; ww < F2_WARPS; ww++) acc += t[ww];
+            qred[v * 32 + lane] = acc;
+        }
+        tile_sync<MODE>(slot);
+    }
     // ---- round 0: who fits within F2_CAP of the base (normally everybody)
     bool part0 = false;
     if (tid < TS) {
@@ -376,13 +392,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             double B = 0.0;
 #pragma unroll
             for (int k = 0; k < K; k++) {
-                double uu = 0.0, vr = 0.0, vi = 0.0;
-#pragma unroll
-                for (int ww = 0; ww < F2_WARPS; ww++) {
-                    uu += qpart[(ww * 3 * K + 3 * k + 0) * 32 + tid];
-                    vr += qpart[(ww * 3 * K + 3 * k + 1) * 32 + tid];
-                    vi += qpart[(ww * 3 * K + 3 * k + 2) * 32 + tid];
-                }
+                const double uu = qred[(3 * k + 0) * 32 + tid], vr = qred[(3 * k + 1) * 32 + tid], vi = qred[(3 * k + 2) * 32 + tid];
                 const double fr = sm.rec[tid][k], fi = sm.rec[tid][4 + k];
                 B += (fr * fr + fi * fi) * uu + ((fr * fr - fi * fi) * vr - 2.0 * fr * fi * vi);
             }
