@@ -1,21 +1,25 @@
-// libile: fused lnL kernel (SURVEY 8(a) steps 5-6).  Design notes in DESIGN.md section 6; the
-// measurements behind it are in profiles/r1_pipes.md: on sm_100a a dependent DMMA.8x8x4 issues
-// every ~150 cycles while the pipe accepts one every 16, and DFMA shares that FP64 datapath.
-// Hence: 8 independent accumulator chains per warp in the contraction, and an epilogue that is
-// branch-free straight-line code over 8 independent (sample, 32-bin) groups with as few FP64
-// instructions per (sample, time bin) as the arithmetic allows.
+// libile: fused lnL kernel (SURVEY 8(a) steps 4-6).  Design notes in DESIGN.md section 6; the
+// measurements behind it are in profiles/r1_pipes.md: on sm_100a DMMA.8x8x4 and DFMA share one FP64
+// datapath (37 TFLOP/s either way), a dependent DMMA waits on the one before it, and every operand
+// fragment that is not register-resident costs 256 bytes of shared-memory/L1 wavefronts - the pipe
+// that is as busy as the FP64 datapath in this kernel.  Hence: 8 independent accumulator chains per
+// warp in the contraction; coefficient fragments read with conflict-free 128-bit loads, Q fragments
+// from a fragment-major global copy (whole 128-byte lines); an epilogue that is branch-free
+// straight-line code over 8 independent (sample, 32-bin) groups with as few FP64 instructions and
+// shared-memory wavefronts per (sample, time bin) as the arithmetic allows.
 //
 //   one CTA = 32 samples (delay-cell sorted), 8 warps, two CTAs per SM
-//   prologue      step 4, the U/V quadratic term B: the tile's harmonics and the packed upper-triangle
-//                 matrices are staged in the (still idle) S ring; warp w sums pairs w, w + 8, ...
-//                 for all 32 samples; then the coefficient fragments are built
+//   prologue      records, harmonics and the packed upper-triangle U/V staged by cp.async in the (still
+//                 idle) S ring; coefficient fragments built in DMMA A-fragment order; step 4, the U/V
+//                 quadratic term B: warp w walks a contiguous run of the upper triangle for all 32 samples
 //   contraction   S_k[s][n] = sum_r coef_k[s][r] Q_k[r][n]  (coef = x Re/Im(F_k Y_m), K-dim 2M):
 //                 unit = (detector k, 8 stored bins) x 32 samples; A fragments (coef) from shared
-//                 memory in fragment order, B fragments (Q) straight from global/L2 into registers,
-//                 loaded one unit ahead; D -> S ring in shared memory
+//                 memory, B fragments (Q) straight from global/L2 into registers, loaded one unit
+//                 ahead; D -> S ring in shared memory; phases of 64 new bins (80 in the first)
 //   epilogue      one warp per 4 sample rows, lanes along time: per-sample delay shift + linear
-//                 interpolation (2 FMA per detector), ln L(t_j) = A_j - x^2 B, streaming log-sum-exp
-//                 with a lazily raised reference and a 13-instruction exp
+//                 interpolation (2 FMA per detector), ln L(t_j) = A_j - x^2 B (or the distance table),
+//                 streaming log-sum-exp with a lazily raised reference and an 8-instruction table exp;
+//                 range logic on the high words in the integer pipe
 #include "common.cuh"
 #include "likelihood_dev.cuh"
 
@@ -43,7 +47,7 @@ struct Fused2Smem {
     double rec[F2_TS][F2_RECS];
     double w1[K][F2_TS];                     // interpolation fraction f
     double2 ew[F2_TS][K];                    // epilogue constants per sample: (1 - f_k, f_k)
-    double2 ec[F2_TS];                       // (x^2 B, B)
+    double2 ec[F2_TS];                       // (x^2 B, B); distance-table mode: (row fraction, row index) of the lookup
     int eoff[F2_TS][4];                      // n_k - base_k, clamped to [0, F2_CAP]
     int n[K][F2_TS];
     int base[4];
