@@ -11,9 +11,11 @@
 #define TWO_PI 6.283185307179586
 
 // ---------------------------------------------------------------- member densities
+template <int D>
 __device__ __forceinline__ double ln_pdf_ac(const IntegDev& I, const SamplerDev& S, const double* zz) {
     double out = 0.0;
-    for (int c = 0; c < I.d; c++) {
+#pragma unroll
+    for (int c = 0; c < D; c++) {
         const long long b = bin_index_dev(zz[c], I.lo[c], I.hi[c], I.nb);
         const double pdf = __ddiv_rn(__dmul_rn(S.pi[c * I.nb + b], (double)I.nb), __dsub_rn(I.hi[c], I.lo[c]));
         out = __dadd_rn(out, log(pdf));
@@ -21,10 +23,12 @@ __device__ __forceinline__ double ln_pdf_ac(const IntegDev& I, const SamplerDev&
     return out;
 }
 
+template <int D>
 __device__ __forceinline__ double ln_pdf_av(const IntegDev& I, const SamplerDev& S, const double* zz) {
     const AvState av = *S.av;
     unsigned long long key = 0, mul = 1;
-    for (int c = 0; c < I.d; c++) {
+#pragma unroll
+    for (int c = 0; c < D; c++) {
         key += (unsigned long long)bin_index_dev(zz[c], I.lo[c], I.hi[c], av.n) * mul;
         mul *= (unsigned long long)av.n;
     }
@@ -52,8 +56,10 @@ __device__ __forceinline__ void gmm_consts(const IntegDev& I, const double* g, d
 }
 
 // ln N(z; mu_c, Sigma_c) + ln omega_c for every component; returns the log-sum-exp
+template <int D>
 __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev& S, const double* zz, double* e_out, const double* gc) {
-    const int d = I.d, C = I.n_gmm;
+    constexpr int d = D;
+    const int C = I.n_gmm;
     const double* omega = S.gmm;
     const double* mu = omega + C;
     const double* L = mu + C * d + C * d * d;
@@ -61,10 +67,12 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
     double mx = neg_inf();
     for (int c = 0; c < C; c++) {
         const double* Lc = L + c * d * d;
-        double y[ILE_MAX_D];
+        double y[D];
         double quad = 0.0;
+#pragma unroll
         for (int i = 0; i < d; i++) {
             double s = zz[i] - mu[c * d + i];
+#pragma unroll
             for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
             y[i] = s / Lc[i * d + i];
             quad = quad + y[i] * y[i];
@@ -79,25 +87,28 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
     return mx + log(sum);
 }
 
+template <int D>
 __device__ __forceinline__ double member_ln_pdf(const IntegDev& I, int a, const double* zz, bool inbox, const double* gc_all) {
     const SamplerDev& S = I.mem[a];
     switch (S.kind) {
         case ILE_KIND_UNIFORM: return inbox ? -log(I.V0) : neg_inf();
-        case ILE_KIND_AC: return inbox ? ln_pdf_ac(I, S, zz) : neg_inf();
-        case ILE_KIND_AV: return inbox ? ln_pdf_av(I, S, zz) : neg_inf();
-        case ILE_KIND_GMM: return ln_pdf_gmm(I, S, zz, nullptr, gc_all + a * GMM_GC);
+        case ILE_KIND_AC: return inbox ? ln_pdf_ac<D>(I, S, zz) : neg_inf();
+        case ILE_KIND_AV: return inbox ? ln_pdf_av<D>(I, S, zz) : neg_inf();
+        case ILE_KIND_GMM: return ln_pdf_gmm<D>(I, S, zz, nullptr, gc_all + a * GMM_GC);
     }
     return neg_inf();
 }
 
+template <int D>
 __device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double* zz, const double* gc_all) {
     bool inbox = true;
-    for (int c = 0; c < I.d; c++) inbox = inbox && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
-    if (I.n_members == 1) return member_ln_pdf(I, 0, zz, inbox, gc_all);
+#pragma unroll
+    for (int c = 0; c < D; c++) inbox = inbox && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
+    if (I.n_members == 1) return member_ln_pdf<D>(I, 0, zz, inbox, gc_all);
     double e[ILE_MAX_MEMBERS];
     double mx = neg_inf();
     for (int a = 0; a < I.n_members; a++) {
-        e[a] = gc_all[ILE_MAX_MEMBERS * GMM_GC + a] + member_ln_pdf(I, a, zz, inbox, gc_all);
+        e[a] = gc_all[ILE_MAX_MEMBERS * GMM_GC + a] + member_ln_pdf<D>(I, a, zz, inbox, gc_all);
         mx = fmax(mx, e[a]);
     }
     if (!is_finite_d(mx)) return neg_inf();
@@ -144,6 +155,7 @@ __device__ __forceinline__ void block_gmm_consts(const IntegDev& I, double* gc_a
     if (any) __syncthreads();
 }
 
+template <int D>
 __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned int g, double* __restrict__ z, double* __restrict__ ln_ps) {
     __shared__ double gc_all[ILE_MAX_MEMBERS * GMM_GC + ILE_MAX_MEMBERS];
     block_gmm_consts(I, gc_all);
@@ -152,8 +164,8 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
     int a = 0;
     while (a + 1 < I.n_members && i >= I.port->offset[a + 1]) a++;
     const SamplerDev& S = I.mem[a];
-    const int d = I.d;
-    double zz[ILE_MAX_D];
+    constexpr int d = D;
+    double zz[D];
     double u0, u1;
     philox_pair(I.seed, (unsigned long long)i, g, 0u, &u0, &u1);
     if (S.kind == ILE_KIND_GMM) {
@@ -168,8 +180,9 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
             if (cw <= u0) comp = c + 1;
         }
         if (comp > C - 1) comp = C - 1;
-        double nrm[ILE_MAX_D + 1];
-        const int npair = (d + 1) / 2;
+        double nrm[D + 1];
+        constexpr int npair = (d + 1) / 2;
+#pragma unroll
         for (int p = 0; p < npair; p++) {
             double ua, ub;
             philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + p), &ua, &ub);
@@ -179,8 +192,10 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
             nrm[2 * p] = r * cs;
             nrm[2 * p + 1] = r * sn;
         }
+#pragma unroll
         for (int r = 0; r < d; r++) {
             double s = mu[comp * d + r];
+#pragma unroll
             for (int k = 0; k <= r; k++) s = s + L[comp * d * d + r * d + k] * nrm[k];
             zz[r] = s;
         }
@@ -195,6 +210,7 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
             key = S.keys[cell];
         }
         double ua = 0.0, ub = 0.0;
+#pragma unroll
         for (int c = 0; c < d; c++) {
             if ((c & 1) == 0) philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + (c >> 1)), &ua, &ub);
             const double u = (c & 1) ? ub : ua;
@@ -223,33 +239,46 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
             zz[c] = fmin(zc, I.below_hi[c]);
         }
     }
+#pragma unroll
     for (int c = 0; c < d; c++) z[(long long)c * N + i] = zz[c];
     // a standalone AV draws inside its own cells: p_s is the constant 1 / (v V0)
-    ln_ps[i] = (I.n_members == 1 && S.kind == ILE_KIND_AV) ? S.av->ln_ps : mixture_ln_pdf(I, zz, gc_all);
+    ln_ps[i] = (I.n_members == 1 && S.kind == ILE_KIND_AV) ? S.av->ln_ps : mixture_ln_pdf<D>(I, zz, gc_all);
 }
 
+template <int D>
 __global__ void __launch_bounds__(128) ln_pdf_kernel(IntegDev I, int N, const double* __restrict__ z, double* __restrict__ ln_ps) {
     __shared__ double gc_all[ILE_MAX_MEMBERS * GMM_GC + ILE_MAX_MEMBERS];
     block_gmm_consts(I, gc_all);
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= N) return;
-    double zz[ILE_MAX_D];
-    for (int c = 0; c < I.d; c++) zz[c] = z[(long long)c * N + i];
-    ln_ps[i] = mixture_ln_pdf(I, zz, gc_all);
+    double zz[D];
+#pragma unroll
+    for (int c = 0; c < D; c++) zz[c] = z[(long long)c * N + i];
+    ln_ps[i] = mixture_ln_pdf<D>(I, zz, gc_all);
 }
 
 int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, double* ln_ps) {
     ile_ctx* ctx = it->ctx;
     alloc_kernel<<<1, 32, 0, ctx->stream>>>(it->I, (long long)N);
     ILE_LAUNCH_CHECK(ctx);
-    draw_kernel<<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, g, z, ln_ps);
+    switch (it->I.d) {
+#define DRAW_CASE(D_) case D_: draw_kernel<D_><<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, g, z, ln_ps); break;
+        DRAW_CASE(1) DRAW_CASE(2) DRAW_CASE(3) DRAW_CASE(4) DRAW_CASE(5) DRAW_CASE(6) DRAW_CASE(7) DRAW_CASE(8)
+#undef DRAW_CASE
+        default: return ile_fail(ctx, ILE_EINVAL, "draw: d = %d", it->I.d);
+    }
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }
 
 int integ_launch_ln_pdf(ile_integrator* it, int N, const double* z, double* ln_ps) {
     ile_ctx* ctx = it->ctx;
-    ln_pdf_kernel<<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, z, ln_ps);
+    switch (it->I.d) {
+#define PDF_CASE(D_) case D_: ln_pdf_kernel<D_><<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, z, ln_ps); break;
+        PDF_CASE(1) PDF_CASE(2) PDF_CASE(3) PDF_CASE(4) PDF_CASE(5) PDF_CASE(6) PDF_CASE(7) PDF_CASE(8)
+#undef PDF_CASE
+        default: return ile_fail(ctx, ILE_EINVAL, "ln_pdf: d = %d", it->I.d);
+    }
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }
