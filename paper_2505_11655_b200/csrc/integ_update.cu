@@ -474,18 +474,22 @@ __global__ void av_commit_kernel(IntegDev I, int a, UpdScratch* us) {
 #define GMM_NACC_MAX 48
 // gc: per-component constants in shared memory (gc[c] = sum_i ln L_c[i][i], gc[16 + c] = ln omega_c), computed
 // once per block; bit-identical to evaluating the logarithms per sample
+template <int D>
 __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g, const double* zz, double* e, const double* gc) {
-    const int d = I.d, C = I.n_gmm;
+    constexpr int d = D;
+    const int C = I.n_gmm;
     const double* omega = g;
     const double* mu = omega + C;
     const double* L = mu + C * d + C * d * d;
     double mx = neg_inf();
     for (int c = 0; c < C; c++) {
         const double* Lc = L + c * d * d;
-        double y[ILE_MAX_D];
+        double y[D];
         double quad = 0.0;
+#pragma unroll
         for (int i = 0; i < d; i++) {
             double s = zz[i] - mu[c * d + i];
+#pragma unroll
             for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
             y[i] = s / Lc[i * d + i];
             quad = quad + y[i] * y[i];
@@ -498,10 +502,12 @@ __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g
 
 // E step: a[c][i] = responsibility of component c for sample i times its importance weight
 // (0 for samples outside the box or with a non-finite weight); one evaluation of the mixture per sample
+template <int D>
 __global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ lnw,
                                                        const UpdScratch* __restrict__ us, double* __restrict__ aw) {
     if (us->abort || us->n_valid == 0) return;
-    const int d = I.d, C = I.n_gmm;
+    constexpr int d = D;
+    const int C = I.n_gmm;
     const double* g = I.mem[a].gmm;
     __shared__ double gc[32];
     if (threadIdx.x < C) {
@@ -516,11 +522,12 @@ __global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N,
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
         const double w = lnw[i];
         const bool ok = is_finite_d(w) && in_box_dev(I, z, N, i);
-        double zz[ILE_MAX_D], e[16];
+        double zz[D], e[16];
+#pragma unroll
         for (int c = 0; c < d; c++) zz[c] = z[(long long)c * N + i];
         double mx = 0.0, sum = 1.0;
         if (ok) {
-            mx = ln_comp_all(I, g, zz, e, gc);
+            mx = ln_comp_all<D>(I, g, zz, e, gc);
             sum = 0.0;
             for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
         }
@@ -777,7 +784,11 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
             ILE_LAUNCH_CHECK(ctx);
             mask_max_kernel<<<grid, 256, 0, st>>>(I, N, z, lnw, nullptr, MASK_BOX, it->us);
             ILE_LAUNCH_CHECK(ctx);
-            gmm_resp_kernel<<<grid, 256, 0, st>>>(I, a, N, z, lnw, it->us, it->gmm_aw);
+            switch (I.d) {
+#define GMM_RESP(D) case D: gmm_resp_kernel<D><<<grid, 256, 0, st>>>(I, a, N, z, lnw, it->us, it->gmm_aw); break;
+                GMM_RESP(1) GMM_RESP(2) GMM_RESP(3) GMM_RESP(4) GMM_RESP(5) GMM_RESP(6) GMM_RESP(7) GMM_RESP(8)
+#undef GMM_RESP
+            }
             ILE_LAUNCH_CHECK(ctx);
             dim3 g(it->gmm_blocks, I.n_gmm);
             switch (I.d) {
