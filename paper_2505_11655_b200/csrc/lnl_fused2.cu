@@ -13,9 +13,10 @@
 //                 idle) S ring; coefficient fragments built in DMMA A-fragment order; step 4, the U/V
 //                 quadratic term B: warp w walks a contiguous run of the upper triangle for all 32 samples
 //   contraction   S_k[s][n] = sum_r coef_k[s][r] Q_k[r][n]  (coef = x Re/Im(F_k Y_m), K-dim 2M):
-//                 unit = (detector k, 8 stored bins) x 32 samples; A fragments (coef) from shared
-//                 memory, B fragments (Q) straight from global/L2 into registers, loaded one unit
-//                 ahead; D -> S ring in shared memory; phases of 64 new bins (80 in the first)
+//                 phases of 64 new bins; in a full phase a warp owns a pair of 8-bin tiles and every
+//                 coefficient fragment it reads from shared memory feeds two DMMAs (Q fragments stream
+//                 from global/L2 two steps ahead); the tail phase runs units of (detector k, 8 bins)
+//                 x 32 samples with the Q fragments loaded one unit ahead; D -> S ring in shared memory
 //   epilogue      one warp per 4 sample rows, lanes along time: per-sample delay shift + linear
 //                 interpolation (2 FMA per detector), ln L(t_j) = A_j - x^2 B (or the distance table),
 //                 streaming log-sum-exp with a lazily raised reference and an 8-instruction table exp;
@@ -39,6 +40,9 @@
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
 #define F2_UVMAX (300 * 3 * 2)   // packed U/V entries staged in shared memory (M <= 24: 300 pairs)
 #define F2_NG 2           // 32-bin groups per phase (at most 64 outputs per phase)
+#ifndef F2_NO_PAIRJOBS
+#define F2_PAIRJOBS       // full phases: contraction by pairs of bin tiles (profiles/r1_pipes.md); -DF2_NO_PAIRJOBS for the A/B
+#endif
 
 template <int K>
 struct Fused2Smem {
@@ -431,7 +435,11 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         const int cap = STRIDE1 ? sm.cap : F2_CAP;
         const int last_bin = stride * (N_t - 1) + 1 + cap;      // highest stored bin (relative to base) any sample reads
         int c_lo = 0, j0 = 0;
+#ifdef F2_PAIRJOBS
+        int ntiles = min((MODE == 0 ? F2_NEW : F2_RING) / 8, (last_bin + 1 - c_lo + 7) / 8);   // MODE 0: every full phase is 4 tile pairs
+#else
         int ntiles = min(F2_RING / 8, (last_bin + 1 - c_lo + 7) / 8);
+#endif
         for (;;) {
             const int c_hi = c_lo + ntiles * 8;
             int j1 = (c_hi - 1 - cap - 1) / stride + 1;         // outputs whose reads are all below c_hi ...
@@ -450,6 +458,105 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                 named_arrive(F3_BAR_EMPTY + slot, 128 + F2_THREADS);   // previous ring reads done, command valid
                 named_sync(F3_BAR_FULL + slot, 128 + F2_THREADS);      // S complete for bins < c_hi
             } else {
+#ifdef F2_PAIRJOBS
+            // ---------------- contraction of a full phase (8 bin tiles): warp (q, h) = (w % 4, w / 4) owns the pair of
+                // tiles (2 q, 2 q + 1) and, for K = 3, the work (detector h, all 4 row blocks) + (detector 2, row
+                // blocks 2 h and 2 h + 1); every coefficient fragment read from shared memory feeds two DMMAs
+                if (MODE == 0 && ntiles == 8)
+                {
+                    static_assert(K == 2 || K == 3, "contraction job split is written for two or three detectors");
+                    const int q = w & 3, h = w >> 2;
+                    if (2 * q < ntiles) {
+                        constexpr int NSTEP = NPAIR + (SINGLE ? 1 : 0);
+                        constexpr int NPART = K == 3 ? 2 : 1;
+                        constexpr int NG_ = NPART * NSTEP;
+                        const int t0 = 2 * q;
+                        const bool two = t0 + 1 < ntiles;                 // the last phase may end on a single tile
+                        const int t1 = two ? t0 + 1 : t0;
+                        const double* qp[NPART][2];
+#pragma unroll
+                        for (int part = 0; part < NPART; part++) {
+                            const int k = part == 0 ? h : 2;
+#pragma unroll
+                            for (int nt = 0; nt < 2; nt++) {
+                                const int row = sm.base[k] + c_lo + 8 * (nt ? t1 : t0) + rq;
+                                qp[part][nt] = P.Qf + (((size_t)k * P.N_Qpad + row) >> 1) * (2 * ILE_QT_ROW) + (row & 1) * 8;
+                            }
+                        }
+                        double2 bb[3][2];
+                        auto issue = [&](const int g) {
+                            const int part = g / NSTEP, st = g % NSTEP;
+#pragma unroll
+                            for (int nt = 0; nt < 2; nt++) {
+                                if (st < NPAIR) bb[g % 3][nt] = __ldg(reinterpret_cast<const double2*>(qp[part][nt] + 16 * st + 2 * c));
+                                else bb[g % 3][nt].x = __ldg(qp[part][nt] + 16 * NPAIR + c);
+                            }
+                        };
+                        issue(0);
+                        if (NG_ > 1) issue(1);
+                        double acc[RB][2][2];
+#pragma unroll
+                        for (int g = 0; g < NG_; g++) {
+                            if (g + 2 < NG_) issue(g + 2);
+                            const int part = g / NSTEP, st = g % NSTEP;
+                            const int k = part == 0 ? h : 2;
+                            const int nrb = part == 0 ? RB : RB / 2, rb0 = part == 0 ? 0 : 2 * h;
+                            if (st == 0) {
+#pragma unroll
+                                for (int r = 0; r < RB; r++) acc[r][0][0] = acc[r][0][1] = acc[r][1][0] = acc[r][1][1] = 0.0;
+                            }
+                            const double2* Ak = &sm.A[k][0][0][lane];
+                            if (st < NPAIR) {
+                                double2 a[RB];
+#pragma unroll
+                                for (int r = 0; r < RB; r++)
+                                    if (r < nrb) a[r] = Ak[(st * RB + rb0 + r) * 32];
+#pragma unroll
+                                for (int r = 0; r < RB; r++)
+                                    if (r < nrb) {
+                                        dmma2(acc[r][0][0], acc[r][0][1], a[r].x, bb[g % 3][0].x);
+                                        dmma2(acc[r][1][0], acc[r][1][1], a[r].x, bb[g % 3][1].x);
+                                    }
+#pragma unroll
+                                for (int r = 0; r < RB; r++)
+                                    if (r < nrb) {
+                                        dmma2(acc[r][0][0], acc[r][0][1], a[r].y, bb[g % 3][0].y);
+                                        dmma2(acc[r][1][0], acc[r][1][1], a[r].y, bb[g % 3][1].y);
+                                    }
+                            } else {
+#pragma unroll
+                                for (int r = 0; r < RB; r += 2)
+                                    if (r < nrb) {
+                                        const double2 as = Ak[(NPAIR * RB + ((rb0 + r) >> 1)) * 32];
+                                        dmma2(acc[r][0][0], acc[r][0][1], as.x, bb[g % 3][0].x);
+                                        dmma2(acc[r][1][0], acc[r][1][1], as.x, bb[g % 3][1].x);
+                                        dmma2(acc[r + 1][0][0], acc[r + 1][0][1], as.y, bb[g % 3][0].x);
+                                        dmma2(acc[r + 1][1][0], acc[r + 1][1][1], as.y, bb[g % 3][1].x);
+                                    }
+                            }
+                            if (st == NSTEP - 1) {
+#pragma unroll
+                                for (int nt = 0; nt < 2; nt++) {
+                                    if (nt == 1 && !two) break;
+                                    int cr = c_lo + 8 * (nt ? t1 : t0);
+                                    cr -= (cr / F2_RING) * F2_RING;
+                                    double* srow = &sm.S[k][8 * rb0 + rq][cr + 2 * c];
+#pragma unroll
+                                    for (int r = 0; r < RB; r++)
+                                        if (r < nrb) *reinterpret_cast<double2*>(srow + r * 8 * F2_SROW) = make_double2(acc[r][nt][0], acc[r][nt][1]);
+                                    if (cr == 0 && c == 0) {      // ring column F2_RING mirrors column 0: the epilogue reads [r], [r+1] unwrapped
+#pragma unroll
+                                        for (int r = 0; r < RB; r++)
+                                            if (r < nrb) srow[r * 8 * F2_SROW + F2_RING] = acc[r][nt][0];
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+
+                else
+#endif
             // ---------------- contraction: unit = (k, 8 bins) x 32 samples.  Q fragments of the next
                 // unit are loaded into the other register set while this one is multiplied.
                 {
