@@ -40,6 +40,9 @@
 #define F2_NP 6           // k-step pairs allocated per detector in the A-fragment table
 #define F2_UVMAX (300 * 3 * 2)   // packed U/V entries staged in shared memory (M <= 24: 300 pairs)
 #define F2_NG 2           // 32-bin groups per phase (at most 64 outputs per phase)
+#ifndef F2_LA
+#define F2_LA 2            // steps the Q fragments of the tile-pair contraction are loaded ahead
+#endif
 #ifndef F2_NO_PAIRJOBS
 #define F2_PAIRJOBS       // full phases: contraction by pairs of bin tiles (profiles/r1_pipes.md); -DF2_NO_PAIRJOBS for the A/B
 #endif
@@ -483,21 +486,21 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                                 qp[part][nt] = P.Qf + (((size_t)k * P.N_Qpad + row) >> 1) * (2 * ILE_QT_ROW) + (row & 1) * 8;
                             }
                         }
-                        double2 bb[3][2];
+                        double2 bb[F2_LA + 1][2];
                         auto issue = [&](const int g) {
                             const int part = g / NSTEP, st = g % NSTEP;
 #pragma unroll
                             for (int nt = 0; nt < 2; nt++) {
-                                if (st < NPAIR) bb[g % 3][nt] = __ldg(reinterpret_cast<const double2*>(qp[part][nt] + 16 * st + 2 * c));
-                                else bb[g % 3][nt].x = __ldg(qp[part][nt] + 16 * NPAIR + c);
+                                if (st < NPAIR) bb[g % (F2_LA + 1)][nt] = __ldg(reinterpret_cast<const double2*>(qp[part][nt] + 16 * st + 2 * c));
+                                else bb[g % (F2_LA + 1)][nt].x = __ldg(qp[part][nt] + 16 * NPAIR + c);
                             }
                         };
                         issue(0);
-                        if (NG_ > 1) issue(1);
+                        if (NG_ > 1 && F2_LA > 1) issue(1);
                         double acc[RB][2][2];
 #pragma unroll
                         for (int g = 0; g < NG_; g++) {
-                            if (g + 2 < NG_) issue(g + 2);
+                            if (g + F2_LA < NG_) issue(g + F2_LA);
                             const int part = g / NSTEP, st = g % NSTEP;
                             const int k = part == 0 ? h : 2;
                             const int nrb = part == 0 ? RB : RB / 2, rb0 = part == 0 ? 0 : 2 * h;
@@ -514,24 +517,24 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
 #pragma unroll
                                 for (int r = 0; r < RB; r++)
                                     if (r < nrb) {
-                                        dmma2(acc[r][0][0], acc[r][0][1], a[r].x, bb[g % 3][0].x);
-                                        dmma2(acc[r][1][0], acc[r][1][1], a[r].x, bb[g % 3][1].x);
+                                        dmma2(acc[r][0][0], acc[r][0][1], a[r].x, bb[g % (F2_LA + 1)][0].x);
+                                        dmma2(acc[r][1][0], acc[r][1][1], a[r].x, bb[g % (F2_LA + 1)][1].x);
                                     }
 #pragma unroll
                                 for (int r = 0; r < RB; r++)
                                     if (r < nrb) {
-                                        dmma2(acc[r][0][0], acc[r][0][1], a[r].y, bb[g % 3][0].y);
-                                        dmma2(acc[r][1][0], acc[r][1][1], a[r].y, bb[g % 3][1].y);
+                                        dmma2(acc[r][0][0], acc[r][0][1], a[r].y, bb[g % (F2_LA + 1)][0].y);
+                                        dmma2(acc[r][1][0], acc[r][1][1], a[r].y, bb[g % (F2_LA + 1)][1].y);
                                     }
                             } else {
 #pragma unroll
                                 for (int r = 0; r < RB; r += 2)
                                     if (r < nrb) {
                                         const double2 as = Ak[(NPAIR * RB + ((rb0 + r) >> 1)) * 32];
-                                        dmma2(acc[r][0][0], acc[r][0][1], as.x, bb[g % 3][0].x);
-                                        dmma2(acc[r][1][0], acc[r][1][1], as.x, bb[g % 3][1].x);
-                                        dmma2(acc[r + 1][0][0], acc[r + 1][0][1], as.y, bb[g % 3][0].x);
-                                        dmma2(acc[r + 1][1][0], acc[r + 1][1][1], as.y, bb[g % 3][1].x);
+                                        dmma2(acc[r][0][0], acc[r][0][1], as.x, bb[g % (F2_LA + 1)][0].x);
+                                        dmma2(acc[r][1][0], acc[r][1][1], as.x, bb[g % (F2_LA + 1)][1].x);
+                                        dmma2(acc[r + 1][0][0], acc[r + 1][0][1], as.y, bb[g % (F2_LA + 1)][0].x);
+                                        dmma2(acc[r + 1][1][0], acc[r + 1][1][1], as.y, bb[g % (F2_LA + 1)][1].x);
                                     }
                             }
                             if (st == NSTEP - 1) {
