@@ -31,7 +31,7 @@
 #define F2_SPW 4          // sample rows per warp in the epilogue
 #define F2_RING 80        // S ring length in stored bins (+ column F2_RING mirroring column 0)
 #define F2_SROW 88        // S row stride (== 8 mod 16: conflict-free 128-bit fragment stores)
-#define F2_NEW 64         // new stored bins per phase (phase 0: F2_RING)
+#define F2_NEW 64         // new stored bins per phase (phase 0 of the warp-specialised variant: F2_RING)
 #define F2_CAP 15         // largest per-sample offset above the tile base handled in one round
 #define F2_YM 24          // mode slots in the prep kernel's Y tile (32-sample sub-tiles)
 #define F2_YS 34          // row stride of the staged Y tile in shared memory (conflict-free fragment-builder reads)
