@@ -25,16 +25,13 @@ __device__ __forceinline__ SampleIn sample_from_angles(double ra, double dec, do
 __device__ __forceinline__ SampleIn sample_from_z(const LnlParams& P, const double* __restrict__ z, long long N, long long i) {
     SampleIn s;
     double v[6];
+    // all coordinate loads first (a check right after each load serialises six memory round trips)
+#pragma unroll
+    for (int c = 0; c < 6; c++) v[c] = c < P.d ? __ldg(z + (long long)c * N + i) : 1.0;
     bool ok = true;
 #pragma unroll
-    for (int c = 0; c < 6; c++) {
-        if (c < P.d) {
-            v[c] = z[(long long)c * N + i];
-            ok = ok && (v[c] >= P.lo[c]) && (v[c] < P.hi[c]);
-        } else {
-            v[c] = 1.0;
-        }
-    }
+    for (int c = 0; c < 6; c++)
+        if (c < P.d) ok = ok & (v[c] >= P.lo[c]) & (v[c] < P.hi[c]);
     s.valid = ok;
     s.ra = v[0];
     s.sd = v[1];
