@@ -289,6 +289,7 @@ class AV:
             R = int(r[kept].sum(dtype=np.uint64))
             v_new = (float(R) * 2.0 ** -FIX_ONE) * math.exp(-mn) / (float(N) * box_volume(self.lo, self.hi))
         dv = v_new / math.sqrt(float(N_min))
+        self.v_new, self.dv = v_new, dv                      # kept for inspection (tests); not used by the method
         inv = 1.0 / dv
         lo_n, hi_n = 1, self.n_max                           # largest n with n^d <= 1/dv (Eq. 13)
         while lo_n < hi_n:

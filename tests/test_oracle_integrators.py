@@ -205,6 +205,64 @@ def test_av_gaussian_volume_and_estimate():
     assert av.ln_pdf(far)[0] == -np.inf
 
 
+def test_av_member_rule_reduces_to_standalone_on_uniform_ps():
+    """SURVEY 8(c) "AV as a portfolio member": with the uniform p_s of the AV's own draw the importance
+    estimate of the kept volume, (1/(N V0)) sum_kept 1/p_s, is v_g N_min / N, so the
+    member rule must leave exactly the state the standalone rule leaves."""
+    d = 3
+    lo, hi = np.array([-2.0, 0.0, 1.0]), np.array([2.0, 3.0, 6.0])       # V0 = 60: a misplaced V0 cannot hide
+    lnf = lambda z: ln_gauss(z, [0.3, 1.2, 3.0], [0.4, 0.5, 0.9])
+    a = og.AV(lo, hi, 5, P_thr=0.98, N_min_star=128)
+    b = og.AV(lo, hi, 5, P_thr=0.98, N_min_star=128)
+    for g in range(4):
+        z, ln_ps = a.draw(1 << 13, g)
+        zb, ln_psb = b.draw(1 << 13, g)
+        assert np.array_equal(z, zb) and np.array_equal(ln_ps, ln_psb)
+        lnw = lnf(z) - ln_ps
+        a.update(z, lnw, None)                                            # standalone rule
+        b.update(z, lnw, ln_ps)                                           # member rule, uniform p_s
+        assert (a.n, a.N_min) == (b.n, b.N_min)
+        assert abs(b.L_thr - (a.L_thr + ln_ps[0])) < 1e-12                # ln f = ln w + ln p_s: a constant shift here
+        assert np.array_equal(a.keys, b.keys)
+        assert abs(b.v_new / a.v_new - 1.0) < 1e-14
+    assert a.n > 1 and len(a.keys) > 1
+
+
+def test_av_member_rule_volume_from_nonuniform_samples():
+    """Same rule on samples from a known non-uniform density: integrand = indicator of a box B of known
+    volume, samples from a product density with hand-set marginals (AC draw, pi set by hand).  With
+    P_thr = 1 every sample inside B is kept, and v' V0 = (1/N) sum_{in B} 1/p_s is the unbiased
+    importance estimate of vol(B): it must equal vol(B) within Monte Carlo error.  A dropped exp(-mn),
+    a V0 on the wrong side or a missing 1/N is off by factors, not per cent."""
+    d = 3
+    lo, hi = np.array([-1.0, 0.0, 2.0]), np.array([3.0, 2.0, 5.0])       # V0 = 24
+    V0 = og.box_volume(lo, hi)
+    ac = og.AC(lo, hi, 77, n_bins=8)
+    ramp = np.linspace(1.0, 3.0, 8)
+    for c in range(d):
+        ac.pi[c] = (ramp if c != 1 else ramp[::-1]) / ramp.sum()
+    ac._scan()
+    N = 1 << 17
+    z, ln_ps = ac.draw(N, 0)
+    blo, bhi = np.array([0.0, 0.5, 2.5]), np.array([2.0, 1.5, 4.0])      # vol(B) = 2 * 1 * 1.5 = 3
+    vol = float(np.prod(bhi - blo))
+    inside = og.in_box(z, blo, bhi)
+    lnw = np.where(inside, -ln_ps, -np.inf)                               # ln(f p / p_s), f = 1 in B, p = 1
+    av = og.AV(lo, hi, 1, P_thr=1.0, N_min_star=1)
+    av.update(z, lnw, ln_ps)
+    assert av.N_min == int(inside.sum())
+    # Monte Carlo error bound: Var(1_B / p_s) <= E[(1_B / p_s)^2] = int_B 1/p_s <= vol(B) max(1/p_s)
+    sigma = math.sqrt(vol * math.exp(-ln_ps.min()) / N)
+    assert abs(av.v_new * V0 - vol) < 5 * sigma
+    assert sigma < 0.03 * vol                                             # ... and the bound is tight enough to matter
+    # Eq. 13 with that volume: n^d <= sqrt(N_min) / v' < (n + 1)^d, and the cells cover B, not more than a layer around it
+    inv_dv = math.sqrt(av.N_min) / av.v_new
+    assert av.n ** d <= inv_dv < (av.n + 1) ** d
+    cover = len(av.keys) / float(av.n) ** d * V0
+    layer = np.prod(bhi - blo + 2 * (hi - lo) / av.n)
+    assert 0.9 * vol < cover <= layer
+
+
 # ------------------------------------------------------------------------------- GMM + P11 portfolio
 def test_gmm_pdf_normalised_and_em_moves_to_target():
     lo, hi = np.array([-8.0, -8.0]), np.array([8.0, 8.0])
