@@ -168,11 +168,12 @@ int ile_lnL(ile_ctx *ctx, int p, int N, const double *ra, const double *dec, con
             double *lnL_t /*[N][N_t] or NULL*/);
 /* Same at integrator coordinates z = (RA, sin Dec, psi, phi_ref, cos incl[, D]), d = 5 or 6; the
  * kernel the integrators call.  Samples outside the prior box get lnL = -inf.  ln_prior
- * (optional) receives ln p(z).  ile_set_lnL_variant: 0 = default (samples ordered by delay cell
- * on the device, then the fused DMMA kernel), 1 = plain one-thread-per-sample kernel (in-library
- * cross-check), 2 = fused kernel without the delay-cell ordering, 3 = first-generation fused kernel,
- * 4 = default fused kernel behind the one-thread-per-sample preparation kernel (which then also
- * computes the quadratic term), 5 = warp-specialised persistent fused kernel (experimental, slower). */
+ * (optional) receives ln p(z).  ile_set_lnL_variant selects the kernel behind this call (and behind the
+ * integrators): 0 = default: samples ordered by delay cell on the device, then the fused kernel whose contraction
+ * (step 5) runs exactly, in signed 8-bit digits, on the Blackwell tensor cores (tcgen05, K <= 3 detectors, M <= 24
+ * modes, time step of one stored bin; other shapes take variant 2); 1 = plain one-thread-per-sample kernel
+ * (in-library cross-check); 2 = delay-cell ordering + the fused FP64 DMMA kernel; 3 = the DMMA kernel without the
+ * ordering.  All variants meet the same tolerance; ILE_EINVAL for other values. */
 int ile_lnL_z(ile_ctx *ctx, int p, int N, int d, const double *z /*[d][N]*/, double *lnL /*[N]*/,
               double *ln_prior /*[N] or NULL*/);
 int ile_set_lnL_variant(ile_ctx *ctx, int variant);

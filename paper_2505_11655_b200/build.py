@@ -19,7 +19,6 @@ LIB = os.path.join(HERE, "libile.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "--expt-extended-lambda"]
-EXTRA = os.environ.get("ILE_NVCC_EXTRA", "").split()      # e.g. -DF2_G=2 for kernel experiments
 PER_FILE = {"integ_draw.cu": ["-fmad=false"], "integ_update.cu": ["-fmad=false"], "integ_api.cu": ["-fmad=false"], "fairdraw.cu": ["-fmad=false"]}
 
 
@@ -44,7 +43,7 @@ def _compile(src: str, force: bool, verbose: bool) -> str:
         t = os.path.getmtime(obj)
         if all(os.path.getmtime(p) <= t for p in [src] + _deps()):
             return obj
-    cmd = [NVCC] + FLAGS + EXTRA + PER_FILE.get(os.path.basename(src), []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+    cmd = [NVCC] + FLAGS + PER_FILE.get(os.path.basename(src), []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)

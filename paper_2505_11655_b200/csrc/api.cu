@@ -105,7 +105,7 @@ extern "C" int ile_create(ile_ctx** out, int device, void* cuda_stream) {
     ctx->D_min = 1.0;
     ctx->D_max = 2.0;
     ctx->sky_sort = 1;
-    ctx->fused_rb = 4;
+    ctx->lnl_split = 1;
     *out = ctx;
     return ILE_OK;
 }
@@ -116,8 +116,11 @@ extern "C" int ile_destroy(ile_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->d_ylm);
     cudaFree(ctx->d_Qc);
-    cudaFree(ctx->d_Qt);
     cudaFree(ctx->d_Qf);
+    cudaFree(ctx->d_Qs);
+    cudaFree(ctx->d_qeb);
+    cudaFree(ctx->d_qhi);
+    free(ctx->h_qeb);
     cudaFree(ctx->pc_buf);
     cudaFree(ctx->d_U);
     cudaFree(ctx->d_V);
@@ -143,13 +146,10 @@ extern "C" int ile_sync(ile_ctx* ctx) {
 }
 
 extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
-    if (!ctx || variant < 0 || variant > 5) return ile_fail(ctx, ILE_EINVAL, "variant must be 0..5");
-    ctx->fused_gen3 = variant == 5 ? 1 : 0;
-    ctx->fused_rb = variant == 4 ? 8 : 4;
+    if (!ctx || variant < 0 || variant > 3) return ile_fail(ctx, ILE_EINVAL, "variant must be 0..3");
     ctx->variant = variant == 1 ? 1 : 0;
-    ctx->sky_sort = variant == 2 ? 0 : 1;
-    ctx->fused_gen1 = variant == 3 ? 1 : 0;
-    ctx->prep_gen1 = (variant == 3 || variant == 4) ? 1 : 0;
+    ctx->lnl_split = variant == 0 ? 1 : 0;
+    ctx->sky_sort = variant == 3 ? 0 : 1;
     return ILE_OK;
 }
 
@@ -254,7 +254,7 @@ extern "C" int ile_set_modes(ile_ctx* ctx, int M, const int* ell, const int* m) 
 // LDS.128 of the fused kernel is bank-conflict free.
 // Qf holds the same values fragment-major, [N_Qpad/2 bin pairs][6 k-step pairs][2 bins][8 columns]:
 // the 8 bins x 4 lanes x 16 bytes of one DMMA B-fragment load are four whole 128-byte lines.
-__global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restrict__ Qt, double* __restrict__ Qf, int PK, int M, int N_Q,
+__global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restrict__ Qf, int PK, int M, int N_Q,
                                 int N_Qpad) {
     long long total = (long long)PK * N_Qpad * ILE_QT_ROW;
     for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
@@ -266,7 +266,6 @@ __global__ void repack_q_kernel(const double* __restrict__ Qc, double* __restric
         int mode = r >> 1, part = r & 1;
         double v = 0.0;
         if (mode < M && n < N_Q) v = Qc[(((long long)pk * M + mode) * N_Q + n) * 2 + part];
-        Qt[idx] = v;
         Qf[(((long long)pk * N_Qpad + n) >> 1) * (2 * ILE_QT_ROW) + (r >> 3) * 16 + (n & 1) * 8 + (r & 7)] = v;
     }
 }
@@ -331,11 +330,16 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     const bool reuse = ctx->have_quv && ctx->P == P && ctx->N_Q == N_Q && ctx->quv_K == K && ctx->quv_M == M;
     ctx->have_quv = false;
     if (!reuse) {
-        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qt); cudaFree(ctx->d_Qf); cudaFree(ctx->d_U); cudaFree(ctx->d_V); cudaFree(ctx->d_UVp);
-        ctx->d_Qc = ctx->d_Qt = ctx->d_Qf = ctx->d_U = ctx->d_V = ctx->d_UVp = nullptr;
-        if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qt, nQt * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qf, nQt * 8) != cudaSuccess ||
+        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qf); cudaFree(ctx->d_U); cudaFree(ctx->d_V); cudaFree(ctx->d_UVp);
+        cudaFree(ctx->d_Qs); cudaFree(ctx->d_qeb); cudaFree(ctx->d_qhi); free(ctx->h_qeb);
+        ctx->d_Qc = ctx->d_Qf = ctx->d_U = ctx->d_V = ctx->d_UVp = nullptr;
+        ctx->d_Qs = nullptr; ctx->d_qeb = nullptr; ctx->d_qhi = nullptr;
+        ctx->h_qeb = (int*)malloc((size_t)P * K * sizeof(int));
+        if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qf, nQt * 8) != cudaSuccess ||
             cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess ||
-            cudaMalloc(&ctx->d_UVp, (size_t)P * ctx->n_pairs * K * 4 * 8) != cudaSuccess) {
+            cudaMalloc(&ctx->d_UVp, (size_t)P * ctx->n_pairs * K * 4 * 8) != cudaSuccess ||
+            cudaMalloc(&ctx->d_Qs, ile_split_qs_bytes(P, K, N_Q)) != cudaSuccess || cudaMalloc(&ctx->d_qeb, (size_t)P * K * sizeof(int)) != cudaSuccess ||
+            cudaMalloc(&ctx->d_qhi, (size_t)P * K * sizeof(int)) != cudaSuccess || !ctx->h_qeb) {
             cudaGetLastError();
             return ile_fail(ctx, ILE_ENOMEM, "load_quv: device allocation failed");
         }
@@ -344,10 +348,16 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_Qc, Q, nQ * 8, kind, ctx->stream));
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_U, U, nU * 8, kind, ctx->stream));
     ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, V, nU * 8, kind, ctx->stream));
-    repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qt, ctx->d_Qf, P * K, M, N_Q, N_Qpad);
+    repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qf, P * K, M, N_Q, N_Qpad);
     ILE_LAUNCH_CHECK(ctx);
     pack_uv_kernel<<<ctx->sm_count * 2, 256, 0, ctx->stream>>>(ctx->d_U, ctx->d_V, ctx->d_pairs, ctx->d_UVp, P, K, M, ctx->n_pairs);
     ILE_LAUNCH_CHECK(ctx);
+    if (K <= 3 && M <= 24) {
+        // signed 8-bit digit image of Q for the tcgen05 contraction (lnl_split.cu)
+        int rc = ile_split_build_q(ctx, P, K, M, N_Q, ctx->d_Qc, ctx->d_Qs, ctx->d_qeb, ctx->d_qhi);
+        if (rc) return rc;
+        ILE_CUDA(ctx, cudaMemcpyAsync(ctx->h_qeb, ctx->d_qeb, (size_t)P * K * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    }
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ctx->P = P; ctx->N_Q = N_Q; ctx->N_Qpad = N_Qpad; ctx->quv_K = K; ctx->quv_M = M; ctx->fs = fs; ctx->t_Q0 = t_Q0; ctx->D_ref = D_ref;
     ctx->have_quv = true;
@@ -419,7 +429,6 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
     L->nA = ctx->nA; L->nB = ctx->nB; L->A_lo = ctx->A_lo; L->A_hi = ctx->A_hi; L->B_lo = ctx->B_lo; L->B_hi = ctx->B_hi;
     L->lnT = ctx->d_lnT;
     L->Qc = ctx->d_Qc + (size_t)p * K * M * ctx->N_Q * 2;
-    L->Qt = ctx->d_Qt + (size_t)p * K * ctx->N_Qpad * ILE_QT_ROW;
     L->Qf = ctx->d_Qf + (size_t)p * K * ctx->N_Qpad * ILE_QT_ROW;
     L->U = ctx->d_U + (size_t)p * K * M * M * 2;
     L->V = ctx->d_V + (size_t)p * K * M * M * 2;
@@ -427,5 +436,11 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
     L->pairs = ctx->d_pairs;
     L->n_pairs = ctx->n_pairs;
     L->UVp = ctx->d_UVp + (size_t)p * ctx->n_pairs * K * 4;
+    L->Qs = nullptr;
+    if (K <= 3 && M <= 24 && ctx->d_Qs) {
+        L->NG8 = ile_split_ng8(ctx->N_Q);
+        L->Qs = ctx->d_Qs + (size_t)p * K * L->NG8 * 2432;
+        for (int k = 0; k < K; k++) L->qeb[k] = ctx->h_qeb[p * K + k];
+    }
     return ILE_OK;
 }

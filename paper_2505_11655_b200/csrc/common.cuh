@@ -48,7 +48,6 @@ struct LnlParams {
     const double* lnT;
     // per intrinsic point data (already offset to point p)
     const double* Qc;             // [K][M][N_Q][2]
-    const double* Qt;             // [K][N_Qpad][48] tiled + swizzled
     const double* Qf;             // [K][N_Qpad/2][6][2][8] fragment-major: one 128-byte line per (bin pair, k-step pair)
     const double* U;              // [K][M][M][2]
     const double* V;              // [K][M][M][2]
@@ -58,6 +57,11 @@ struct LnlParams {
     const int2* pairs;
     int n_pairs;
     const double* UVp;
+    // signed 8-bit digits of Q for the tcgen05 contraction (lnl_split.cu): image of point p, groups of 8 bins per
+    // detector, biased exponent of max |Q_k| (the integer scale is 2^(45 - (qeb - 1023)))
+    const unsigned char* Qs;
+    int NG8;
+    int qeb[ILE_MAX_K];
 };
 
 struct ile_ctx {
@@ -71,7 +75,11 @@ struct ile_ctx {
     YlmTable h_ylm;
     YlmTable* d_ylm;
     double fs, t_Q0, D_ref;
-    double *d_Qc, *d_Qt, *d_Qf, *d_U, *d_V, *d_UVp;
+    double *d_Qc, *d_Qf, *d_U, *d_V, *d_UVp;
+    unsigned char* d_Qs;          // Q digits for the tcgen05 contraction, [P][K][NG8][2432 bytes]
+    int* d_qeb;                   // [P][K] biased exponent of max |Q|
+    unsigned int* d_qhi;          // scratch of the same size
+    int* h_qeb;                   // host copy of d_qeb
     int2* d_pairs;
     int n_pairs;
     double t_lo, dt;
@@ -84,10 +92,7 @@ struct ile_ctx {
     int ylm_max_pow, ylm_max_abs_m;   // sizes of the harmonics' power and phase tables (shared-memory scratch of the prep kernel)
     void* pc_buf;                 // scratch of ile_precompute_quv (grow-only, freed at destroy)
     size_t pc_bytes;
-    int fused_rb;                 // row blocks of 8 samples per CTA of the fused kernel: 4 (default, two CTAs per SM) or 8
-    int fused_gen3;               // 1: warp-specialised persistent fused kernel
-    int prep_gen1;                // 1: one-thread-per-sample prep kernel (A/B timing)
-    int fused_gen1;               // 1: first-generation fused kernel (kept for A/B timing)
+    int lnl_split;                // 1 (default): tcgen05 integer-digit fused kernel (lnl_split.cu) where the shape allows
     int sky_sort;                 // 1 (default): order samples by delay cell before the fused kernel
     int sm_count;
     // scratch
@@ -109,6 +114,19 @@ int ile_launch_lnL_z(ile_ctx* ctx, int p, int N, int d, const double* z, const i
                      double* ln_prior);
 int ile_launch_reduce(ile_ctx* ctx, int N, const double* lnw, ile_result* out_dev, int accumulate);
 uint64_t ile_launch_count(ile_ctx* ctx);
+// tcgen05 path (lnl_split.cu)
+struct SpTile;
+size_t ile_split_qs_bytes(int P, int K, int N_Q);
+int ile_split_ng8(int N_Q);
+int ile_split_build_q(ile_ctx* ctx, int P, int K, int M, int N_Q, const double* d_Qc, unsigned char* d_Qs, int* d_qeb, unsigned int* d_qhi);
+bool ile_split_supported(const LnlParams& P);
+int ile_split_cell_bits(int n_min, int n_max);
+int ile_split_max_tiles(int N, int cell_bits, int K);
+size_t ile_split_tile_bytes(int max_tiles);
+int ile_launch_split_keys(ile_ctx* ctx, const LnlParams& P, int N, const double* z, int n_min, int cell_bits, unsigned long long* key,
+                          unsigned int* val, long long* n_dev, int* bits_dev, int* ntiles_dev);
+int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int cell_bits, const unsigned long long* key, const double* rec, const double2* yt,
+                     const int* perm, double* lnL, int* tstart, SpTile* tiles, int* ntiles_dev);
 int ile_timing_begin(ile_ctx* ctx);            // returns a slot (or -1 when timing is off)
 void ile_timing_end(ile_ctx* ctx, int slot);
 int ile_timing_drain(ile_ctx* ctx);

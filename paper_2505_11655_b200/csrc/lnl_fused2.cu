@@ -23,6 +23,7 @@
 //                 range logic on the high words in the integer pipe
 #include "common.cuh"
 #include "likelihood_dev.cuh"
+#include "exp_tab.cuh"
 
 #define F2_THREADS 256
 #define F2_WARPS 8
@@ -31,7 +32,7 @@
 #define F2_SPW 4          // sample rows per warp in the epilogue
 #define F2_RING 80        // S ring length in stored bins (+ column F2_RING mirroring column 0)
 #define F2_SROW 88        // S row stride (== 8 mod 16: conflict-free 128-bit fragment stores)
-#define F2_NEW 64         // new stored bins per phase (phase 0 of the warp-specialised variant: F2_RING)
+#define F2_NEW 64         // new stored bins per phase
 #define F2_CAP 15         // largest per-sample offset above the tile base handled in one round
 #define F2_YM 24          // mode slots in the prep kernel's Y tile (32-sample sub-tiles)
 #define F2_YS 34          // row stride of the staged Y tile in shared memory (conflict-free fragment-builder reads)
@@ -93,25 +94,6 @@ __device__ __forceinline__ double exp_small(double d) {
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
 }
 
-// 2^(j/64), j = 0..63, correctly rounded
-__device__ const double f2_exp2_tab[64] = {
-    0x1.0000000000000p+0, 0x1.02c9a3e778061p+0, 0x1.059b0d3158574p+0, 0x1.0874518759bc8p+0,
-    0x1.0b5586cf9890fp+0, 0x1.0e3ec32d3d1a2p+0, 0x1.11301d0125b51p+0, 0x1.1429aaea92de0p+0,
-    0x1.172b83c7d517bp+0, 0x1.1a35beb6fcb75p+0, 0x1.1d4873168b9aap+0, 0x1.2063b88628cd6p+0,
-    0x1.2387a6e756238p+0, 0x1.26b4565e27cddp+0, 0x1.29e9df51fdee1p+0, 0x1.2d285a6e4030bp+0,
-    0x1.306fe0a31b715p+0, 0x1.33c08b26416ffp+0, 0x1.371a7373aa9cbp+0, 0x1.3a7db34e59ff7p+0,
-    0x1.3dea64c123422p+0, 0x1.4160a21f72e2ap+0, 0x1.44e086061892dp+0, 0x1.486a2b5c13cd0p+0,
-    0x1.4bfdad5362a27p+0, 0x1.4f9b2769d2ca7p+0, 0x1.5342b569d4f82p+0, 0x1.56f4736b527dap+0,
-    0x1.5ab07dd485429p+0, 0x1.5e76f15ad2148p+0, 0x1.6247eb03a5585p+0, 0x1.6623882552225p+0,
-    0x1.6a09e667f3bcdp+0, 0x1.6dfb23c651a2fp+0, 0x1.71f75e8ec5f74p+0, 0x1.75feb564267c9p+0,
-    0x1.7a11473eb0187p+0, 0x1.7e2f336cf4e62p+0, 0x1.82589994cce13p+0, 0x1.868d99b4492edp+0,
-    0x1.8ace5422aa0dbp+0, 0x1.8f1ae99157736p+0, 0x1.93737b0cdc5e5p+0, 0x1.97d829fde4e50p+0,
-    0x1.9c49182a3f090p+0, 0x1.a0c667b5de565p+0, 0x1.a5503b23e255dp+0, 0x1.a9e6b5579fdbfp+0,
-    0x1.ae89f995ad3adp+0, 0x1.b33a2b84f15fbp+0, 0x1.b7f76f2fb5e47p+0, 0x1.bcc1e904bc1d2p+0,
-    0x1.c199bdd85529cp+0, 0x1.c67f12e57d14bp+0, 0x1.cb720dcef9069p+0, 0x1.d072d4a07897cp+0,
-    0x1.d5818dcfba487p+0, 0x1.da9e603db3285p+0, 0x1.dfc97337b9b5fp+0, 0x1.e502ee78b3ff6p+0,
-    0x1.ea4afa2a490dap+0, 0x1.efa1bee615a27p+0, 0x1.f50765b6e4540p+0, 0x1.fa7c1819e90d8p+0,
-};
 
 // exp(d) for d in [-40, 31] in 8 FP64 instructions: k = rint(64 d / ln2) by the magic-number add,
 // r = d - k ln2/64 (|r| <= 0.00542; the rounding of ln2/64 costs < 3e-15 for |d| <= 40),
@@ -136,13 +118,6 @@ __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
 }
-
-#ifdef F2_TIMERS
-__device__ unsigned long long f2_timers[16];
-#define F2_T(i) do { const long long t__ = clock64(); if (lane == 0) atomicAdd(&f2_timers[i], (unsigned long long)(t__ - tmark)); tmark = t__; } while (0)
-#else
-#define F2_T(i)
-#endif
 
 // general round set-up (warp 0): tile base = even floor of the per-detector minimum first bin over
 // the unfinished samples; a sample takes part when all its offsets are within F2_CAP; when none
@@ -205,43 +180,8 @@ __device__ __forceinline__ void sample_consts(Fused2Smem<K>& sm, const LnlParams
     }
 }
 
-// ---------------------------------------------------------------- synchronisation policies
-// MODE 0: the tile is processed by a whole CTA (256 threads) that also does its own contraction.
-// MODE 1: the tile is processed by one 8-warp epilogue group of a warp-specialised persistent CTA;
-//         the contraction is done by the CTA's dedicated warps (lnl_fused3_kernel), handed over
-//         through a command block and two named barriers per slot.
-#define F3_MW 4                       // contraction warps (warpgroup 0)
-#ifndef F3_MREGS
-#define F3_MREGS 224                  // registers per thread of the contraction warps after setmaxnreg
-#endif
-#ifndef F3_EREGS
-#define F3_EREGS 64                   // ... and of the epilogue warps
-#endif
-#define F3_THREADS (128 + 2 * F2_THREADS)
-enum { F3_BAR_GROUP = 1, F3_BAR_FULL = 3, F3_BAR_EMPTY = 5 };   // + slot
-struct F3Cmd {
-    int go;                           // 0: this slot's group has no more tiles
-    int c_lo, ntiles;                 // ring bins [c_lo, c_lo + 8 ntiles) are to be computed
-    int base[3];                      // tile base bin per detector
-    int pad[2];
-};
-__device__ __forceinline__ void named_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
-__device__ __forceinline__ void named_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
-template <int MODE>
-__device__ __forceinline__ void tile_sync(int slot) {
-    if (MODE == 0) __syncthreads();
-    else named_sync(F3_BAR_GROUP + slot, F2_THREADS);
-}
-template <int MODE>
-__device__ __forceinline__ int tile_count(int slot, bool pred) {
-    if (MODE == 0) return __syncthreads_count(pred);
-    int r;
-    asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n bar.red.popc.u32 %0, %1, %2, p;\n}" : "=r"(r) : "r"(F3_BAR_GROUP + slot), "r"(F2_THREADS), "r"((int)pred) : "memory");
-    return r;
-}
-
-template <int MODE, int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
-__device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const int slot, const int tid, const int tile, const LnlParams& P,
+template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
+__device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, const int tid, const int tile, const LnlParams& P,
                                           const int N, const int quad, const double* __restrict__ rec, const double2* __restrict__ ytile,
                                           const int* __restrict__ perm, double* __restrict__ lnL) {
     constexpr int RB = F2_RB, TS = F2_TS, SPW = F2_SPW, NG = F2_NG;
@@ -254,9 +194,6 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
     double* qpart = reinterpret_cast<double*>(ysm + F2_YM * F2_YS);            // [8 warps][3 K][32] partial quadratic sums
     double* qred = qpart + F2_WARPS * 3 * K * 32;                           // [3 K][32] their sums
     double2* uvsm = reinterpret_cast<double2*>(qred + 3 * K * 32);          // packed U/V, up to F2_UVMAX entries
-#ifdef F2_TIMERS
-    long long tmark = clock64();
-#endif
 
     // ---- stage the tile's records; tile base by shared-memory atomicMin
     {
@@ -279,9 +216,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         if (tid >= 64 && tid < 128) sm.etab[tid - 64] = f2_exp2_tab[tid - 64];
         asm volatile("cp.async.commit_group;\n cp.async.wait_group 0;" ::: "memory");
     }
-    F2_T(8);
-    tile_sync<MODE>(slot);
-    F2_T(9);
+    __syncthreads();
     bool valid = false;
     if (tid < TS) {
         valid = sm.rec[tid][14] != 0.0;
@@ -324,7 +259,6 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             }
         }
     }
-    F2_T(10);
     // ---- step 4, the U/V quadratic term (Eq. 7 with the Eq. 17-18 symmetries): warp w sums the
     //      upper-triangle pairs w, w + 8, ... for all 32 samples (lane = sample; the packed matrix
     //      entries are warp-uniform loads); partial sums meet in shared memory
@@ -373,9 +307,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             qpart[(w * 3 * K + 3 * k + 2) * 32 + lane] = vi[k];
         }
     }
-    F2_T(11);
-    const int n_valid = tile_count<MODE>(slot, valid);      // also publishes n, w1, base, A
-    F2_T(12);
+    const int n_valid = __syncthreads_count(valid);      // also publishes n, w1, base, A
     if (n_valid == 0) return;
     // the 8 partial sums of each of the 3 K quadratic-form components are added by all warps (8 components
     // at a time): left to warp 0 alone it is a serial chain of ~100 FP64 instructions queueing behind the
@@ -390,7 +322,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             for (int ww = 1; ww < F2_WARPS; ww++) acc += t[ww];
             qred[v * 32 + lane] = acc;
         }
-        tile_sync<MODE>(slot);
+        __syncthreads();
     }
     // ---- round 0: who fits within F2_CAP of the base (normally everybody)
     bool part0 = false;
@@ -411,21 +343,19 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         }
         sample_consts<K, TABLE>(sm, P, tid);
     }
-    F2_T(13);
-    const int n_part0 = tile_count<MODE>(slot, part0);
+    const int n_part0 = __syncthreads_count(part0);
     bool last_round = n_part0 == n_valid;
     bool need_setup = n_part0 == 0;                       // nobody fits: the general set-up pivots
-    F2_T(0);
 
     for (int round = 0;; round++) {   // rounds: normally one; more only when the tile's delay spread exceeds F2_CAP
         if (round > 0 || need_setup) {
-            tile_sync<MODE>(slot);
+            __syncthreads();
             if (tid < 32) round_setup<K>(sm, lane);
-            tile_sync<MODE>(slot);
+            __syncthreads();
             if (sm.n_left == 0) break;
             last_round = sm.n_part == sm.n_left;
             if (tid < TS) sample_consts<K, TABLE>(sm, P, tid);
-            tile_sync<MODE>(slot);
+            __syncthreads();
             need_setup = false;
         }
         // per-sample epilogue state of this warp's rows: reference m (warp-uniform), lane-partial sum
@@ -439,7 +369,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
         const int last_bin = stride * (N_t - 1) + 1 + cap;      // highest stored bin (relative to base) any sample reads
         int c_lo = 0, j0 = 0;
 #ifdef F2_PAIRJOBS
-        int ntiles = min((MODE == 0 ? F2_NEW : F2_RING) / 8, (last_bin + 1 - c_lo + 7) / 8);   // MODE 0: every full phase is 4 tile pairs
+        int ntiles = min(F2_NEW / 8, (last_bin + 1 - c_lo + 7) / 8);   // every full phase is 4 tile pairs
 #else
         int ntiles = min(F2_RING / 8, (last_bin + 1 - c_lo + 7) / 8);
 #endif
@@ -447,25 +377,12 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
             const int c_hi = c_lo + ntiles * 8;
             int j1 = (c_hi - 1 - cap - 1) / stride + 1;         // outputs whose reads are all below c_hi ...
             j1 = min(min(j1, j0 + 32 * NG), N_t);               // ... as many as one epilogue pass takes
-            F2_T(1);
-            if (MODE == 1) {
-                // ---------------- hand the phase to the contraction warps and wait for S
-                if (tid == 0) {
-                    cmd->c_lo = c_lo;
-                    cmd->ntiles = ntiles;
-#pragma unroll
-                    for (int k = 0; k < K; k++) cmd->base[k] = sm.base[k];
-                    cmd->go = 1;
-                }
-                __threadfence_block();
-                named_arrive(F3_BAR_EMPTY + slot, 128 + F2_THREADS);   // previous ring reads done, command valid
-                named_sync(F3_BAR_FULL + slot, 128 + F2_THREADS);      // S complete for bins < c_hi
-            } else {
+            {
 #ifdef F2_PAIRJOBS
             // ---------------- contraction of a full phase (8 bin tiles): warp (q, h) = (w % 4, w / 4) owns the pair of
                 // tiles (2 q, 2 q + 1) and, for K = 3, the work (detector h, all 4 row blocks) + (detector 2, row
                 // blocks 2 h and 2 h + 1); every coefficient fragment read from shared memory feeds two DMMAs
-                if (MODE == 0 && ntiles == 8)
+                if (ntiles == 8)
                 {
                     static_assert(K == 2 || K == 3, "contraction job split is written for two or three detectors");
                     const int q = w & 3, h = w >> 2;
@@ -633,9 +550,7 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                     }
                 }
     }
-            F2_T(2);
-            if (MODE == 0) tile_sync<MODE>(slot);   // S complete for bins < c_hi
-            F2_T(3);
+            __syncthreads();   // S complete for bins < c_hi
             // ---------------- epilogue: shift + interpolate + sum detectors, then a streaming
             // log-sum-exp.  Straight-line code over SPW x NG independent (sample row, 32-bin group)
             // chains; rows that do not take part in this round run on clamped offsets and are discarded.
@@ -746,13 +661,11 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                         run_s[i] += exp_tab(__hiloint2double((int)hc, dlo[i][gi]), sm.etab);
                     }
             }
-            F2_T(4);
             if (j1 >= N_t) break;
             j0 = j1;
             c_lo = c_hi;
             ntiles = min(F2_NEW / 8, (last_bin + 1 - c_lo + 7) / 8);
-            if (MODE == 0) tile_sync<MODE>(slot);   // ring reads done before the next phase overwrites old bins (MODE 1: the EMPTY barrier)
-            F2_T(5);
+            __syncthreads();   // ring reads done before the next phase overwrites old bins
         }
         // ---------------- finalise this round's samples: lane q < SPW writes sample row q
         {
@@ -771,7 +684,6 @@ __device__ __forceinline__ void tile_body(Fused2Smem<K>& sm, F3Cmd* cmd, const i
                 }
             }
         }
-        F2_T(6);
         if (last_round) break;
     }
 }
@@ -783,21 +695,14 @@ lnl_fused2_kernel(LnlParams P, int N, int quad, const double* __restrict__ rec, 
                   const int* __restrict__ perm, double* __restrict__ lnL) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Fused2Smem<K>& sm = *reinterpret_cast<Fused2Smem<K>*>(smem_raw);
-    tile_body<0, K, NPAIR, SINGLE, TABLE, STRIDE1>(sm, nullptr, 0, threadIdx.x, blockIdx.x, P, N, quad, rec, ytile, perm, lnL);
+    tile_body<K, NPAIR, SINGLE, TABLE, STRIDE1>(sm, threadIdx.x, blockIdx.x, P, N, quad, rec, ytile, perm, lnL);
 }
 
 template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
 static int launch_fused2_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
-    static bool configured = false;
-#ifdef F2_SMEM_PAD
-    const int smem = (int)sizeof(Fused2Smem<K>) + F2_SMEM_PAD;      // experiment: force one CTA per SM
-#else
     const int smem = (int)sizeof(Fused2Smem<K>);
-#endif
-    if (!configured) {
-        ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        configured = true;
-    }
+    // per device, cheap: set on every launch (a per-process flag would miss a second device)
+    ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     const int tiles = (N + F2_TS - 1) / F2_TS;
     const int slot = ile_timing_begin(ctx);
     lnl_fused2_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1><<<tiles, F2_THREADS, smem, ctx->stream>>>(P, N, quad ? 1 : 0, rec, yt, perm, lnL);
@@ -817,7 +722,7 @@ static int launch_fused2_k(ile_ctx* ctx, const LnlParams& P, int N, const double
 
 // rec / yt as written by lnl_prep_kernel (quad = false) or lnl_prep3_kernel (quad = true: the
 // quadratic term is computed here) for ceil(N/64)*64 padded samples.  Returns 1 when the
-// shape has no instantiation (the caller falls back to the first-generation kernel).
+// shape has no instantiation (the caller falls back to the plain kernel).
 int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
     const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
     if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4) return launch_fused2_k<3, 5, true>(ctx, P, N, rec, yt, perm, lnL, quad);
@@ -825,229 +730,3 @@ int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec
     return 1;
 }
 
-#ifdef F2_TIMERS
-extern "C" int ile_dbg_timers(unsigned long long* out16) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out16, f2_timers, sizeof(f2_timers));
-    unsigned long long z[16] = {0};
-    cudaMemcpyToSymbol(f2_timers, z, sizeof(z));
-    return 0;
-}
-#endif
-
-// ================================================================ warp-specialised persistent kernel
-// One CTA per SM: warpgroup 0 = 4 contraction warps (one per SM sub-partition) with a large
-// register budget (setmaxnreg), warpgroups 1-4 = two epilogue groups of 8 warps, each working on
-// its own 32-sample tile ("slot") with tile_body<1>.  The contraction warps alternate between the
-// two slots, so the FP64 pipe is fed while either group is in its epilogue or prologue.
-template <int K>
-struct Fused3Smem {
-    Fused2Smem<K> slot[2];
-    F3Cmd cmd[2];
-};
-
-// contraction of one phase of one slot by the 4 contraction warps: warp mw takes the 8-bin tiles
-// t = mw, mw + 4, ... of every detector, two tiles of the same detector at a time (they share the
-// A fragments): 16 independent DMMA chains per warp
-template <int K, int NPAIR, bool SINGLE>
-__device__ __forceinline__ void contract_phase(Fused2Smem<K>& sm, const LnlParams& P, const int c_lo, const int ntiles, const int* base,
-                                               const int mw, const int lane) {
-    constexpr int RB = F2_RB;
-    const int c = lane & 3, rq = lane >> 2;
-    const int nper = ntiles > mw ? (ntiles - mw + 7) / 8 : 0;       // items per detector for this warp
-    const int nitems = K * nper;
-    auto item_kt = [&](int j, int& k, int& t0, int& nu) {
-        k = nper == 2 ? (j >> 1) : j;
-        t0 = mw + 8 * (nper == 2 ? (j & 1) : 0);
-        nu = (t0 + 4 < ntiles) ? 2 : 1;
-    };
-    auto load_b = [&](int j, double2 (&b)[2][NPAIR], double (&bs)[2]) {
-        int k, t0, nu;
-        item_kt(j, k, t0, nu);
-#pragma unroll
-        for (int u = 0; u < 2; u++) {
-            if (u < nu) {
-                const int row = base[k] + c_lo + 8 * (t0 + 4 * u) + rq;
-                const double* qrow = P.Qf + (((size_t)k * P.N_Qpad + row) >> 1) * (2 * ILE_QT_ROW) + (row & 1) * 8;
-#pragma unroll
-                for (int p = 0; p < NPAIR; p++) b[u][p] = __ldg(reinterpret_cast<const double2*>(qrow + 16 * p + 2 * c));
-                if (SINGLE) bs[u] = __ldg(qrow + 16 * NPAIR + c);
-            }
-        }
-    };
-    auto store_unit = [&](int k, int t, const double (&d)[RB][2]) {
-        int cr = c_lo + 8 * t;
-        cr -= (cr / F2_RING) * F2_RING;
-        double* srow = &sm.S[k][rq][cr + 2 * c];
-#pragma unroll
-        for (int rb = 0; rb < RB; rb++) *reinterpret_cast<double2*>(srow + rb * 8 * F2_SROW) = make_double2(d[rb][0], d[rb][1]);
-        if (cr == 0 && c == 0) {
-#pragma unroll
-            for (int rb = 0; rb < RB; rb++) srow[rb * 8 * F2_SROW + F2_RING] = d[rb][0];
-        }
-    };
-    auto compute = [&](int j, const double2 (&b)[2][NPAIR], const double (&bs)[2]) {
-        int k, t0, nu;
-        item_kt(j, k, t0, nu);
-        const double2* Ak = &sm.A[k][0][0][lane];
-        if (nu == 2) {
-            double d[2][RB][2], e[2][RB][2];
-#pragma unroll
-            for (int u = 0; u < 2; u++)
-#pragma unroll
-                for (int rb = 0; rb < RB; rb++) d[u][rb][0] = d[u][rb][1] = e[u][rb][0] = e[u][rb][1] = 0.0;
-#pragma unroll
-            for (int p = 0; p < NPAIR; p++) {
-                const double2 bp[2] = {b[0][p], b[1][p]};
-                double2 a[RB];
-#pragma unroll
-                for (int rb = 0; rb < RB; rb++) a[rb] = Ak[(p * RB + rb) * 32];
-#pragma unroll
-                for (int u = 0; u < 2; u++)
-#pragma unroll
-                    for (int rb = 0; rb < RB; rb++) dmma2(d[u][rb][0], d[u][rb][1], a[rb].x, bp[u].x);
-#pragma unroll
-                for (int u = 0; u < 2; u++)
-#pragma unroll
-                    for (int rb = 0; rb < RB; rb++) dmma2(e[u][rb][0], e[u][rb][1], a[rb].y, bp[u].y);
-            }
-            if (SINGLE) {
-#pragma unroll
-                for (int u = 0; u < 2; u++)
-#pragma unroll
-                    for (int rb = 0; rb < RB; rb += 2) {
-                        const double2 as = Ak[(NPAIR * RB + (rb >> 1)) * 32];
-                        dmma2(d[u][rb][0], d[u][rb][1], as.x, bs[u]);
-                        dmma2(d[u][rb + 1][0], d[u][rb + 1][1], as.y, bs[u]);
-                    }
-            }
-#pragma unroll
-            for (int u = 0; u < 2; u++) {
-#pragma unroll
-                for (int rb = 0; rb < RB; rb++) { d[u][rb][0] += e[u][rb][0]; d[u][rb][1] += e[u][rb][1]; }
-                store_unit(k, t0 + 4 * u, d[u]);
-            }
-        } else {
-            double d[RB][2], e[RB][2];
-#pragma unroll
-            for (int rb = 0; rb < RB; rb++) d[rb][0] = d[rb][1] = e[rb][0] = e[rb][1] = 0.0;
-#pragma unroll
-            for (int p = 0; p < NPAIR; p++) {
-                const double2 bp = b[0][p];
-                double2 a[RB];
-#pragma unroll
-                for (int rb = 0; rb < RB; rb++) a[rb] = Ak[(p * RB + rb) * 32];
-#pragma unroll
-                for (int rb = 0; rb < RB; rb++) dmma2(d[rb][0], d[rb][1], a[rb].x, bp.x);
-#pragma unroll
-                for (int rb = 0; rb < RB; rb++) dmma2(e[rb][0], e[rb][1], a[rb].y, bp.y);
-            }
-            if (SINGLE) {
-#pragma unroll
-                for (int rb = 0; rb < RB; rb += 2) {
-                    const double2 as = Ak[(NPAIR * RB + (rb >> 1)) * 32];
-                    dmma2(d[rb][0], d[rb][1], as.x, bs[0]);
-                    dmma2(d[rb + 1][0], d[rb + 1][1], as.y, bs[0]);
-                }
-            }
-#pragma unroll
-            for (int rb = 0; rb < RB; rb++) { d[rb][0] += e[rb][0]; d[rb][1] += e[rb][1]; }
-            store_unit(k, t0, d);
-        }
-    };
-    double2 bA[2][NPAIR], bB[2][NPAIR];
-    double sA[2] = {0.0, 0.0}, sB[2] = {0.0, 0.0};
-    int j = 0;
-    if (j < nitems) load_b(j, bA, sA);
-    while (j < nitems) {
-        if (j + 1 < nitems) load_b(j + 1, bB, sB);
-        compute(j, bA, sA);
-        j++;
-        if (j >= nitems) break;
-        if (j + 1 < nitems) load_b(j + 1, bA, sA);
-        compute(j, bB, sB);
-        j++;
-    }
-}
-
-template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
-__global__ void __launch_bounds__(F3_THREADS, 1)
-lnl_fused3_kernel(LnlParams P, int N, int ntiles_total, int quad, const double* __restrict__ rec, const double2* __restrict__ ytile,
-                  const int* __restrict__ perm, double* __restrict__ lnL) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    Fused3Smem<K>& cta = *reinterpret_cast<Fused3Smem<K>*>(smem_raw);
-    const int wg = threadIdx.x >> 7;
-    if (wg == 0) {
-        // ---------------- contraction warps
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(F3_MREGS));
-        const int mw = threadIdx.x >> 5, lane = threadIdx.x & 31;
-        int alive = 3, slot = 0;
-        while (alive) {
-            if (alive & (1 << slot)) {
-#ifdef F2_TIMERS
-                long long tmark = clock64();
-#endif
-                named_sync(F3_BAR_EMPTY + slot, 128 + F2_THREADS);
-                F2_T(7);
-                const volatile F3Cmd* cm = &cta.cmd[slot];
-                if (!cm->go) {
-                    alive &= ~(1 << slot);
-                } else {
-                    int base[3];
-#pragma unroll
-                    for (int k = 0; k < K; k++) base[k] = cm->base[k];
-                    contract_phase<K, NPAIR, SINGLE>(cta.slot[slot], P, cm->c_lo, cm->ntiles, base, mw, lane);
-                    __threadfence_block();
-                    named_arrive(F3_BAR_FULL + slot, 128 + F2_THREADS);
-                }
-            }
-            slot ^= 1;
-        }
-    } else {
-        // ---------------- epilogue groups: slot 0 = warpgroups 1-2, slot 1 = warpgroups 3-4
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(F3_EREGS));
-        const int slot = (wg - 1) >> 1;
-        const int tid = threadIdx.x - 128 - slot * F2_THREADS;
-        for (int tile = 2 * blockIdx.x + slot; tile < ntiles_total; tile += 2 * gridDim.x) {
-            named_sync(F3_BAR_GROUP + slot, F2_THREADS);   // the previous tile's finalisation is done with this slot's memory
-            tile_body<1, K, NPAIR, SINGLE, TABLE, STRIDE1>(cta.slot[slot], &cta.cmd[slot], slot, tid, tile, P, N, quad, rec, ytile, perm, lnL);
-        }
-        if (tid == 0) cta.cmd[slot].go = 0;
-        __threadfence_block();
-        named_arrive(F3_BAR_EMPTY + slot, 128 + F2_THREADS);
-    }
-}
-
-template <int K, int NPAIR, bool SINGLE, bool TABLE, bool STRIDE1>
-static int launch_fused3_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
-    static bool configured = false;
-    const int smem = (int)sizeof(Fused3Smem<K>);
-    if (!configured) {
-        ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_fused3_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        configured = true;
-    }
-    const int tiles = (N + F2_TS - 1) / F2_TS;
-    int grid = (tiles + 1) / 2;
-    if (grid > ctx->sm_count) grid = ctx->sm_count;
-    const int slot = ile_timing_begin(ctx);
-    lnl_fused3_kernel<K, NPAIR, SINGLE, TABLE, STRIDE1><<<grid, F3_THREADS, smem, ctx->stream>>>(P, N, tiles, quad ? 1 : 0, rec, yt, perm, lnL);
-    ile_timing_end(ctx, slot);
-    ILE_LAUNCH_CHECK(ctx);
-    return ILE_OK;
-}
-
-template <int K, int NPAIR, bool SINGLE>
-static int launch_fused3_k(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
-    const bool tb = P.use_table != 0, s1 = P.stride == 1;
-    if (tb) return s1 ? launch_fused3_t<K, NPAIR, SINGLE, true, true>(ctx, P, N, rec, yt, perm, lnL, quad)
-                      : launch_fused3_t<K, NPAIR, SINGLE, true, false>(ctx, P, N, rec, yt, perm, lnL, quad);
-    return s1 ? launch_fused3_t<K, NPAIR, SINGLE, false, true>(ctx, P, N, rec, yt, perm, lnL, quad)
-              : launch_fused3_t<K, NPAIR, SINGLE, false, false>(ctx, P, N, rec, yt, perm, lnL, quad);
-}
-
-int ile_launch_fused3(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL, bool quad) {
-    const int n2 = 2 * P.M, np = n2 / 8, rem = n2 % 8;
-    if (P.K == 3 && np == 5 && rem >= 1 && rem <= 4) return launch_fused3_k<3, 5, true>(ctx, P, N, rec, yt, perm, lnL, quad);
-    if (P.K == 2 && np == 1 && rem >= 1 && rem <= 4) return launch_fused3_k<2, 1, true>(ctx, P, N, rec, yt, perm, lnL, quad);
-    return 1;
-}

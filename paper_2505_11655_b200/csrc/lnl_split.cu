@@ -1,0 +1,641 @@
+// libile: fused lnL kernel on the Blackwell tensor path.
+//
+// Step 5 of the hot path, S_k[i][n] = sum_r coef_k[i][r] Q_k[r][n] (Eq. 7's Re[(F Y)^* Q] on the
+// (time) x (extrinsic) array), is a dense real contraction with K-dimension 2M <= 48.  FP64 has no tcgen05 kind, so
+// the contraction is done EXACTLY in integers instead: both operands are scaled by a power of two (per sample and
+// detector for the coefficients, per intrinsic point and detector for Q), rounded to 47-bit integers and cut into
+// six signed 8-bit digits, C = sum_a c_a 256^(5-a), Qi = sum_b q_b 256^(5-b).  Then
+//     C Qi = sum_s 256^(10-s) acc_s,   acc_s = sum_{a+b=s} sum_r c_a[r] q_b[r]
+// and each acc_s is one tcgen05.mma kind::i8 accumulation (int32, |acc_s| < 6 * 42 * 2^14: no overflow, no
+// rounding) with the digit pairs of equal weight stacked along K.  Sums s <= 5 are kept (21 digit pairs); the
+// dropped pairs are below 2^-43 of max|coef| max|Q| (DESIGN.md section 6 derives the bound against the 1e-9
+// tolerance).  The six accumulators are recombined in FP64 by the epilogue.
+//
+//   operand A (coefficients): [c_0 | c_1 | ... | c_5], 48 bytes per digit block (2M <= 42 used), written to tensor
+//              memory by the thread that owns the sample (tcgen05.st); stationary for the whole tile
+//   operand B (Q digits): per stored bin 304 bytes [q_5 | q_4 | ... | q_0 | 16 zero bytes], built once per intrinsic
+//              point at ile_load_quv in the K-major no-swizzle core-matrix layout, so that a 16-bin chunk is one
+//              contiguous 4864-byte TMA bulk copy; sum s reads the view that starts at block 5 - s, which pairs
+//              c_a with q_{s-a} (descriptor start addresses move in 16-byte steps)
+//   tile       128 samples of one delay cell (16 stored bins per detector) = the 128 lanes of tensor memory
+//   work item  (16-bin chunk, detector): 33 MMAs of 128 x 16 x 32 into one of two accumulator sets
+//   warps      0-3: one thread per sample: coefficients and digits, the U/V quadratic term (step 4), then per item
+//              accumulators -> FP64, interpolation weights, accumulation of A_j = sum_k S_k(t_j + tau_k) into a
+//              thread-private column of a shared-memory ring (the per-sample delay shift is an address offset),
+//              and the streaming log-sum-exp over complete time bins (step 6);  warp 4: TMA producer + MMA issuer
+#include "common.cuh"
+#include "likelihood_dev.cuh"
+#include "radix_sort.cuh"
+#include "sm100_ptx.cuh"
+#include "exp_tab.cuh"
+
+#define SP_TS 128             // samples per tile
+#define SP_NB 16              // stored bins per work item (MMA N)
+#define SP_BLK 48             // bytes per digit block
+#define SP_NCH 19             // 16-byte chunks per stored bin in the Q digit image (304 bytes)
+#define SP_GRP (SP_NCH * 128) // bytes per group of 8 bins
+#define SP_STAGE (2 * SP_GRP) // bytes per 16-bin chunk
+#define SP_NSTAGE 6
+#define SP_RING 64            // rows (time bins) of the accumulation ring
+#define SP_CAPMAX 24          // largest per-sample offset above the tile base
+#define SP_CELL_SHIFT 4       // delay cells of 16 stored bins
+#define SP_ACOLS 72           // tensor-memory columns of A per detector (288 bytes)
+#define SP_DCOL 256           // first accumulator column; set b, sum s at SP_DCOL + 96 b + 16 s
+#define SP_THREADS 160
+#define SP_UVMAX (300 * 3 * 2)
+#define SP_MAGIC 6755399441055744.0   // 1.5 * 2^52
+
+struct SpTile {
+    int start, cnt;           // sorted positions [start, start + cnt)
+    int base[3];              // first stored bin of the tile's window per detector (multiple of 8)
+    int cap;                  // largest offset n_k - base_k in the tile
+    int nchunk;               // 16-bin chunks to contract
+    int flags;                // 1: samples outside the prior box (lnL = -inf), 2: delay spread too large (NaN)
+};
+
+// ---------------------------------------------------------------- Q digits (ile_load_quv)
+// biased exponent of max |Q| per (point, detector)
+__global__ void sp_qmax_kernel(const double* __restrict__ Qc, int M, int N_Q, unsigned int* __restrict__ qhi) {
+    const int pk = blockIdx.y;
+    const double* src = Qc + (size_t)pk * M * N_Q * 2;
+    const long long total = (long long)M * N_Q * 2;
+    unsigned int mx = 0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
+        mx = max(mx, (unsigned int)__double2hiint(src[i]) & 0x7fffffffu);
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0) atomicMax(&qhi[pk], mx);
+}
+
+// digits of rint(v), |v| < 2^46: c = sum_p d_p 256^p with d_p in [-128, 127]; lo = (d_0..d_3), hi bytes 0, 1 = d_4, d_5
+__device__ __forceinline__ void sp_digits(double v, uint32_t& lo, uint32_t& hi) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v + SP_MAGIC);   // 0x4338000000000000 + rint(v)
+    const unsigned long long c = (b + 0xBCC8808080808080ull) ^ 0x0000808080808080ull;
+    lo = (uint32_t)c;
+    hi = (uint32_t)(c >> 32);
+}
+// digit words of four values: w[a] = digit of weight 256^(5-a) of (v0, v1, v2, v3), one per byte
+__device__ __forceinline__ void sp_digit_words(const uint32_t (&lo)[4], const uint32_t (&hi)[4], uint32_t (&w)[6]) {
+    const uint32_t a01 = __byte_perm(lo[0], lo[1], 0x5140), b01 = __byte_perm(lo[0], lo[1], 0x7362);
+    const uint32_t a23 = __byte_perm(lo[2], lo[3], 0x5140), b23 = __byte_perm(lo[2], lo[3], 0x7362);
+    const uint32_t h01 = __byte_perm(hi[0], hi[1], 0x5140), h23 = __byte_perm(hi[2], hi[3], 0x5140);
+    w[5] = __byte_perm(a01, a23, 0x5410);
+    w[4] = __byte_perm(a01, a23, 0x7632);
+    w[3] = __byte_perm(b01, b23, 0x5410);
+    w[2] = __byte_perm(b01, b23, 0x7632);
+    w[1] = __byte_perm(h01, h23, 0x5410);
+    w[0] = __byte_perm(h01, h23, 0x7632);
+}
+
+// one thread per (point-detector, stored bin, group of four reals r = 4 q .. 4 q + 3, r = 2 mode + part)
+__global__ void sp_qslice_kernel(const double* __restrict__ Qc, int PK, int M, int N_Q, int NG8, const unsigned int* __restrict__ qhi,
+                                 int* __restrict__ qeb, unsigned char* __restrict__ Qs) {
+    const long long total = (long long)PK * NG8 * 8 * 12;
+    for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total; idx += (long long)gridDim.x * blockDim.x) {
+        const int q = (int)(idx % 12);
+        const long long rest = idx / 12;
+        const int n = (int)(rest % (NG8 * 8));
+        const int pk = (int)(rest / (NG8 * 8));
+        const int eb = min(max((int)(qhi[pk] >> 20), 200), 1800);
+        if (n == 0 && q == 0) qeb[pk] = eb;
+        const double sc = __hiloint2double((2091 - eb) << 20, 0);            // 2^(45 - (eb - 1023))
+        uint32_t lo[4], hi[4], w[6];
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+            const int rr = 4 * q + r, mode = rr >> 1, part = rr & 1;
+            double v = 0.0;
+            if (mode < M && n < N_Q) v = Qc[(((size_t)pk * M + mode) * N_Q + n) * 2 + part];
+            sp_digits(v * sc, lo[r], hi[r]);
+        }
+        sp_digit_words(lo, hi, w);
+        unsigned char* row = Qs + ((size_t)pk * NG8 + (n >> 3)) * SP_GRP + (n & 7) * 16;
+#pragma unroll
+        for (int b = 0; b < 6; b++) {
+            const int off = SP_BLK * (5 - b) + 4 * q;                         // block 5 - b holds digit b
+            *reinterpret_cast<uint32_t*>(row + (off >> 4) * 128 + (off & 15)) = w[b];
+        }
+    }
+}
+
+size_t ile_split_qs_bytes(int P, int K, int N_Q) { return (size_t)P * K * ((N_Q + 64 + 7) / 8) * SP_GRP; }
+int ile_split_ng8(int N_Q) { return (N_Q + 64 + 7) / 8; }
+
+int ile_split_build_q(ile_ctx* ctx, int P, int K, int M, int N_Q, const double* d_Qc, unsigned char* d_Qs, int* d_qeb, unsigned int* d_qhi) {
+    const int NG8 = ile_split_ng8(N_Q);
+    ILE_CUDA(ctx, cudaMemsetAsync(d_Qs, 0, ile_split_qs_bytes(P, K, N_Q), ctx->stream));
+    ILE_CUDA(ctx, cudaMemsetAsync(d_qhi, 0, (size_t)P * K * sizeof(unsigned int), ctx->stream));
+    sp_qmax_kernel<<<dim3(32, P * K), 256, 0, ctx->stream>>>(d_Qc, M, N_Q, d_qhi);
+    ILE_LAUNCH_CHECK(ctx);
+    sp_qslice_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(d_Qc, P * K, M, N_Q, NG8, d_qhi, d_qeb, d_Qs);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}
+
+// ---------------------------------------------------------------- delay-cell keys and tiles
+__global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const double* __restrict__ z, int n_min, int cell_bits,
+                                                     unsigned long long* __restrict__ key, unsigned int* __restrict__ val, long long* n_dev,
+                                                     int* bits_dev, int* ntiles_dev) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) {
+        *n_dev = N;
+        *bits_dev = cell_bits * P.K + 1;
+        *ntiles_dev = 0;
+    }
+    if (i >= N) return;
+    const double ra = z[i], sd = z[(size_t)N + i];
+    bool ok = true;
+    for (int c = 0; c < P.d; c++) {
+        const double v = z[(size_t)c * N + i];
+        ok = ok && (v >= P.lo[c]) && (v < P.hi[c]);
+    }
+    unsigned long long k = 1ull << (cell_bits * P.K);      // out-of-box samples last
+    if (ok) {
+        const double cd = sqrt(fmax((1.0 - sd) * (1.0 + sd), 0.0));
+        double sg, cg;
+        sincos(P.gmst - ra, &sg, &cg);
+        const double n0 = cd * cg, n1 = -cd * sg, n2 = sd;
+        k = 0;
+        for (int kk = 0; kk < P.K; kk++) {
+            const double tau = -(P.pos[kk][0] * n0 + P.pos[kk][1] * n1 + P.pos[kk][2] * n2) / ILE_C_LIGHT;
+            double u = (P.t_lo + tau - P.t_Q0) * P.fs;
+            if (!P.interp) u = floor(u + 0.5);
+            int cell = ((int)floor(u) - n_min) >> SP_CELL_SHIFT;
+            cell = max(0, min(cell, (1 << cell_bits) - 1));
+            k = (k << cell_bits) | (unsigned long long)cell;
+        }
+    }
+    key[i] = k;
+    val[i] = (unsigned int)i;
+}
+
+// a tile starts at every multiple of 128 of the sorted order and wherever the cell changes
+__global__ void __launch_bounds__(256) sp_tile_flag_kernel(int N, const unsigned long long* __restrict__ key, int* __restrict__ tstart, int* ntiles_dev) {
+    const int pos = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= N) return;
+    if ((pos & (SP_TS - 1)) == 0 || key[pos] != key[pos - 1]) tstart[atomicAdd(ntiles_dev, 1)] = pos;
+}
+
+// one warp per tile: extent, window base per detector, largest offset
+__global__ void __launch_bounds__(256) sp_tile_info_kernel(LnlParams P, int N, int invalid_shift, const unsigned long long* __restrict__ key,
+                                                           const int* __restrict__ tstart, const int* __restrict__ ntiles_dev,
+                                                           const double* __restrict__ rec, SpTile* __restrict__ tiles) {
+    const int id = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (id >= *ntiles_dev) return;
+    const int start = tstart[id];
+    const unsigned long long k0 = key[start];
+    int cnt = 0, nmin[3] = {0x7fffffff, 0x7fffffff, 0x7fffffff}, nmax[3] = {0, 0, 0};
+    bool open = true;
+    for (int q = 0; q < SP_TS / 32; q++) {
+        const int pos = start + 32 * q + lane;
+        const bool mem = open && pos < N && key[pos] == k0 && (pos == start || (pos & (SP_TS - 1)) != 0);
+        const unsigned b = __ballot_sync(0xffffffffu, mem);
+        const int lead = b == 0xffffffffu ? 32 : __ffs(~b) - 1;      // members are a prefix
+        if (lane < lead) {
+#pragma unroll
+            for (int k = 0; k < 3; k++)
+                if (k < P.K) {
+                    const int nk = (int)floor(rec[(size_t)pos * 16 + 8 + k]);
+                    nmin[k] = min(nmin[k], nk);
+                    nmax[k] = max(nmax[k], nk);
+                }
+        }
+        cnt += lead;
+        if (lead < 32) open = false;
+    }
+    SpTile t;
+    t.start = start;
+    t.cnt = cnt;
+    t.flags = (k0 >> invalid_shift) ? 1 : 0;
+    t.cap = 0;
+#pragma unroll
+    for (int k = 0; k < 3; k++) {
+        const int lo = __reduce_min_sync(0xffffffffu, nmin[k]), hi = __reduce_max_sync(0xffffffffu, nmax[k]);
+        t.base[k] = k < P.K ? (max(lo, 0) & ~7) : 0;
+        if (k < P.K) t.cap = max(t.cap, hi - t.base[k]);
+    }
+    if (t.flags == 0 && t.cap > SP_CAPMAX) t.flags = 2;
+    t.nchunk = t.flags ? 0 : (P.N_t + 1 + t.cap + SP_NB - 1) / SP_NB;
+    if (lane == 0) tiles[id] = t;
+}
+
+// ---------------------------------------------------------------- the fused kernel
+struct SplitSmem {
+    unsigned char bst[SP_NSTAGE][SP_STAGE];   // Q digit chunks (TMA destination, MMA operand B)
+    double ring[SP_RING][SP_TS];              // A_j accumulation: row = time bin mod 64, column = sample (thread-private)
+    double2 Y[24][SP_TS];                     // harmonics of the tile, column = sample
+    double2 uv[SP_UVMAX];                     // packed upper-triangle U/V of the intrinsic point
+    double etab[64][16];                      // 2^(j/64), 16 copies: lane l reads copy l % 16 (conflict-free)
+    uint64_t a_full, d_full[2], d_empty[2], b_full[SP_NSTAGE], b_empty[SP_NSTAGE];
+    uint32_t tmem_base;
+};
+
+// exp(d), d in [-40, 31]: 2^(k >> 6) tab[k & 63] (1 + r (1 + r/2 + r^2/6 + r^3/24)), k = rint(64 d / ln 2) (R2)
+__device__ __forceinline__ double sp_exp_tab(double d, const double* __restrict__ tab_lane) {
+    const double t = fma(d, 0x1.71547652b82fep+6, SP_MAGIC);
+    const int k = __double2loint(t);
+    const double kf = t - SP_MAGIC;
+    const double r = fma(kf, -0x1.62e42fefa39efp-7, d);
+    const double T = tab_lane[(k & 63) * 16];
+    double p = fma(r, 1.0 / 24.0, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    const double e = fma(T * r, p, T);
+    return __hiloint2double(__double2hiint(e) + ((k >> 6) << 20), __double2loint(e));
+}
+// exp(d) for d in (-690, 0]: degree-10 Taylor after range reduction (used only when a reference is raised)
+__device__ __forceinline__ double sp_exp_small(double d) {
+    const double t = fma(d, 1.4426950408889634, SP_MAGIC);
+    const int k = __double2loint(t);
+    const double kf = t - SP_MAGIC;
+    double r = fma(kf, -6.93147180369123816490e-01, d);
+    r = fma(kf, -1.90821492927058770002e-10, r);
+    double p = 1.0 / 3628800.0;
+    p = fma(p, r, 1.0 / 362880.0);
+    p = fma(p, r, 1.0 / 40320.0);
+    p = fma(p, r, 1.0 / 5040.0);
+    p = fma(p, r, 1.0 / 720.0);
+    p = fma(p, r, 1.0 / 120.0);
+    p = fma(p, r, 1.0 / 24.0);
+    p = fma(p, r, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// cursor over the work items (tile, chunk, detector) of this CTA, in the order both warp roles walk them
+struct SpCursor {
+    int t, c, k, nchunk;
+    int base[3];
+};
+template <int K>
+__device__ __forceinline__ void sp_cursor_load(SpCursor& cu, const SpTile* __restrict__ tiles, int ntiles, int step) {
+    while (cu.t < ntiles) {
+        const SpTile ti = tiles[cu.t];
+        if (ti.nchunk > 0) {
+            cu.nchunk = ti.nchunk;
+#pragma unroll
+            for (int k = 0; k < 3; k++) cu.base[k] = ti.base[k];
+            cu.c = 0;
+            cu.k = 0;
+            return;
+        }
+        cu.t += step;
+    }
+    cu.nchunk = 0;
+}
+template <int K>
+__device__ __forceinline__ void sp_cursor_next(SpCursor& cu, const SpTile* __restrict__ tiles, int ntiles, int step) {
+    if (++cu.k < K) return;
+    cu.k = 0;
+    if (++cu.c < cu.nchunk) return;
+    cu.t += step;
+    sp_cursor_load<K>(cu, tiles, ntiles, step);
+}
+
+template <int K, bool TABLE>
+__global__ void __launch_bounds__(SP_THREADS, 1)
+lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const double2* __restrict__ ytile, const int* __restrict__ perm,
+                 double* __restrict__ lnL, const SpTile* __restrict__ tiles, const int* __restrict__ ntiles_dev) {
+    extern __shared__ __align__(1024) unsigned char sp_smem_raw[];
+    SplitSmem& sm = *reinterpret_cast<SplitSmem*>(sp_smem_raw);
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int ntiles = *ntiles_dev;
+
+    if (w == 4) tmem_alloc512(&sm.tmem_base);
+    if (tid == 0) {
+        mbar_init(&sm.a_full, SP_TS);
+        for (int b = 0; b < 2; b++) { mbar_init(&sm.d_full[b], 1); mbar_init(&sm.d_empty[b], SP_TS); }
+        for (int s = 0; s < SP_NSTAGE; s++) { mbar_init(&sm.b_full[s], 1); mbar_init(&sm.b_empty[s], 1); }
+        mbar_init_fence();
+    }
+    for (int q = tid; q < 64 * 16; q += SP_THREADS) sm.etab[q >> 4][q & 15] = f2_exp2_tab[q >> 4];
+    {
+        const double2* usrc = reinterpret_cast<const double2*>(P.UVp);
+        const int nuv = min(P.n_pairs * K * 2, SP_UVMAX);
+        for (int q = tid; q < nuv; q += SP_THREADS) sm.uv[q] = usrc[q];
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = sm.tmem_base;
+
+    if (w == 4) {
+        // ================================================================ producer: TMA loads and MMA issue
+        const bool el = elect_one();
+        const uint32_t idesc = umma_idesc_s8_m128(SP_NB);
+        SpCursor L, Mc;
+        L.t = Mc.t = blockIdx.x;
+        sp_cursor_load<K>(L, tiles, ntiles, gridDim.x);
+        sp_cursor_load<K>(Mc, tiles, ntiles, gridDim.x);
+        unsigned nl = 0, nm = 0, tile_par = 0;
+        while (Mc.nchunk > 0) {
+            while (L.nchunk > 0 && nl < nm + (SP_NSTAGE - 1)) {
+                const unsigned s = nl % SP_NSTAGE;
+                if (nl >= SP_NSTAGE) mbar_wait(&sm.b_empty[s], ((nl / SP_NSTAGE) - 1) & 1);
+                if (el) {
+                    const unsigned char* src = P.Qs + ((size_t)L.k * P.NG8 + ((L.base[L.k] + SP_NB * L.c) >> 3)) * SP_GRP;
+                    mbar_expect_tx(&sm.b_full[s], SP_STAGE);
+                    bulk_g2s(sm.bst[s], src, SP_STAGE, &sm.b_full[s]);
+                }
+                nl++;
+                sp_cursor_next<K>(L, tiles, ntiles, gridDim.x);
+            }
+            if (Mc.c == 0 && Mc.k == 0) {             // the tile's coefficient digits are in tensor memory
+                mbar_wait(&sm.a_full, tile_par);
+                tile_par ^= 1;
+            }
+            const unsigned b = nm & 1, s = nm % SP_NSTAGE;
+            if (nm >= 2) mbar_wait(&sm.d_empty[b], ((nm >> 1) - 1) & 1);
+            mbar_wait(&sm.b_full[s], (nm / SP_NSTAGE) & 1);
+            tc_fence_after();
+            if (el) {
+                const uint64_t b0 = umma_desc_kmajor_noswizzle(smem_u32(sm.bst[s]), 128, SP_GRP);
+                const uint32_t a0 = tmem + SP_ACOLS * Mc.k, d0 = tmem + SP_DCOL + 96 * b;
+                // sum s reads K_s = 64, 96, 160, 192, 256, 288 bytes of A against the view of B starting at 16-byte chunk 3 (5 - s);
+                // k-step major, so that consecutive MMAs go to different accumulators
+#pragma unroll
+                for (int t = 0; t < 9; t++) {
+#pragma unroll
+                    for (int sidx = 0; sidx < 6; sidx++) {
+                        const int Ks = sidx == 0 ? 64 : sidx == 1 ? 96 : sidx == 2 ? 160 : sidx == 3 ? 192 : sidx == 4 ? 256 : 288;
+                        if (32 * t < Ks) umma_i8_ts(d0 + SP_NB * sidx, a0 + 8 * t, b0 + (uint64_t)(((3 * (5 - sidx) + 2 * t) * 128) >> 4), idesc, t > 0 ? 1u : 0u);
+                    }
+                }
+                umma_commit(&sm.b_empty[s]);
+                umma_commit(&sm.d_full[b]);
+            }
+            __syncwarp();
+            nm++;
+            sp_cursor_next<K>(Mc, tiles, ntiles, gridDim.x);
+        }
+    } else {
+        // ================================================================ one thread per sample
+        const int i = tid;                                     // sample of the tile = tensor-memory lane
+        const uint32_t tlane = tmem + ((uint32_t)(32 * w) << 16);
+        double* const rcol = &sm.ring[0][i];
+        const double* const etab = &sm.etab[0][lane & 15];
+        const double tabA_s = TABLE ? (double)(P.nA - 1) / (P.A_hi - P.A_lo) : 0.0, tabA_o = -P.A_lo * tabA_s;
+        unsigned im = 0, tile_seq = 0;
+        (void)tile_seq;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            const SpTile ti = tiles[t];
+            const int pos = ti.start + i;
+            const bool member = i < ti.cnt;
+            if (ti.nchunk == 0) {
+                if (member) lnL[perm ? perm[pos] : pos] = (ti.flags & 2) ? __longlong_as_double(0x7ff8000000000000LL) : neg_inf();
+                continue;
+            }
+            const int N_t = P.N_t;
+            // ---- the sample's record: F_k = F+ - i Fx, stored-bin coordinate u_k of grid time 0, x = D_ref / D
+            double fr[K], fi[K], w0[K], w1[K], x = 0.0;
+            int off[K];
+            {
+                const double* r = rec + (size_t)pos * 16;
+                double u[K];
+#pragma unroll
+                for (int k = 0; k < K; k++) { fr[k] = fi[k] = 0.0; u[k] = (double)ti.base[k]; }
+                if (member) {
+                    const double2 r0 = *reinterpret_cast<const double2*>(r), r1 = *reinterpret_cast<const double2*>(r + 2);
+                    const double2 r2 = *reinterpret_cast<const double2*>(r + 4), r3 = *reinterpret_cast<const double2*>(r + 6);
+                    const double2 r4 = *reinterpret_cast<const double2*>(r + 8), r5 = *reinterpret_cast<const double2*>(r + 10);
+                    const double fr_[4] = {r0.x, r0.y, r1.x, r1.y}, fi_[4] = {r2.x, r2.y, r3.x, r3.y}, u_[4] = {r4.x, r4.y, r5.x, r5.y};
+#pragma unroll
+                    for (int k = 0; k < K; k++) { fr[k] = fr_[k]; fi[k] = fi_[k]; u[k] = u_[k]; }
+                    x = r[12];
+                }
+#pragma unroll
+                for (int k = 0; k < K; k++) {
+                    const double fl = floor(u[k]);
+                    w1[k] = u[k] - fl;
+                    w0[k] = 1.0 - w1[k];
+                    off[k] = min(max((int)fl - ti.base[k], 0), SP_CAPMAX);
+                }
+            }
+            // ---- harmonics: own column of the tile
+#pragma unroll 4
+            for (int m = 0; m < 24; m++)
+                sm.Y[m][i] = member ? __ldg(ytile + ((size_t)(pos >> 5) * 24 + m) * 32 + (pos & 31)) : make_double2(0.0, 0.0);
+            // ---- step 3: coefficients x F_k Y_m -> six signed 8-bit digits -> tensor memory (operand A)
+#pragma unroll
+            for (int k = 0; k < K; k++) {
+                const double xr = x * fr[k], xi = x * fi[k];
+                int mh = 0;
+#pragma unroll 4
+                for (int m = 0; m < 24; m++) {
+                    const double2 y = sm.Y[m][i];
+                    const double cr = xr * y.x - xi * y.y, ci = xr * y.y + xi * y.x;
+                    mh = max(mh, max(__double2hiint(cr) & 0x7fffffff, __double2hiint(ci) & 0x7fffffff));
+                }
+                const int eb = min(max(mh >> 20, 200), 1800);
+                const double sc = __hiloint2double((2091 - eb) << 20, 0);         // 2^(45 - (eb - 1023)): |coef sc| < 2^46
+                const double un = __hiloint2double(min(max(eb + P.qeb[k] - 1023 - 50, 1), 2046) << 20, 0);   // 2^40 / (sc sq_k)
+                w0[k] *= un;
+                w1[k] *= un;
+                uint32_t col[6][12];
+#pragma unroll
+                for (int q = 0; q < 12; q++) {
+                    const double2 y0 = sm.Y[2 * q][i], y1 = sm.Y[2 * q + 1][i];
+                    uint32_t lo[4], hi[4], wd[6];
+                    sp_digits((xr * y0.x - xi * y0.y) * sc, lo[0], hi[0]);
+                    sp_digits((xr * y0.y + xi * y0.x) * sc, lo[1], hi[1]);
+                    sp_digits((xr * y1.x - xi * y1.y) * sc, lo[2], hi[2]);
+                    sp_digits((xr * y1.y + xi * y1.x) * sc, lo[3], hi[3]);
+                    sp_digit_words(lo, hi, wd);
+#pragma unroll
+                    for (int a = 0; a < 6; a++) col[a][q] = wd[a];
+                }
+#pragma unroll
+                for (int g = 0; g < 9; g++) {
+                    uint32_t v[8];
+#pragma unroll
+                    for (int e = 0; e < 8; e++) v[e] = col[(8 * g + e) / 12][(8 * g + e) % 12];
+                    tmem_st8(tlane + SP_ACOLS * k + 8 * g, v);
+                }
+            }
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(&sm.a_full);
+            // ---- step 4: B = 1/4 sum_k [ |F_k|^2 Re(y^H U_k y) + Re(F_k^2 y^T V_k y) ] over the upper triangle (Eq. 17-18)
+            double Bq = 0.0;
+            {
+                double uu[K], vr[K], vi[K];
+#pragma unroll
+                for (int k = 0; k < K; k++) uu[k] = vr[k] = vi[k] = 0.0;
+                const int M = P.M;
+                const double2* uv = sm.uv;
+                for (int a = 0; a < M; a++) {
+                    const double2 ya = sm.Y[a][i];
+                    for (int b = a; b < M; b++) {
+                        const double2 yb = sm.Y[b][i];
+                        const double t2 = ya.y * yb.y, t4 = ya.y * yb.x;
+                        const double pr = fma(ya.x, yb.x, t2), qr = fma(ya.x, yb.x, -t2), pi = fma(ya.x, yb.y, -t4), qi = fma(ya.x, yb.y, t4);
+#pragma unroll
+                        for (int k = 0; k < K; k++) {
+                            const double2 u = uv[2 * k], v = uv[2 * k + 1];
+                            uu[k] = fma(-u.y, pi, fma(u.x, pr, uu[k]));
+                            vr[k] = fma(-v.y, qi, fma(v.x, qr, vr[k]));
+                            vi[k] = fma(v.y, qr, fma(v.x, qi, vi[k]));
+                        }
+                        uv += 2 * K;
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < K; k++)
+                    Bq += (fr[k] * fr[k] + fi[k] * fi[k]) * uu[k] + ((fr[k] * fr[k] - fi[k] * fi[k]) * vr[k] - 2.0 * fr[k] * fi[k] * vi[k]);
+                Bq *= 0.25;
+            }
+            // per-sample constants of the time marginalisation
+            double init = -(x * x * Bq), tb_f = 0.0;
+            const double* tb_row = nullptr;
+            if (TABLE) {
+                double b = (Bq - P.B_lo) / (P.B_hi - P.B_lo) * (double)(P.nB - 1);
+                b = fmin(fmax(b, 0.0), (double)(P.nB - 1));
+                const int ib = min((int)floor(b), P.nB - 2);
+                tb_f = b - ib;
+                tb_row = P.lnT + (size_t)ib * P.nA;
+                init = 0.0;
+            }
+#pragma unroll 8
+            for (int r = 0; r < SP_RING; r++) rcol[r * SP_TS] = init;
+            double run_m = -1.0e300, run_s = 0.0;
+            int jdone = 0;
+            double prev[K];
+#pragma unroll
+            for (int k = 0; k < K; k++) prev[k] = 0.0;
+
+            // rows [jdone, jend) of the ring are complete: lnL(t_j) and the streaming log-sum-exp (step 6)
+            auto lse_rows = [&](const int jend) {
+                for (int j0 = jdone; j0 < jend; j0 += 4) {
+                    double v[4];
+                    bool need = false;
+#pragma unroll
+                    for (int e = 0; e < 4; e++) {
+                        double* p = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
+                        double A = *p;
+                        if (j0 + e < jend) *p = init;
+                        if (TABLE) {
+                            double a = fma(A, tabA_s, tabA_o);
+                            a = fmin(fmax(a, 0.0), (double)(P.nA - 1));
+                            const int ia = min((int)a, P.nA - 2);
+                            const double fa = a - (double)ia;
+                            const double* T0 = tb_row + ia;
+                            const double t00 = __ldg(T0), t01 = __ldg(T0 + 1), t10 = __ldg(T0 + P.nA), t11 = __ldg(T0 + P.nA + 1);
+                            const double t0 = fma(fa, t01 - t00, t00), t1 = fma(fa, t11 - t10, t10);
+                            A = fma(tb_f, t1 - t0, t0);
+                        }
+                        v[e] = j0 + e < jend ? A : neg_inf();
+                        need = need || (v[e] - run_m >= 30.0);
+                    }
+                    if (__any_sync(0xffffffffu, need)) {
+                        // raise the reference to the largest new value (rare); the running sum is rescaled exactly
+                        const double mx = fmax(fmax(v[0], v[1]), fmax(v[2], v[3]));
+                        if (mx - run_m >= 30.0) {
+                            const double dm = run_m - mx;
+                            run_s = dm > -690.0 ? run_s * sp_exp_small(dm) : 0.0;
+                            run_m = mx;
+                        }
+                    }
+#pragma unroll
+                    for (int e = 0; e < 4; e++) {
+                        // terms below e^-40 of the reference (and rows past the end) are clamped to e^-40 (R2)
+                        const double dl = v[e] - run_m;
+                        const unsigned hc = min((unsigned)__double2hiint(dl), 0xC0440000u);
+                        run_s += sp_exp_tab(__hiloint2double((int)hc, __double2loint(dl)), etab);
+                    }
+                }
+                jdone = max(jdone, jend);
+            };
+
+            // ---- work items: accumulators -> FP64 -> interpolation -> ring
+            for (int c = 0; c < ti.nchunk; c++) {
+#pragma unroll
+                for (int k = 0; k < K; k++) {
+                    const unsigned b = im & 1;
+                    mbar_wait(&sm.d_full[b], (im >> 1) & 1);
+                    tc_fence_after();
+                    const int jb = SP_NB * c - 1 - off[k];              // time bin of the pair (previous, first) of this chunk
+#pragma unroll
+                    for (int h = 0; h < 2; h++) {
+                        uint32_t acc[6][8];
+#pragma unroll
+                        for (int s = 0; s < 6; s++) tmem_ld8(tlane + SP_DCOL + 96 * b + SP_NB * s + 8 * h, acc[s]);
+                        tmem_wait_ld();
+                        if (h == 1) {
+                            tc_fence_before();
+                            mbar_arrive(&sm.d_empty[b]);
+                        }
+#pragma unroll
+                        for (int e = 0; e < 8; e++) {
+                            const int t0 = (int)acc[0][e] * 256 + (int)acc[1][e];
+                            const int t1 = (int)acc[2][e] * 256 + (int)acc[3][e];
+                            const int t2 = (int)acc[4][e] * 256 + (int)acc[5][e];
+                            const double V = fma((double)t0, 4294967296.0, fma((double)t1, 65536.0, (double)t2));
+                            const int j = jb + 8 * h + e;
+                            if ((unsigned)j < (unsigned)N_t) {
+                                double* p = rcol + (j & (SP_RING - 1)) * SP_TS;
+                                *p = fma(w1[k], V, fma(w0[k], prev[k], *p));
+                            }
+                            prev[k] = V;
+                        }
+                    }
+                    im++;
+                }
+                lse_rows(min(N_t, SP_NB * c + SP_NB - 1 - ti.cap));
+            }
+            lse_rows(N_t);
+            if (member) lnL[perm ? perm[pos] : pos] = run_m + log(run_s) - P.ln_Nt;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (w == 4) tmem_free512(tmem);
+}
+
+// ---------------------------------------------------------------- launch
+template <int K, bool TABLE>
+static int launch_split_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL,
+                          const SpTile* tiles, const int* ntiles_dev) {
+    const int smem = (int)sizeof(SplitSmem) + 1024;
+    ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_split_kernel<K, TABLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    const int slot = ile_timing_begin(ctx);
+    lnl_split_kernel<K, TABLE><<<ctx->sm_count, SP_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
+    ile_timing_end(ctx, slot);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}
+
+bool ile_split_supported(const LnlParams& P) { return P.K >= 1 && P.K <= 3 && P.M <= 24 && P.stride == 1 && P.Qs != nullptr && P.n_pairs * P.K * 2 <= SP_UVMAX; }
+
+// scratch layout helpers for the caller (ile_launch_lnL_fused): tile list capacity for N samples
+int ile_split_max_tiles(int N, int cell_bits, int K) {
+    const long long cells = (1ll << (cell_bits * K)) + 1;
+    const long long t = (N + SP_TS - 1) / SP_TS + (cells < N ? cells : N) + 1;
+    return (int)t;
+}
+size_t ile_split_tile_bytes(int max_tiles) { return ((size_t)max_tiles * (sizeof(SpTile) + sizeof(int)) + 255) / 256 * 256; }
+int ile_split_cell_bits(int n_min, int n_max) {
+    int cell_bits = 1;
+    while ((1 << cell_bits) <= ((n_max - n_min) >> SP_CELL_SHIFT)) cell_bits++;
+    return cell_bits;
+}
+
+int ile_launch_split_keys(ile_ctx* ctx, const LnlParams& P, int N, const double* z, int n_min, int cell_bits, unsigned long long* key,
+                          unsigned int* val, long long* n_dev, int* bits_dev, int* ntiles_dev) {
+    sp_key_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(P, N, z, n_min, cell_bits, key, val, n_dev, bits_dev, ntiles_dev);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}
+
+// rec / yt as written by lnl_prep3_kernel in the order of perm (sorted by sp_key_kernel's keys, in key[])
+int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int cell_bits, const unsigned long long* key, const double* rec, const double2* yt,
+                     const int* perm, double* lnL, int* tstart, SpTile* tiles, int* ntiles_dev) {
+    sp_tile_flag_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(N, key, tstart, ntiles_dev);
+    ILE_LAUNCH_CHECK(ctx);
+    const int max_tiles = ile_split_max_tiles(N, cell_bits, P.K);
+    sp_tile_info_kernel<<<(max_tiles * 32 + 255) / 256, 256, 0, ctx->stream>>>(P, N, cell_bits * P.K, key, tstart, ntiles_dev, rec, tiles);
+    ILE_LAUNCH_CHECK(ctx);
+    const bool tb = P.use_table != 0;
+    if (P.K == 3) return tb ? launch_split_t<3, true>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev) : launch_split_t<3, false>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
+    if (P.K == 2) return tb ? launch_split_t<2, true>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev) : launch_split_t<2, false>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
+    return tb ? launch_split_t<1, true>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev) : launch_split_t<1, false>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
+}

@@ -304,6 +304,30 @@ def make_problem(cfg: int, P: int | None = None, N: int | None = None, n_iter: i
                    n_iter=n_iter, opts=opts, table=table, inj=inj)
 
 
+def make_custom_problem(K: int, lmax: int, snr: float, seed: int, N_Q: int = 820, N_t: int = 300) -> Problem:
+    """A one-point problem with a detector / mode count outside the five configs (parity of the kernels' other
+    shapes).  The template's mode coefficients are seeded random numbers with the usual amplitude law, not a
+    physical signal (no injection fixture is needed): Q = q0 A_m(t - tau_k) + coloured noise as in make_q."""
+    rng = _rng(SEED_BASE + 900000 + seed)
+    D, pos = make_network(K, rng)
+    ell, m = make_modes(lmax)
+    M = len(ell)
+    t_Q0 = -(N_Q // 2) / FS
+    U, V, G = make_uv(K, ell, m, rng, profile=0)
+    tpl = dict(F=(rng.standard_normal(K) + 1j * rng.standard_normal(K)) * 0.5,
+               Y=(rng.standard_normal(M) + 1j * rng.standard_normal(M)) * 0.3,
+               tau=rng.uniform(-0.5, 0.5, K) * R_EARTH / C_LIGHT)
+    Q, D_ref, rho2 = make_q(U, V, G, ell, m, [tpl], snr, N_Q, t_Q0, rng)
+    t_lo = -(N_t // 2) / FS
+    D_min, D_max = 100.0, 2000.0
+    lo = np.array([0.0, -1.0, 0.0, 0.0, -1.0, D_min])
+    hi = np.array([2.0 * np.pi, 1.0, np.pi, 2.0 * np.pi, 1.0, D_max])
+    return Problem(cfg=0, K=K, M=M, P=1, N_Q=N_Q, fs=FS, t_Q0=t_Q0, D=D, pos=pos, gmst=0.0, ell=ell, m=m,
+                   Q=Q[None], U=U[None], V=V[None], D_ref=D_ref, rho2=rho2, t_lo=t_lo, dt=1.0 / FS, N_t=N_t, interp=1,
+                   D_min=D_min, D_max=D_max, d=6, lo=lo, hi=hi, kind="UNIFORM", N=1 << 12, n_iter=1,
+                   opts=dict(seed=seed), table=None, inj=None)
+
+
 def uniform_box_samples(lo, hi, N, seed):
     """N points uniform in the box [lo, hi) (numpy Philox; for parity inputs, not the
     integrators' own counter-based draws)."""

@@ -90,7 +90,7 @@ def test_all_samples_outside_the_box_and_empty_batch():
 
 
 def test_delay_spread_beyond_one_round():
-    """Unsorted samples all over the sky in one tile force the multi-round path (variant 2)."""
+    """Unsorted samples all over the sky in one tile force the DMMA kernel's multi-round path (variant 3: no delay-cell sort)."""
     import torch
     from paper_2505_11655_b200 import Ile
     from oracle import likelihood as lk
@@ -98,7 +98,7 @@ def test_delay_spread_beyond_one_round():
     prob = make_problem(3, P=1)
     ile = Ile(0)
     ile.load_problem(prob)
-    ile.set_lnL_variant(2)
+    ile.set_lnL_variant(3)
     z = uniform_box_samples(prob.lo, prob.hi, 257, seed=4)
     ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
                    prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z)

@@ -10,6 +10,10 @@ from synth.workloads import uniform_box_samples
 pytestmark = pytest.mark.gpu
 
 
+VARIANTS = (0, 1, 2, 3)        # every value ile_set_lnL_variant accepts
+FUSED = (0, 2)                 # the two fused kernels (tcgen05 digits, FP64 DMMA)
+
+
 def _tol(ref):
     return 1e-9 * np.maximum(1.0, np.abs(ref))      # north_star: per-sample lnL within 1e-9 relative (fp64)
 
@@ -61,13 +65,14 @@ def test_lnL_parity_all_entry_points(torch_mod, cfg, N):
     ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
                    prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z)
     zd = _dev(torch, z)
-    got, lp = ile.lnL_z(0, zd, want_prior=True)                     # fused DMMA kernel (unsorted: multi-round path)
-    got = got.cpu().numpy()
-    assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
-    np.testing.assert_allclose(lp.cpu().numpy(), lk.ln_prior_z(z, prob.D_min, prob.D_max), rtol=1e-14)
-    ile.set_lnL_variant(1)                                          # plain reference kernel
-    got1 = ile.lnL_z(0, zd).cpu().numpy()
-    assert np.all(np.abs(got1 - ref) <= _tol(ref))
+    # every kernel the ABI can select: 0 = tcgen05 integer-digit kernel where the shape allows (config 1's stride-2
+    # grid runs the DMMA kernel), 1 = plain, 2 = DMMA kernel behind the delay-cell sort, 3 = DMMA kernel, unsorted
+    for variant in VARIANTS:
+        ile.set_lnL_variant(variant)
+        got, lp = ile.lnL_z(0, zd, want_prior=True)
+        got = got.cpu().numpy()
+        assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
+        np.testing.assert_allclose(lp.cpu().numpy(), lk.ln_prior_z(z, prob.D_min, prob.D_max), rtol=1e-14)
     ang = lk.z_to_angles(z)
     got2, dump = ile.lnL(0, *[_dev(torch, a) for a in ang], N_t_dump=prob.N_t)
     assert np.all(np.abs(got2.cpu().numpy() - ref) <= _tol(ref))
@@ -91,11 +96,13 @@ def test_lnL_localised_samples_single_round(torch_mod):
     z[:, 7] = [7.0, 0.0, 1.0, 1.0, 0.0, 500.0]                        # one out-of-box sample
     ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
                    prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, np.delete(z, 7, axis=1))
-    got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
-    assert got[7] == -np.inf
-    got = np.delete(got, 7)
     assert ref.max() > 1000.0                                         # loud source: lnL dynamic range
-    assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
+    for variant in FUSED:
+        ile.set_lnL_variant(variant)
+        got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
+        assert got[7] == -np.inf
+        got = np.delete(got, 7)
+        assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
 
 
 def test_lnL_nearest_bin_and_table(torch_mod):
@@ -109,12 +116,15 @@ def test_lnL_nearest_bin_and_table(torch_mod):
             prob.t_Q0, prob.t_lo, prob.dt, prob.N_t)
     ref = lk.lnL_z(*args, z, table=prob.table)
     zd = _dev(torch, z)
-    got = ile.lnL_z(0, zd).cpu().numpy()
-    assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
-    ile.set_time_grid(prob.t_lo, prob.dt, prob.N_t, 0)                # nearest-bin mode
     ref0 = lk.lnL_z(*args, z, interp=0, table=prob.table)
-    got0 = ile.lnL_z(0, zd).cpu().numpy()
-    assert np.all(np.abs(got0 - ref0) <= _tol(ref0))
+    for variant in FUSED:
+        ile.set_lnL_variant(variant)
+        ile.set_time_grid(prob.t_lo, prob.dt, prob.N_t, 1)
+        got = ile.lnL_z(0, zd).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
+        ile.set_time_grid(prob.t_lo, prob.dt, prob.N_t, 0)            # nearest-bin mode
+        got0 = ile.lnL_z(0, zd).cpu().numpy()
+        assert np.all(np.abs(got0 - ref0) <= _tol(ref0)), (variant, np.abs(got0 - ref0).max())
 
 
 def test_reduce_parity(torch_mod):
@@ -158,14 +168,17 @@ def test_error_paths(torch_mod):
         ile.set_time_grid(prob.t_lo, 1.5 / prob.fs, 10)              # non-integer stride
 
 
-@pytest.mark.parametrize("N_t,stride", [(1, 1), (7, 1), (63, 1), (64, 1), (65, 1), (129, 1), (333, 1), (50, 2), (131, 3)])
-def test_time_grid_shapes(torch_mod, N_t, stride):
-    """Window lengths around the 64-output phases of the fused kernel (one phase, exactly full, one bin over, a
-    short tail) and time steps of 2 and 3 stored bins, on the l <= 4 three-detector problem."""
+@pytest.mark.parametrize("variant", FUSED)
+@pytest.mark.parametrize("N_t,stride", [(1, 1), (7, 1), (15, 1), (16, 1), (17, 1), (63, 1), (64, 1), (65, 1), (129, 1), (333, 1), (50, 2), (131, 3)])
+def test_time_grid_shapes(torch_mod, N_t, stride, variant):
+    """Window lengths around the 64-output phases of the DMMA kernel and the 16-bin work items of the tcgen05 kernel
+    (one phase, exactly full, one bin over, a short tail) and time steps of 2 and 3 stored bins (DMMA kernel in
+    both variants), on the l <= 4 three-detector problem."""
     from oracle import likelihood as lk
     torch = torch_mod
     prob = make_problem(2)
     ile = _ile(prob)
+    ile.set_lnL_variant(variant)
     dt = stride / prob.fs
     t_lo = -0.5 * (N_t - 1) * dt
     t_lo = round(t_lo * prob.fs) / prob.fs                              # on the stored grid
@@ -176,3 +189,22 @@ def test_time_grid_shapes(torch_mod, N_t, stride):
                    prob.t_Q0, t_lo, dt, N_t, z)
     got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
     assert np.all(np.abs(got - ref) <= _tol(ref)), np.abs(got - ref).max()
+
+
+@pytest.mark.parametrize("K,lmax", [(1, 2), (2, 3), (3, 3), (3, 4)])
+def test_lnL_other_shapes(torch_mod, K, lmax):
+    """Detector and mode counts other than the configs': K = 1..3, l <= 2, 3, 4 (M = 5, 12, 21) through the tcgen05
+    kernel (any M <= 24) and whatever the DMMA variant falls back to."""
+    from oracle import likelihood as lk
+    from synth.workloads import make_custom_problem
+    torch = torch_mod
+    prob = make_custom_problem(K=K, lmax=lmax, snr=30.0, seed=40 + 10 * K + lmax)
+    ile = _ile(prob)
+    N = 700
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=3)
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z)
+    for variant in FUSED:
+        ile.set_lnL_variant(variant)
+        got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
