@@ -465,18 +465,31 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                 const double2* uv = sm.uv;
                 for (int a = 0; a < M; a++) {
                     const double2 ya = sm.Y[a][i];
-                    for (int b = a; b < M; b++) {
-                        const double2 yb = sm.Y[b][i];
-                        const double t2 = ya.y * yb.y, t4 = ya.y * yb.x;
-                        const double pr = fma(ya.x, yb.x, t2), qr = fma(ya.x, yb.x, -t2), pi = fma(ya.x, yb.y, -t4), qi = fma(ya.x, yb.y, t4);
+                    for (int b = a; b < M; b += 4) {
+                        // four pairs (a, b .. b + 3) per step, all operands loaded before the arithmetic; pairs past the
+                        // end of the row multiply a zero harmonic (the matrix index stays inside the packed array)
+                        double2 yb[4], u[4][K], v[4][K];
 #pragma unroll
-                        for (int k = 0; k < K; k++) {
-                            const double2 u = uv[2 * k], v = uv[2 * k + 1];
-                            uu[k] = fma(-u.y, pi, fma(u.x, pr, uu[k]));
-                            vr[k] = fma(-v.y, qi, fma(v.x, qr, vr[k]));
-                            vi[k] = fma(v.y, qr, fma(v.x, qi, vi[k]));
+                        for (int q = 0; q < 4; q++) {
+                            const bool in = b + q < M;
+                            yb[q] = sm.Y[in ? b + q : a][i];
+                            if (!in) yb[q] = make_double2(0.0, 0.0);
+                            const double2* uq = uv + (in ? q : 0) * 2 * K;
+#pragma unroll
+                            for (int k = 0; k < K; k++) { u[q][k] = uq[2 * k]; v[q][k] = uq[2 * k + 1]; }
                         }
-                        uv += 2 * K;
+#pragma unroll
+                        for (int q = 0; q < 4; q++) {
+                            const double t2 = ya.y * yb[q].y, t4 = ya.y * yb[q].x;
+                            const double pr = fma(ya.x, yb[q].x, t2), qr = fma(ya.x, yb[q].x, -t2), pi = fma(ya.x, yb[q].y, -t4), qi = fma(ya.x, yb[q].y, t4);
+#pragma unroll
+                            for (int k = 0; k < K; k++) {
+                                uu[k] = fma(-u[q][k].y, pi, fma(u[q][k].x, pr, uu[k]));
+                                vr[k] = fma(-v[q][k].y, qi, fma(v[q][k].x, qr, vr[k]));
+                                vi[k] = fma(v[q][k].y, qr, fma(v[q][k].x, qi, vi[k]));
+                            }
+                        }
+                        uv += 2 * K * min(4, M - b);
                     }
                 }
 #pragma unroll
@@ -505,14 +518,21 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
 
             // rows [jdone, jend) of the ring are complete: lnL(t_j) and the streaming log-sum-exp (step 6)
             auto lse_rows = [&](const int jend) {
-                for (int j0 = jdone; j0 < jend; j0 += 4) {
-                    double v[4];
+                for (int j0 = jdone; j0 < jend; j0 += 8) {
+                    double v[8];
+                    double* pr[8];
+#pragma unroll
+                    for (int e = 0; e < 8; e++) {
+                        pr[e] = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
+                        v[e] = *pr[e];
+                    }
+#pragma unroll
+                    for (int e = 0; e < 8; e++)
+                        if (j0 + e < jend) *pr[e] = init;
                     bool need = false;
 #pragma unroll
-                    for (int e = 0; e < 4; e++) {
-                        double* p = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
-                        double A = *p;
-                        if (j0 + e < jend) *p = init;
+                    for (int e = 0; e < 8; e++) {
+                        double A = v[e];
                         if (TABLE) {
                             double a = fma(A, tabA_s, tabA_o);
                             a = fmin(fmax(a, 0.0), (double)(P.nA - 1));
@@ -528,20 +548,22 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     }
                     if (__any_sync(0xffffffffu, need)) {
                         // raise the reference to the largest new value (rare); the running sum is rescaled exactly
-                        const double mx = fmax(fmax(v[0], v[1]), fmax(v[2], v[3]));
+                        const double mx = fmax(fmax(fmax(v[0], v[1]), fmax(v[2], v[3])), fmax(fmax(v[4], v[5]), fmax(v[6], v[7])));
                         if (mx - run_m >= 30.0) {
                             const double dm = run_m - mx;
                             run_s = dm > -690.0 ? run_s * sp_exp_small(dm) : 0.0;
                             run_m = mx;
                         }
                     }
+                    double part[2] = {0.0, 0.0};
 #pragma unroll
-                    for (int e = 0; e < 4; e++) {
+                    for (int e = 0; e < 8; e++) {
                         // terms below e^-40 of the reference (and rows past the end) are clamped to e^-40 (R2)
                         const double dl = v[e] - run_m;
                         const unsigned hc = min((unsigned)__double2hiint(dl), 0xC0440000u);
-                        run_s += sp_exp_tab(__hiloint2double((int)hc, __double2loint(dl)), etab);
+                        part[e & 1] += sp_exp_tab(__hiloint2double((int)hc, __double2loint(dl)), etab);
                     }
+                    run_s += part[0] + part[1];
                 }
                 jdone = max(jdone, jend);
             };
@@ -564,19 +586,31 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                             tc_fence_before();
                             mbar_arrive(&sm.d_empty[b]);
                         }
+                        // all loads of the ring first, then the arithmetic, then all stores: the eight rows are distinct, which
+                        // the compiler cannot see through the run-time row index (it would serialise load -> store -> load)
+                        double V[8], rv[8];
+                        double* pr[8];
+                        bool ok[8];
+#pragma unroll
+                        for (int e = 0; e < 8; e++) {
+                            const int j = jb + 8 * h + e;
+                            ok[e] = (unsigned)j < (unsigned)N_t;
+                            pr[e] = rcol + (j & (SP_RING - 1)) * SP_TS;
+                            rv[e] = ok[e] ? *pr[e] : 0.0;
+                        }
 #pragma unroll
                         for (int e = 0; e < 8; e++) {
                             const int t0 = (int)acc[0][e] * 256 + (int)acc[1][e];
                             const int t1 = (int)acc[2][e] * 256 + (int)acc[3][e];
                             const int t2 = (int)acc[4][e] * 256 + (int)acc[5][e];
-                            const double V = fma((double)t0, 4294967296.0, fma((double)t1, 65536.0, (double)t2));
-                            const int j = jb + 8 * h + e;
-                            if ((unsigned)j < (unsigned)N_t) {
-                                double* p = rcol + (j & (SP_RING - 1)) * SP_TS;
-                                *p = fma(w1[k], V, fma(w0[k], prev[k], *p));
-                            }
-                            prev[k] = V;
+                            V[e] = fma((double)t0, 4294967296.0, fma((double)t1, 65536.0, (double)t2));
                         }
+#pragma unroll
+                        for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e], fma(w0[k], e == 0 ? prev[k] : V[e - 1], rv[e]));
+#pragma unroll
+                        for (int e = 0; e < 8; e++)
+                            if (ok[e]) *pr[e] = rv[e];
+                        prev[k] = V[7];
                     }
                     im++;
                 }
