@@ -30,18 +30,20 @@
 #include "exp_tab.cuh"
 
 #define SP_TS 128             // samples per tile
-#define SP_NB 16              // stored bins per work item (MMA N)
+#define SP_NB 32              // stored bins per work item (MMA N)
 #define SP_BLK 48             // bytes per digit block
 #define SP_NCH 19             // 16-byte chunks per stored bin in the Q digit image (304 bytes)
 #define SP_GRP (SP_NCH * 128) // bytes per group of 8 bins
-#define SP_STAGE (2 * SP_GRP) // bytes per 16-bin chunk
-#define SP_NSTAGE 6
+#define SP_STAGE ((SP_NB / 8) * SP_GRP) // bytes per chunk of SP_NB bins
+#define SP_NSTAGE 4
 #define SP_RING 64            // rows (time bins) of the accumulation ring
 #define SP_CAPMAX 24          // largest per-sample offset above the tile base
 #define SP_CELL_SHIFT 4       // delay cells of 16 stored bins
 #define SP_ACOLS 72           // tensor-memory columns of A per detector (288 bytes)
-#define SP_DCOL 256           // first accumulator column; set b, sum s at SP_DCOL + 96 b + 16 s
-#define SP_THREADS 160
+#define SP_DCOL 256           // first accumulator column; sum s at SP_DCOL + SP_NB s (one set: it is free again as soon as every warp has loaded its bins)
+#define SP_G 4                // threads per sample (warp groups): digits by detector, bins, triangle rows, log-sum-exp rows
+#define SP_MATH (SP_G * SP_TS)
+#define SP_THREADS (SP_MATH + 32)
 #define SP_UVMAX (300 * 3 * 2)
 #define SP_MAGIC 6755399441055744.0   // 1.5 * 2^52
 
@@ -224,7 +226,10 @@ struct SplitSmem {
     double2 Y[24][SP_TS];                     // harmonics of the tile, column = sample
     double2 uv[SP_UVMAX];                     // packed upper-triangle U/V of the intrinsic point
     double etab[64][16];                      // 2^(j/64), 16 copies: lane l reads copy l % 16 (conflict-free)
-    uint64_t a_full, d_full[2], d_empty[2], b_full[SP_NSTAGE], b_empty[SP_NSTAGE];
+    double xch[2][3][SP_TS];                  // last bin of a chunk, from group 3 to group 0 of the next chunk (slot = chunk parity)
+    double lse[SP_G][2][SP_TS];               // partial (reference, sum) of the four threads of a sample
+    int eb[3][SP_TS];                         // biased exponent of max |coefficient| per detector
+    uint64_t a_full, d_full, d_empty, b_full[SP_NSTAGE], b_empty[SP_NSTAGE];
     uint32_t tmem_base;
 };
 
@@ -260,6 +265,14 @@ __device__ __forceinline__ double sp_exp_small(double d) {
     p = fma(p, r, 1.0);
     p = fma(p, r, 1.0);
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// V = sum_s acc_s 256^(5-s) = t0 2^32 + t1 2^16 + t2 with t = acc_even 256 + acc_odd (int32, no overflow), exact in 64-bit
+// integers (|V| < 2^63), then one conversion (rounded to 53 bits: 2^-53 of |V|, far below the digits dropped)
+__device__ __forceinline__ double sp_recombine(uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t a4, uint32_t a5) {
+    const int t0 = (int)a0 * 256 + (int)a1, t1 = (int)a2 * 256 + (int)a3, t2 = (int)a4 * 256 + (int)a5;
+    const long long v = ((long long)t0 << 32) + ((long long)t1 * 65536LL + (long long)t2);
+    return (double)v;
 }
 
 // cursor over the work items (tile, chunk, detector) of this CTA, in the order both warp roles walk them
@@ -301,10 +314,11 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     const int ntiles = *ntiles_dev;
 
-    if (w == 4) tmem_alloc512(&sm.tmem_base);
+    if (w == SP_MATH / 32) tmem_alloc512(&sm.tmem_base);
     if (tid == 0) {
-        mbar_init(&sm.a_full, SP_TS);
-        for (int b = 0; b < 2; b++) { mbar_init(&sm.d_full[b], 1); mbar_init(&sm.d_empty[b], SP_TS); }
+        mbar_init(&sm.a_full, SP_MATH);
+        mbar_init(&sm.d_full, 1);
+        mbar_init(&sm.d_empty, SP_MATH);
         for (int s = 0; s < SP_NSTAGE; s++) { mbar_init(&sm.b_full[s], 1); mbar_init(&sm.b_empty[s], 1); }
         mbar_init_fence();
     }
@@ -319,7 +333,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
     tc_fence_after();
     const uint32_t tmem = sm.tmem_base;
 
-    if (w == 4) {
+    if (w == SP_MATH / 32) {
         // ================================================================ producer: TMA loads and MMA issue
         const bool el = elect_one();
         const uint32_t idesc = umma_idesc_s8_m128(SP_NB);
@@ -344,13 +358,13 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                 mbar_wait(&sm.a_full, tile_par);
                 tile_par ^= 1;
             }
-            const unsigned b = nm & 1, s = nm % SP_NSTAGE;
-            if (nm >= 2) mbar_wait(&sm.d_empty[b], ((nm >> 1) - 1) & 1);
+            const unsigned s = nm % SP_NSTAGE;
+            if (nm >= 1) mbar_wait(&sm.d_empty, (nm - 1) & 1);
             mbar_wait(&sm.b_full[s], (nm / SP_NSTAGE) & 1);
             tc_fence_after();
             if (el) {
                 const uint64_t b0 = umma_desc_kmajor_noswizzle(smem_u32(sm.bst[s]), 128, SP_GRP);
-                const uint32_t a0 = tmem + SP_ACOLS * Mc.k, d0 = tmem + SP_DCOL + 96 * b;
+                const uint32_t a0 = tmem + SP_ACOLS * Mc.k, d0 = tmem + SP_DCOL;
                 // sum s reads K_s = 64, 96, 160, 192, 256, 288 bytes of A against the view of B starting at 16-byte chunk 3 (5 - s);
                 // k-step major, so that consecutive MMAs go to different accumulators
 #pragma unroll
@@ -362,27 +376,31 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     }
                 }
                 umma_commit(&sm.b_empty[s]);
-                umma_commit(&sm.d_full[b]);
+                umma_commit(&sm.d_full);
             }
             __syncwarp();
             nm++;
             sp_cursor_next<K>(Mc, tiles, ntiles, gridDim.x);
         }
     } else {
-        // ================================================================ one thread per sample
-        const int i = tid;                                     // sample of the tile = tensor-memory lane
-        const uint32_t tlane = tmem + ((uint32_t)(32 * w) << 16);
+        // ================================================================ SP_G threads per sample
+        // thread (g, i): sample i of the tile = tensor-memory lane i (warp % 4 is the lane quarter), group g = warp / 4.
+        // The four threads of a sample split its work: detectors (digits), rows of the U/V triangle (step 4), bins of
+        // every work item (4 each) and rows of the log-sum-exp.  They meet at a named barrier per lane quarter.
+        const int g = w >> 2, qd = w & 3;
+        const int i = 32 * qd + lane;
+        const uint32_t tlane = tmem + ((uint32_t)(32 * qd) << 16);
         double* const rcol = &sm.ring[0][i];
         const double* const etab = &sm.etab[0][lane & 15];
         const double tabA_s = TABLE ? (double)(P.nA - 1) / (P.A_hi - P.A_lo) : 0.0, tabA_o = -P.A_lo * tabA_s;
-        unsigned im = 0, tile_seq = 0;
-        (void)tile_seq;
+        auto qbar = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + qd), "r"(32 * SP_G) : "memory"); };
+        unsigned im = 0;
         for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
             const SpTile ti = tiles[t];
             const int pos = ti.start + i;
             const bool member = i < ti.cnt;
             if (ti.nchunk == 0) {
-                if (member) lnL[perm ? perm[pos] : pos] = (ti.flags & 2) ? __longlong_as_double(0x7ff8000000000000LL) : neg_inf();
+                if (member && g == 0) lnL[perm ? perm[pos] : pos] = (ti.flags & 2) ? __longlong_as_double(0x7ff8000000000000LL) : neg_inf();
                 continue;
             }
             const int N_t = P.N_t;
@@ -411,13 +429,15 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     off[k] = min(max((int)fl - ti.base[k], 0), SP_CAPMAX);
                 }
             }
-            // ---- harmonics: own column of the tile
-#pragma unroll 4
-            for (int m = 0; m < 24; m++)
+            // ---- harmonics: group g fetches modes g, g + 4, ... of the sample's column
+#pragma unroll
+            for (int m = g; m < 24; m += SP_G)
                 sm.Y[m][i] = member ? __ldg(ytile + ((size_t)(pos >> 5) * 24 + m) * 32 + (pos & 31)) : make_double2(0.0, 0.0);
-            // ---- step 3: coefficients x F_k Y_m -> six signed 8-bit digits -> tensor memory (operand A)
+            qbar();
+            // ---- step 3 (group k does detector k): coefficients x F_k Y_m -> six signed 8-bit digits -> tensor memory (operand A)
 #pragma unroll
             for (int k = 0; k < K; k++) {
+                if (k != g) continue;
                 const double xr = x * fr[k], xi = x * fi[k];
                 int mh = 0;
 #pragma unroll 4
@@ -427,10 +447,8 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     mh = max(mh, max(__double2hiint(cr) & 0x7fffffff, __double2hiint(ci) & 0x7fffffff));
                 }
                 const int eb = min(max(mh >> 20, 200), 1800);
+                sm.eb[k][i] = eb;
                 const double sc = __hiloint2double((2091 - eb) << 20, 0);         // 2^(45 - (eb - 1023)): |coef sc| < 2^46
-                const double un = __hiloint2double(min(max(eb + P.qeb[k] - 1023 - 50, 1), 2046) << 20, 0);   // 2^40 / (sc sq_k)
-                w0[k] *= un;
-                w1[k] *= un;
                 uint32_t col[6][12];
 #pragma unroll
                 for (int q = 0; q < 12; q++) {
@@ -445,58 +463,77 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     for (int a = 0; a < 6; a++) col[a][q] = wd[a];
                 }
 #pragma unroll
-                for (int g = 0; g < 9; g++) {
+                for (int gg = 0; gg < 9; gg++) {
                     uint32_t v[8];
 #pragma unroll
-                    for (int e = 0; e < 8; e++) v[e] = col[(8 * g + e) / 12][(8 * g + e) % 12];
-                    tmem_st8(tlane + SP_ACOLS * k + 8 * g, v);
+                    for (int e = 0; e < 8; e++) v[e] = col[(8 * gg + e) / 12][(8 * gg + e) % 12];
+                    tmem_st8(tlane + SP_ACOLS * k + 8 * gg, v);
                 }
+                tmem_wait_st();
             }
-            tmem_wait_st();
             tc_fence_before();
             mbar_arrive(&sm.a_full);
-            // ---- step 4: B = 1/4 sum_k [ |F_k|^2 Re(y^H U_k y) + Re(F_k^2 y^T V_k y) ] over the upper triangle (Eq. 17-18)
-            double Bq = 0.0;
+            // ---- step 4: B = 1/4 sum_k [ |F_k|^2 Re(y^H U_k y) + Re(F_k^2 y^T V_k y) ] over the upper triangle (Eq. 17-18).
+            //      Group g walks the rows a with a % 8 == g or 7 - g (equal pair counts); the partial sums meet in the ring's memory.
+            double* const qpart = &sm.ring[0][0];                // [SP_G][3 K][128], the ring is idle until the first work item
             {
                 double uu[K], vr[K], vi[K];
 #pragma unroll
                 for (int k = 0; k < K; k++) uu[k] = vr[k] = vi[k] = 0.0;
                 const int M = P.M;
-                const double2* uv = sm.uv;
                 for (int a = 0; a < M; a++) {
+                    if ((a & 7) != g && (a & 7) != 7 - g) continue;
                     const double2 ya = sm.Y[a][i];
-                    for (int b = a; b < M; b += 4) {
-                        // four pairs (a, b .. b + 3) per step, all operands loaded before the arithmetic; pairs past the
-                        // end of the row multiply a zero harmonic (the matrix index stays inside the packed array)
-                        double2 yb[4], u[4][K], v[4][K];
+                    const double2* uv = sm.uv + (size_t)(a * M - (a * (a - 1)) / 2) * 2 * K;
+                    for (int b = a; b < M; b += 2) {
+                        // two pairs per step; a pair past the end of the row multiplies a zero harmonic
+                        const bool in1 = b + 1 < M;
+                        double2 yb[2];
+                        yb[0] = sm.Y[b][i];
+                        yb[1] = sm.Y[in1 ? b + 1 : b][i];
+                        if (!in1) yb[1] = make_double2(0.0, 0.0);
+                        const double2* u1 = uv + (in1 ? 2 * K : 0);
 #pragma unroll
-                        for (int q = 0; q < 4; q++) {
-                            const bool in = b + q < M;
-                            yb[q] = sm.Y[in ? b + q : a][i];
-                            if (!in) yb[q] = make_double2(0.0, 0.0);
-                            const double2* uq = uv + (in ? q : 0) * 2 * K;
-#pragma unroll
-                            for (int k = 0; k < K; k++) { u[q][k] = uq[2 * k]; v[q][k] = uq[2 * k + 1]; }
-                        }
-#pragma unroll
-                        for (int q = 0; q < 4; q++) {
+                        for (int q = 0; q < 2; q++) {
+                            const double2* uq = q ? u1 : uv;
                             const double t2 = ya.y * yb[q].y, t4 = ya.y * yb[q].x;
                             const double pr = fma(ya.x, yb[q].x, t2), qr = fma(ya.x, yb[q].x, -t2), pi = fma(ya.x, yb[q].y, -t4), qi = fma(ya.x, yb[q].y, t4);
 #pragma unroll
                             for (int k = 0; k < K; k++) {
-                                uu[k] = fma(-u[q][k].y, pi, fma(u[q][k].x, pr, uu[k]));
-                                vr[k] = fma(-v[q][k].y, qi, fma(v[q][k].x, qr, vr[k]));
-                                vi[k] = fma(v[q][k].y, qr, fma(v[q][k].x, qi, vi[k]));
+                                const double2 u = uq[2 * k], v = uq[2 * k + 1];
+                                uu[k] = fma(-u.y, pi, fma(u.x, pr, uu[k]));
+                                vr[k] = fma(-v.y, qi, fma(v.x, qr, vr[k]));
+                                vi[k] = fma(v.y, qr, fma(v.x, qi, vi[k]));
                             }
                         }
-                        uv += 2 * K * min(4, M - b);
+                        uv += 4 * K;
                     }
                 }
 #pragma unroll
-                for (int k = 0; k < K; k++)
-                    Bq += (fr[k] * fr[k] + fi[k] * fi[k]) * uu[k] + ((fr[k] * fr[k] - fi[k] * fi[k]) * vr[k] - 2.0 * fr[k] * fi[k] * vi[k]);
-                Bq *= 0.25;
+                for (int k = 0; k < K; k++) {
+                    qpart[((g * 3 * K) + 3 * k + 0) * SP_TS + i] = uu[k];
+                    qpart[((g * 3 * K) + 3 * k + 1) * SP_TS + i] = vr[k];
+                    qpart[((g * 3 * K) + 3 * k + 2) * SP_TS + i] = vi[k];
+                }
             }
+            qbar();
+            double Bq = 0.0;
+#pragma unroll
+            for (int k = 0; k < K; k++) {
+                double uu = 0.0, vr = 0.0, vi = 0.0;
+#pragma unroll
+                for (int gg = 0; gg < SP_G; gg++) {
+                    uu += qpart[((gg * 3 * K) + 3 * k + 0) * SP_TS + i];
+                    vr += qpart[((gg * 3 * K) + 3 * k + 1) * SP_TS + i];
+                    vi += qpart[((gg * 3 * K) + 3 * k + 2) * SP_TS + i];
+                }
+                Bq += (fr[k] * fr[k] + fi[k] * fi[k]) * uu + ((fr[k] * fr[k] - fi[k] * fi[k]) * vr - 2.0 * fr[k] * fi[k] * vi);
+                // 2^40 / (sc sq_k): the weight of the integer contraction, folded into the interpolation weights
+                const double un = __hiloint2double(min(max(sm.eb[k][i] + P.qeb[k] - 1023 - 50, 1), 2046) << 20, 0);
+                w0[k] *= un;
+                w1[k] *= un;
+            }
+            Bq *= 0.25;
             // per-sample constants of the time marginalisation
             double init = -(x * x * Bq), tb_f = 0.0;
             const double* tb_row = nullptr;
@@ -508,30 +545,34 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                 tb_row = P.lnT + (size_t)ib * P.nA;
                 init = 0.0;
             }
-#pragma unroll 8
-            for (int r = 0; r < SP_RING; r++) rcol[r * SP_TS] = init;
+            qbar();                                              // partial sums read by everybody before the ring is initialised
+#pragma unroll 4
+            for (int r = g; r < SP_RING; r += SP_G) rcol[r * SP_TS] = init;
+            if (g == 0) {
+#pragma unroll
+                for (int k = 0; k < K; k++) sm.xch[0][k][i] = sm.xch[1][k][i] = 0.0;
+            }
+            qbar();
             double run_m = -1.0e300, run_s = 0.0;
             int jdone = 0;
-            double prev[K];
-#pragma unroll
-            for (int k = 0; k < K; k++) prev[k] = 0.0;
 
-            // rows [jdone, jend) of the ring are complete: lnL(t_j) and the streaming log-sum-exp (step 6)
+            // rows jdone + g, jdone + g + 4, ... below jend are complete: lnL(t_j) and this thread's share of the streaming
+            // log-sum-exp (step 6); four rows per batch, loads first
             auto lse_rows = [&](const int jend) {
-                for (int j0 = jdone; j0 < jend; j0 += 8) {
-                    double v[8];
-                    double* pr[8];
+                for (int j0 = jdone + g; j0 < jend; j0 += 4 * SP_G) {
+                    double v[4];
+                    double* pr[4];
 #pragma unroll
-                    for (int e = 0; e < 8; e++) {
-                        pr[e] = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
+                    for (int e = 0; e < 4; e++) {
+                        pr[e] = rcol + ((j0 + SP_G * e) & (SP_RING - 1)) * SP_TS;
                         v[e] = *pr[e];
                     }
 #pragma unroll
-                    for (int e = 0; e < 8; e++)
-                        if (j0 + e < jend) *pr[e] = init;
+                    for (int e = 0; e < 4; e++)
+                        if (j0 + SP_G * e < jend) *pr[e] = init;
                     bool need = false;
 #pragma unroll
-                    for (int e = 0; e < 8; e++) {
+                    for (int e = 0; e < 4; e++) {
                         double A = v[e];
                         if (TABLE) {
                             double a = fma(A, tabA_s, tabA_o);
@@ -543,12 +584,12 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                             const double t0 = fma(fa, t01 - t00, t00), t1 = fma(fa, t11 - t10, t10);
                             A = fma(tb_f, t1 - t0, t0);
                         }
-                        v[e] = j0 + e < jend ? A : neg_inf();
+                        v[e] = j0 + SP_G * e < jend ? A : neg_inf();
                         need = need || (v[e] - run_m >= 30.0);
                     }
                     if (__any_sync(0xffffffffu, need)) {
                         // raise the reference to the largest new value (rare); the running sum is rescaled exactly
-                        const double mx = fmax(fmax(fmax(v[0], v[1]), fmax(v[2], v[3])), fmax(fmax(v[4], v[5]), fmax(v[6], v[7])));
+                        const double mx = fmax(fmax(v[0], v[1]), fmax(v[2], v[3]));
                         if (mx - run_m >= 30.0) {
                             const double dm = run_m - mx;
                             run_s = dm > -690.0 ? run_s * sp_exp_small(dm) : 0.0;
@@ -557,7 +598,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     }
                     double part[2] = {0.0, 0.0};
 #pragma unroll
-                    for (int e = 0; e < 8; e++) {
+                    for (int e = 0; e < 4; e++) {
                         // terms below e^-40 of the reference (and rows past the end) are clamped to e^-40 (R2)
                         const double dl = v[e] - run_m;
                         const unsigned hc = min((unsigned)__double2hiint(dl), 0xC0440000u);
@@ -568,61 +609,72 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                 jdone = max(jdone, jend);
             };
 
-            // ---- work items: accumulators -> FP64 -> interpolation -> ring
+            // ---- work items: accumulators -> FP64 -> interpolation -> ring; this thread takes bins 8 g .. 8 g + 7 of each item
             for (int c = 0; c < ti.nchunk; c++) {
+                // rows of this chunk all inside [0, N_t) for every sample of the tile: no per-row guard
+                const bool guard = !(SP_NB * c - 1 - ti.cap >= 0 && SP_NB * c + SP_NB - 2 < N_t);
 #pragma unroll
                 for (int k = 0; k < K; k++) {
-                    const unsigned b = im & 1;
-                    mbar_wait(&sm.d_full[b], (im >> 1) & 1);
+                    mbar_wait(&sm.d_full, im & 1);
                     tc_fence_after();
-                    const int jb = SP_NB * c - 1 - off[k];              // time bin of the pair (previous, first) of this chunk
+                    uint32_t acc[6][8], accp[6];
 #pragma unroll
-                    for (int h = 0; h < 2; h++) {
-                        uint32_t acc[6][8];
+                    for (int s = 0; s < 6; s++) tmem_ld8(tlane + SP_DCOL + SP_NB * s + 8 * g, acc[s]);
+                    if (g > 0) {
 #pragma unroll
-                        for (int s = 0; s < 6; s++) tmem_ld8(tlane + SP_DCOL + 96 * b + SP_NB * s + 8 * h, acc[s]);
-                        tmem_wait_ld();
-                        if (h == 1) {
-                            tc_fence_before();
-                            mbar_arrive(&sm.d_empty[b]);
-                        }
-                        // all loads of the ring first, then the arithmetic, then all stores: the eight rows are distinct, which
-                        // the compiler cannot see through the run-time row index (it would serialise load -> store -> load)
-                        double V[8], rv[8];
-                        double* pr[8];
-                        bool ok[8];
-#pragma unroll
-                        for (int e = 0; e < 8; e++) {
-                            const int j = jb + 8 * h + e;
-                            ok[e] = (unsigned)j < (unsigned)N_t;
-                            pr[e] = rcol + (j & (SP_RING - 1)) * SP_TS;
-                            rv[e] = ok[e] ? *pr[e] : 0.0;
-                        }
-#pragma unroll
-                        for (int e = 0; e < 8; e++) {
-                            const int t0 = (int)acc[0][e] * 256 + (int)acc[1][e];
-                            const int t1 = (int)acc[2][e] * 256 + (int)acc[3][e];
-                            const int t2 = (int)acc[4][e] * 256 + (int)acc[5][e];
-                            V[e] = fma((double)t0, 4294967296.0, fma((double)t1, 65536.0, (double)t2));
-                        }
-#pragma unroll
-                        for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e], fma(w0[k], e == 0 ? prev[k] : V[e - 1], rv[e]));
-#pragma unroll
-                        for (int e = 0; e < 8; e++)
-                            if (ok[e]) *pr[e] = rv[e];
-                        prev[k] = V[7];
+                        for (int s = 0; s < 6; s++) tmem_ld1(tlane + SP_DCOL + SP_NB * s + 8 * g - 1, accp[s]);
                     }
+                    tmem_wait_ld();
+                    tc_fence_before();
+                    mbar_arrive(&sm.d_empty);                           // the accumulators are free for the next item's MMAs
                     im++;
+                    // the bin before this thread's eight: the neighbour group's last (reloaded) or, for group 0, the last bin of
+                    // the previous chunk, handed over by group 3 through shared memory (two slots: chunk parity)
+                    double V[9];
+                    if (g > 0) V[0] = sp_recombine(accp[0], accp[1], accp[2], accp[3], accp[4], accp[5]);
+                    else V[0] = sm.xch[(c + 1) & 1][k][i];
+#pragma unroll
+                    for (int e = 0; e < 8; e++) V[e + 1] = sp_recombine(acc[0][e], acc[1][e], acc[2][e], acc[3][e], acc[4][e], acc[5][e]);
+                    if (g == SP_G - 1) sm.xch[c & 1][k][i] = V[8];
+                    const int j0 = SP_NB * c + 8 * g - 1 - off[k];      // time bin of the pair (V[0], V[1])
+                    double rv[8];
+                    double* pr[8];
+                    bool ok[8];
+#pragma unroll
+                    for (int e = 0; e < 8; e++) {
+                        ok[e] = !guard || (unsigned)(j0 + e) < (unsigned)N_t;
+                        pr[e] = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
+                        rv[e] = ok[e] ? *pr[e] : 0.0;
+                    }
+#pragma unroll
+                    for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e + 1], fma(w0[k], V[e], rv[e]));
+#pragma unroll
+                    for (int e = 0; e < 8; e++)
+                        if (ok[e]) *pr[e] = rv[e];
+                    qbar();                                             // the next item's rows overlap this one's (other detector, other offset)
                 }
                 lse_rows(min(N_t, SP_NB * c + SP_NB - 1 - ti.cap));
+                qbar();                                                 // rows consumed before the next chunk wraps onto them
             }
             lse_rows(N_t);
-            if (member) lnL[perm ? perm[pos] : pos] = run_m + log(run_s) - P.ln_Nt;
+            // ---- the four partial log-sum-exps of the sample
+            sm.lse[g][0][i] = run_m;
+            sm.lse[g][1][i] = run_s;
+            qbar();
+            if (g == 0 && member) {
+                double mx = sm.lse[0][0][i];
+#pragma unroll
+                for (int gg = 1; gg < SP_G; gg++) mx = fmax(mx, sm.lse[gg][0][i]);
+                double tot = 0.0;
+#pragma unroll
+                for (int gg = 0; gg < SP_G; gg++) tot += sm.lse[gg][1][i] * exp(sm.lse[gg][0][i] - mx);
+                lnL[perm ? perm[pos] : pos] = mx + log(tot) - P.ln_Nt;
+            }
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (w == 4) tmem_free512(tmem);
+    if (w == SP_MATH / 32) tmem_free512(tmem);
 }
 
 // ---------------------------------------------------------------- launch
