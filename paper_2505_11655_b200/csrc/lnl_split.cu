@@ -271,8 +271,9 @@ __device__ __forceinline__ double sp_exp_small(double d) {
 // integers (|V| < 2^63), then one conversion (rounded to 53 bits: 2^-53 of |V|, far below the digits dropped)
 __device__ __forceinline__ double sp_recombine(uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t a4, uint32_t a5) {
     const int t0 = (int)a0 * 256 + (int)a1, t1 = (int)a2 * 256 + (int)a3, t2 = (int)a4 * 256 + (int)a5;
-    const long long v = ((long long)t0 << 32) + ((long long)t1 * 65536LL + (long long)t2);
-    return (double)v;
+    const long long wl = (long long)t1 * 65536LL + (long long)t2;
+    const unsigned hi = (unsigned)(wl >> 32) + (unsigned)t0;                  // + t0 2^32: no carry into the low word
+    return (double)(long long)(((unsigned long long)hi << 32) | (unsigned)wl);
 }
 
 // cursor over the work items (tile, chunk, detector) of this CTA, in the order both warp roles walk them
@@ -571,6 +572,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     for (int e = 0; e < 4; e++)
                         if (j0 + SP_G * e < jend) *pr[e] = init;
                     bool need = false;
+                    double dl[4];
 #pragma unroll
                     for (int e = 0; e < 4; e++) {
                         double A = v[e];
@@ -585,7 +587,8 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                             A = fma(tb_f, t1 - t0, t0);
                         }
                         v[e] = j0 + SP_G * e < jend ? A : neg_inf();
-                        need = need || (v[e] - run_m >= 30.0);
+                        dl[e] = v[e] - run_m;
+                        need = need || (__double2hiint(dl[e]) >= 0x403E0000);   // dl >= 30 (or NaN): test on the high word
                     }
                     if (__any_sync(0xffffffffu, need)) {
                         // raise the reference to the largest new value (rare); the running sum is rescaled exactly
@@ -595,14 +598,15 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                             run_s = dm > -690.0 ? run_s * sp_exp_small(dm) : 0.0;
                             run_m = mx;
                         }
+#pragma unroll
+                        for (int e = 0; e < 4; e++) dl[e] = v[e] - run_m;
                     }
                     double part[2] = {0.0, 0.0};
 #pragma unroll
                     for (int e = 0; e < 4; e++) {
                         // terms below e^-40 of the reference (and rows past the end) are clamped to e^-40 (R2)
-                        const double dl = v[e] - run_m;
-                        const unsigned hc = min((unsigned)__double2hiint(dl), 0xC0440000u);
-                        part[e & 1] += sp_exp_tab(__hiloint2double((int)hc, __double2loint(dl)), etab);
+                        const unsigned hc = min((unsigned)__double2hiint(dl[e]), 0xC0440000u);
+                        part[e & 1] += sp_exp_tab(__hiloint2double((int)hc, __double2loint(dl[e])), etab);
                     }
                     run_s += part[0] + part[1];
                 }
@@ -637,20 +641,34 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                     for (int e = 0; e < 8; e++) V[e + 1] = sp_recombine(acc[0][e], acc[1][e], acc[2][e], acc[3][e], acc[4][e], acc[5][e]);
                     if (g == SP_G - 1) sm.xch[c & 1][k][i] = V[8];
                     const int j0 = SP_NB * c + 8 * g - 1 - off[k];      // time bin of the pair (V[0], V[1])
-                    double rv[8];
-                    double* pr[8];
-                    bool ok[8];
+                    if (guard) {
+                        double rv[8];
+                        double* pr[8];
+                        bool ok[8];
 #pragma unroll
-                    for (int e = 0; e < 8; e++) {
-                        ok[e] = !guard || (unsigned)(j0 + e) < (unsigned)N_t;
-                        pr[e] = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
-                        rv[e] = ok[e] ? *pr[e] : 0.0;
+                        for (int e = 0; e < 8; e++) {
+                            ok[e] = (unsigned)(j0 + e) < (unsigned)N_t;
+                            pr[e] = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
+                            rv[e] = ok[e] ? *pr[e] : 0.0;
+                        }
+#pragma unroll
+                        for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e + 1], fma(w0[k], V[e], rv[e]));
+#pragma unroll
+                        for (int e = 0; e < 8; e++)
+                            if (ok[e]) *pr[e] = rv[e];
+                    } else {
+                        double rv[8];
+                        double* pr[8];
+#pragma unroll
+                        for (int e = 0; e < 8; e++) {
+                            pr[e] = rcol + ((j0 + e) & (SP_RING - 1)) * SP_TS;
+                            rv[e] = *pr[e];
+                        }
+#pragma unroll
+                        for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e + 1], fma(w0[k], V[e], rv[e]));
+#pragma unroll
+                        for (int e = 0; e < 8; e++) *pr[e] = rv[e];
                     }
-#pragma unroll
-                    for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e + 1], fma(w0[k], V[e], rv[e]));
-#pragma unroll
-                    for (int e = 0; e < 8; e++)
-                        if (ok[e]) *pr[e] = rv[e];
                     qbar();                                             // the next item's rows overlap this one's (other detector, other offset)
                 }
                 lse_rows(min(N_t, SP_NB * c + SP_NB - 1 - ti.cap));
