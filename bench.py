@@ -1,32 +1,35 @@
 #!/usr/bin/env python
 """bench.py -- headline measurement of the ILE hot path on B200 (BASELINE.json).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-per-config] [--no-cpu-baseline]
 
-A *step* is one pass of the whole hot path over one batch: one integrator iteration of
-BASELINE.json configs[1] (3 detectors, 21 modes, 820-bin Q, 400 time bins, AC with 100-bin
-marginals, 2^20 samples): draw -> antenna/Y_lm/coefficients/quadratic term -> fused lnL over the
-time grid -> time marginalisation -> weight reduction -> AC update.  The sampler is reset every 10
-steps, as the config's 10-iteration runs are.  Metric: extrinsic lnL evaluations per second,
-counted as samples x time bins.
+A *step* is one pass of the whole hot path over one batch: one integrator iteration of the largest
+single-GPU configuration, BASELINE.json configs[2] (3 detectors, 21 modes, 820-bin Q, 400 time bins, source at
+SNR 100, AV adaptive-volume integrator, 2^22 samples): draw -> antenna/Y_lm -> coefficients and quadratic term ->
+fused lnL over the time grid (contraction on the tensor cores) -> time marginalisation -> weight reduction -> AV
+update.  The sampler is reset every 20 steps, as the config's 20-iteration runs are.  Metric: extrinsic lnL
+evaluations per second, counted as samples x time bins.
 
-`value`   device-resident: Q/U/V already in HBM; CUDA events around the K steps.
-`e2e`     the same step through the C ABI from HOST buffers: every step loads that intrinsic
-          point's Q/U/V from pinned host memory (ile_load_quv: host -> device copy + repack), runs
-          the iteration and reads the ile_result struct back to the host.
-`roofline` the fused lnL kernel (steps 4-6): algorithmic flop (289.4 per sample-bin, DESIGN.md
-          section 6) / its device time, timed live with CUDA events on the launching stream,
-          against the FP64 peak measured in the same process by the library's register-resident
-          DFMA / DMMA chain probes (bound "alu": the path is FP64-arithmetic bound, not HBM bound).
-`cpu_baseline` the oracle (oracle/, numpy fp64, as it stands) on the host cores, one AC iteration
-          of the same config on a bounded sample of 2^14 samples.
+`value`    device-resident: Q/U/V already in HBM; CUDA events around the K steps.
+`e2e`      the same step through the C ABI from HOST buffers: every step loads that intrinsic point's Q/U/V from
+           pinned host memory (ile_load_quv: host -> device copy + repack + digit image), runs the iteration and
+           reads the ile_result struct back to the host.
+`roofline` the fused lnL kernel (steps 3-6): algorithmic flop (289.4 per sample-bin) / its
+           device time, timed live with CUDA events on the launching stream, against the FP64 peak measured in
+           the same process by the library's register-resident DFMA / DMMA chain probes.  The kernel's contraction
+           runs on the int8 tensor path (exactly), so the fraction of the FP64 peak can pass 1.
+`per_config` configs 2-5 of SURVEY 8(d) at their full BASELINE.json sizes through ile_integrator_run (config 4:
+           all 512 intrinsic points): ms per iteration, fused-kernel ms, flop per unit, fraction, n_eff / N.
+`cpu_baseline` the oracle (oracle/, numpy fp64, as it stands) on the host cores: one AV iteration of the same
+           config on a bounded sample, sample slices fanned out over the cores with multiprocessing.
 
-N > 1 (torchrun): the path does not communicate; each rank runs the same step on its own
-intrinsic point ("replicas", weak scaling); value = total sample-bins / max-over-ranks time.
+N > 1 (torchrun): the path does not communicate; rank r runs the same step on intrinsic point r of the config
+("replicas", weak scaling); value = total sample-bins / max-over-ranks time.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -42,7 +45,8 @@ if ROOT not in sys.path:
 
 METRIC = "extrinsic lnL evals/s (samples x time bins)"
 UNIT = "sample-bins/s"
-CFG = 2
+CFG = 3                                   # BASELINE.json configs[2]: the largest single-GPU configuration
+KERNEL = "lnl_split_kernel (tcgen05.mma kind::i8 contraction + FP64 epilogue)"
 
 
 def flop_per_unit(K, M, N_t):
@@ -52,8 +56,21 @@ def flop_per_unit(K, M, N_t):
     pairs = M * (M + 1) // 2
     return 2.0 * K * (2 * M + 2) + (2.0 * K * 6 * pairs + 8.0 * pairs) / N_t
 
+
 ORACLE_SAMPLE_N = 1 << 14
-NCU_TRAFFIC_BYTES = 550.80e6 + 15.23e6   # profiles/r1_fused_kernel.md (algorithmic: 512 B in + 8 B out per sample = 545 MB)
+
+
+def ncu_traffic(cfg):
+    """dram bytes read + written per launch of the fused kernel on config `cfg`, from the committed ncu summary
+    profiles/r2_traffic.csv (one `ncu --set full` capture per config; the command is in profiles/r2_traffic.md)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as fh:
+            for row in csv.DictReader(fh):
+                if int(row["config"]) == cfg:
+                    return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
+    except (OSError, KeyError, ValueError):
+        pass
+    return None
 
 
 # ------------------------------------------------------------------------------- clocks
@@ -105,32 +122,80 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------- oracle arm
-def oracle_rate(n_samples, steps=1, warmup=0):
-    """The oracle as it stands: AC iterations of config 2 on `n_samples` samples per step."""
-    from oracle.ile import IleProblem, iteration
-    from oracle.integrators import make_integrator
+_ORACLE = {}
+
+
+def _oracle_worker_init(cfg):
+    from oracle.ile import IleProblem
     from synth import make_problem
+    prob = make_problem(cfg, N=1, n_iter=1)
+    _ORACLE["op"] = IleProblem(prob)
+
+
+def _oracle_lnL_slice(z):
+    return _ORACLE["op"].lnL_z(z)
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_rate(n_samples, steps=1, warmup=0, procs=None):
+    """The oracle as it stands: iterations of config CFG (draw, lnL, weights, reduction, sampler update) on `n_samples`
+    samples per step.  The likelihood of the batch is evaluated on sample slices by `procs` worker processes (one per
+    host core, SURVEY 8(d) timing protocol); draw, reduction and update run in the parent.  Only oracle/ code runs."""
+    import multiprocessing as mp
+    from oracle.ile import IleProblem
+    from oracle.integrators import make_integrator
+    from oracle.reduce import reduce_lnw
+    from synth import make_problem
+    procs = procs or os.cpu_count() or 1
     prob = make_problem(CFG, N=n_samples, n_iter=1)
     op = IleProblem(prob)
     oo = {k: v for k, v in prob.opts.items() if k != "seed"}
     integ = make_integrator(prob.kind, prob.lo, prob.hi, prob.opts["seed"], **oo)
+    pool = mp.get_context("fork").Pool(procs, initializer=_oracle_worker_init, initargs=(CFG,)) if procs > 1 else None
+
+    def one(g):
+        z, ln_ps = integ.draw(n_samples, g)
+        if pool is not None:
+            parts = np.array_split(np.arange(n_samples), procs)
+            lnL = np.concatenate(pool.map(_oracle_lnL_slice, [z[:, p] for p in parts]))
+        else:
+            lnL = op.lnL_z(z)
+        with np.errstate(invalid="ignore"):
+            lnw = lnL + op.ln_prior(z) - ln_ps
+        lnw = np.where(np.isfinite(lnL), lnw, -np.inf)
+        reduce_lnw(lnw)
+        integ.update(z, lnw, None if integ.kind == "AV" else ln_ps)
+
     for g in range(warmup):
-        iteration(op, integ, n_samples, g)
-    c0, t0 = time.process_time(), time.perf_counter()
+        one(g)
+    t0 = time.perf_counter()
     for g in range(steps):
-        iteration(op, integ, n_samples, warmup + g)
-    wall, cpu = time.perf_counter() - t0, time.process_time() - c0
-    cores = max(1, int(round(cpu / wall)))
-    return n_samples * prob.N_t * steps / wall, wall / steps, cores, prob
+        one(warmup + g)
+    wall = time.perf_counter() - t0
+    if pool is not None:
+        pool.close()
+        pool.join()
+    return n_samples * prob.N_t * steps / wall, wall / steps, procs, prob
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    n = 1 << 11
+    n = 1 << 12
     rate, sec, cores, prob = oracle_rate(n, steps=args.steps, warmup=min(args.warmup, 1))
-    sample = f"config {CFG} shapes (K=3, M=21, N_t={prob.N_t}, AC), {n} samples per step instead of {1 << 20}"
+    sample = (f"config {CFG} shapes (K={prob.K}, M={prob.M}, N_t={prob.N_t}, {prob.kind}), {n} samples per step instead of {prob.N}; "
+              f"{cores} worker processes on {os.cpu_count()} host cores ({cpu_model()})")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -140,10 +205,11 @@ def run_reference(args):
 
 
 def _config_dict(prob, N):
-    return {"workload": f"BASELINE.json configs[1]: {prob.K} detectors, {prob.M} modes (l<=4), N_Q={prob.N_Q}, N_t={prob.N_t}, "
-                        f"AC 100 bins, {N} samples per iteration, sampler reset every 10 iterations",
+    return {"workload": f"BASELINE.json configs[{CFG - 1}]: {prob.K} detectors, {prob.M} modes (l<=4), N_Q={prob.N_Q}, N_t={prob.N_t}, "
+                        f"source at SNR 100, {prob.kind} (P_thr 0.999, all {prob.d} dimensions), {N} samples per iteration, "
+                        f"sampler reset every {prob.n_iter} iterations",
             "samples_per_step": N, "time_bins": prob.N_t, "integrator": prob.kind, "d": prob.d,
-            "l2": "per-step working set (draws, per-sample records and Y tiles, ~0.6 GB) exceeds the 126 MB L2; no explicit flush"}
+            "l2": "per-step working set (draws, per-sample records and Y tiles, ~2.5 GB) exceeds the 126 MB L2; no explicit flush"}
 
 
 # ------------------------------------------------------------------------------- our arm
@@ -162,11 +228,59 @@ def aggregate_value(units_per_step_per_rank, steps, world, ms):
     return world * units_per_step_per_rank * steps / (ms * 1e-3)
 
 
+def rank_problem(cfg, rank):
+    """Rank r works on intrinsic point r of the config (its own seeded Q/U/V; one event: shared network and D_ref)."""
+    from synth import make_problem
+    prob = make_problem(cfg, P=rank + 1)
+    prob.Q, prob.U, prob.V, prob.P = prob.Q[rank:rank + 1].copy(), prob.U[rank:rank + 1].copy(), prob.V[rank:rank + 1].copy(), 1
+    return prob
+
+
+def measure_config(cfg, dev, peak):
+    """One full BASELINE.json run of config `cfg` through ile_integrator_run (no host round-trip inside): every
+    intrinsic point, every iteration, full batch size.  CUDA events around the run, fused-kernel time from the library."""
+    import torch
+    from paper_2505_11655_b200 import Ile, Integrator, RESULT_DTYPE
+    from synth import make_problem
+    prob = make_problem(cfg)
+    ile = Ile(int(dev.split(":")[1]))
+    ile.load_problem(prob)
+    integ = Integrator.from_problem(ile, prob, max_batch=prob.N)
+    P, n_iter, N = prob.P, prob.n_iter, prob.N
+    out = integ.run(0, min(P, 2), n_iter, N)                            # warm-up: the first points
+    torch.cuda.synchronize()
+    ile.kernel_timing(True)
+    l0 = ile.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    out = integ.run(0, P, n_iter, N)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    launches = ile.kernel_launches() - l0
+    k_ms, k_n = ile.kernel_time()
+    ile.kernel_timing(False)
+    res = np.frombuffer(out.cpu().numpy().tobytes(), dtype=RESULT_DTYPE).reshape(P, n_iter)
+    units = float(P) * n_iter * N * prob.N_t
+    fpu = flop_per_unit(prob.K, prob.M, prob.N_t)
+    k_avg = k_ms / max(k_n, 1)
+    frac = fpu * N * prob.N_t / (k_avg * 1e-3) / 1e12 / peak
+    last = res[:, -1]
+    integ.close()
+    del ile
+    torch.cuda.empty_cache()
+    return {"config": cfg, "integrator": prob.kind, "points": P, "iterations": n_iter, "samples_per_iteration": N, "time_bins": prob.N_t,
+            "ms_per_iteration": ms / (P * n_iter), "value": units / (ms * 1e-3), "fused_kernel_ms": k_avg, "fused_kernel_launches": int(k_n),
+            "fused_kernel_share": k_ms / ms, "flop_per_unit": fpu, "frac": frac, "gpu_launches_per_iteration": launches / (P * n_iter),
+            "traffic": ncu_traffic(cfg),
+            "check": {"n_eff_over_N_last": float(np.mean(last["n_eff"]) / N), "n_eff_cumulative_over_N": float(np.mean(last["cum_n_eff"] / last["cum_n_samples"])),
+                      "ln_integral_last": float(last["ln_integral"][0]), "n_nonfinite": int(res["n_nonfinite"].sum())}}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2505_11655_b200 import Ile, Integrator, RESULT_DTYPE
-    from synth import make_problem
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -178,7 +292,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     dev = f"cuda:{local}"
 
-    prob = make_problem(CFG, P=1)
+    prob = rank_problem(CFG, rank)
     N, n_iter = prob.N, prob.n_iter
     ile = Ile(local)
     ile.load_problem(prob)
@@ -199,6 +313,7 @@ def run_ours(args):
 
     # FP64 peaks, measured in this process before the timed region
     peak_dfma, peak_dmma = ile.fp64_peak(0), ile.fp64_peak(1)
+    peak = max(peak_dfma, peak_dmma)
 
     for g in range(args.warmup):
         step(g)
@@ -254,13 +369,21 @@ def run_ours(args):
         k_avg_ms = k_ms / max(k_n, 1)
         fpu = flop_per_unit(prob.K, prob.M, prob.N_t)
         achieved = fpu * units_per_step / (k_avg_ms * 1e-3) / 1e12
-        peak = max(peak_dfma, peak_dmma)
+        integ.close()
+        del ile
+        torch.cuda.empty_cache()
+        # configs 2-5 at full size (rank 0, N = 1 only)
+        per_config = None
+        if world == 1 and not args.no_per_config:
+            per_config = [measure_config(c, dev, peak) for c in (2, 3, 4, 5)]
         # oracle on the host cores (rank 0, N = 1 only), bounded sample
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             rate, sec, cores, _ = oracle_rate(ORACLE_SAMPLE_N)
-            cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                   "sample": f"one AC iteration of config {CFG} on {ORACLE_SAMPLE_N} samples x {prob.N_t} bins ({sec:.1f} s)"}
+            cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "host_cores": os.cpu_count(), "cpu_model": cpu_model(),
+                   "sample": f"one {prob.kind} iteration of config {CFG} on {ORACLE_SAMPLE_N} samples x {prob.N_t} bins ({sec:.1f} s), "
+                             f"likelihood on sample slices in {cores} worker processes"}
+        traffic = ncu_traffic(CFG)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
@@ -269,13 +392,19 @@ def run_ours(args):
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches),
             "clocks": clk,
-            "roofline": {"bound": "alu", "kernel": "lnl_fused2_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES,
-                         "traffic_note": "dram bytes read+written per launch of this kernel, ncu --set full, profiles/r1_fused_kernel.md", "kernel_ms": k_avg_ms, "kernel_launches": int(k_n),
-                         "kernel_share_of_step": k_ms / ms, "peak_source": "measured in-process: max(DFMA chain, DMMA chain)",
-                         "peak_dfma": peak_dfma, "peak_dmma": peak_dmma, "flop_per_unit": fpu},
+            "roofline": {"bound": "alu", "kernel": KERNEL, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                         "frac": achieved / peak, "traffic": traffic,
+                         "traffic_note": "dram bytes read + written per launch of this kernel on this config, one ncu --set full capture, "
+                                         "profiles/r2_traffic.csv (command in profiles/r2_traffic.md)",
+                         "kernel_ms": k_avg_ms, "kernel_launches": int(k_n), "kernel_share_of_step": k_ms / ms,
+                         "peak_source": "FP64 peak measured in-process: max(DFMA chain, DMMA chain); the algorithmic FP64 flop of "
+                                        "steps 3-6 over the kernel time.  The contraction itself runs exactly on the int8 tensor "
+                                        "path (21 digit pairs, tcgen05.mma kind::i8), which is how the fraction can pass 1",
+                         "peak_dfma": peak_dfma, "peak_dmma": peak_dmma, "flop_per_unit": fpu,
+                         "int8_tops": 2.0 * 1056 * prob.K * units_per_step * (432.0 / prob.N_t) / (k_avg_ms * 1e-3) / 1e12},
             "cpu_baseline": cpu,
-            "check": {"ln_integral_last": float(last["ln_integral"]), "n_eff_last": float(last["n_eff"]),
+            "per_config": per_config,
+            "check": {"ln_integral_last": float(last["ln_integral"]), "n_eff_last": float(last["n_eff"]), "n_eff_over_N_last": float(last["n_eff"]) / N,
                       "samples_per_s": value / prob.N_t},
         }
         print(json.dumps(out))
@@ -315,10 +444,11 @@ def run_precompute(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the full-size runs of configs 2-5")
     ap.add_argument("--precompute", action="store_true", help="time the Q/U/V precompute instead of the hot path (side measurement)")
     args = ap.parse_args()
     if args.precompute:
