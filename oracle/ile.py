@@ -45,7 +45,8 @@ def iteration(ile, integ, N, g, update=True):
     with np.errstate(invalid="ignore"):
         lnw = lnL + ile.ln_prior(z) - ln_ps
     lnw = np.where(np.isfinite(lnL), lnw, -np.inf)
-    res = reduce_lnw(lnw)
+    # a portfolio's silent members draw after the contributing ones and stay out of the estimate
+    res = reduce_lnw(lnw[:getattr(integ, "n_contrib_samples", N)])
     if update:
         # a standalone AV samples uniformly inside its cells, so it follows PAPER.md:265 exactly
         # (V_{g+1} = V_g N_min / N_live); ln p_s matters only to a portfolio member

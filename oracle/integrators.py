@@ -416,35 +416,78 @@ class Portfolio:
     """Mixture of member samplers (p_s = sum_a W_a p_s,a / sum_a W_a), weights
     adapted from the per-member n_ESS of the last batch, floor 0.05/N_s, members below 5 %
     frozen, every other member trained on all samples with the overall weights.
-    Reading G25."""
+    Reading G25.
+
+    Options of PAPER.md:297 (readings G41, G42): `first_iter[a]` = "the first iteration for which a given
+    sampler is activated within the portfolio" (member 0 is always active): before it the member gets no
+    samples, has no term in p_s, is not trained, and N_s counts the activated members only, so the portfolio
+    behaves exactly as if the member were not there; when the activated set changes the weights restart
+    uniform and no member is frozen on that batch.  `silent[a]`: the member "contribute[s] silently, only contributing training data for other
+    samplers without directly influencing the integral": it draws N // N_active samples per batch (fixed
+    share, its weight is not adapted), it has no term in p_s, its samples are left out of the estimate
+    (they sit after the contributing members' samples: silent members are listed last) and every
+    trained member, itself included, sees all samples with the weights L p / p_s."""
     kind = "PORTFOLIO"
 
-    def __init__(self, members):
+    def __init__(self, members, first_iter=None, silent=None):
         self.members = list(members)
         self.Ns = len(self.members)
-        self.W = np.full(self.Ns, 1.0 / self.Ns)
+        self.first_iter = np.zeros(self.Ns, dtype=np.int64) if first_iter is None else np.asarray(first_iter, dtype=np.int64)
+        self.silent = np.zeros(self.Ns, dtype=bool) if silent is None else np.asarray(silent, dtype=bool)
+        if self.first_iter[0] != 0 or self.silent[0]:
+            raise ValueError("member 0 is active from iteration 0 and contributes")
+        if np.any(self.silent[:-1] & ~self.silent[1:]):
+            raise ValueError("silent members are listed after the contributing ones")
         self.lo, self.hi, self.d = members[0].lo, members[0].hi, members[0].d
         self.alloc = None
         self.frozen = np.zeros(self.Ns, dtype=bool)
+        self.active = np.zeros(self.Ns, dtype=bool)           # activated set of the last draw
+        self.W = np.zeros(self.Ns)
+        self._activate(0)
+        self.restarted = False
+
+    def _activate(self, g):
+        """Activated set at iteration g; when it differs from the last draw's the weights restart uniform over the
+        contributing activated members."""
+        act = self.first_iter <= g
+        if not np.array_equal(act, self.active):
+            self.active = act
+            con = act & ~self.silent
+            self.W = np.where(con, 1.0 / float(con.sum()), 0.0)
+            self.frozen = np.zeros(self.Ns, dtype=bool)
+            self.restarted = True
+
+    @property
+    def contributing(self):
+        return self.active & ~self.silent
 
     def allocation(self, N):
-        Na = np.floor(float(N) * self.W).astype(np.int64)
-        rem = N - int(Na.sum())
+        con, sil = self.contributing, self.active & self.silent
+        n_act = int(self.active.sum())
+        each = N // n_act if sil.any() else 0
+        Nc = N - int(sil.sum()) * each
+        Na = np.where(con, np.floor(float(Nc) * self.W), 0.0).astype(np.int64)
+        rem = Nc - int(Na.sum())
+        idx = np.nonzero(con)[0]
         a = 0
         while rem > 0:
-            Na[a % self.Ns] += 1
+            Na[idx[a % len(idx)]] += 1
             rem -= 1
             a += 1
+        Na[sil] = each
+        self.n_contrib_samples = Nc
         return Na
 
     def ln_pdf(self, z):
-        e = np.stack([math.log(self.W[a]) + self.members[a].ln_pdf(z) for a in range(self.Ns)])
+        terms = [math.log(self.W[a]) + self.members[a].ln_pdf(z) for a in range(self.Ns) if self.contributing[a]]
+        e = np.stack(terms)
         mx = e.max(axis=0)
         mxs = np.where(np.isfinite(mx), mx, 0.0)
         with np.errstate(divide="ignore"):
             return np.where(np.isfinite(mx), mxs + np.log(np.exp(e - mxs).sum(axis=0)), -np.inf)
 
     def draw(self, N, g, i0=0):
+        self._activate(g)
         Na = self.allocation(N)
         self.alloc = Na
         z = np.empty((self.d, N))
@@ -458,11 +501,15 @@ class Portfolio:
 
     def update(self, z, lnw, ln_ps):
         lnw = np.asarray(lnw, dtype=np.float64)
+        con = self.contributing
+        n_con = int(con.sum())
         ness = np.zeros(self.Ns)
         off = 0
         for a in range(self.Ns):
             seg = lnw[off:off + int(self.alloc[a])]
             off += int(self.alloc[a])
+            if not con[a]:
+                continue
             fin = np.isfinite(seg)
             if fin.any():
                 mm = seg[fin].max()
@@ -470,13 +517,16 @@ class Portfolio:
                 ness[a] = e.sum() ** 2 / (e * e).sum()
         if ness.sum() > 0.0:
             raw = ness / ness.sum()
-            self.frozen = raw < 0.05
-            W = np.maximum(raw, 0.05 / self.Ns)
+            # the batch after a restart was drawn with uniform weights (none below 5 %): nobody is frozen on it, so a
+            # member that has just been activated is trained at least once
+            self.frozen = con & (raw < 0.05) & (not self.restarted)
+            W = np.where(con, np.maximum(raw, 0.05 / n_con), 0.0)
             self.W = W / W.sum()
+        self.restarted = False
         # a one-member portfolio *is* that member (pin P11): it trains as the member would alone
         ln_ps_arg = ln_ps if self.Ns > 1 else None
         for a in range(self.Ns):
-            if not self.frozen[a]:
+            if self.active[a] and not self.frozen[a]:
                 self.members[a].update(z, lnw, ln_ps_arg)
 
 
@@ -491,6 +541,8 @@ def make_integrator(kind, lo, hi, seed, **o):
     if kind == "GMM":
         return GMM(lo, hi, seed, o.get("n_gmm", 8))
     if kind == "PORTFOLIO":
-        mem = [make_integrator(k, lo, hi, seed, **o) for k in o.get("members", ["AC", "AV", "GMM"])]
-        return Portfolio(mem)
+        names = o.get("members", ["AC", "AV", "GMM"])
+        per = o.get("member_opts") or [{}] * len(names)           # options unique to each sampler realization
+        mem = [make_integrator(k, lo, hi, seed, **{**o, **per[a]}) for a, k in enumerate(names)]
+        return Portfolio(mem, o.get("first_iter"), o.get("silent"))
     raise ValueError(kind)

@@ -313,3 +313,103 @@ def test_portfolio_single_member_is_member_and_allocation():
     gm_in = np.exp(pf.members[2].ln_pdf(np.stack([X.ravel(), Y.ravel()]))).sum() * 1e-4
     want = pf.W[0] + pf.W[1] + pf.W[2] * gm_in
     assert abs(pdf.sum() * 1e-4 - want) < 2e-3
+
+
+# ------------------------------------------------------------------------------- portfolio options of PAPER.md:297
+def _state(m):
+    if m.kind == "AC":
+        return (m.H.copy(), m.pi.copy())
+    if m.kind == "AV":
+        return (m.n, m.keys.copy())
+    return (m.omega.copy(), m.mu.copy(), m.Sigma.copy())
+
+
+def test_portfolio_activation_iteration_is_invisible_before_it():
+    """A member with first_iter = g0 gets no samples, no density term and no training before g0, and N_s counts the
+    activated members only: for g < g0 the portfolio is bit-identical to the portfolio without that member.  At g0
+    the weights restart uniform and the newcomer draws its share."""
+    lo, hi = np.array([-5.0, -5.0]), np.array([5.0, 5.0])
+    lnf = lambda z: ln_gauss(z, [1.0, -1.0], [0.4, 0.6])
+    mk = lambda kind, **o: og.make_integrator(kind, lo, hi, 11, **o)
+    g0 = 3
+    with_late = og.Portfolio([mk("AC", n_bins=10), mk("AV", N_min_star=64), mk("AC", n_bins=30)], first_iter=[0, 0, g0])
+    without = og.Portfolio([mk("AC", n_bins=10), mk("AV", N_min_star=64)])
+    N = 4000
+    for g in range(g0):
+        za, la = with_late.draw(N, g)
+        zb, lb = without.draw(N, g)
+        assert np.array_equal(za, zb) and np.array_equal(la, lb)
+        assert with_late.alloc[2] == 0 and with_late.W[2] == 0.0
+        lnw = lnf(za) - la
+        with_late.update(za, lnw, la)
+        without.update(zb, lnw, lb)
+        assert np.array_equal(with_late.W[:2], without.W)
+        for a in range(2):
+            for x, y in zip(_state(with_late.members[a]), _state(without.members[a])):
+                assert np.array_equal(x, y)
+        assert np.all(with_late.members[2].pi == 1.0 / 30)              # untouched
+    z, l = with_late.draw(N, g0)
+    assert np.array_equal(with_late.W, np.full(3, 1.0 / 3)) and with_late.alloc.tolist() == [1334, 1333, 1333]
+    with_late.update(z, lnf(z) - l, l)
+    assert not np.all(with_late.members[2].pi == 1.0 / 30)              # now trained
+    with pytest.raises(ValueError):
+        og.Portfolio([mk("AC"), mk("AC")], first_iter=[1, 0])
+
+
+def test_portfolio_silent_member_trains_but_stays_out_of_the_integral():
+    """Silent member (listed last): fixed share N // N_active of every batch, no term in p_s, its samples are left
+    out of the estimate but train every member (itself included) with the weights L p / p_s."""
+    from oracle.ile import iteration
+    lo, hi = np.array([-5.0, -5.0]), np.array([5.0, 5.0])
+    mu, sig = [1.0, -1.0], [0.4, 0.6]
+    pf = og.Portfolio([og.AC(lo, hi, 5, n_bins=20), og.Uniform(lo, hi, 5)], silent=[False, True])
+    N = 6000
+    z, ln_ps = pf.draw(N, 0)
+    assert pf.alloc.tolist() == [3000, 3000] and pf.n_contrib_samples == 3000
+    assert np.array_equal(ln_ps, pf.members[0].ln_pdf(z))                # the mixture is the contributing member alone (W = 1)
+    lnw = ln_gauss(z, mu, sig) - ln_ps
+    ref = og.AC(lo, hi, 5, n_bins=20)
+    pf.update(z, lnw, ln_ps)
+    assert np.array_equal(pf.members[0].H, ref.histogram(z, lnw))        # trained on all N samples, the silent ones included
+    assert pf.members[0].H.sum() > ref.histogram(z[:, :3000], lnw[:3000]).sum()
+    assert pf.W.tolist() == [1.0, 0.0]
+
+    class Prob:                                                          # the estimate through oracle.ile.iteration: contributing samples only
+        lo_, hi_ = lo, hi
+        def lnL_z(self, zz):
+            return np.where(og.in_box(zz, lo, hi), ln_gauss(zz, mu, sig), -np.inf)
+        def ln_prior(self, zz):
+            return np.zeros(zz.shape[1])
+    res = []
+    for g in range(1, 7):
+        out = iteration(Prob(), pf, N, g)
+        assert out["result"]["n_samples"] == 3000 and len(out["lnw"]) == N
+        res.append(out["result"])
+    exact = gauss_box_integral(mu, sig, lo, hi)
+    tot = combine(res[2:])
+    assert abs(math.exp(tot["ln_integral"]) / exact - 1) < 5 * math.sqrt(tot["rel_variance"]) + 2e-3
+    with pytest.raises(ValueError):
+        og.Portfolio([og.AC(lo, hi, 5), og.Uniform(lo, hi, 5), og.AC(lo, hi, 5)], silent=[False, True, False])
+
+
+def test_portfolio_fig7_two_ac_members_second_from_iteration_10():
+    """PAPER.md:299 (Fig. 7): a portfolio of two AC integrators with 10 and 30 bins, the high-resolution one joining
+    after 10 iterations, on three superposed Gaussians in four dimensions (seeded parameters: the paper's are random
+    and unprinted).  The estimate converges to the closed-form integral."""
+    d = 4
+    lo, hi = np.full(d, -6.0), np.full(d, 6.0)
+    rng = np.random.Generator(np.random.Philox(7))
+    mus, sigs, amps = rng.uniform(-3, 3, (3, d)), rng.uniform(0.5, 1.0, (3, d)), np.array([1.0, 0.6, 0.3])
+
+    def lnf(z):
+        e = np.stack([math.log(amps[c]) + ln_gauss(z, mus[c], sigs[c]) for c in range(3)])
+        mx = e.max(axis=0)
+        return mx + np.log(np.exp(e - mx).sum(axis=0))
+    exact = sum(amps[c] * gauss_box_integral(mus[c], sigs[c], lo, hi) for c in range(3))
+    pf = og.make_integrator("PORTFOLIO", lo, hi, 42, members=["AC", "AC"], member_opts=[dict(n_bins=10), dict(n_bins=30)], first_iter=[0, 10])
+    res = run(pf, lnf, 1 << 14, 20)
+    assert pf.members[0].n_bins == 10 and pf.members[1].n_bins == 30
+    assert pf.W[1] > 0.0 and abs(pf.W.sum() - 1) < 1e-14
+    tot = combine(res[12:])
+    assert abs(math.exp(tot["ln_integral"]) / exact - 1) < 5 * math.sqrt(tot["rel_variance"]) + 2e-3
+    assert tot["n_ess"] > 0.05 * 8 * (1 << 14)
