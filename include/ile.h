@@ -93,6 +93,22 @@ typedef struct {
     /* PORTFOLIO */
     int32_t n_members;
     int32_t member_kind[ILE_MAX_MEMBERS]; /* AC / AV / GMM / UNIFORM */
+    /* "a list of N_s - 1 integers specifying the first iteration for which a given sampler is
+     * activated within the portfolio" (entry 0 must be 0): before it the member gets no samples, has no term in p_s
+     * and is not trained; N_s counts the activated members; the weights restart uniform when the set changes. */
+    int32_t member_first_iter[ILE_MAX_MEMBERS];
+    /* members that "contribute silently, only contributing training data for other samplers without
+     * directly influencing the integral": a silent member draws N / N_active samples of every batch, has no term in
+     * p_s and its samples (stored after the contributing members': silent members must be listed last) are left out
+     * of the estimate (ile_result.n_samples counts the contributing ones); every trained member sees all N. */
+    int32_t member_silent[ILE_MAX_MEMBERS];
+    /* PAPER.md:297 "a list of options unique to each sampler realization": bins per dimension of an AC member,
+     * 0 = n_bins (the paper's Fig. 7 portfolio: two AC members with 10 and 30 bins). */
+    int32_t member_n_bins[ILE_MAX_MEMBERS];
+    /* PAPER.md:107 "Gaussian mixture models ... for any user-specified subset of dimensions": bit c set = dimension c
+     * is modelled by the mixture, the others are sampled uniformly; 0 = all d dimensions. */
+    uint32_t gmm_dims_mask;
+    int32_t pad1;
 } ile_integrator_opts;
 
 /* ------------------------------------------------------------------ lifecycle */
@@ -209,7 +225,7 @@ int ile_integrator_last_batch(ile_integrator *it, const double **z, const double
  *   AC      int64 n_bins; uint64 H[d][n_bins]; double pi[d][n_bins]; double cdf[d][n_bins+1]
  *   AV      int64 n, C, N_min; double L_thr; uint64 keys[C]
  *   GMM     int64 n_comp; double omega[C], mu[C][d], Sigma[C][d][d], L[C][d][d]
- *   PORTF.  int64 n_members; double W[8]; int64 frozen[8]; int64 alloc[8];
+ *   PORTF.  int64 n_members; double W[8]; int64 frozen[8]; int64 alloc[8]; int64 active[8];
  *           then per member: int64 bytes_m, followed by that member's blob (with header)
  *   UNIFORM nothing more */
 int ile_integrator_get_state(ile_integrator *it, void *buf, size_t *bytes);

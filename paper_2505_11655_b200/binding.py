@@ -68,7 +68,9 @@ class IntegratorOpts(C.Structure):
     _fields_ = [("kind", C.c_int32), ("d", C.c_int32), ("lo", C.c_double * ILE_MAX_D), ("hi", C.c_double * ILE_MAX_D),
                 ("seed", C.c_uint64), ("max_batch", C.c_int64), ("n_bins", C.c_int32), ("pad0", C.c_int32), ("eps", C.c_double),
                 ("beta", C.c_double), ("P_thr", C.c_double), ("N_min_star", C.c_int64), ("n_gmm", C.c_int32),
-                ("n_members", C.c_int32), ("member_kind", C.c_int32 * ILE_MAX_MEMBERS)]
+                ("n_members", C.c_int32), ("member_kind", C.c_int32 * ILE_MAX_MEMBERS),
+                ("member_first_iter", C.c_int32 * ILE_MAX_MEMBERS), ("member_silent", C.c_int32 * ILE_MAX_MEMBERS),
+                ("member_n_bins", C.c_int32 * ILE_MAX_MEMBERS), ("gmm_dims_mask", C.c_uint32), ("pad1", C.c_int32)]
 
 
 _lib = None
@@ -307,7 +309,7 @@ def parse_state(blob: bytes):
     pos = 16
     Ns = int(i64()[0])
     out = dict(kind=kind, d=d, n_members=Ns, W=arr("<f8", ILE_MAX_MEMBERS), frozen=arr("<i8", ILE_MAX_MEMBERS),
-               alloc=arr("<i8", ILE_MAX_MEMBERS), members=[])
+               alloc=arr("<i8", ILE_MAX_MEMBERS), active=arr("<i8", ILE_MAX_MEMBERS), members=[])
     for _ in range(Ns):
         i64()
         out["members"].append(member())
@@ -334,7 +336,8 @@ def pack_state(st: dict) -> bytes:
         return member(st)
     parts = [np.array([st["kind"], st["d"], st["n_members"]], dtype="<i8").tobytes(),
              np.ascontiguousarray(st["W"], dtype="<f8").tobytes(), np.ascontiguousarray(st["frozen"], dtype="<i8").tobytes(),
-             np.ascontiguousarray(st["alloc"], dtype="<i8").tobytes()]
+             np.ascontiguousarray(st["alloc"], dtype="<i8").tobytes(),
+             np.ascontiguousarray(st.get("active", np.ones(ILE_MAX_MEMBERS)), dtype="<i8").tobytes()]
     for m in st["members"]:
         b = member(m)
         parts += [np.array([len(b)], dtype="<i8").tobytes(), b]
@@ -352,7 +355,8 @@ class Integrator:
     """Handle over ile_integrator_* (include/ile.h).  Buffers are torch CUDA float64 tensors."""
 
     def __init__(self, ile: Ile, kind: str, d: int, lo, hi, seed: int, max_batch: int, n_bins=100, eps=0.1, beta=1.0,
-                 P_thr=0.999, N_min_star=4096, n_gmm=8, members=("AC", "AV", "GMM")):
+                 P_thr=0.999, N_min_star=4096, n_gmm=8, members=("AC", "AV", "GMM"), first_iter=None, silent=None, member_opts=None,
+                 gmm_dims=None):
         self.ile = ile
         self.lib = ile.lib
         self.torch = ile.torch
@@ -367,6 +371,11 @@ class Integrator:
             o.n_members = len(members)
             for a, k in enumerate(members):
                 o.member_kind[a] = KINDS[k]
+                o.member_first_iter[a] = int(first_iter[a]) if first_iter is not None else 0
+                o.member_silent[a] = int(bool(silent[a])) if silent is not None else 0
+                o.member_n_bins[a] = int((member_opts[a] or {}).get("n_bins", 0)) if member_opts is not None else 0
+        if gmm_dims is not None:
+            o.gmm_dims_mask = sum(1 << int(c) for c in gmm_dims)
         self.opts = o
         self.h = C.c_void_p()
         self.ile._ck(self.lib.ile_integrator_create(ile.ctx, C.byref(o), C.byref(self.h)))

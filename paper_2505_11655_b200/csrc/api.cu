@@ -62,6 +62,7 @@ int ile_timing_drain(ile_ctx* ctx) {
 }
 extern "C" int ile_kernel_timing(ile_ctx* ctx, int on) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     int rc = ile_timing_drain(ctx);
     if (rc) return rc;
     if (on && !ctx->tev) {
@@ -76,6 +77,7 @@ extern "C" int ile_kernel_timing(ile_ctx* ctx, int on) {
 }
 extern "C" int ile_kernel_time(ile_ctx* ctx, double* total_ms, uint64_t* launches) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     int rc = ile_timing_drain(ctx);
     if (rc) return rc;
     if (total_ms) *total_ms = ctx->t_ms_total;
@@ -112,6 +114,7 @@ extern "C" int ile_create(ile_ctx** out, int device, void* cuda_stream) {
 
 extern "C" int ile_destroy(ile_ctx* ctx) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->d_ylm);
@@ -140,6 +143,7 @@ extern "C" const char* ile_last_error(const ile_ctx* ctx) { return ctx ? ctx->er
 
 extern "C" int ile_sync(ile_ctx* ctx) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ILE_CUDA(ctx, cudaGetLastError());
     return ILE_OK;
@@ -155,6 +159,7 @@ extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
 
 extern "C" int ile_set_network(ile_ctx* ctx, int K, const double* D, const double* pos_m, double gmst) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     if (K < 1 || K > ILE_MAX_K || !D || !pos_m) return ile_fail(ctx, ILE_EINVAL, "set_network: K in 1..%d", ILE_MAX_K);
     for (int k = 0; k < K; k++)
         for (int a = 0; a < 3; a++)
@@ -193,6 +198,7 @@ static long double binom_ld(int n, int k) {
 // (Goldberg et al. 1967 closed form with s = -2).
 extern "C" int ile_set_modes(ile_ctx* ctx, int M, const int* ell, const int* m) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     if (M < 1 || M > ILE_MAX_M || !ell || !m) return ile_fail(ctx, ILE_EINVAL, "set_modes: M in 1..%d", ILE_MAX_M);
     if (ctx->have_quv && M != ctx->M) return ile_fail(ctx, ILE_ESTATE, "set_modes: M differs from the loaded Q/U/V");
     YlmTable& T = ctx->h_ylm;
@@ -288,6 +294,7 @@ __global__ void pack_uv_kernel(const double* __restrict__ U, const double* __res
 extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U,
                             const double* V, double D_ref, int src_is_device) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);
     if (!ctx->have_net || !ctx->have_modes) return ile_fail(ctx, ILE_ESTATE, "load_quv: set_network and set_modes first");
     if (P < 1 || N_Q < 4 || !(fs > 0) || !Q || !U || !V || !(D_ref > 0))
         return ile_fail(ctx, ILE_EINVAL, "load_quv: bad argument");
@@ -300,6 +307,7 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     if (src_is_device) {
         hU.resize(nU);
         hV.resize(nU);
+        ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));      // producers of U, V on the context's (possibly non-blocking) stream
         ILE_CUDA(ctx, cudaMemcpy(hU.data(), U, nU * 8, cudaMemcpyDeviceToHost));
         ILE_CUDA(ctx, cudaMemcpy(hV.data(), V, nU * 8, cudaMemcpyDeviceToHost));
         pU = hU.data();
@@ -367,6 +375,7 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
 
 extern "C" int ile_set_time_grid(ile_ctx* ctx, double t_lo, double dt, int N_t, int interp) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     if (!ctx->have_quv) return ile_fail(ctx, ILE_ESTATE, "set_time_grid: load_quv first");
     if (N_t < 1 || !(dt > 0) || (interp != 0 && interp != 1)) return ile_fail(ctx, ILE_EINVAL, "set_time_grid: bad argument");
     double s = dt * ctx->fs;
@@ -384,6 +393,7 @@ extern "C" int ile_set_time_grid(ile_ctx* ctx, double t_lo, double dt, int N_t, 
 
 extern "C" int ile_set_prior(ile_ctx* ctx, double D_min, double D_max) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     if (!(D_min > 0) || !(D_max > D_min)) return ile_fail(ctx, ILE_EINVAL, "set_prior: need 0 < D_min < D_max");
     ctx->D_min = D_min; ctx->D_max = D_max; ctx->have_prior = true;
     return ILE_OK;
@@ -410,6 +420,7 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
         return ile_fail(ctx, ILE_ESTATE, "lnL: network, modes, Q/U/V and time grid must be set first");
     if (p < 0 || p >= ctx->P) return ile_fail(ctx, ILE_EINVAL, "lnL: intrinsic point %d out of range [0,%d)", p, ctx->P);
     bool table = ctx->d_lnT != nullptr;
+    if (d == 6 && !ctx->have_prior) return ile_fail(ctx, ILE_ESTATE, "lnL: set_prior (distance range) before evaluating with d = 6");
     if (!((d == 6 && !table) || (d == 5 && table)))
         return ile_fail(ctx, ILE_EINVAL, "lnL: d = %d does not match the distance-table state (6 without table, 5 with)", d);
     memset(L, 0, sizeof(*L));

@@ -19,8 +19,10 @@ struct AvState {
 };
 
 struct PortState {
-    double W[ILE_MAX_MEMBERS];
-    int frozen[ILE_MAX_MEMBERS];
+    double W[ILE_MAX_MEMBERS];        // mixture weights of the contributing activated members (sum 1), 0 for the others
+    int frozen[ILE_MAX_MEMBERS];      // 1: not trained on this batch (below 5 %, or not activated yet)
+    int active[ILE_MAX_MEMBERS];      // activated set of the last draw
+    int restarted, n_contrib;         // the weights were restarted uniform at the last draw; samples of contributing members
     long long alloc[ILE_MAX_MEMBERS];
     long long offset[ILE_MAX_MEMBERS + 1];
 };
@@ -53,7 +55,7 @@ struct UpdScratch {           // per-update scalars
 
 struct SamplerDev {
     int kind;
-    int pad;
+    int nb;                   // AC: bins per dimension of this member
     // AC
     unsigned long long* H;    // [d][nb]
     double* pi;               // [d][nb]
@@ -73,6 +75,7 @@ struct IntegDev {
     double eps, beta, P_thr;
     long long N_min_star, n_max;
     SamplerDev mem[ILE_MAX_MEMBERS];
+    int first_iter[ILE_MAX_MEMBERS], silent[ILE_MAX_MEMBERS];   // portfolio options
     PortState* port;
 };
 

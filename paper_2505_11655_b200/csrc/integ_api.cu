@@ -56,9 +56,10 @@ static ArenaPlan plan_arena(const IntegDev& I) {
         const int k = I.mem[a].kind;
         if (k == ILE_KIND_AV) { A.av[a] = off; off = align256(off + sizeof(AvState)); }
         if (k == ILE_KIND_AC) {
-            A.H[a] = off; off = align256(off + (size_t)I.d * I.nb * 8);
-            A.pi[a] = off; off = align256(off + (size_t)I.d * I.nb * 8);
-            A.cdf[a] = off; off = align256(off + (size_t)I.d * (I.nb + 1) * 8);
+            const int nb = I.mem[a].nb;
+            A.H[a] = off; off = align256(off + (size_t)I.d * nb * 8);
+            A.pi[a] = off; off = align256(off + (size_t)I.d * nb * 8);
+            A.cdf[a] = off; off = align256(off + (size_t)I.d * (nb + 1) * 8);
         }
         if (k == ILE_KIND_GMM) { A.gmm[a] = off; off = align256(off + gmm_doubles(I.n_gmm, I.d) * 8); }
     }
@@ -80,7 +81,13 @@ static void host_chol(int d, const double* S, double* L) {
 // covariances; portfolio equal weights
 static void fill_initial(const IntegDev& I, const ArenaPlan& A, unsigned char* h) {
     PortState* P = (PortState*)(h + A.port);
-    for (int a = 0; a < I.n_members; a++) P->W[a] = 1.0 / (double)I.n_members;
+    // iteration 0: the members whose first iteration is 0 are activated; uniform weights over the contributing ones
+    int n_con = 0;
+    for (int a = 0; a < I.n_members; a++) {
+        P->active[a] = I.first_iter[a] <= 0 ? 1 : 0;
+        n_con += P->active[a] && !I.silent[a];
+    }
+    for (int a = 0; a < I.n_members; a++) P->W[a] = (P->active[a] && !I.silent[a]) ? 1.0 / (double)n_con : 0.0;
     for (int a = 0; a < I.n_members; a++) {
         const int k = I.mem[a].kind;
         if (k == ILE_KIND_AV) {
@@ -95,11 +102,12 @@ static void fill_initial(const IntegDev& I, const ArenaPlan& A, unsigned char* h
             double* cdf = (double*)(h + A.cdf[a]);
             for (int c = 0; c < I.d; c++) {
                 double acc = 0.0;
-                cdf[c * (I.nb + 1)] = 0.0;
-                for (int b = 0; b < I.nb; b++) {
-                    pi[c * I.nb + b] = 1.0 / (double)I.nb;
-                    acc = acc + pi[c * I.nb + b];
-                    cdf[c * (I.nb + 1) + b + 1] = acc;
+                const int nb = I.mem[a].nb;
+                cdf[c * (nb + 1)] = 0.0;
+                for (int b = 0; b < nb; b++) {
+                    pi[c * nb + b] = 1.0 / (double)nb;
+                    acc = acc + pi[c * nb + b];
+                    cdf[c * (nb + 1) + b + 1] = acc;
                 }
             }
         }
@@ -213,20 +221,30 @@ extern "C" int ile_integrator_reset(ile_integrator* it);
 
 extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o, ile_integrator** out) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     if (!o || !out) return ile_fail(ctx, ILE_EINVAL, "integrator_create: null argument");
     *out = nullptr;
-    if (o->kind < 0 || o->kind > ILE_KIND_PORTFOLIO || o->d < 1 || o->d > ILE_MAX_D || o->max_batch < 1 || o->max_batch > (1ll << 30))
-        return ile_fail(ctx, ILE_EINVAL, "integrator_create: kind, d (1..%d) or max_batch out of range", ILE_MAX_D);
+    // max_batch: the fixed-point sums (q <= 2^40 per sample, uint64) cannot overflow up to 2^24 samples with flat weights
+    if (o->kind < 0 || o->kind > ILE_KIND_PORTFOLIO || o->d < 1 || o->d > ILE_MAX_D || o->max_batch < 1 || o->max_batch > (1ll << 24))
+        return ile_fail(ctx, ILE_EINVAL, "integrator_create: kind, d (1..%d) or max_batch (1..2^24) out of range", ILE_MAX_D);
     for (int c = 0; c < o->d; c++)
         if (!(o->hi[c] > o->lo[c])) return ile_fail(ctx, ILE_EINVAL, "integrator_create: empty box in dimension %d", c);
-    int kinds[ILE_MAX_MEMBERS], Ns = 1;
+    int kinds[ILE_MAX_MEMBERS], nbs[ILE_MAX_MEMBERS], Ns = 1;
     kinds[0] = o->kind;
+    nbs[0] = o->n_bins;
     if (o->kind == ILE_KIND_PORTFOLIO) {
         Ns = o->n_members;
         if (Ns < 1 || Ns > ILE_MAX_MEMBERS) return ile_fail(ctx, ILE_EINVAL, "integrator_create: n_members in 1..%d", ILE_MAX_MEMBERS);
         for (int a = 0; a < Ns; a++) {
             kinds[a] = o->member_kind[a];
             if (kinds[a] < 0 || kinds[a] > ILE_KIND_GMM) return ile_fail(ctx, ILE_EINVAL, "integrator_create: member %d has kind %d", a, kinds[a]);
+            nbs[a] = o->member_n_bins[a] ? o->member_n_bins[a] : o->n_bins;
+            if (o->member_first_iter[a] < 0 || (a == 0 && o->member_first_iter[0] != 0))
+                return ile_fail(ctx, ILE_EINVAL, "integrator_create: member_first_iter must be >= 0 and 0 for member 0 (PAPER.md:297)");
+            if (o->member_silent[a] != 0 && o->member_silent[a] != 1) return ile_fail(ctx, ILE_EINVAL, "integrator_create: member_silent is 0 or 1");
+            if (o->member_silent[a] && a == 0) return ile_fail(ctx, ILE_EINVAL, "integrator_create: member 0 contributes to the integral");
+            if (a > 0 && o->member_silent[a - 1] && !o->member_silent[a])
+                return ile_fail(ctx, ILE_EINVAL, "integrator_create: silent members are listed after the contributing ones");
         }
     }
     bool has_ac = false, has_av = false, has_gmm = false;
@@ -235,8 +253,11 @@ extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o,
         has_av |= kinds[a] == ILE_KIND_AV;
         has_gmm |= kinds[a] == ILE_KIND_GMM;
     }
-    if (has_ac && (o->n_bins < 1 || o->n_bins > 4096 || !(o->eps >= 0.0 && o->eps <= 1.0) || !(o->beta > 0.0)))
-        return ile_fail(ctx, ILE_EINVAL, "integrator_create: AC needs n_bins in 1..4096, eps in [0,1], beta > 0");
+    if (has_ac && (!(o->eps >= 0.0 && o->eps <= 1.0) || !(o->beta > 0.0)))
+        return ile_fail(ctx, ILE_EINVAL, "integrator_create: AC needs eps in [0,1], beta > 0");
+    for (int a = 0; a < Ns; a++)   // the histogram kernel keeps d x n_bins 64-bit counters in shared memory (48 KB without opt-in)
+        if (kinds[a] == ILE_KIND_AC && (nbs[a] < 1 || nbs[a] > 4096 || (long long)o->d * nbs[a] > 6144))
+            return ile_fail(ctx, ILE_EINVAL, "integrator_create: AC needs n_bins in 1..4096 and d * n_bins <= 6144");
     if (has_av && (!(o->P_thr > 0.0 && o->P_thr <= 1.0) || o->N_min_star < 1))
         return ile_fail(ctx, ILE_EINVAL, "integrator_create: AV needs P_thr in (0,1], N_min_star >= 1");
     if (has_gmm && (o->n_gmm < 1 || o->n_gmm > 16)) return ile_fail(ctx, ILE_EINVAL, "integrator_create: n_gmm in 1..16");
@@ -248,6 +269,11 @@ extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o,
     it->cap = o->max_batch;
     IntegDev& I = it->I;
     I.kind = o->kind; I.d = o->d; I.n_members = Ns; I.nb = has_ac ? o->n_bins : 1; I.n_gmm = has_gmm ? o->n_gmm : 1;
+    for (int a = 0; a < Ns; a++) {
+        I.mem[a].nb = kinds[a] == ILE_KIND_AC ? nbs[a] : 1;
+        I.first_iter[a] = o->kind == ILE_KIND_PORTFOLIO ? o->member_first_iter[a] : 0;
+        I.silent[a] = o->kind == ILE_KIND_PORTFOLIO ? o->member_silent[a] : 0;
+    }
     I.V0 = 1.0;
     for (int c = 0; c < o->d; c++) {
         I.lo[c] = o->lo[c];
@@ -320,6 +346,7 @@ extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o,
 extern "C" int ile_integrator_destroy(ile_integrator* it) {
     if (!it) return ILE_EINVAL;
     cudaSetDevice(it->ctx->device);
+    cudaSetDevice(it->ctx->device);
     cudaStreamSynchronize(it->ctx->stream);
     free_integrator(it);
     return ILE_OK;
@@ -327,6 +354,7 @@ extern "C" int ile_integrator_destroy(ile_integrator* it) {
 
 extern "C" int ile_integrator_reset(ile_integrator* it) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     ile_ctx* ctx = it->ctx;
     const ArenaPlan A = plan_arena(it->I);
     unsigned char* base = (unsigned char*)it->arena;
@@ -347,6 +375,7 @@ static int check_N(ile_integrator* it, int N, const char* what) {
 
 extern "C" int ile_integrator_draw(ile_integrator* it, int N, uint64_t iter, double* z, double* ln_ps) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     int rc = check_N(it, N, "integrator_draw");
     if (rc) return rc;
     if (!z || !ln_ps) return ile_fail(it->ctx, ILE_EINVAL, "integrator_draw: null output");
@@ -359,12 +388,14 @@ extern "C" int ile_integrator_draw(ile_integrator* it, int N, uint64_t iter, dou
 
 extern "C" int ile_integrator_ln_pdf(ile_integrator* it, int N, const double* z, double* ln_ps) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     if (N < 1 || !z || !ln_ps) return ile_fail(it->ctx, ILE_EINVAL, "integrator_ln_pdf: bad argument");
     return integ_launch_ln_pdf(it, N, z, ln_ps);
 }
 
 extern "C" int ile_integrator_update(ile_integrator* it, int N, const double* z, const double* lnw, const double* ln_ps) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     int rc = check_N(it, N, "integrator_update");
     if (rc) return rc;
     if (!z || !lnw) return ile_fail(it->ctx, ILE_EINVAL, "integrator_update: null input");
@@ -374,6 +405,18 @@ extern "C" int ile_integrator_update(ile_integrator* it, int N, const double* z,
             return ile_fail(it->ctx, ILE_ESTATE, "integrator_update: a portfolio must have drawn this batch (member allocation)");
     }
     return integ_launch_update(it, N, z, lnw, ln_ps);
+}
+
+// samples of the contributing members in a batch of N at iteration g (alloc_kernel's N_c): silent
+// activated members take N / N_active each and sit after the contributing ones
+static int contributing_samples(const IntegDev& I, int N, uint64_t g) {
+    int n_act = 0, n_sil = 0;
+    for (int a = 0; a < I.n_members; a++) {
+        const bool act = (uint64_t)I.first_iter[a] <= g;
+        n_act += act;
+        n_sil += act && I.silent[a];
+    }
+    return n_sil ? N - n_sil * (N / n_act) : N;
 }
 
 // ---------------------------------------------------------------- step / run
@@ -388,7 +431,7 @@ static int step_internal(ile_integrator* it, int p, int N, uint64_t iter, ile_re
     if (rc) return rc;
     lnw_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(N, it->lnL, it->ln_prior, it->ln_ps, it->lnw);
     ILE_LAUNCH_CHECK(ctx);
-    rc = ile_launch_reduce(ctx, N, it->lnw, it->res, 1);
+    rc = ile_launch_reduce(ctx, contributing_samples(I, N, iter), it->lnw, it->res, 1);   // silent members' samples stay out of the estimate
     if (rc) return rc;
     annotate_kernel<<<1, 32, 0, ctx->stream>>>(I, it->res, 1);
     ILE_LAUNCH_CHECK(ctx);
@@ -445,6 +488,7 @@ __global__ void __launch_bounds__(256) integrand_kernel(IntegDev I, ile_integran
 
 extern "C" int ile_integrator_step_integrand(ile_integrator* it, const ile_integrand* f, int N, uint64_t iter, ile_result* out_dev) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     ile_ctx* ctx = it->ctx;
     int rc = check_N(it, N, "integrator_step_integrand");
     if (rc) return rc;
@@ -459,7 +503,7 @@ extern "C" int ile_integrator_step_integrand(ile_integrator* it, const ile_integ
     it->last_N = N;
     integrand_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(I, *f, N, it->z, it->ln_ps, it->lnL, it->lnw);
     ILE_LAUNCH_CHECK(ctx);
-    rc = ile_launch_reduce(ctx, N, it->lnw, it->res, 1);
+    rc = ile_launch_reduce(ctx, contributing_samples(I, N, iter), it->lnw, it->res, 1);
     if (rc) return rc;
     annotate_kernel<<<1, 32, 0, ctx->stream>>>(I, it->res, 1);
     ILE_LAUNCH_CHECK(ctx);
@@ -474,6 +518,7 @@ extern "C" int ile_integrator_step_integrand(ile_integrator* it, const ile_integ
 
 extern "C" int ile_integrator_step(ile_integrator* it, int p, int N, uint64_t iter, ile_result* out_dev) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     int rc = check_N(it, N, "integrator_step");
     if (rc) return rc;
     return step_internal(it, p, N, iter, out_dev);
@@ -481,6 +526,7 @@ extern "C" int ile_integrator_step(ile_integrator* it, int p, int N, uint64_t it
 
 extern "C" int ile_integrator_run(ile_integrator* it, int p_first, int p_count, int n_iter, int N, ile_result* out_dev) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     int rc = check_N(it, N, "integrator_run");
     if (rc) return rc;
     if (p_count < 1 || n_iter < 1 || p_first < 0 || !out_dev) return ile_fail(it->ctx, ILE_EINVAL, "integrator_run: bad argument");
@@ -509,7 +555,7 @@ extern "C" int ile_integrator_last_batch(ile_integrator* it, const double** z, c
 static size_t member_blob_bytes(const IntegDev& I, int a, long long C_av) {
     size_t b = 16;   // header: kind, d
     switch (I.mem[a].kind) {
-        case ILE_KIND_AC: b += 8 + (size_t)I.d * I.nb * 16 + (size_t)I.d * (I.nb + 1) * 8; break;
+        case ILE_KIND_AC: b += 8 + (size_t)I.d * I.mem[a].nb * 16 + (size_t)I.d * (I.mem[a].nb + 1) * 8; break;
         case ILE_KIND_AV: b += 32 + (size_t)C_av * 8; break;
         case ILE_KIND_GMM: b += 8 + gmm_doubles(I.n_gmm, I.d) * 8; break;
         default: break;
@@ -519,6 +565,7 @@ static size_t member_blob_bytes(const IntegDev& I, int a, long long C_av) {
 
 extern "C" int ile_integrator_get_state(ile_integrator* it, void* buf, size_t* bytes) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     ile_ctx* ctx = it->ctx;
     if (!bytes) return ile_fail(ctx, ILE_EINVAL, "integrator_get_state: bytes is null");
     const IntegDev& I = it->I;
@@ -529,7 +576,7 @@ extern "C" int ile_integrator_get_state(ile_integrator* it, void* buf, size_t* b
         if (I.mem[a].kind == ILE_KIND_AV) ILE_CUDA(ctx, cudaMemcpy(&av[a], I.mem[a].av, sizeof(AvState), cudaMemcpyDeviceToHost));
     size_t need = 0;
     if (I.kind == ILE_KIND_PORTFOLIO) {
-        need = 16 + 8 + 3 * 8 * ILE_MAX_MEMBERS;
+        need = 16 + 8 + 4 * 8 * ILE_MAX_MEMBERS;
         for (int a = 0; a < I.n_members; a++) need += 8 + member_blob_bytes(I, a, av[a].C);
     } else {
         need = member_blob_bytes(I, 0, av[0].C);
@@ -555,8 +602,8 @@ extern "C" int ile_integrator_get_state(ile_integrator* it, void* buf, size_t* b
         put_i64(S.kind);
         put_i64(I.d);
         if (S.kind == ILE_KIND_AC) {
-            put_i64(I.nb);
-            if (put_dev(S.H, (size_t)I.d * I.nb * 8) || put_dev(S.pi, (size_t)I.d * I.nb * 8) || put_dev(S.cdf, (size_t)I.d * (I.nb + 1) * 8)) return 1;
+            put_i64(S.nb);
+            if (put_dev(S.H, (size_t)I.d * S.nb * 8) || put_dev(S.pi, (size_t)I.d * S.nb * 8) || put_dev(S.cdf, (size_t)I.d * (S.nb + 1) * 8)) return 1;
         } else if (S.kind == ILE_KIND_AV) {
             put_i64(av[a].n); put_i64(av[a].C); put_i64(av[a].N_min);
             memcpy(w, &av[a].L_thr, 8); w += 8;
@@ -577,6 +624,7 @@ extern "C" int ile_integrator_get_state(ile_integrator* it, void* buf, size_t* b
         memcpy(w, P.W, 8 * ILE_MAX_MEMBERS); w += 8 * ILE_MAX_MEMBERS;
         for (int a = 0; a < ILE_MAX_MEMBERS; a++) put_i64(P.frozen[a]);
         for (int a = 0; a < ILE_MAX_MEMBERS; a++) put_i64(P.alloc[a]);
+        for (int a = 0; a < ILE_MAX_MEMBERS; a++) put_i64(P.active[a]);
         for (int a = 0; a < I.n_members && !bad; a++) {
             put_i64((long long)member_blob_bytes(I, a, av[a].C));
             bad = put_member(a);
@@ -593,6 +641,7 @@ extern "C" int ile_integrator_get_state(ile_integrator* it, void* buf, size_t* b
 
 extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, size_t bytes) {
     if (!it) return ILE_EINVAL;
+    cudaSetDevice(it->ctx->device);
     ile_ctx* ctx = it->ctx;
     if (!buf) return ile_fail(ctx, ILE_EINVAL, "integrator_set_state: null buffer");
     const IntegDev& I = it->I;
@@ -618,8 +667,8 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
         if (!get_i64(&kind) || !get_i64(&d) || kind != S.kind || d != I.d) return false;
         if (S.kind == ILE_KIND_AC) {
             long long nb;
-            if (!get_i64(&nb) || nb != I.nb) return false;
-            return get_dev(S.H, (size_t)I.d * I.nb * 8) && get_dev(S.pi, (size_t)I.d * I.nb * 8) && get_dev(S.cdf, (size_t)I.d * (I.nb + 1) * 8);
+            if (!get_i64(&nb) || nb != S.nb) return false;
+            return get_dev(S.H, (size_t)I.d * S.nb * 8) && get_dev(S.pi, (size_t)I.d * S.nb * 8) && get_dev(S.cdf, (size_t)I.d * (S.nb + 1) * 8);
         }
         if (S.kind == ILE_KIND_AV) {
             AvState s;
@@ -629,6 +678,16 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
             memcpy(&s.L_thr, r, 8);
             r += 8;
             if (s.n < 1 || s.n > I.n_max || s.C < 1 || s.C > it->cap) return false;
+            if (r + (size_t)s.C * 8 > end) return false;
+            {   // the draw's binary search and ln p_s assume sorted unique keys below n^d
+                unsigned long long lim = 1, prev = 0, k;
+                for (int c = 0; c < I.d; c++) lim *= (unsigned long long)s.n;
+                for (long long q = 0; q < s.C; q++) {
+                    memcpy(&k, r + 8 * q, 8);
+                    if (k >= lim || (q > 0 && k <= prev)) return false;
+                    prev = k;
+                }
+            }
             if (!dry && cudaMemcpy(S.av, &s, sizeof(s), cudaMemcpyHostToDevice) != cudaSuccess) return false;
             if (!get_dev(S.keys, (size_t)s.C * 8)) return false;
             if (!dry) {
@@ -640,7 +699,9 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
         if (S.kind == ILE_KIND_GMM) {
             long long C;
             if (!get_i64(&C) || C != I.n_gmm) return false;
-            return get_dev(S.gmm, gmm_doubles(I.n_gmm, I.d) * 8);
+            if (!get_dev(S.gmm, gmm_doubles(I.n_gmm, I.d) * 8)) return false;
+            if (!dry && integ_gmm_refresh(it, a) != ILE_OK) return false;     // Cholesky factors from the restored Sigma, not from the blob
+            return true;
         }
         return true;
     };
@@ -658,11 +719,15 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
             r += 8 * ILE_MAX_MEMBERS;
         } else ok = false;
         for (int a = 0; a < ILE_MAX_MEMBERS && ok; a++) { long long v; ok = get_i64(&v); P.frozen[a] = (int)v; }
-        for (int a = 0; a < ILE_MAX_MEMBERS && ok; a++) { long long v; ok = get_i64(&v); P.alloc[a] = v; }
+        for (int a = 0; a < ILE_MAX_MEMBERS && ok; a++) { long long v; ok = get_i64(&v) && v >= 0 && v <= it->cap; P.alloc[a] = v; }
+        for (int a = 0; a < ILE_MAX_MEMBERS && ok; a++) { long long v; ok = get_i64(&v) && (v == 0 || v == 1); P.active[a] = (int)v; }
         if (ok) {
             long long off = 0;
             for (int a = 0; a < I.n_members; a++) { P.offset[a] = off; off += P.alloc[a]; }
             P.offset[I.n_members] = off;
+            ok = off <= it->cap;
+            // the allocation belongs to a batch of that size: an update needs a draw first unless it is the resident one
+            if (!dry && off != it->last_N) it->drew = false;
             ok = dry || cudaMemcpy(I.port, &P, sizeof(P), cudaMemcpyHostToDevice) == cudaSuccess;
         }
         for (int a = 0; a < I.n_members && ok; a++) {

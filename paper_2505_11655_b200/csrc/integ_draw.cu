@@ -16,8 +16,8 @@ __device__ __forceinline__ double ln_pdf_ac(const IntegDev& I, const SamplerDev&
     double out = 0.0;
 #pragma unroll
     for (int c = 0; c < D; c++) {
-        const long long b = bin_index_dev(zz[c], I.lo[c], I.hi[c], I.nb);
-        const double pdf = __ddiv_rn(__dmul_rn(S.pi[c * I.nb + b], (double)I.nb), __dsub_rn(I.hi[c], I.lo[c]));
+        const long long b = bin_index_dev(zz[c], I.lo[c], I.hi[c], S.nb);
+        const double pdf = __ddiv_rn(__dmul_rn(S.pi[c * S.nb + b], (double)S.nb), __dsub_rn(I.hi[c], I.lo[c]));
         out = __dadd_rn(out, log(pdf));
     }
     return out;
@@ -108,7 +108,9 @@ __device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double
     double e[ILE_MAX_MEMBERS];
     double mx = neg_inf();
     for (int a = 0; a < I.n_members; a++) {
-        e[a] = gc_all[ILE_MAX_MEMBERS * GMM_GC + a] + member_ln_pdf<D>(I, a, zz, inbox, gc_all);
+        // members that are not activated yet or contribute silently have weight 0 (ln W = -inf): no term
+        const double lw = gc_all[ILE_MAX_MEMBERS * GMM_GC + a];
+        e[a] = lw == neg_inf() ? neg_inf() : lw + member_ln_pdf<D>(I, a, zz, inbox, gc_all);
         mx = fmax(mx, e[a]);
     }
     if (!is_finite_d(mx)) return neg_inf();
@@ -117,36 +119,65 @@ __device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double
     return mx + log(sum);
 }
 
-// ---------------------------------------------------------------- allocation (portfolio, reading G25)
-// N_a = floor(N W_a), remainder to the members in index order.
-__global__ void alloc_kernel(IntegDev I, long long N) {
+// ---------------------------------------------------------------- allocation (portfolio, readings G25, G41, G42)
+// Activated set at iteration g; when it changes the weights restart uniform over the contributing
+// members.  Silent activated members take N / N_active samples each; the contributing ones share the rest,
+// N_a = floor(N_c W_a) with the remainder to them in index order.
+__global__ void alloc_kernel(IntegDev I, long long N, unsigned int g) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     PortState* P = I.port;
+    const int Ns = I.n_members;
+    bool changed = false;
+    int n_act = 0, n_sil = 0, n_con = 0;
+    for (int a = 0; a < Ns; a++) {
+        const int act = (unsigned int)I.first_iter[a] <= g ? 1 : 0;
+        changed = changed || (act != P->active[a]);
+        P->active[a] = act;
+        n_act += act;
+        n_sil += act && I.silent[a];
+        n_con += act && !I.silent[a];
+    }
+    P->restarted = 0;
+    if (changed) {
+        for (int a = 0; a < Ns; a++) {
+            P->W[a] = (P->active[a] && !I.silent[a]) ? __ddiv_rn(1.0, (double)n_con) : 0.0;
+            P->frozen[a] = 0;
+        }
+        P->restarted = 1;
+    }
+    const long long each = n_sil ? N / n_act : 0;
+    const long long Nc = N - n_sil * each;
     long long tot = 0;
-    for (int a = 0; a < I.n_members; a++) {
-        P->alloc[a] = (long long)floor(__dmul_rn((double)N, P->W[a]));
+    for (int a = 0; a < Ns; a++) {
+        const bool con = P->active[a] && !I.silent[a];
+        P->alloc[a] = con ? (long long)floor(__dmul_rn((double)Nc, P->W[a])) : 0;
         tot += P->alloc[a];
     }
-    long long rem = N - tot;
+    long long rem = Nc - tot;
     int a = 0;
     while (rem > 0) {
-        P->alloc[a % I.n_members] += 1;
-        rem--;
+        if (P->active[a % Ns] && !I.silent[a % Ns]) {
+            P->alloc[a % Ns] += 1;
+            rem--;
+        }
         a++;
     }
+    for (int b = 0; b < Ns; b++)
+        if (P->active[b] && I.silent[b]) P->alloc[b] = each;
     long long off = 0;
-    for (int b = 0; b < I.n_members; b++) {
+    for (int b = 0; b < Ns; b++) {
         P->offset[b] = off;
         off += P->alloc[b];
     }
-    P->offset[I.n_members] = off;
+    P->offset[Ns] = off;
+    P->n_contrib = (int)Nc;
 }
 
 // ---------------------------------------------------------------- draw
 // every GMM member's per-component constants and the members' ln W_a, once per block
 __device__ __forceinline__ void block_gmm_consts(const IntegDev& I, double* gc_all) {
     bool any = I.n_members > 1;
-    if (I.n_members > 1 && threadIdx.x < I.n_members) gc_all[ILE_MAX_MEMBERS * GMM_GC + threadIdx.x] = log(I.port->W[threadIdx.x]);   // ln W_a
+    if (I.n_members > 1 && threadIdx.x < I.n_members) gc_all[ILE_MAX_MEMBERS * GMM_GC + threadIdx.x] = I.port->W[threadIdx.x] > 0.0 ? log(I.port->W[threadIdx.x]) : neg_inf();   // ln W_a
     for (int a = 0; a < I.n_members; a++)
         if (I.mem[a].kind == ILE_KIND_GMM) {
             gmm_consts(I, I.mem[a].gmm, gc_all + a * GMM_GC, threadIdx.x, blockDim.x);
@@ -219,16 +250,16 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
             if (S.kind == ILE_KIND_UNIFORM) {
                 zc = __dadd_rn(lo, __dmul_rn(u, __dsub_rn(hi, lo)));
             } else if (S.kind == ILE_KIND_AC) {
-                const double* cdf = S.cdf + c * (I.nb + 1);
-                const double* pi = S.pi + c * I.nb;
-                int b0 = 0, b1 = I.nb;            // last b in [0, nb) with cdf[b] <= u
+                const double* cdf = S.cdf + c * (S.nb + 1);
+                const double* pi = S.pi + c * S.nb;
+                int b0 = 0, b1 = S.nb;            // last b in [0, nb) with cdf[b] <= u
                 while (b1 - b0 > 1) {
                     const int mid = (b0 + b1) >> 1;
                     if (cdf[mid] <= u) b0 = mid; else b1 = mid;
                 }
                 double r = __ddiv_rn(__dsub_rn(u, cdf[b0]), pi[b0]);
                 r = fmin(r, 1.0 - 0x1.0p-53);
-                const double delta = __ddiv_rn(__dsub_rn(hi, lo), (double)I.nb);
+                const double delta = __ddiv_rn(__dsub_rn(hi, lo), (double)S.nb);
                 zc = __dadd_rn(lo, __dmul_rn(__dadd_rn((double)b0, r), delta));
             } else {                                // AV
                 const unsigned long long ic = key % (unsigned long long)n;
@@ -259,7 +290,7 @@ __global__ void __launch_bounds__(128) ln_pdf_kernel(IntegDev I, int N, const do
 
 int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, double* ln_ps) {
     ile_ctx* ctx = it->ctx;
-    alloc_kernel<<<1, 32, 0, ctx->stream>>>(it->I, (long long)N);
+    alloc_kernel<<<1, 32, 0, ctx->stream>>>(it->I, (long long)N, g);
     ILE_LAUNCH_CHECK(ctx);
     switch (it->I.d) {
 #define DRAW_CASE(D_) case D_: draw_kernel<D_><<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, g, z, ln_ps); break;

@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(256) ac_hist_kernel(IntegDev I, int a, int N, 
                                                       const UpdScratch* __restrict__ us) {
     if (us->abort || us->n_valid == 0) return;
     extern __shared__ unsigned long long sh_h[];
-    const int nb = I.nb, tot = I.d * nb;
+    const int nb = I.mem[a].nb, tot = I.d * nb;
     for (int q = threadIdx.x; q < tot; q += blockDim.x) sh_h[q] = 0ull;
     __syncthreads();
     const double m = double_from_ord(us->m_ord);
@@ -110,7 +110,7 @@ __global__ void ac_finish_kernel(IntegDev I, int a, const UpdScratch* __restrict
     if (us->abort) return;
     const int c = threadIdx.x;
     if (c >= I.d) return;
-    const int nb = I.nb;
+    const int nb = I.mem[a].nb;
     const unsigned long long* H = I.mem[a].H + c * nb;
     double* pi = I.mem[a].pi + c * nb;
     double* cdf = I.mem[a].cdf + c * (nb + 1);
@@ -650,7 +650,7 @@ __global__ void gmm_chol_kernel(IntegDev I, int a) {
 // ---------------------------------------------------------------- PORTFOLIO weights
 __global__ void __launch_bounds__(256) port_ness_kernel(IntegDev I, const double* __restrict__ lnw, double* __restrict__ part) {
     const int a = blockIdx.y;
-    const long long off = I.port->offset[a], cnt = I.port->alloc[a];
+    const long long off = I.port->offset[a], cnt = (I.port->active[a] && !I.silent[a]) ? I.port->alloc[a] : 0;   // n_ESS of contributing members only
     double m = neg_inf(), s1 = 0.0, s2 = 0.0;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < cnt; i += (long long)gridDim.x * blockDim.x) {
         const double v = lnw[off + i];
@@ -708,15 +708,33 @@ __global__ void port_weights_kernel(IntegDev I, const double* __restrict__ part,
         ness[a] = (bm == neg_inf() || !(t2 > 0.0)) ? 0.0 : t1 * t1 / t2;
         tot += ness[a];
     }
-    if (!(tot > 0.0)) return;
+    // members that are not activated are never trained; silent ones always are
+    int n_con = 0;
+    for (int a = 0; a < Ns; a++) {
+        const bool con = P->active[a] && !I.silent[a];
+        n_con += con;
+        if (!P->active[a]) P->frozen[a] = 1;
+        else if (!con) P->frozen[a] = 0;
+    }
+    if (!(tot > 0.0)) {
+        P->restarted = 0;
+        return;
+    }
     double W[ILE_MAX_MEMBERS], ws = 0.0;
     for (int a = 0; a < Ns; a++) {
+        const bool con = P->active[a] && !I.silent[a];
+        if (!con) {
+            W[a] = 0.0;
+            continue;
+        }
         const double raw = ness[a] / tot;
-        P->frozen[a] = raw < 0.05 ? 1 : 0;
-        W[a] = fmax(raw, 0.05 / (double)Ns);
+        // the batch after a restart was drawn with uniform weights (none below 5 %): nobody is frozen on it
+        P->frozen[a] = (raw < 0.05 && !P->restarted) ? 1 : 0;
+        W[a] = fmax(raw, 0.05 / (double)n_con);
         ws += W[a];
     }
     for (int a = 0; a < Ns; a++) P->W[a] = W[a] / ws;
+    P->restarted = 0;
 }
 
 // ---------------------------------------------------------------- host: update dispatch
@@ -730,11 +748,11 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
         case ILE_KIND_UNIFORM:
             return ILE_OK;
         case ILE_KIND_AC: {
-            upd_init_kernel<<<8, 256, 0, st>>>(it->us, skip, S.H, I.d * I.nb, nullptr);
+            upd_init_kernel<<<8, 256, 0, st>>>(it->us, skip, S.H, I.d * S.nb, nullptr);
             ILE_LAUNCH_CHECK(ctx);
             mask_max_kernel<<<grid, 256, 0, st>>>(I, N, z, lnw, nullptr, 0, it->us);
             ILE_LAUNCH_CHECK(ctx);
-            ac_hist_kernel<<<grid, 256, (size_t)I.d * I.nb * 8, st>>>(I, a, N, z, lnw, it->us);
+            ac_hist_kernel<<<grid, 256, (size_t)I.d * S.nb * 8, st>>>(I, a, N, z, lnw, it->us);
             ILE_LAUNCH_CHECK(ctx);
             ac_finish_kernel<<<1, 32, 0, st>>>(I, a, it->us);
             ILE_LAUNCH_CHECK(ctx);

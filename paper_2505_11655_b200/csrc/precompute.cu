@@ -251,6 +251,7 @@ static void launch_fft_cols(int P, int M, int K, int N_f, int N1, const double2*
 extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, double f_low, const double* h, const double* d, const double* S,
                                   double t_Q0, int N_Q, double D_ref) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);
     if (!ctx->have_net || !ctx->have_modes) return ile_fail(ctx, ILE_ESTATE, "precompute_quv: set_network and set_modes first");
     if (P < 1 || N_f < 8 || (N_f & 1) || !(df > 0) || !h || !d || !S || N_Q < 4 || N_Q > N_f || !(D_ref > 0))
         return ile_fail(ctx, ILE_EINVAL, "precompute_quv: bad argument");
@@ -324,6 +325,7 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
 // Copies the resident Q/U/V of intrinsic point p to host arrays (caller layout of ile_load_quv).
 extern "C" int ile_get_quv(ile_ctx* ctx, int p, double* Q, double* U, double* V) {
     if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
     if (!ctx->have_quv) return ile_fail(ctx, ILE_ESTATE, "get_quv: nothing loaded");
     if (p < 0 || p >= ctx->P) return ile_fail(ctx, ILE_EINVAL, "get_quv: point out of range");
     const size_t nQ = (size_t)ctx->K * ctx->M * ctx->N_Q * 2, nU = (size_t)ctx->K * ctx->M * ctx->M * 2;

@@ -38,4 +38,4 @@ def test_create_fails_loudly_without_a_gpu_or_with_bad_arguments():
 def test_binding_struct_layouts_match_the_header():
     from paper_2505_11655_b200 import binding
     assert ctypes.sizeof(binding.Result) == binding.RESULT_DTYPE.itemsize == 8 * (14 + 8 + 8)
-    assert ctypes.sizeof(binding.IntegratorOpts) == 8 + 128 + 16 + 8 + 16 + 16 + 8 + 32
+    assert ctypes.sizeof(binding.IntegratorOpts) == 8 + 128 + 16 + 8 + 16 + 16 + 8 + 32 + 3 * 32 + 8

@@ -51,7 +51,8 @@ def test_portfolio_blob_round_trip():
     W = np.zeros(8)
     W[:3] = [0.2, 0.3, 0.5]
     st = dict(kind=b.KINDS["PORTFOLIO"], d=3, n_members=3, W=W, frozen=np.array([0, 1, 0, 0, 0, 0, 0, 0], dtype=np.int64),
-              alloc=np.array([10, 20, 30, 0, 0, 0, 0, 0], dtype=np.int64), members=[_ac(), _av(), _gmm()])
+              alloc=np.array([10, 20, 30, 0, 0, 0, 0, 0], dtype=np.int64), active=np.array([1, 1, 1, 0, 0, 0, 0, 0], dtype=np.int64),
+              members=[_ac(), _av(), _gmm()])
     _same(b.parse_state(b.pack_state(st)), st)
 
 

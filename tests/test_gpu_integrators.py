@@ -338,3 +338,82 @@ def test_run_matches_steps_and_resets_between_points(env):
             assert r["ln_integral"] == out[p * 2 + it]["ln_integral"]
             assert r["cum_ln_integral"] == out[p * 2 + it]["cum_ln_integral"]
     assert len({float(out[p * 2]["ln_integral"]) for p in range(3)}) == 3     # different intrinsic points
+
+
+# ------------------------------------------------------------------------------- portfolio options of PAPER.md:297
+def test_portfolio_activation_iteration_teacher_forced(env):
+    """member_first_iter: two AC members with 10 and 30 bins, the second activated at iteration 3 (the paper's Fig. 7
+    portfolio in small).  Same draws (bit-exact), the oracle's ln w into both updates: identical allocations,
+    histograms and weights at every iteration, before, at and after the activation."""
+    torch, ile, _ = env
+    N, d, g0 = 40000, 4, 3
+    kw = dict(members=("AC", "AC"), member_opts=[dict(n_bins=10), dict(n_bins=30)], first_iter=[0, g0])
+    g = _make(ile, "PORTFOLIO", d, N, **kw)
+    o = _oracle("PORTFOLIO", d, members=["AC", "AC"], member_opts=kw["member_opts"], first_iter=kw["first_iter"])
+    lo, hi = LO6[:d], HI6[:d]
+    for it in range(6):
+        z, lp = g.draw(N, it)
+        zo, lpo = o.draw(N, it)
+        st = g.get_state()
+        assert np.array_equal(st["alloc"][:2], o.alloc) and np.array_equal(st["active"][:2].astype(bool), o.active)
+        if it < g0:
+            assert st["alloc"][1] == 0 and st["W"][1] == 0.0
+        zg = z.cpu().numpy()
+        assert np.array_equal(zg, zo)                                        # AC draws: bit-exact
+        np.testing.assert_allclose(lp.cpu().numpy(), lpo, rtol=0, atol=1e-10)
+        lnw = _gauss_lnw(zg, lo, hi, width=0.08) - lpo
+        o.update(zo, lnw, lpo)
+        g.update(z, _dev(torch, lnw), _dev(torch, lpo))
+        st = g.get_state()
+        np.testing.assert_allclose(st["W"][:2], o.W, rtol=1e-11)
+        assert np.array_equal(st["frozen"][:2].astype(bool)[o.active], o.frozen[o.active])
+        for a in range(2):
+            assert st["members"][a]["n_bins"] == (10, 30)[a]
+            assert np.array_equal(st["members"][a]["H"], o.members[a].H), (it, a)
+    assert st["W"][1] > 0.0
+
+
+def test_portfolio_silent_member_and_estimate(env):
+    """member_silent: [AC, UNIFORM (silent)]: the silent member draws N / 2 samples of every batch, the density is the
+    AC member's alone, the estimate counts the contributing samples only and the AC histogram is trained on all N."""
+    from paper_2505_11655_b200 import Integrand, result_from_device
+    torch, ile, _ = env
+    N, d = 30000, 3
+    g = _make(ile, "PORTFOLIO", d, N, members=("AC", "UNIFORM"), silent=[False, True], n_bins=20)
+    o = _oracle("PORTFOLIO", d, members=["AC", "UNIFORM"], silent=[False, True], n_bins=20)
+    lo, hi = LO6[:d], HI6[:d]
+    for it in range(3):
+        z, lp = g.draw(N, it)
+        zo, lpo = o.draw(N, it)
+        st = g.get_state()
+        assert st["alloc"][:2].tolist() == [N // 2, N // 2] == o.alloc.tolist()
+        zg = z.cpu().numpy()
+        assert np.array_equal(zg, zo)
+        np.testing.assert_allclose(lp.cpu().numpy(), lpo, rtol=0, atol=1e-10)
+        lnw = _gauss_lnw(zg, lo, hi, width=0.1) - lpo
+        o.update(zo, lnw, lpo)
+        g.update(z, _dev(torch, lnw), _dev(torch, lpo))
+        st = g.get_state()
+        assert np.array_equal(st["members"][0]["H"], o.members[0].H)          # trained on the silent samples too
+        assert st["W"][:2].tolist() == [1.0, 0.0]
+    # free-running step on a built-in integrand: n_samples = contributing samples; the estimate matches the closed form
+    f = Integrand.gaussian_mix([[3.0, 0.0, 1.5]], [0.3], [0.0])
+    g2 = _make(ile, "PORTFOLIO", d, N, members=("AC", "UNIFORM"), silent=[False, True], n_bins=40)
+    for it in range(8):
+        r = result_from_device(g2.step_integrand(f, N, it))
+    assert r["n_samples"] == N - N // 2 and r["cum_n_samples"] == 8 * (N - N // 2)
+    exact = (0.3 * math.sqrt(2 * math.pi)) ** 3                              # the Gaussian sits well inside the box
+    assert abs(math.exp(float(r["cum_ln_integral"])) / exact - 1) < 5 * math.sqrt(float(r["cum_rel_variance"])) + 5e-3
+
+
+def test_integrator_option_validation(env):
+    from paper_2505_11655_b200 import IleError
+    torch, ile, _ = env
+    with pytest.raises(IleError):
+        _make(ile, "PORTFOLIO", 3, 1000, members=("AC", "AC"), first_iter=[1, 0])        # member 0 is always active
+    with pytest.raises(IleError):
+        _make(ile, "PORTFOLIO", 3, 1000, members=("AC", "UNIFORM", "AC"), silent=[False, True, False])   # silent members last
+    with pytest.raises(IleError):
+        _make(ile, "AC", 6, 1000, n_bins=2000)                                            # d * n_bins beyond the histogram kernel's shared memory
+    with pytest.raises(IleError):
+        _make(ile, "UNIFORM", 3, (1 << 24) + 1)                                           # fixed-point sums could overflow
