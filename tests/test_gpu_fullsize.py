@@ -13,6 +13,38 @@ def _tol(ref):
     return 1e-9 * np.maximum(1.0, np.abs(ref))
 
 
+def _strata(prob, z, rng, n_random=192):
+    """Indices of the batch to compare with the oracle, chosen where the fused kernel's full-size paths are
+    (DESIGN.md section 6): it orders the samples by the cell (16 stored bins per detector) of their first-bin
+    indices n_k = floor((t_lo + tau_k - t_Q0) fs) and cuts the order into tiles at every multiple of 128 and at every
+    cell change.  Taken: every sample of the first and of the last tile of the order, of the three smallest (ragged)
+    tiles and of the tile with the widest spread of n_k; the samples with the extreme n_k of each detector; the
+    samples nearest the edges of the prior box; and a random set."""
+    from oracle import likelihood as lk
+    N = z.shape[1]
+    ang = lk.z_to_angles(np.clip(z, prob.lo[:, None], prob.hi[:, None]))         # GMM draws may leave the box (lnL = -inf there)
+    _, _, tau = lk.antenna(prob.D, prob.pos, prob.gmst, ang[0], ang[1], ang[2])
+    n = np.floor((prob.t_lo + tau - prob.t_Q0) * prob.fs).astype(np.int64)               # [K, N]
+    inbox = np.all((z >= prob.lo[:, None]) & (z < prob.hi[:, None]), axis=0)
+    cell = (n - n.min()) >> 4
+    key = np.where(inbox, 0, 1 << 40)
+    for k in range(prob.K):
+        key = key * 4096 + np.where(inbox, cell[k], 0)
+    order = np.argsort(key, kind="stable")
+    ks = key[order]
+    start = np.nonzero((np.arange(N) % 128 == 0) | (np.r_[True, ks[1:] != ks[:-1]]))[0]
+    cnt = np.diff(np.r_[start, N])
+    spread = np.array([(n[:, order[s:s + c]].max(axis=1) - n[:, order[s:s + c]].min(axis=1)).max() for s, c in zip(start, cnt)])
+    tiles = {0, len(start) - 1, int(np.argmax(spread))} | set(np.argsort(cnt, kind="stable")[:3].tolist())
+    pick = [order[start[t]:start[t] + cnt[t]] for t in tiles]
+    for k in range(prob.K):
+        pick.append(np.array([np.argmin(np.where(inbox, n[k], 1 << 30)), np.argmax(np.where(inbox, n[k], -1))]))
+    y = (z - prob.lo[:, None]) / (prob.hi - prob.lo)[:, None]
+    pick.append(np.argsort(np.minimum(y, 1 - y).min(axis=0))[:32])                          # nearest the box edges
+    pick.append(rng.choice(N, size=n_random, replace=False))
+    return np.unique(np.concatenate(pick))
+
+
 @pytest.mark.parametrize("cfg,P,n_iter", [(2, 1, 3), (3, 1, 3), (4, 3, 1), (5, 1, 3)])
 def test_full_batch_sampled_parity(cfg, P, n_iter):
     import torch
@@ -31,7 +63,8 @@ def test_full_batch_sampled_parity(cfg, P, n_iter):
         for it in range(n_iter):
             res = result_from_device(g.step(p, N, it))[0]
             z, lp, lnL, lnw = g.last_batch(N)
-            idx = np.sort(rng.choice(N, size=192, replace=False))
+            idx = _strata(prob, z.cpu().numpy(), rng)
+            assert len(idx) >= 300
             tidx = torch.from_numpy(idx).cuda()
             zs = z[:, tidx].cpu().numpy()
             got = lnL[tidx].cpu().numpy()

@@ -56,6 +56,35 @@ def test_precompute_parity_and_lnL_from_it(lmax, K, N_f, P):
     assert np.all(np.abs(got - ref) <= 1e-9 * np.maximum(1.0, np.abs(ref))), np.abs(got - ref).max()
 
 
+def test_precompute_parity_at_the_bench_shape():
+    """The shape bench.py --precompute times (M = 21, K = 3, N_f = 32768, N_Q = 1024: the eight-column FFT
+    instantiation and the tiled U/V grid), P = 2.  The oracle's Q is O(N_Q N_f K M): compared on two 32-bin windows
+    (the first stored bins and the last), U and V in full."""
+    import torch
+    from paper_2505_11655_b200 import Ile
+    from oracle.precompute import precompute_q, precompute_uv
+    fs, N_f, K, P, N_Q = 4096.0, 32768, 3, 2, 1024
+    ell, m = make_modes(4)
+    M = len(ell)
+    D, pos = make_network(K, np.random.Generator(np.random.Philox(99)))
+    h, d, S, df = make_spectra(K, ell, m, N_f, fs, seed=77, P=P)
+    f_low, n0 = 20.0, -(N_Q // 2)
+    ile = Ile(0)
+    ile.set_network(D, pos, 0.0)
+    ile.set_modes(ell, m)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    ile.precompute_quv(dev(h), dev(d), dev(S), df, f_low, n0 / fs, N_Q, D_ref=500.0)
+    for p in range(P):
+        Q, U, V = ile.get_quv(p, K, M, N_Q)
+        rU, rV = precompute_uv(h[p], S, df, f_low)
+        _close(U, rU, 1e-12)
+        _close(V, rV, 1e-12)
+        scale = np.abs(Q).max()
+        for first in (0, N_Q // 2 - 16, N_Q - 32):
+            rQ = precompute_q(h[p], d, S, df, f_low, (n0 + first) / fs, 32)
+            assert np.all(np.abs(Q[:, :, first:first + 32] - rQ) <= 1e-11 * scale), np.abs(Q[:, :, first:first + 32] - rQ).max() / scale
+
+
 def test_precompute_argument_errors():
     import torch
     from paper_2505_11655_b200 import Ile, IleError
