@@ -304,25 +304,30 @@ class AV:
 
 # =============================================================================== GMM
 class GMM:
-    """Gaussian-mixture sampling prior in all d dimensions, one weighted EM
-    step per batch (G26).  Not bit-exact (exp / log / sincos); compared to 1e-10 relative."""
+    """Gaussian-mixture sampling prior ("Gaussian mixture models (GMMs) to generate sampling priors
+    for any user-specified subset of dimensions"), one weighted EM step per batch (G26).  `dims` = the modelled
+    dimensions (default: all d); the others are sampled uniformly over the box and their density factor is
+    1/(hi - lo) inside it, 0 outside (reading G43).  Not bit-exact (exp / log / sincos); compared to 1e-10 relative."""
     kind = "GMM"
     REG = 1.0e-6
 
-    def __init__(self, lo, hi, seed, n_comp=8):
+    def __init__(self, lo, hi, seed, n_comp=8, dims=None):
         self.lo = np.asarray(lo, dtype=np.float64)
         self.hi = np.asarray(hi, dtype=np.float64)
         self.d = len(lo)
+        self.dims = list(range(self.d)) if dims is None else sorted(int(c) for c in dims)
+        self.other = [c for c in range(self.d) if c not in self.dims]
+        self.gd = len(self.dims)
         self.seed = seed
         self.C = int(n_comp)
         u = uniforms(seed, np.arange(self.C, dtype=np.uint64), 0xFFFFFFFF, self.d)
         self.omega = np.full(self.C, 1.0 / self.C)
-        self.mu = (self.lo[:, None] + u * (self.hi - self.lo)[:, None]).T.copy()     # [C, d]
-        self.Sigma = np.stack([np.diag((0.5 * (self.hi - self.lo)) ** 2) for _ in range(self.C)])
+        self.mu = (self.lo[:, None] + u * (self.hi - self.lo)[:, None]).T[:, self.dims].copy()     # [C, gd]
+        self.Sigma = np.stack([np.diag((0.5 * (self.hi - self.lo)[self.dims]) ** 2) for _ in range(self.C)])
         self._chol()
 
     def _chol(self):
-        d = self.d
+        d = self.gd
         self.L = np.zeros((self.C, d, d))
         for c in range(self.C):
             S = self.Sigma[c]
@@ -335,15 +340,16 @@ class GMM:
                     L[i, j] = math.sqrt(s) if i == j else s / L[j, j]
 
     def _ln_comp(self, z):
-        """ln N(z; mu_c, Sigma_c) for every component: [C, N]."""
-        d = self.d
+        """ln N(z_dims; mu_c, Sigma_c) for every component: [C, N]."""
+        d = self.gd
+        zg = z[self.dims]
         N = z.shape[1]
         out = np.empty((self.C, N))
         for c in range(self.C):
             L = self.L[c]
             y = np.empty((d, N))
             for i in range(d):                                 # forward substitution L y = z - mu
-                s = z[i] - self.mu[c, i]
+                s = zg[i] - self.mu[c, i]
                 for k in range(i):
                     s = s - L[i, k] * y[k]
                 y[i] = s / L[i, i]
@@ -358,12 +364,20 @@ class GMM:
     def ln_pdf(self, z):
         e = self._ln_comp(z) + np.log(self.omega)[:, None]
         mx = e.max(axis=0)
-        return mx + np.log(np.exp(e - mx).sum(axis=0))
+        out = mx + np.log(np.exp(e - mx).sum(axis=0))
+        if self.other:                                         # uniform factor of the dimensions the mixture leaves alone
+            lnu = 0.0
+            ok = np.ones(z.shape[1], dtype=bool)
+            for c in self.other:
+                lnu = lnu + math.log(self.hi[c] - self.lo[c])
+                ok &= (z[c] >= self.lo[c]) & (z[c] < self.hi[c])
+            out = np.where(ok, out - lnu, -np.inf)
+        return out
 
     def draw(self, N, g, i0=0):
-        d = self.d
+        d = self.gd
         npair = (d + 1) // 2
-        u = uniforms(self.seed, i0 + np.arange(N, dtype=np.uint64), g, 2 + 2 * npair)
+        u = uniforms(self.seed, i0 + np.arange(N, dtype=np.uint64), g, 2 + 2 * npair + len(self.other))
         cw = np.cumsum(self.omega)
         comp = np.minimum(np.searchsorted(cw, u[0], side="right"), self.C - 1)
         nrm = np.empty((2 * npair, N))
@@ -372,16 +386,18 @@ class GMM:
             ang = 2.0 * math.pi * u[3 + 2 * p]
             nrm[2 * p] = r * np.cos(ang)
             nrm[2 * p + 1] = r * np.sin(ang)
-        z = np.empty((d, N))
+        z = np.empty((self.d, N))
         for i in range(d):
             s = self.mu[comp, i]
             for k in range(i + 1):
                 s = s + self.L[comp, i, k] * nrm[k]
-            z[i] = s
+            z[self.dims[i]] = s
+        for q, c in enumerate(self.other):                     # the other dimensions: uniform over the box, as Uniform.draw
+            zc = self.lo[c] + u[2 + 2 * npair + q] * (self.hi[c] - self.lo[c])
+            z[c] = np.minimum(zc, _below(self.hi[c], self.lo[c]))
         return z, self.ln_pdf(z)
 
     def update(self, z, lnw, ln_ps=None):
-        d = self.d
         lnw = np.asarray(lnw, dtype=np.float64)
         ok = np.isfinite(lnw) & in_box(z, self.lo, self.hi)
         if not ok.any():
@@ -397,11 +413,12 @@ class GMM:
         if not (s0.sum() > 0.0):
             return
         new_omega = s0 / s0.sum()
-        rng2 = (self.hi - self.lo) ** 2
+        rng2 = ((self.hi - self.lo) ** 2)[self.dims]
+        zg = z[self.dims]
         for c in range(self.C):
             if not (s0[c] > 1.0e-300):
                 continue                                       # dead component: keep it
-            dz = z - self.mu[c][:, None]                       # shifted moments about the old mean
+            dz = zg - self.mu[c][:, None]                      # shifted moments about the old mean
             s1 = (a[c][None, :] * dz).sum(axis=1)
             s2 = np.einsum("n,in,jn->ij", a[c], dz, dz)
             mean = s1 / s0[c]
@@ -539,7 +556,7 @@ def make_integrator(kind, lo, hi, seed, **o):
     if kind == "AV":
         return AV(lo, hi, seed, o.get("P_thr", 0.999), o.get("N_min_star", 4096))
     if kind == "GMM":
-        return GMM(lo, hi, seed, o.get("n_gmm", 8))
+        return GMM(lo, hi, seed, o.get("n_gmm", 8), o.get("gmm_dims"))
     if kind == "PORTFOLIO":
         names = o.get("members", ["AC", "AV", "GMM"])
         per = o.get("member_opts") or [{}] * len(names)           # options unique to each sampler realization

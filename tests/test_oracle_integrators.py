@@ -413,3 +413,46 @@ def test_portfolio_fig7_two_ac_members_second_from_iteration_10():
     tot = combine(res[12:])
     assert abs(math.exp(tot["ln_integral"]) / exact - 1) < 5 * math.sqrt(tot["rel_variance"]) + 2e-3
     assert tot["n_ess"] > 0.05 * 8 * (1 << 14)
+
+
+# ------------------------------------------------------------------------------- GMM over a subset of dimensions
+def test_gmm_dimension_subset():
+    """`dims` = the modelled dimensions, the others uniform over the box.  Pins: every dimension listed = the default
+    (bit for bit); the density factorises into a lower-dimensional mixture times 1/range and integrates to one;
+    draws in the other dimensions are uniform; the EM step moves the modelled marginal onto the target."""
+    lo, hi = np.array([-3.0, -8.0, 1.0]), np.array([5.0, 8.0, 4.0])
+    full, alld = og.GMM(lo, hi, 9, n_comp=3), og.GMM(lo, hi, 9, n_comp=3, dims=[2, 0, 1])
+    za, la = full.draw(2000, 4)
+    zb, lb = alld.draw(2000, 4)
+    assert np.array_equal(za, zb) and np.array_equal(la, lb)
+    # factorisation: a mixture in dimension 1 only == the one-dimensional mixture with the same parameters / (range_0 range_2)
+    sub = og.GMM(lo, hi, 9, n_comp=3, dims=[1])
+    one = og.GMM(lo[1:2], hi[1:2], 9, n_comp=3)
+    one.omega, one.mu, one.Sigma = sub.omega.copy(), sub.mu.copy(), sub.Sigma.copy()
+    one._chol()
+    z, ln_ps = sub.draw(20000, 0)
+    assert np.array_equal(ln_ps, sub.ln_pdf(z))
+    np.testing.assert_allclose(ln_ps, one.ln_pdf(z[1:2]) - math.log(8.0 * 3.0), rtol=0, atol=1e-13)
+    outside = z.copy()
+    outside[0, :5] = 5.5                                                  # outside the box in a uniform dimension: density 0
+    assert np.all(sub.ln_pdf(outside)[:5] == -np.inf)
+    # the uniform dimensions: inside the box, flat (Kolmogorov-Smirnov), and untouched by the mixture parameters
+    for c in (0, 2):
+        y = (z[c] - lo[c]) / (hi[c] - lo[c])
+        assert y.min() >= 0.0 and y.max() < 1.0 and stats.kstest(y, "uniform").pvalue > 1e-3
+    # normalisation by quadrature over (x0 in the box) x (x1 on a wide grid) at fixed x2
+    g0 = np.linspace(lo[0], hi[0], 401)[:-1] + (hi[0] - lo[0]) / 800
+    g1 = np.linspace(-80.0, 80.0, 8001)[:-1] + 0.01
+    X0, X1 = np.meshgrid(g0, g1, indexing="ij")
+    pdf = np.exp(sub.ln_pdf(np.stack([X0.ravel(), X1.ravel(), np.full(X0.size, 2.0)])))
+    assert abs(pdf.sum() * (hi[0] - lo[0]) / 400 * 0.02 * (hi[2] - lo[2]) - 1.0) < 1e-6
+    # EM on a target that is Gaussian in dimension 1 (mean 2.5, sigma 0.7) and flat elsewhere
+    for g in range(12):
+        z, ln_ps = sub.draw(20000, g + 1)
+        lnw = -0.5 * ((z[1] - 2.5) / 0.7) ** 2 - ln_ps
+        lnw = np.where(og.in_box(z, lo, hi), lnw, -np.inf)
+        sub.update(z, lnw, ln_ps)
+    mean = float((sub.omega * sub.mu[:, 0]).sum())
+    var = float((sub.omega * (sub.Sigma[:, 0, 0] + (sub.mu[:, 0] - mean) ** 2)).sum())
+    assert abs(mean - 2.5) < 0.05 and abs(math.sqrt(var) - 0.7) < 0.08
+    assert sub.mu.shape == (3, 1) and sub.Sigma.shape == (3, 1, 1)
