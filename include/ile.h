@@ -224,7 +224,7 @@ int ile_integrator_last_batch(ile_integrator *it, const double **z, const double
  *   header  int64 kind, d
  *   AC      int64 n_bins; uint64 H[d][n_bins]; double pi[d][n_bins]; double cdf[d][n_bins+1]
  *   AV      int64 n, C, N_min; double L_thr; uint64 keys[C]
- *   GMM     int64 n_comp; double omega[C], mu[C][d], Sigma[C][d][d], L[C][d][d]
+ *   GMM     int64 n_comp, gd (modelled dimensions); double omega[C], mu[C][gd], Sigma[C][gd][gd], L[C][gd][gd]
  *   PORTF.  int64 n_members; double W[8]; int64 frozen[8]; int64 alloc[8]; int64 active[8];
  *           then per member: int64 bytes_m, followed by that member's blob (with header)
  *   UNIFORM nothing more */

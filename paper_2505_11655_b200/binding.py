@@ -299,8 +299,8 @@ def parse_state(blob: bytes):
             n, Cn, N_min = (int(v) for v in i64(3))
             out.update(n=n, C=Cn, N_min=N_min, L_thr=float(arr("<f8", 1)[0]), keys=arr("<u8", Cn))
         elif kind == KINDS["GMM"]:
-            Cn = int(i64()[0])
-            out.update(n_comp=Cn, omega=arr("<f8", Cn), mu=arr("<f8", Cn, d), Sigma=arr("<f8", Cn, d, d), L=arr("<f8", Cn, d, d))
+            Cn, gd = int(i64()[0]), int(i64()[0])
+            out.update(n_comp=Cn, gd=gd, omega=arr("<f8", Cn), mu=arr("<f8", Cn, gd), Sigma=arr("<f8", Cn, gd, gd), L=arr("<f8", Cn, gd, gd))
         return out
 
     kind, d = (int(v) for v in np.frombuffer(buf, dtype="<i8", count=2, offset=0))
@@ -328,7 +328,7 @@ def pack_state(st: dict) -> bytes:
             parts += [np.array([m["n"], len(keys), m.get("N_min", 0)], dtype="<i8").tobytes(),
                       np.array([m.get("L_thr", -np.inf)], dtype="<f8").tobytes(), keys.tobytes()]
         elif m["kind"] == KINDS["GMM"]:
-            parts += [np.array([len(m["omega"])], dtype="<i8").tobytes()]
+            parts += [np.array([len(m["omega"]), np.asarray(m["mu"]).shape[1]], dtype="<i8").tobytes()]
             parts += [np.ascontiguousarray(m[k], dtype="<f8").tobytes() for k in ("omega", "mu", "Sigma", "L")]
         return b"".join(parts)
 

@@ -76,6 +76,10 @@ struct IntegDev {
     long long N_min_star, n_max;
     SamplerDev mem[ILE_MAX_MEMBERS];
     int first_iter[ILE_MAX_MEMBERS], silent[ILE_MAX_MEMBERS];   // portfolio options
+    // GMM over a subset of the dimensions (reading G43): gd modelled dimensions gdim[0..gd), the other
+    // d - gd dimensions udim[] are uniform over the box; ln_uvol = sum of ln(hi - lo) over them
+    int gd, gdim[ILE_MAX_D], udim[ILE_MAX_D];
+    double ln_uvol;
     PortState* port;
 };
 

@@ -61,7 +61,7 @@ static ArenaPlan plan_arena(const IntegDev& I) {
             A.pi[a] = off; off = align256(off + (size_t)I.d * nb * 8);
             A.cdf[a] = off; off = align256(off + (size_t)I.d * (nb + 1) * 8);
         }
-        if (k == ILE_KIND_GMM) { A.gmm[a] = off; off = align256(off + gmm_doubles(I.n_gmm, I.d) * 8); }
+        if (k == ILE_KIND_GMM) { A.gmm[a] = off; off = align256(off + gmm_doubles(I.n_gmm, I.gd) * 8); }
     }
     A.total = off;
     return A;
@@ -112,7 +112,7 @@ static void fill_initial(const IntegDev& I, const ArenaPlan& A, unsigned char* h
             }
         }
         if (k == ILE_KIND_GMM) {
-            const int C = I.n_gmm, d = I.d;
+            const int C = I.n_gmm, d = I.gd;                         // modelled dimensions only
             double* omega = (double*)(h + A.gmm[a]);
             double* mu = omega + C;
             double* Sigma = mu + C * d;
@@ -120,9 +120,10 @@ static void fill_initial(const IntegDev& I, const ArenaPlan& A, unsigned char* h
             for (int c = 0; c < C; c++) {
                 omega[c] = 1.0 / (double)C;
                 for (int i = 0; i < d; i++) {
-                    const double u = uniform_host(I.seed, (uint64_t)c, 0xFFFFFFFFu, i);
-                    mu[c * d + i] = I.lo[i] + u * (I.hi[i] - I.lo[i]);
-                    const double hw = 0.5 * (I.hi[i] - I.lo[i]);
+                    const int dim = I.gdim[i];                        // the uniform of that dimension, as with every dimension modelled
+                    const double u = uniform_host(I.seed, (uint64_t)c, 0xFFFFFFFFu, dim);
+                    mu[c * d + i] = I.lo[dim] + u * (I.hi[dim] - I.lo[dim]);
+                    const double hw = 0.5 * (I.hi[dim] - I.lo[dim]);
                     Sigma[c * d * d + i * d + i] = hw * hw;
                 }
                 host_chol(d, Sigma + c * d * d, L + c * d * d);
@@ -261,6 +262,7 @@ extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o,
     if (has_av && (!(o->P_thr > 0.0 && o->P_thr <= 1.0) || o->N_min_star < 1))
         return ile_fail(ctx, ILE_EINVAL, "integrator_create: AV needs P_thr in (0,1], N_min_star >= 1");
     if (has_gmm && (o->n_gmm < 1 || o->n_gmm > 16)) return ile_fail(ctx, ILE_EINVAL, "integrator_create: n_gmm in 1..16");
+    if (o->gmm_dims_mask >> o->d) return ile_fail(ctx, ILE_EINVAL, "integrator_create: gmm_dims_mask names a dimension >= d");
 
     ile_integrator* it = (ile_integrator*)calloc(1, sizeof(ile_integrator));
     if (!it) return ile_fail(ctx, ILE_ENOMEM, "integrator_create: out of host memory");
@@ -282,6 +284,20 @@ extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o,
         I.V0 = I.V0 * (o->hi[c] - o->lo[c]);
     }
     I.seed = o->seed; I.eps = o->eps; I.beta = o->beta; I.P_thr = o->P_thr; I.N_min_star = o->N_min_star;
+    {   // the mixture models the dimensions of the mask (0 = all), the others are uniform over the box
+        const unsigned mask = o->gmm_dims_mask ? o->gmm_dims_mask : (1u << o->d) - 1u;
+        int nu = 0;
+        I.gd = 0;
+        I.ln_uvol = 0.0;
+        for (int c = 0; c < ILE_MAX_D; c++) { I.gdim[c] = -1; I.udim[c] = -1; }
+        for (int c = 0; c < o->d; c++) {
+            if ((mask >> c) & 1u) I.gdim[I.gd++] = c;
+            else {
+                I.udim[nu++] = c;
+                I.ln_uvol = I.ln_uvol + log(o->hi[c] - o->lo[c]);
+            }
+        }
+    }
     I.n_max = av_n_max_host(o->d);
     for (int a = 0; a < Ns; a++) I.mem[a].kind = kinds[a];
 
@@ -557,7 +573,7 @@ static size_t member_blob_bytes(const IntegDev& I, int a, long long C_av) {
     switch (I.mem[a].kind) {
         case ILE_KIND_AC: b += 8 + (size_t)I.d * I.mem[a].nb * 16 + (size_t)I.d * (I.mem[a].nb + 1) * 8; break;
         case ILE_KIND_AV: b += 32 + (size_t)C_av * 8; break;
-        case ILE_KIND_GMM: b += 8 + gmm_doubles(I.n_gmm, I.d) * 8; break;
+        case ILE_KIND_GMM: b += 16 + gmm_doubles(I.n_gmm, I.gd) * 8; break;
         default: break;
     }
     return b;
@@ -610,7 +626,8 @@ extern "C" int ile_integrator_get_state(ile_integrator* it, void* buf, size_t* b
             if (put_dev(S.keys, (size_t)av[a].C * 8)) return 1;
         } else if (S.kind == ILE_KIND_GMM) {
             put_i64(I.n_gmm);
-            if (put_dev(S.gmm, gmm_doubles(I.n_gmm, I.d) * 8)) return 1;
+            put_i64(I.gd);
+            if (put_dev(S.gmm, gmm_doubles(I.n_gmm, I.gd) * 8)) return 1;
         }
         return 0;
     };
@@ -698,8 +715,9 @@ extern "C" int ile_integrator_set_state(ile_integrator* it, const void* buf, siz
         }
         if (S.kind == ILE_KIND_GMM) {
             long long C;
-            if (!get_i64(&C) || C != I.n_gmm) return false;
-            if (!get_dev(S.gmm, gmm_doubles(I.n_gmm, I.d) * 8)) return false;
+            long long gd;
+            if (!get_i64(&C) || C != I.n_gmm || !get_i64(&gd) || gd != I.gd) return false;
+            if (!get_dev(S.gmm, gmm_doubles(I.n_gmm, I.gd) * 8)) return false;
             if (!dry && integ_gmm_refresh(it, a) != ILE_OK) return false;     // Cholesky factors from the restored Sigma, not from the blob
             return true;
         }

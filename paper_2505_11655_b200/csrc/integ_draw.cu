@@ -45,7 +45,7 @@ __device__ __forceinline__ double ln_pdf_av(const IntegDev& I, const SamplerDev&
 // The densities below are bit-identical to evaluating these logarithms in place.
 #define GMM_GC 32
 __device__ __forceinline__ void gmm_consts(const IntegDev& I, const double* g, double* gc, int t, int nt) {
-    const int d = I.d, C = I.n_gmm;
+    const int d = I.gd, C = I.n_gmm;
     const double* L = g + C + C * d + C * d * d;
     for (int c = t; c < C; c += nt) {
         double lndet = 0.0;
@@ -56,13 +56,35 @@ __device__ __forceinline__ void gmm_consts(const IntegDev& I, const double* g, d
 }
 
 // ln N(z; mu_c, Sigma_c) + ln omega_c for every component; returns the log-sum-exp
+// the modelled coordinates of a sample, in the mixture's order (static register indices: gdim is matched, not indexed)
+template <int D>
+__device__ __forceinline__ void gmm_gather(const IntegDev& I, const double* zz, double* zg) {
+#pragma unroll
+    for (int r = 0; r < D; r++) {
+        zg[r] = 0.0;
+#pragma unroll
+        for (int c = 0; c < D; c++)
+            if (I.gdim[r] == c) zg[r] = zz[c];
+    }
+}
+
 template <int D>
 __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev& S, const double* zz, double* e_out, const double* gc) {
-    constexpr int d = D;
+    const int d = I.gd;
     const int C = I.n_gmm;
     const double* omega = S.gmm;
     const double* mu = omega + C;
     const double* L = mu + C * d + C * d * d;
+    double zg[D];
+    gmm_gather<D>(I, zz, zg);
+    bool uok = true;                       // the dimensions the mixture leaves alone: uniform over the box, zero outside
+#pragma unroll
+    for (int q = 0; q < D; q++)
+        if (q < D - d) {
+#pragma unroll
+            for (int c = 0; c < D; c++)
+                if (I.udim[q] == c) uok = uok && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
+        }
     double e[16];
     double mx = neg_inf();
     for (int c = 0; c < C; c++) {
@@ -70,13 +92,14 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
         double y[D];
         double quad = 0.0;
 #pragma unroll
-        for (int i = 0; i < d; i++) {
-            double s = zz[i] - mu[c * d + i];
+        for (int i = 0; i < D; i++)
+            if (i < d) {
+                double s = zg[i] - mu[c * d + i];
 #pragma unroll
-            for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
-            y[i] = s / Lc[i * d + i];
-            quad = quad + y[i] * y[i];
-        }
+                for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
+                y[i] = s / Lc[i * d + i];
+                quad = quad + y[i] * y[i];
+            }
         e[c] = -0.5 * quad - gc[c] - 0.5 * d * log(TWO_PI) + gc[16 + c];
         mx = fmax(mx, e[c]);
     }
@@ -84,7 +107,9 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
     for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
     if (e_out)
         for (int c = 0; c < C; c++) e_out[c] = e[c];
-    return mx + log(sum);
+    const double out = mx + log(sum);
+    if (d == D) return out;
+    return uok ? out - I.ln_uvol : neg_inf();
 }
 
 template <int D>
@@ -200,10 +225,10 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
     double u0, u1;
     philox_pair(I.seed, (unsigned long long)i, g, 0u, &u0, &u1);
     if (S.kind == ILE_KIND_GMM) {
-        const int C = I.n_gmm;
+        const int C = I.n_gmm, gd = I.gd;
         const double* omega = S.gmm;
         const double* mu = omega + C;
-        const double* L = mu + C * d + C * d * d;
+        const double* L = mu + C * gd + C * gd * gd;
         int comp = 0;
         double cw = 0.0;
         for (int c = 0; c < C; c++) {     // number of cumulative weights <= u0
@@ -212,24 +237,47 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
         }
         if (comp > C - 1) comp = C - 1;
         double nrm[D + 1];
-        constexpr int npair = (d + 1) / 2;
+        const int npair = (gd + 1) / 2;
 #pragma unroll
-        for (int p = 0; p < npair; p++) {
-            double ua, ub;
-            philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + p), &ua, &ub);
-            const double r = sqrt(-2.0 * log(1.0 - ua));
-            double sn, cs;
-            sincos(TWO_PI * ub, &sn, &cs);
-            nrm[2 * p] = r * cs;
-            nrm[2 * p + 1] = r * sn;
-        }
+        for (int p = 0; p < (D + 1) / 2; p++)
+            if (p < npair) {
+                double ua, ub;
+                philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + p), &ua, &ub);
+                const double r = sqrt(-2.0 * log(1.0 - ua));
+                double sn, cs;
+                sincos(TWO_PI * ub, &sn, &cs);
+                nrm[2 * p] = r * cs;
+                nrm[2 * p + 1] = r * sn;
+            }
+        double zg[D];
 #pragma unroll
-        for (int r = 0; r < d; r++) {
-            double s = mu[comp * d + r];
+        for (int r = 0; r < D; r++)
+            if (r < gd) {
+                double s = mu[comp * gd + r];
 #pragma unroll
-            for (int k = 0; k <= r; k++) s = s + L[comp * d * d + r * d + k] * nrm[k];
-            zz[r] = s;
-        }
+                for (int k = 0; k <= r; k++) s = s + L[comp * gd * gd + r * gd + k] * nrm[k];
+                zg[r] = s;
+            }
+        // scatter to the modelled dimensions; the others are uniform over the box (streams after the Box-Muller pairs)
+#pragma unroll
+        for (int c = 0; c < D; c++) zz[c] = 0.0;
+#pragma unroll
+        for (int r = 0; r < D; r++)
+            if (r < gd) {
+#pragma unroll
+                for (int c = 0; c < D; c++)
+                    if (I.gdim[r] == c) zz[c] = zg[r];
+            }
+        double ua = 0.0, ub = 0.0;
+#pragma unroll
+        for (int q = 0; q < D; q++)
+            if (q < D - gd) {
+                if ((q & 1) == 0) philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + npair + (q >> 1)), &ua, &ub);
+                const double u = (q & 1) ? ub : ua;
+#pragma unroll
+                for (int c = 0; c < D; c++)
+                    if (I.udim[q] == c) zz[c] = fmin(__dadd_rn(I.lo[c], __dmul_rn(u, __dsub_rn(I.hi[c], I.lo[c]))), I.below_hi[c]);
+            }
     } else {
         unsigned long long key = 0;
         long long n = 1;

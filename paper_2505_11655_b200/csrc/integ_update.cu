@@ -475,8 +475,8 @@ __global__ void av_commit_kernel(IntegDev I, int a, UpdScratch* us) {
 // gc: per-component constants in shared memory (gc[c] = sum_i ln L_c[i][i], gc[16 + c] = ln omega_c), computed
 // once per block; bit-identical to evaluating the logarithms per sample
 template <int D>
-__device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g, const double* zz, double* e, const double* gc) {
-    constexpr int d = D;
+__device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g, const double* zg, double* e, const double* gc) {
+    const int d = I.gd;                      // modelled dimensions (zg: their coordinates, in the mixture's order)
     const int C = I.n_gmm;
     const double* omega = g;
     const double* mu = omega + C;
@@ -487,13 +487,14 @@ __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g
         double y[D];
         double quad = 0.0;
 #pragma unroll
-        for (int i = 0; i < d; i++) {
-            double s = zz[i] - mu[c * d + i];
+        for (int i = 0; i < D; i++)
+            if (i < d) {
+                double s = zg[i] - mu[c * d + i];
 #pragma unroll
-            for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
-            y[i] = s / Lc[i * d + i];
-            quad = quad + y[i] * y[i];
-        }
+                for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
+                y[i] = s / Lc[i * d + i];
+                quad = quad + y[i] * y[i];
+            }
         e[c] = -0.5 * quad - gc[c] - 0.5 * d * log(6.283185307179586) + gc[16 + c];
         mx = fmax(mx, e[c]);
     }
@@ -506,7 +507,7 @@ template <int D>
 __global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ lnw,
                                                        const UpdScratch* __restrict__ us, double* __restrict__ aw) {
     if (us->abort || us->n_valid == 0) return;
-    constexpr int d = D;
+    const int d = I.gd;
     const int C = I.n_gmm;
     const double* g = I.mem[a].gmm;
     __shared__ double gc[32];
@@ -524,7 +525,8 @@ __global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N,
         const bool ok = is_finite_d(w) && in_box_dev(I, z, N, i);
         double zz[D], e[16];
 #pragma unroll
-        for (int c = 0; c < d; c++) zz[c] = z[(long long)c * N + i];
+        for (int c = 0; c < D; c++)
+            if (c < d) zz[c] = z[(long long)I.gdim[c] * N + i];
         double mx = 0.0, sum = 1.0;
         if (ok) {
             mx = ln_comp_all<D>(I, g, zz, e, gc);
@@ -542,11 +544,11 @@ __global__ void __launch_bounds__(256) gmm_moments_kernel(IntegDev I, int a, int
                                                           const UpdScratch* __restrict__ us, double* __restrict__ part) {
     if (us->abort || us->n_valid == 0) return;
     constexpr int NACC = 1 + D + D * (D + 1) / 2;
-    const int C = I.n_gmm, comp = blockIdx.y;
-    const double* mu = I.mem[a].gmm + C + comp * D;
+    const int C = I.n_gmm, comp = blockIdx.y, gd = I.gd;
+    const double* mu = I.mem[a].gmm + C + comp * gd;
     double mu_r[D];
 #pragma unroll
-    for (int r = 0; r < D; r++) mu_r[r] = mu[r];
+    for (int r = 0; r < D; r++) mu_r[r] = r < gd ? mu[r] : 0.0;
     double acc[NACC];
 #pragma unroll
     for (int q = 0; q < NACC; q++) acc[q] = 0.0;
@@ -556,9 +558,9 @@ __global__ void __launch_bounds__(256) gmm_moments_kernel(IntegDev I, int a, int
         if (wgt == 0.0) continue;
         double dz[D];
 #pragma unroll
-        for (int r = 0; r < D; r++) dz[r] = z[(long long)r * N + i] - mu_r[r];
+        for (int r = 0; r < D; r++) dz[r] = r < gd ? z[(long long)I.gdim[r] * N + i] - mu_r[r] : 0.0;
         acc[0] += wgt;
-        int q = 1 + D;
+        int q = 1 + D;                      // accumulator layout by the total dimension D (static indices); entries past gd stay 0
 #pragma unroll
         for (int r = 0; r < D; r++) {
             const double t = wgt * dz[r];
@@ -594,8 +596,8 @@ __device__ void gmm_chol_dev(int d, const double* S, double* L) {
 
 __global__ void gmm_finish_kernel(IntegDev I, int a, const UpdScratch* __restrict__ us, const double* __restrict__ part, int blocks) {
     if (us->abort || us->n_valid == 0) return;
-    const int d = I.d, C = I.n_gmm, c = threadIdx.x;
-    const int nacc = 1 + d + d * (d + 1) / 2;
+    const int d = I.gd, dt = I.d, C = I.n_gmm, c = threadIdx.x;
+    const int nacc = 1 + dt + dt * (dt + 1) / 2;             // the moments kernel lays its accumulators out by the total dimension
     double* g = I.mem[a].gmm;
     double* omega = g;
     double* mu = omega + C;
@@ -623,12 +625,11 @@ __global__ void gmm_finish_kernel(IntegDev I, int a, const UpdScratch* __restric
     if (acc[0] > 1.0e-300) {
         double mean[ILE_MAX_D];
         for (int r = 0; r < d; r++) mean[r] = acc[1 + r] / acc[0];
-        int q = 1 + d;
         for (int r = 0; r < d; r++)
             for (int s = 0; s <= r; s++) {
-                double v = acc[q++] / acc[0] - mean[r] * mean[s];
+                double v = acc[1 + dt + r * (r + 1) / 2 + s] / acc[0] - mean[r] * mean[s];
                 if (r == s) {
-                    const double rg = I.hi[r] - I.lo[r];
+                    const double rg = I.hi[I.gdim[r]] - I.lo[I.gdim[r]];
                     v = v + 1.0e-6 * (rg * rg);
                 }
                 Sigma[c * d * d + r * d + s] = v;
@@ -641,7 +642,7 @@ __global__ void gmm_finish_kernel(IntegDev I, int a, const UpdScratch* __restric
 }
 
 __global__ void gmm_chol_kernel(IntegDev I, int a) {
-    const int d = I.d, C = I.n_gmm, c = threadIdx.x;
+    const int d = I.gd, C = I.n_gmm, c = threadIdx.x;
     if (c >= C) return;
     double* Sigma = I.mem[a].gmm + C + C * d;
     gmm_chol_dev(d, Sigma + c * d * d, Sigma + C * d * d + c * d * d);

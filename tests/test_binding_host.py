@@ -20,7 +20,7 @@ def _av(d=3, C_=11, seed=1):
 
 def _gmm(d=3, C_=4, seed=2):
     rng = np.random.default_rng(seed)
-    return dict(kind=b.KINDS["GMM"], d=d, n_comp=C_, omega=rng.random(C_), mu=rng.random((C_, d)), Sigma=rng.random((C_, d, d)),
+    return dict(kind=b.KINDS["GMM"], d=d, n_comp=C_, gd=d, omega=rng.random(C_), mu=rng.random((C_, d)), Sigma=rng.random((C_, d, d)),
                 L=rng.random((C_, d, d)))
 
 

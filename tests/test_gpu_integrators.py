@@ -181,6 +181,38 @@ def test_gmm_parity(env):
             np.testing.assert_allclose(st[k], ref, rtol=1e-10, atol=1e-10 * np.abs(ref).max(), err_msg=f"iteration {it}: {k}")
 
 
+def test_gmm_dimension_subset_parity(env):
+    """gmm_dims_mask: the mixture models dimensions {1, 3} of five, the others are uniform over the box."""
+    torch, ile, _ = env
+    N, d, dims = 30011, 5, [1, 3]
+    g = _make(ile, "GMM", d, N, n_gmm=4, gmm_dims=dims)
+    o = _oracle("GMM", d, n_gmm=4, gmm_dims=dims)
+    lo, hi = LO6[:d], HI6[:d]
+    st = g.get_state()
+    assert st["gd"] == 2 and st["mu"].shape == (4, 2)
+    assert np.array_equal(st["mu"], o.mu) and np.array_equal(st["L"], o.L)      # seeded initial state
+    for it in range(3):
+        z, lp = g.draw(N, it)
+        zo, lpo = o.draw(N, it)
+        zg = z.cpu().numpy()
+        np.testing.assert_allclose(zg[dims], zo[dims], rtol=0, atol=1e-10 * np.abs(hi - lo).max())
+        assert np.array_equal(zg[[0, 2, 4]], zo[[0, 2, 4]])                     # the uniform dimensions: bit-exact
+        ref = o.ln_pdf(zg)
+        assert np.array_equal(np.isfinite(ref), np.isfinite(lp.cpu().numpy()))
+        np.testing.assert_allclose(lp.cpu().numpy(), ref, rtol=0, atol=1e-10)
+        out = zg.copy()
+        out[0, :7] = hi[0] + 1.0                                               # outside the box in a uniform dimension: density 0
+        assert np.all(g.ln_pdf(_dev(torch, out)).cpu().numpy()[:7] == -np.inf)
+        lnw = _gauss_lnw(zg, lo, hi, width=0.1) - ref
+        o.update(zg, lnw)
+        g.update(z, _dev(torch, lnw))
+        st = g.get_state()
+        for k, r in (("omega", o.omega), ("mu", o.mu), ("Sigma", o.Sigma), ("L", o.L)):
+            np.testing.assert_allclose(st[k], r, rtol=1e-10, atol=1e-10 * np.abs(r).max(), err_msg=f"iteration {it}: {k}")
+    with pytest.raises(Exception):
+        _make(ile, "GMM", 3, 100, gmm_dims=[4])                                # a dimension >= d
+
+
 def _load_portfolio_state(o, st):
     """Copy a parsed GPU state into the oracle portfolio (teacher forcing: same state in)."""
     o.W = st["W"][:o.Ns].copy()
@@ -400,7 +432,7 @@ def test_portfolio_silent_member_and_estimate(env):
     f = Integrand.gaussian_mix([[3.0, 0.0, 1.5]], [0.3], [0.0])
     g2 = _make(ile, "PORTFOLIO", d, N, members=("AC", "UNIFORM"), silent=[False, True], n_bins=40)
     for it in range(8):
-        r = result_from_device(g2.step_integrand(f, N, it))
+        r = result_from_device(g2.step_integrand(f, N, it))[0]
     assert r["n_samples"] == N - N // 2 and r["cum_n_samples"] == 8 * (N - N // 2)
     exact = (0.3 * math.sqrt(2 * math.pi)) ** 3                              # the Gaussian sits well inside the box
     assert abs(math.exp(float(r["cum_ln_integral"])) / exact - 1) < 5 * math.sqrt(float(r["cum_rel_variance"])) + 5e-3
