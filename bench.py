@@ -52,7 +52,8 @@ KERNEL = "lnl_split_kernel (tcgen05.mma kind::i8 contraction + FP64 epilogue)"
 def flop_per_unit(K, M, N_t):
     """Algorithmic flop of the fused kernel per (sample, time bin): contraction +
     interpolation 2 K (2M + 2), plus the U/V quadratic term (K 6 M(M+1)/2 FMA + 8 M(M+1)/2 flop per
-    sample) spread over the N_t bins.  264 + 25.4 = 289.4 at K = 3, M = 21, N_t = 400."""
+    sample) spread over the N_t bins.  264 + 25.4 = 289.4 at K = 3, M = 21, N_t = 400.  (Steps 1-3, which the
+    kernel now also does - SURVEY 8(d): 45 K + 15 M + 6 K M flop per sample, 2 more per bin - are not counted.)"""
     pairs = M * (M + 1) // 2
     return 2.0 * K * (2 * M + 2) + (2.0 * K * 6 * pairs + 8.0 * pairs) / N_t
 

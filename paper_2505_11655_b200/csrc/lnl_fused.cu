@@ -122,13 +122,15 @@ int ile_launch_fused2(ile_ctx* ctx, const LnlParams& P, int N, const double* rec
 
 int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* z, const int* perm, double* lnL, double* ln_prior) {
     if (P.K > 3 || 2 * P.M > ILE_QT_ROW) return ile_launch_lnL_plain_z(ctx, P, N, z, lnL, ln_prior);
+    // the tcgen05 path (lnl_split.cu) orders by cells of 16 bins, builds its tiles on the device and does steps 1-2 itself;
+    // the DMMA path runs the preparation kernel into per-sample records and Y tiles first
+    const bool split = ctx->lnl_split && perm == nullptr && ile_split_supported(P);
     const int tiles = (N + 63) / 64 * 2;                       // 32-sample sub-tiles, padded to whole 64-sample tiles
-    const size_t rec_bytes = ((size_t)tiles * FT_TS * FT_REC * sizeof(double) + 255) / 256 * 256;
-    const size_t y_bytes = ((size_t)tiles * FT_YM * FT_TS * sizeof(double2) + 255) / 256 * 256;
+    const size_t rec_bytes = split ? 0 : ((size_t)tiles * FT_TS * FT_REC * sizeof(double) + 255) / 256 * 256;
+    const size_t y_bytes = split ? 0 : ((size_t)tiles * FT_YM * FT_TS * sizeof(double2) + 255) / 256 * 256;
+    const size_t uk_bytes = split ? ((size_t)N * 32 + 255) / 256 * 256 : 0;
     const size_t key_bytes = ((size_t)N * 8 + 255) / 256 * 256, val_bytes = ((size_t)N * 4 + 255) / 256 * 256;
     const size_t sort_bytes = (radix_sort_scratch_bytes(N) + 255) / 256 * 256;
-    // the tcgen05 path (lnl_split.cu) orders by cells of 16 bins and builds its tiles on the device
-    const bool split = ctx->lnl_split && perm == nullptr && ile_split_supported(P);
     const bool sort = perm == nullptr && (split || (ctx->sky_sort && N > FT_TS));
     // cells of stored bins over the range of delays the network allows
     const int n_min = ((int)floor((P.t_lo - ctx->max_delay - P.t_Q0) * P.fs) - 1) & ~7;
@@ -137,15 +139,16 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
     const int sp_tiles = split ? ile_split_max_tiles(N, sp_bits, P.K) : 0;
     const size_t tile_bytes = split ? ile_split_tile_bytes(sp_tiles) : 0;
     void* scratch = nullptr;
-    int rc = ile_scratch(ctx, rec_bytes + y_bytes + (sort ? 2 * key_bytes + 2 * val_bytes + sort_bytes + 256 : 0) + tile_bytes, &scratch);
+    int rc = ile_scratch(ctx, rec_bytes + y_bytes + uk_bytes + (sort ? 2 * key_bytes + 2 * val_bytes + sort_bytes + 256 : 0) + tile_bytes, &scratch);
     if (rc) return rc;
     char* base = (char*)scratch;
     double* rec = (double*)base;
     double2* yt = (double2*)(base + rec_bytes);
+    double* uk = (double*)(base + rec_bytes + y_bytes);
     unsigned long long* k0 = nullptr;
     int* ntiles_dev = nullptr;
     if (sort) {
-        char* sb = base + rec_bytes + y_bytes;
+        char* sb = base + rec_bytes + y_bytes + uk_bytes;
         k0 = (unsigned long long*)sb;
         unsigned long long* k1 = (unsigned long long*)(sb + key_bytes);
         unsigned int* v0 = (unsigned int*)(sb + 2 * key_bytes);
@@ -157,7 +160,7 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         int cell_bits = 1;
         if (split) {
             cell_bits = sp_bits;
-            rc = ile_launch_split_keys(ctx, P, N, z, n_min, cell_bits, k0, v0, n_dev, bits_dev, ntiles_dev);
+            rc = ile_launch_split_keys(ctx, P, N, z, n_min, cell_bits, k0, v0, uk, n_dev, bits_dev, ntiles_dev);
             if (rc) return rc;
         } else {
             while ((1 << cell_bits) <= ((n_max - n_min) >> SKY_CELL_SHIFT)) cell_bits++;
@@ -168,18 +171,18 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         if (rc) return rc;
         perm = (const int*)v0;
     }
+    if (split) {
+        char* tb = base + rec_bytes + y_bytes + uk_bytes + 2 * key_bytes + 2 * val_bytes + sort_bytes + 256;
+        SpTile* tl = (SpTile*)tb;
+        int* tstart = (int*)(tb + (size_t)sp_tiles * 32);
+        return ile_launch_split(ctx, P, N, sp_bits, k0, z, uk, perm, lnL, ln_prior, tstart, tl, ntiles_dev);
+    }
     // shared-memory scratch of the harmonics: (2 (max_pow + 1) + 2 (max_abs_m + 1)) doubles per thread
     // ... and a copy of the mode table
     const int scr_d = (2 * (ctx->ylm_max_pow + 1) + 2 * (ctx->ylm_max_abs_m + 1)) * 128;
     const size_t scr = (size_t)scr_d * sizeof(double) + sizeof(YlmTable) + 16;
     lnl_prep3_kernel<<<(tiles * FT_TS + 127) / 128, 128, scr, ctx->stream>>>(P, N, tiles * FT_TS, scr_d, z, perm, rec, yt, ln_prior);
     ILE_LAUNCH_CHECK(ctx);
-    if (split) {
-        char* tb = base + rec_bytes + y_bytes + 2 * key_bytes + 2 * val_bytes + sort_bytes + 256;
-        SpTile* tl = (SpTile*)tb;
-        int* tstart = (int*)(tb + (size_t)sp_tiles * 32);
-        return ile_launch_split(ctx, P, N, sp_bits, k0, rec, yt, perm, lnL, tstart, tl, ntiles_dev);
-    }
     rc = ile_launch_fused2(ctx, P, N, rec, yt, perm, lnL, true);
     if (rc != 1) return rc;
     return ile_launch_lnL_plain_z(ctx, P, N, z, lnL, ln_prior);   // shape without a fused instantiation

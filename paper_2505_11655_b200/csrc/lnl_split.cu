@@ -134,8 +134,8 @@ int ile_split_build_q(ile_ctx* ctx, int P, int K, int M, int N_Q, const double* 
 
 // ---------------------------------------------------------------- delay-cell keys and tiles
 __global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const double* __restrict__ z, int n_min, int cell_bits,
-                                                     unsigned long long* __restrict__ key, unsigned int* __restrict__ val, long long* n_dev,
-                                                     int* bits_dev, int* ntiles_dev) {
+                                                     unsigned long long* __restrict__ key, unsigned int* __restrict__ val, double* __restrict__ uk,
+                                                     long long* n_dev, int* bits_dev, int* ntiles_dev) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) {
         *n_dev = N;
@@ -160,6 +160,7 @@ __global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const d
             const double tau = -(P.pos[kk][0] * n0 + P.pos[kk][1] * n1 + P.pos[kk][2] * n2) / ILE_C_LIGHT;
             double u = (P.t_lo + tau - P.t_Q0) * P.fs;
             if (!P.interp) u = floor(u + 0.5);
+            uk[(size_t)i * 4 + kk] = u;                      // the fused kernel and the tile builder use this very value
             int cell = ((int)floor(u) - n_min) >> SP_CELL_SHIFT;
             cell = max(0, min(cell, (1 << cell_bits) - 1));
             k = (k << cell_bits) | (unsigned long long)cell;
@@ -179,7 +180,7 @@ __global__ void __launch_bounds__(256) sp_tile_flag_kernel(int N, const unsigned
 // one warp per tile: extent, window base per detector, largest offset
 __global__ void __launch_bounds__(256) sp_tile_info_kernel(LnlParams P, int N, int invalid_shift, const unsigned long long* __restrict__ key,
                                                            const int* __restrict__ tstart, const int* __restrict__ ntiles_dev,
-                                                           const double* __restrict__ rec, SpTile* __restrict__ tiles) {
+                                                           const double* __restrict__ uk, const int* __restrict__ perm, SpTile* __restrict__ tiles) {
     const int id = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (id >= *ntiles_dev) return;
     const int start = tstart[id];
@@ -191,11 +192,12 @@ __global__ void __launch_bounds__(256) sp_tile_info_kernel(LnlParams P, int N, i
         const bool mem = open && pos < N && key[pos] == k0 && (pos == start || (pos & (SP_TS - 1)) != 0);
         const unsigned b = __ballot_sync(0xffffffffu, mem);
         const int lead = b == 0xffffffffu ? 32 : __ffs(~b) - 1;      // members are a prefix
-        if (lane < lead) {
+        if (lane < lead && !(k0 >> invalid_shift)) {
+            const size_t sidx = (size_t)perm[pos];
 #pragma unroll
             for (int k = 0; k < 3; k++)
                 if (k < P.K) {
-                    const int nk = (int)floor(rec[(size_t)pos * 16 + 8 + k]);
+                    const int nk = (int)floor(uk[sidx * 4 + k]);
                     nmin[k] = min(nmin[k], nk);
                     nmax[k] = max(nmax[k], nk);
                 }
@@ -229,6 +231,7 @@ struct SplitSmem {
     double xch[2][3][SP_TS];                  // last bin of a chunk, from group 3 to group 0 of the next chunk (slot = chunk parity)
     double lse[SP_G][2][SP_TS];               // partial (reference, sum) of the four threads of a sample
     int eb[3][SP_TS];                         // biased exponent of max |coefficient| per detector
+    YlmTable ytab;                            // term table of the harmonics (Eq. 4), copied once per CTA
     uint64_t a_full, d_full, d_empty, b_full[SP_NSTAGE], b_empty[SP_NSTAGE];
     uint32_t tmem_base;
 };
@@ -308,8 +311,8 @@ __device__ __forceinline__ void sp_cursor_next(SpCursor& cu, const SpTile* __res
 
 template <int K, bool TABLE>
 __global__ void __launch_bounds__(SP_THREADS, 1)
-lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const double2* __restrict__ ytile, const int* __restrict__ perm,
-                 double* __restrict__ lnL, const SpTile* __restrict__ tiles, const int* __restrict__ ntiles_dev) {
+lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double* __restrict__ uk, const int* __restrict__ perm,
+                 double* __restrict__ lnL, double* __restrict__ ln_prior, const SpTile* __restrict__ tiles, const int* __restrict__ ntiles_dev) {
     extern __shared__ __align__(1024) unsigned char sp_smem_raw[];
     SplitSmem& sm = *reinterpret_cast<SplitSmem*>(sp_smem_raw);
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
@@ -324,6 +327,11 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
         mbar_init_fence();
     }
     for (int q = tid; q < 64 * 16; q += SP_THREADS) sm.etab[q >> 4][q & 15] = f2_exp2_tab[q >> 4];
+    {
+        const int4* src = reinterpret_cast<const int4*>(P.ylm);
+        int4* dst = reinterpret_cast<int4*>(&sm.ytab);
+        for (int q = tid; q < (int)(sizeof(YlmTable) / 16); q += SP_THREADS) dst[q] = src[q];
+    }
     {
         const double2* usrc = reinterpret_cast<const double2*>(P.UVp);
         const int nuv = min(P.n_pairs * K * 2, SP_UVMAX);
@@ -401,40 +409,120 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
             const int pos = ti.start + i;
             const bool member = i < ti.cnt;
             if (ti.nchunk == 0) {
-                if (member && g == 0) lnL[perm ? perm[pos] : pos] = (ti.flags & 2) ? __longlong_as_double(0x7ff8000000000000LL) : neg_inf();
+                if (member && g == 0) {
+                    lnL[perm[pos]] = (ti.flags & 2) ? __longlong_as_double(0x7ff8000000000000LL) : neg_inf();
+                    if (ln_prior && (ti.flags & 1)) ln_prior[perm[pos]] = neg_inf();
+                }
                 continue;
             }
             const int N_t = P.N_t;
-            // ---- the sample's record: F_k = F+ - i Fx, stored-bin coordinate u_k of grid time 0, x = D_ref / D
-            double fr[K], fi[K], w0[K], w1[K], x = 0.0;
+            // ---- steps 1-2 in place (no preparation kernel, no per-sample record in HBM).  The four threads of a sample
+            //      share the work and meet in shared memory (arrays that are idle during the prologue): group 0 the antenna
+            //      patterns F_k = F+ - i Fx, group 1 the powers of cos, sin(iota/2), group 2 the phases e^{i m phi}, group 3
+            //      x = D_ref / D, ln prior and the stored-bin coordinates u_k of grid time 0 (from the key kernel: the very
+            //      values the tile's window was built from).  Coordinates are gathered through the sort permutation.
+            double fr[K], fi[K], w0[K], w1[K], x;
             int off[K];
             {
-                const double* r = rec + (size_t)pos * 16;
-                double u[K];
+                const size_t sidx = member ? (size_t)perm[pos] : 0;
+                double* const shr = &sm.lse[0][0][i];                     // rows 0..2 Re F_k, 3..5 Im F_k, 6 x
+                double* const shu = &sm.xch[0][0][i];                     // rows 0..2 u_k
+                double* const scr = &sm.ring[0][i];                       // harmonics' tables: row q of table t at scr[(t0 + q) * SP_TS]
+                const int mp = sm.ytab.max_pow, mm = sm.ytab.max_abs_m;
+                double* const pc = scr;
+                double* const ps = pc + (mp + 1) * SP_TS;
+                double* const cm = ps + (mp + 1) * SP_TS;
+                double* const sn = cm + (mm + 1) * SP_TS;
+                if (g == 0) {
+                    SampleIn sp;
+                    sp.ra = 0.0; sp.sd = 0.0; sp.cd = 1.0; sp.psi = 0.0; sp.phi_ref = 0.0; sp.ch = 1.0; sp.sh = 0.0; sp.dist = 1.0; sp.valid = member;
+                    if (member) {
+                        sp.ra = __ldg(z + sidx);
+                        sp.sd = __ldg(z + (size_t)N + sidx);
+                        sp.psi = __ldg(z + 2 * (size_t)N + sidx);
+                        sp.cd = sqrt(fmax((1.0 - sp.sd) * (1.0 + sp.sd), 0.0));
+                    }
+                    double Fp[ILE_MAX_K], Fx[ILE_MAX_K], tau[ILE_MAX_K];
+                    antenna_dev(P, sp, Fp, Fx, tau);
 #pragma unroll
-                for (int k = 0; k < K; k++) { fr[k] = fi[k] = 0.0; u[k] = (double)ti.base[k]; }
-                if (member) {
-                    const double2 r0 = *reinterpret_cast<const double2*>(r), r1 = *reinterpret_cast<const double2*>(r + 2);
-                    const double2 r2 = *reinterpret_cast<const double2*>(r + 4), r3 = *reinterpret_cast<const double2*>(r + 6);
-                    const double2 r4 = *reinterpret_cast<const double2*>(r + 8), r5 = *reinterpret_cast<const double2*>(r + 10);
-                    const double fr_[4] = {r0.x, r0.y, r1.x, r1.y}, fi_[4] = {r2.x, r2.y, r3.x, r3.y}, u_[4] = {r4.x, r4.y, r5.x, r5.y};
+                    for (int k = 0; k < K; k++) {
+                        shr[k * SP_TS] = Fp[k];
+                        shr[(3 + k) * SP_TS] = -Fx[k];
+                    }
+                } else if (g == 1) {
+                    const double ci = member ? __ldg(z + 4 * (size_t)N + sidx) : 1.0;
+                    const double ch = sqrt(fmax(0.5 * (1.0 + ci), 0.0)), sh = sqrt(fmax(0.5 * (1.0 - ci), 0.0));
+                    double a = 1.0, b = 1.0;
+                    pc[0] = 1.0;
+                    ps[0] = 1.0;
+                    for (int q = 1; q <= mp; q++) {
+                        a *= ch;
+                        b *= sh;
+                        pc[q * SP_TS] = a;
+                        ps[q * SP_TS] = b;
+                    }
+                } else if (g == 2) {
+                    const double phi = member ? -__ldg(z + 3 * (size_t)N + sidx) : 0.0;   // -2Y_lm(iota, -phi_ref) (reading G7)
+                    cm[0] = 1.0;
+                    sn[0] = 0.0;
+                    for (int q = 1; q <= mm; q++) {
+                        double sq, cq;
+                        sincos((double)q * phi, &sq, &cq);
+                        cm[q * SP_TS] = cq;
+                        sn[q * SP_TS] = sq;
+                    }
+                } else {
+                    double xs = 0.0;
+                    if (member) {
+                        SampleIn sp;
+                        sp.dist = P.d > 5 ? __ldg(z + 5 * (size_t)N + sidx) : 1.0;
+                        xs = TABLE ? 1.0 : P.D_ref / sp.dist;
+                        if (ln_prior) ln_prior[sidx] = ln_prior_dev(P, sp);
+                    }
+                    shr[6 * SP_TS] = xs;
 #pragma unroll
-                    for (int k = 0; k < K; k++) { fr[k] = fr_[k]; fi[k] = fi_[k]; u[k] = u_[k]; }
-                    x = r[12];
+                    for (int k = 0; k < K; k++) shu[k * SP_TS] = member ? __ldg(uk + sidx * 4 + k) : (double)ti.base[k];
                 }
+                qbar();
+                x = shr[6 * SP_TS];
 #pragma unroll
                 for (int k = 0; k < K; k++) {
-                    const double fl = floor(u[k]);
-                    w1[k] = u[k] - fl;
+                    fr[k] = shr[k * SP_TS];
+                    fi[k] = shr[(3 + k) * SP_TS];
+                    const double u = shu[k * SP_TS], fl = floor(u);
+                    w1[k] = u - fl;
                     w0[k] = 1.0 - w1[k];
                     off[k] = min(max((int)fl - ti.base[k], 0), SP_CAPMAX);
                 }
+                // ---- harmonics (Eq. 4): group g evaluates modes g, g + 4, ... from the tables
+                const int M = sm.ytab.M;
+                for (int m = g; m < 24; m += SP_G) {
+                    double2 y = make_double2(0.0, 0.0);
+                    if (m < M) {
+                        const YlmMode& Ym = sm.ytab.mode[m];
+                        double acc = 0.0;
+                        for (int t = 0; t < Ym.nterms; t++) acc += Ym.coef[t] * pc[Ym.pc[t] * SP_TS] * ps[Ym.ps[t] * SP_TS];
+                        const int am = Ym.m < 0 ? -Ym.m : Ym.m;
+                        const double c = cm[am * SP_TS], sgn = Ym.m < 0 ? -sn[am * SP_TS] : sn[am * SP_TS];
+                        y = make_double2(acc * c, acc * sgn);
+                    }
+                    sm.Y[m][i] = y;
+                }
             }
-            // ---- harmonics: group g fetches modes g, g + 4, ... of the sample's column
-#pragma unroll
-            for (int m = g; m < 24; m += SP_G)
-                sm.Y[m][i] = member ? __ldg(ytile + ((size_t)(pos >> 5) * 24 + m) * 32 + (pos & 31)) : make_double2(0.0, 0.0);
             qbar();
+            // ---- the next tile's coordinates are gathered through the sort permutation (scattered 8-byte reads): ask for
+            //      them now, so that its prologue finds them in L2 instead of waiting two dependent DRAM round trips
+            if (t + (int)gridDim.x < ntiles) {
+                const SpTile tn = tiles[t + gridDim.x];
+                if (tn.nchunk > 0 && i < tn.cnt) {
+                    const size_t sn_ = (size_t)perm[tn.start + i];
+                    auto pf = [](const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); };
+                    if (g == 0) { pf(z + sn_); pf(z + (size_t)N + sn_); pf(z + 2 * (size_t)N + sn_); }
+                    else if (g == 1) pf(z + 4 * (size_t)N + sn_);
+                    else if (g == 2) pf(z + 3 * (size_t)N + sn_);
+                    else { if (P.d > 5) pf(z + 5 * (size_t)N + sn_); pf(uk + sn_ * 4); }
+                }
+            }
             // ---- step 3 (group k does detector k): coefficients x F_k Y_m -> six signed 8-bit digits -> tensor memory (operand A)
 #pragma unroll
             for (int k = 0; k < K; k++) {
@@ -686,8 +774,9 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
                 double tot = 0.0;
 #pragma unroll
                 for (int gg = 0; gg < SP_G; gg++) tot += sm.lse[gg][1][i] * exp(sm.lse[gg][0][i] - mx);
-                lnL[perm ? perm[pos] : pos] = mx + log(tot) - P.ln_Nt;
+                lnL[perm[pos]] = mx + log(tot) - P.ln_Nt;
             }
+            qbar();                                                     // the next tile's prologue reuses sm.lse
         }
     }
     tc_fence_before();
@@ -697,12 +786,12 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const doubl
 
 // ---------------------------------------------------------------- launch
 template <int K, bool TABLE>
-static int launch_split_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const double2* yt, const int* perm, double* lnL,
-                          const SpTile* tiles, const int* ntiles_dev) {
+static int launch_split_t(ile_ctx* ctx, const LnlParams& P, int N, const double* z, const double* uk, const int* perm, double* lnL,
+                          double* ln_prior, const SpTile* tiles, const int* ntiles_dev) {
     const int smem = (int)sizeof(SplitSmem) + 1024;
     ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_split_kernel<K, TABLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     const int slot = ile_timing_begin(ctx);
-    lnl_split_kernel<K, TABLE><<<ctx->sm_count, SP_THREADS, smem, ctx->stream>>>(P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
+    lnl_split_kernel<K, TABLE><<<ctx->sm_count, SP_THREADS, smem, ctx->stream>>>(P, N, z, uk, perm, lnL, ln_prior, tiles, ntiles_dev);
     ile_timing_end(ctx, slot);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
@@ -724,22 +813,24 @@ int ile_split_cell_bits(int n_min, int n_max) {
 }
 
 int ile_launch_split_keys(ile_ctx* ctx, const LnlParams& P, int N, const double* z, int n_min, int cell_bits, unsigned long long* key,
-                          unsigned int* val, long long* n_dev, int* bits_dev, int* ntiles_dev) {
-    sp_key_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(P, N, z, n_min, cell_bits, key, val, n_dev, bits_dev, ntiles_dev);
+                          unsigned int* val, double* uk, long long* n_dev, int* bits_dev, int* ntiles_dev) {
+    sp_key_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(P, N, z, n_min, cell_bits, key, val, uk, n_dev, bits_dev, ntiles_dev);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }
 
-// rec / yt as written by lnl_prep3_kernel in the order of perm (sorted by sp_key_kernel's keys, in key[])
-int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int cell_bits, const unsigned long long* key, const double* rec, const double2* yt,
-                     const int* perm, double* lnL, int* tstart, SpTile* tiles, int* ntiles_dev) {
+// z [d][N] in the caller's order; key / perm = the sorted keys of sp_key_kernel and the sort permutation; uk = its u_k [N][4]
+int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int cell_bits, const unsigned long long* key, const double* z, const double* uk,
+                     const int* perm, double* lnL, double* ln_prior, int* tstart, SpTile* tiles, int* ntiles_dev) {
     sp_tile_flag_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(N, key, tstart, ntiles_dev);
     ILE_LAUNCH_CHECK(ctx);
     const int max_tiles = ile_split_max_tiles(N, cell_bits, P.K);
-    sp_tile_info_kernel<<<(max_tiles * 32 + 255) / 256, 256, 0, ctx->stream>>>(P, N, cell_bits * P.K, key, tstart, ntiles_dev, rec, tiles);
+    sp_tile_info_kernel<<<(max_tiles * 32 + 255) / 256, 256, 0, ctx->stream>>>(P, N, cell_bits * P.K, key, tstart, ntiles_dev, uk, perm, tiles);
     ILE_LAUNCH_CHECK(ctx);
     const bool tb = P.use_table != 0;
-    if (P.K == 3) return tb ? launch_split_t<3, true>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev) : launch_split_t<3, false>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
-    if (P.K == 2) return tb ? launch_split_t<2, true>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev) : launch_split_t<2, false>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
-    return tb ? launch_split_t<1, true>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev) : launch_split_t<1, false>(ctx, P, N, rec, yt, perm, lnL, tiles, ntiles_dev);
+#define SP_LAUNCH(K_, T_) launch_split_t<K_, T_>(ctx, P, N, z, uk, perm, lnL, ln_prior, tiles, ntiles_dev)
+    if (P.K == 3) return tb ? SP_LAUNCH(3, true) : SP_LAUNCH(3, false);
+    if (P.K == 2) return tb ? SP_LAUNCH(2, true) : SP_LAUNCH(2, false);
+    return tb ? SP_LAUNCH(1, true) : SP_LAUNCH(1, false);
+#undef SP_LAUNCH
 }
