@@ -130,6 +130,7 @@ extern "C" int ile_destroy(ile_ctx* ctx) {
     cudaFree(ctx->d_UVp);
     cudaFree(ctx->d_pairs);
     cudaFree(ctx->d_lnT);
+    cudaFree(ctx->d_lnT4);
     cudaFree(ctx->d_scratch);
     if (ctx->tev) {
         for (int s = 0; s < 2 * ILE_TIMING_SLOTS; s++) cudaEventDestroy(ctx->tev[s]);
@@ -404,13 +405,25 @@ extern "C" int ile_load_distance_table(ile_ctx* ctx, int nA, int nB, double A_lo
     if (!ctx) return ILE_EINVAL;
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (nA == 0) {
-        cudaFree(ctx->d_lnT); ctx->d_lnT = nullptr; ctx->nA = ctx->nB = 0;
+        cudaFree(ctx->d_lnT); ctx->d_lnT = nullptr; cudaFree(ctx->d_lnT4); ctx->d_lnT4 = nullptr; ctx->nA = ctx->nB = 0;
         return ILE_OK;
     }
     if (nA < 2 || nB < 2 || !(A_hi > A_lo) || !(B_hi > B_lo) || !lnT) return ile_fail(ctx, ILE_EINVAL, "load_distance_table: bad argument");
     cudaFree(ctx->d_lnT); ctx->d_lnT = nullptr;
     if (cudaMalloc(&ctx->d_lnT, (size_t)nA * nB * 8) != cudaSuccess) { cudaGetLastError(); return ile_fail(ctx, ILE_ENOMEM, "table allocation failed"); }
     ILE_CUDA(ctx, cudaMemcpy(ctx->d_lnT, lnT, (size_t)nA * nB * 8, cudaMemcpyHostToDevice));
+    {   // cell copy for the fused kernel: the four corners of a bilinear lookup in one 32-byte sector
+        std::vector<double> cells((size_t)(nA - 1) * (nB - 1) * 4);
+        for (int b = 0; b < nB - 1; b++)
+            for (int a = 0; a < nA - 1; a++) {
+                double* c = &cells[((size_t)b * (nA - 1) + a) * 4];
+                c[0] = lnT[(size_t)b * nA + a]; c[1] = lnT[(size_t)b * nA + a + 1];
+                c[2] = lnT[(size_t)(b + 1) * nA + a]; c[3] = lnT[(size_t)(b + 1) * nA + a + 1];
+            }
+        cudaFree(ctx->d_lnT4); ctx->d_lnT4 = nullptr;
+        if (cudaMalloc(&ctx->d_lnT4, cells.size() * 8) != cudaSuccess) { cudaGetLastError(); return ile_fail(ctx, ILE_ENOMEM, "table allocation failed"); }
+        ILE_CUDA(ctx, cudaMemcpy(ctx->d_lnT4, cells.data(), cells.size() * 8, cudaMemcpyHostToDevice));
+    }
     ctx->nA = nA; ctx->nB = nB; ctx->A_lo = A_lo; ctx->A_hi = A_hi; ctx->B_lo = B_lo; ctx->B_hi = B_hi;
     return ILE_OK;
 }
@@ -439,6 +452,7 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
     L->ln_Nt = log((double)ctx->N_t);
     L->nA = ctx->nA; L->nB = ctx->nB; L->A_lo = ctx->A_lo; L->A_hi = ctx->A_hi; L->B_lo = ctx->B_lo; L->B_hi = ctx->B_hi;
     L->lnT = ctx->d_lnT;
+    L->lnT4 = ctx->d_lnT4;
     L->Qc = ctx->d_Qc + (size_t)p * K * M * ctx->N_Q * 2;
     L->Qf = ctx->d_Qf + (size_t)p * K * ctx->N_Qpad * ILE_QT_ROW;
     L->U = ctx->d_U + (size_t)p * K * M * M * 2;

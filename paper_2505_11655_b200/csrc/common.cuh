@@ -46,6 +46,7 @@ struct LnlParams {
     int nA, nB;
     double A_lo, A_hi, B_lo, B_hi;
     const double* lnT;
+    const double* lnT4;           // cells of the table, see ile_ctx
     // per intrinsic point data (already offset to point p)
     const double* Qc;             // [K][M][N_Q][2]
     const double* Qf;             // [K][N_Qpad/2][6][2][8] fragment-major: one 128-byte line per (bin pair, k-step pair)
@@ -88,6 +89,7 @@ struct ile_ctx {
     int nA, nB;
     double A_lo, A_hi, B_lo, B_hi;
     double* d_lnT;
+    double* d_lnT4;               // the same table as cells: [nB-1][nA-1][4] = (T[b][a], T[b][a+1], T[b+1][a], T[b+1][a+1]): one 32-byte read per bilinear lookup
     int variant;
     int ylm_max_pow, ylm_max_abs_m;   // sizes of the harmonics' power and phase tables (shared-memory scratch of the prep kernel)
     void* pc_buf;                 // scratch of ile_precompute_quv (grow-only, freed at destroy)

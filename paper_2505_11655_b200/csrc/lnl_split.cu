@@ -140,7 +140,8 @@ __global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const d
     if (i == 0) {
         *n_dev = N;
         *bits_dev = cell_bits * P.K + 1;
-        *ntiles_dev = 0;
+        ntiles_dev[0] = 0;                                 // tile count, run count
+        ntiles_dev[1] = 0;
     }
     if (i >= N) return;
     const double ra = z[i], sd = z[(size_t)N + i];
@@ -170,11 +171,34 @@ __global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const d
     val[i] = (unsigned int)i;
 }
 
-// a tile starts at every multiple of 128 of the sorted order and wherever the cell changes
-__global__ void __launch_bounds__(256) sp_tile_flag_kernel(int N, const unsigned long long* __restrict__ key, int* __restrict__ tstart, int* ntiles_dev) {
+// Tiles: the sorted order is cut at every cell change (run start) and every 128 samples after it.
+// pass 1: run starts, appended in any order
+__global__ void __launch_bounds__(256) sp_run_flag_kernel(int N, const unsigned long long* __restrict__ key, int* __restrict__ runs, int* nruns_dev) {
     const int pos = blockIdx.x * blockDim.x + threadIdx.x;
     if (pos >= N) return;
-    if ((pos & (SP_TS - 1)) == 0 || key[pos] != key[pos - 1]) tstart[atomicAdd(ntiles_dev, 1)] = pos;
+    if (pos == 0 || key[pos] != key[pos - 1]) runs[atomicAdd(nruns_dev, 1)] = pos;
+}
+// pass 2: one block per run: its end by binary search, then its tile starts
+__global__ void __launch_bounds__(256) sp_run_tiles_kernel(int N, const unsigned long long* __restrict__ key, const int* __restrict__ runs,
+                                                          const int* __restrict__ nruns_dev, int* __restrict__ tstart, int* ntiles_dev) {
+    const int nruns = *nruns_dev;
+    __shared__ int sh_first, sh_nt;
+    for (int r = blockIdx.x; r < nruns; r += gridDim.x) {
+        const int rs = runs[r];
+        if (threadIdx.x == 0) {
+            const unsigned long long k0 = key[rs];
+            int lo = rs + 1, hi = N;                     // first position with a larger key
+            while (lo < hi) {
+                const int mid = (int)(((long long)lo + hi) >> 1);
+                if (key[mid] > k0) hi = mid; else lo = mid + 1;
+            }
+            sh_nt = (lo - rs + SP_TS - 1) / SP_TS;
+            sh_first = atomicAdd(ntiles_dev, sh_nt);
+        }
+        __syncthreads();
+        for (int q = threadIdx.x; q < sh_nt; q += blockDim.x) tstart[sh_first + q] = rs + q * SP_TS;
+        __syncthreads();
+    }
 }
 
 // one warp per tile: extent, window base per detector, largest offset
@@ -189,7 +213,7 @@ __global__ void __launch_bounds__(256) sp_tile_info_kernel(LnlParams P, int N, i
     bool open = true;
     for (int q = 0; q < SP_TS / 32; q++) {
         const int pos = start + 32 * q + lane;
-        const bool mem = open && pos < N && key[pos] == k0 && (pos == start || (pos & (SP_TS - 1)) != 0);
+        const bool mem = open && pos < N && key[pos] == k0;
         const unsigned b = __ballot_sync(0xffffffffu, mem);
         const int lead = b == 0xffffffffu ? 32 : __ffs(~b) - 1;      // members are a prefix
         if (lane < lead && !(k0 >> invalid_shift)) {
@@ -631,7 +655,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                 b = fmin(fmax(b, 0.0), (double)(P.nB - 1));
                 const int ib = min((int)floor(b), P.nB - 2);
                 tb_f = b - ib;
-                tb_row = P.lnT + (size_t)ib * P.nA;
+                tb_row = P.lnT4 + (size_t)ib * (P.nA - 1) * 4;
                 init = 0.0;
             }
             qbar();                                              // partial sums read by everybody before the ring is initialised
@@ -669,9 +693,9 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                             a = fmin(fmax(a, 0.0), (double)(P.nA - 1));
                             const int ia = min((int)a, P.nA - 2);
                             const double fa = a - (double)ia;
-                            const double* T0 = tb_row + ia;
-                            const double t00 = __ldg(T0), t01 = __ldg(T0 + 1), t10 = __ldg(T0 + P.nA), t11 = __ldg(T0 + P.nA + 1);
-                            const double t0 = fma(fa, t01 - t00, t00), t1 = fma(fa, t11 - t10, t10);
+                            const double2* T0 = reinterpret_cast<const double2*>(tb_row + 4 * ia);       // one 32-byte cell
+                            const double2 lo2 = __ldg(T0), hi2 = __ldg(T0 + 1);
+                            const double t0 = fma(fa, lo2.y - lo2.x, lo2.x), t1 = fma(fa, hi2.y - hi2.x, hi2.x);
                             A = fma(tb_f, t1 - t0, t0);
                         }
                         v[e] = j0 + SP_G * e < jend ? A : neg_inf();
@@ -805,7 +829,7 @@ int ile_split_max_tiles(int N, int cell_bits, int K) {
     const long long t = (N + SP_TS - 1) / SP_TS + (cells < N ? cells : N) + 1;
     return (int)t;
 }
-size_t ile_split_tile_bytes(int max_tiles) { return ((size_t)max_tiles * (sizeof(SpTile) + sizeof(int)) + 255) / 256 * 256; }
+size_t ile_split_tile_bytes(int max_tiles) { return ((size_t)max_tiles * (sizeof(SpTile) + 2 * sizeof(int)) + 255) / 256 * 256; }   // tiles, tile starts, run starts
 int ile_split_cell_bits(int n_min, int n_max) {
     int cell_bits = 1;
     while ((1 << cell_bits) <= ((n_max - n_min) >> SP_CELL_SHIFT)) cell_bits++;
@@ -822,9 +846,13 @@ int ile_launch_split_keys(ile_ctx* ctx, const LnlParams& P, int N, const double*
 // z [d][N] in the caller's order; key / perm = the sorted keys of sp_key_kernel and the sort permutation; uk = its u_k [N][4]
 int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int cell_bits, const unsigned long long* key, const double* z, const double* uk,
                      const int* perm, double* lnL, double* ln_prior, int* tstart, SpTile* tiles, int* ntiles_dev) {
-    sp_tile_flag_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(N, key, tstart, ntiles_dev);
-    ILE_LAUNCH_CHECK(ctx);
     const int max_tiles = ile_split_max_tiles(N, cell_bits, P.K);
+    int* runs = tstart + max_tiles;                     // run starts; their count sits behind the tile count
+    int* nruns_dev = ntiles_dev + 1;
+    sp_run_flag_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(N, key, runs, nruns_dev);
+    ILE_LAUNCH_CHECK(ctx);
+    sp_run_tiles_kernel<<<ctx->sm_count * 2, 256, 0, ctx->stream>>>(N, key, runs, nruns_dev, tstart, ntiles_dev);
+    ILE_LAUNCH_CHECK(ctx);
     sp_tile_info_kernel<<<(max_tiles * 32 + 255) / 256, 256, 0, ctx->stream>>>(P, N, cell_bits * P.K, key, tstart, ntiles_dev, uk, perm, tiles);
     ILE_LAUNCH_CHECK(ctx);
     const bool tb = P.use_table != 0;
