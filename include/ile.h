@@ -130,6 +130,10 @@ int ile_kernel_time(ile_ctx *ctx, double *total_ms, uint64_t *launches);
  * the FP64 ALUs, mode 1 = independent DMMA.8x8x4 chains on the FP64 tensor pipe.  Synchronises;
  * *tflops (host) receives the best of three timed runs. */
 int ile_fp64_peak(ile_ctx *ctx, int mode, double *tflops);
+/* Probe of the int8 tensor path the fused kernel's contraction runs on (tcgen05.mma kind::i8, 128 x 32 x 32, A from tensor
+ * memory, B from shared memory, the kernel's 33-MMA schedule and nothing else): mode 0 = k-step-major issue (the kernel's),
+ * 1 = sum-major.  Synchronises; *tops (host) receives int8 operations (2 per multiply-add) per second / 1e12, best of three. */
+int ile_int8_mma_peak(ile_ctx *ctx, int mode, double *tops);
 
 /* ------------------------------------------------------------------ problem definition (host pointers)
  * detector response functions and positions.  D[k] is the 3x3 response tensor

@@ -217,6 +217,11 @@ class Ile:
         self._ck(self.lib.ile_fp64_peak(self.ctx, C.c_int(mode), C.byref(tf)))
         return tf.value
 
+    def int8_mma_peak(self, mode: int = 0) -> float:
+        t = C.c_double(0.0)
+        self._ck(self.lib.ile_int8_mma_peak(self.ctx, C.c_int(mode), C.byref(t)))
+        return t.value
+
     def load_quv_ptr(self, P, N_Q, fs, t_Q0, Q_ptr, U_ptr, V_ptr, D_ref):
         """ile_load_quv from raw host addresses (e.g. pinned torch tensors): no marshalling copies."""
         self._ck(self.lib.ile_load_quv(self.ctx, C.c_int(P), C.c_int(N_Q), C.c_double(fs), C.c_double(t_Q0), C.c_void_p(Q_ptr),
