@@ -26,6 +26,7 @@
 #include "common.cuh"
 #include "likelihood_dev.cuh"
 #include "radix_sort.cuh"
+#include <type_traits>
 #include "sm100_ptx.cuh"
 #include "exp_tab.cuh"
 
@@ -43,6 +44,7 @@
 #define SP_DCOL 256           // first accumulator column; sum s at SP_DCOL + SP_NB s (one set: it is free again as soon as every warp has loaded its bins)
 #define SP_G 4                // threads per sample (warp groups): digits by detector, bins, triangle rows, log-sum-exp rows
 #define SP_MATH (SP_G * SP_TS)
+#define SP_RAISE_HI 0x40800000   // high word of 512.0: the streaming log-sum-exp raises its reference beyond e^512
 #define SP_THREADS (SP_MATH + 32)
 #define SP_UVMAX (300 * 3 * 2)
 #define SP_MAGIC 6755399441055744.0   // 1.5 * 2^52
@@ -594,31 +596,31 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
 #pragma unroll
                 for (int k = 0; k < K; k++) uu[k] = vr[k] = vi[k] = 0.0;
                 const int M = P.M;
+                auto pair = [&](const double2 ya, const double2 yb, const double2* __restrict__ uq) {
+                    const double t2 = ya.y * yb.y, t4 = ya.y * yb.x;
+                    const double pr = fma(ya.x, yb.x, t2), qr = fma(ya.x, yb.x, -t2), pi = fma(ya.x, yb.y, -t4), qi = fma(ya.x, yb.y, t4);
+#pragma unroll
+                    for (int k = 0; k < K; k++) {
+                        const double2 u = uq[2 * k], v = uq[2 * k + 1];
+                        uu[k] = fma(-u.y, pi, fma(u.x, pr, uu[k]));
+                        vr[k] = fma(-v.y, qi, fma(v.x, qr, vr[k]));
+                        vi[k] = fma(v.y, qr, fma(v.x, qi, vi[k]));
+                    }
+                };
                 for (int a = 0; a < M; a++) {
                     if ((a & 7) != g && (a & 7) != 7 - g) continue;
                     const double2 ya = sm.Y[a][i];
                     const double2* uv = sm.uv + (size_t)(a * M - (a * (a - 1)) / 2) * 2 * K;
-                    for (int b = a; b < M; b += 2) {
-                        // two pairs per step; a pair past the end of the row multiplies a zero harmonic
-                        const bool in1 = b + 1 < M;
-                        double2 yb[2];
-                        yb[0] = sm.Y[b][i];
-                        yb[1] = sm.Y[in1 ? b + 1 : b][i];
-                        if (!in1) yb[1] = make_double2(0.0, 0.0);
-                        const double2* u1 = uv + (in1 ? 2 * K : 0);
-#pragma unroll
-                        for (int q = 0; q < 2; q++) {
-                            const double2* uq = q ? u1 : uv;
-                            const double t2 = ya.y * yb[q].y, t4 = ya.y * yb[q].x;
-                            const double pr = fma(ya.x, yb[q].x, t2), qr = fma(ya.x, yb[q].x, -t2), pi = fma(ya.x, yb[q].y, -t4), qi = fma(ya.x, yb[q].y, t4);
-#pragma unroll
-                            for (int k = 0; k < K; k++) {
-                                const double2 u = uq[2 * k], v = uq[2 * k + 1];
-                                uu[k] = fma(-u.y, pi, fma(u.x, pr, uu[k]));
-                                vr[k] = fma(-v.y, qi, fma(v.x, qr, vr[k]));
-                                vi[k] = fma(v.y, qr, fma(v.x, qi, vi[k]));
-                            }
-                        }
+                    int b = a;
+                    if ((M - a) & 1) {                                   // odd row length: the diagonal pair alone
+                        pair(ya, ya, uv);
+                        uv += 2 * K;
+                        b++;
+                    }
+                    for (; b < M; b += 2) {                              // two pairs per step, loads first
+                        const double2 yb0 = sm.Y[b][i], yb1 = sm.Y[b + 1][i];
+                        pair(ya, yb0, uv);
+                        pair(ya, yb1, uv + 2 * K);
                         uv += 4 * K;
                     }
                 }
@@ -671,57 +673,62 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
 
             // rows jdone + g, jdone + g + 4, ... below jend are complete: lnL(t_j) and this thread's share of the streaming
             // log-sum-exp (step 6); four rows per batch, loads first
-            auto lse_rows = [&](const int jend) {
-                for (int j0 = jdone + g; j0 < jend; j0 += 4 * SP_G) {
-                    double v[4];
-                    double* pr[4];
+            auto lse_batch = [&](const int j0, const int jend, auto fullc) {
+                constexpr bool FULL = decltype(fullc)::value;          // all four rows below jend: no guards
+                double v[4];
+                double* pr[4];
 #pragma unroll
-                    for (int e = 0; e < 4; e++) {
-                        pr[e] = rcol + ((j0 + SP_G * e) & (SP_RING - 1)) * SP_TS;
-                        v[e] = *pr[e];
-                    }
-#pragma unroll
-                    for (int e = 0; e < 4; e++)
-                        if (j0 + SP_G * e < jend) *pr[e] = init;
-                    bool need = false;
-                    double dl[4];
-#pragma unroll
-                    for (int e = 0; e < 4; e++) {
-                        double A = v[e];
-                        if (TABLE) {
-                            double a = fma(A, tabA_s, tabA_o);
-                            a = fmin(fmax(a, 0.0), (double)(P.nA - 1));
-                            const int ia = min((int)a, P.nA - 2);
-                            const double fa = a - (double)ia;
-                            const double2* T0 = reinterpret_cast<const double2*>(tb_row + 4 * ia);       // one 32-byte cell
-                            const double2 lo2 = __ldg(T0), hi2 = __ldg(T0 + 1);
-                            const double t0 = fma(fa, lo2.y - lo2.x, lo2.x), t1 = fma(fa, hi2.y - hi2.x, hi2.x);
-                            A = fma(tb_f, t1 - t0, t0);
-                        }
-                        v[e] = j0 + SP_G * e < jend ? A : neg_inf();
-                        dl[e] = v[e] - run_m;
-                        need = need || (__double2hiint(dl[e]) >= 0x403E0000);   // dl >= 30 (or NaN): test on the high word
-                    }
-                    if (__any_sync(0xffffffffu, need)) {
-                        // raise the reference to the largest new value (rare); the running sum is rescaled exactly
-                        const double mx = fmax(fmax(v[0], v[1]), fmax(v[2], v[3]));
-                        if (mx - run_m >= 30.0) {
-                            const double dm = run_m - mx;
-                            run_s = dm > -690.0 ? run_s * sp_exp_small(dm) : 0.0;
-                            run_m = mx;
-                        }
-#pragma unroll
-                        for (int e = 0; e < 4; e++) dl[e] = v[e] - run_m;
-                    }
-                    double part[2] = {0.0, 0.0};
-#pragma unroll
-                    for (int e = 0; e < 4; e++) {
-                        // terms below e^-40 of the reference (and rows past the end) are clamped to e^-40 (R2)
-                        const unsigned hc = min((unsigned)__double2hiint(dl[e]), 0xC0440000u);
-                        part[e & 1] += sp_exp_tab(__hiloint2double((int)hc, __double2loint(dl[e])), etab);
-                    }
-                    run_s += part[0] + part[1];
+                for (int e = 0; e < 4; e++) {
+                    pr[e] = rcol + ((j0 + SP_G * e) & (SP_RING - 1)) * SP_TS;
+                    v[e] = *pr[e];
                 }
+#pragma unroll
+                for (int e = 0; e < 4; e++)
+                    if (FULL || j0 + SP_G * e < jend) *pr[e] = init;
+                bool need = false;
+                double dl[4];
+#pragma unroll
+                for (int e = 0; e < 4; e++) {
+                    double A = v[e];
+                    if (TABLE) {
+                        double a = fma(A, tabA_s, tabA_o);
+                        a = fmin(fmax(a, 0.0), (double)(P.nA - 1));
+                        const int ia = min((int)a, P.nA - 2);
+                        const double fa = a - (double)ia;
+                        const double2* T0 = reinterpret_cast<const double2*>(tb_row + 4 * ia);       // one 32-byte cell
+                        const double2 lo2 = __ldg(T0), hi2 = __ldg(T0 + 1);
+                        const double t0 = fma(fa, lo2.y - lo2.x, lo2.x), t1 = fma(fa, hi2.y - hi2.x, hi2.x);
+                        A = fma(tb_f, t1 - t0, t0);
+                    }
+                    v[e] = (FULL || j0 + SP_G * e < jend) ? A : neg_inf();
+                    dl[e] = v[e] - run_m;
+                    need = need || (__double2hiint(dl[e]) >= SP_RAISE_HI);   // dl >= 512 (or NaN): test on the high word
+                }
+                if (__any_sync(0xffffffffu, need)) {
+                    // raise the reference to the largest new value (rare); the running sum is rescaled exactly
+                    const double mx = fmax(fmax(v[0], v[1]), fmax(v[2], v[3]));
+                    if (mx - run_m >= 512.0) {
+                        const double dm = run_m - mx;
+                        run_s = dm > -690.0 ? run_s * sp_exp_small(dm) : 0.0;
+                        run_m = mx;
+                    }
+#pragma unroll
+                    for (int e = 0; e < 4; e++) dl[e] = v[e] - run_m;
+                }
+                double part = 0.0;
+#pragma unroll
+                for (int e = 0; e < 4; e++) {
+                    // terms below e^-40 of the reference (and rows past the end) are clamped to e^-40 (R2)
+                    const unsigned hc = min((unsigned)__double2hiint(dl[e]), 0xC0440000u);
+                    const double t = sp_exp_tab(__hiloint2double((int)hc, __double2loint(dl[e])), etab);
+                    part = e == 0 ? t : part + t;
+                }
+                run_s += part;
+            };
+            auto lse_rows = [&](const int jend) {
+                int j0 = jdone + g;
+                for (; j0 + 3 * SP_G < jend; j0 += 4 * SP_G) lse_batch(j0, jend, std::true_type{});
+                if (j0 < jend) lse_batch(j0, jend, std::false_type{});
                 jdone = max(jdone, jend);
             };
 
