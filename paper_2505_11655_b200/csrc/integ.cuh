@@ -100,7 +100,6 @@ struct ile_integrator {
     void* sort_scratch;
     double* gmm_part;                               // [C][blocks][28+] partial moments
     int gmm_blocks;
-    double* gmm_aw;                                 // [C][cap] responsibility x weight of the last batch
     double* port_part;                              // [members][blocks][3]
     int port_blocks;
     ile_result* res;                                // device: last iteration + cumulative

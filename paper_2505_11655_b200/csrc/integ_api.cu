@@ -203,7 +203,7 @@ static void free_integrator(ile_integrator* it) {
     if (!it) return;
     cudaFree(it->z); cudaFree(it->ln_ps); cudaFree(it->lnL); cudaFree(it->lnw); cudaFree(it->ln_prior);
     cudaFree(it->us); cudaFree(it->skey); cudaFree(it->q); cudaFree(it->kbuf0); cudaFree(it->kbuf1);
-    cudaFree(it->sel_hist); cudaFree(it->blk_count); cudaFree(it->sort_scratch); cudaFree(it->gmm_part); cudaFree(it->gmm_aw);
+    cudaFree(it->sel_hist); cudaFree(it->blk_count); cudaFree(it->sort_scratch); cudaFree(it->gmm_part);
     cudaFree(it->port_part); cudaFree(it->res); cudaFree(it->arena);
     for (int a = 0; a < ILE_MAX_MEMBERS; a++) cudaFree(it->I.mem[a].keys);
     free(it);
@@ -322,9 +322,8 @@ extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o,
         IT_ALLOC(it->sort_scratch, radix_sort_scratch_bytes((int)cap));
     }
     if (has_gmm) {
-        it->gmm_blocks = ctx->sm_count * 2;
+        it->gmm_blocks = ctx->sm_count * 4;
         IT_ALLOC(it->gmm_part, (size_t)I.n_gmm * it->gmm_blocks * 48 * 8);
-        IT_ALLOC(it->gmm_aw, (size_t)I.n_gmm * cap * 8);
     }
     it->port_blocks = ctx->sm_count;
     IT_ALLOC(it->port_part, (size_t)Ns * it->port_blocks * 3 * 8);

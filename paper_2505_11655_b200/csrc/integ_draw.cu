@@ -13,14 +13,14 @@
 // ---------------------------------------------------------------- member densities
 template <int D>
 __device__ __forceinline__ double ln_pdf_ac(const IntegDev& I, const SamplerDev& S, const double* zz) {
-    double out = 0.0;
+    // one logarithm of the product of the D marginal densities (each within [1e-30, 1e30]: no overflow for D <= 8)
+    double prod = 1.0;
 #pragma unroll
     for (int c = 0; c < D; c++) {
         const long long b = bin_index_dev(zz[c], I.lo[c], I.hi[c], S.nb);
-        const double pdf = __ddiv_rn(__dmul_rn(S.pi[c * S.nb + b], (double)S.nb), __dsub_rn(I.hi[c], I.lo[c]));
-        out = __dadd_rn(out, log(pdf));
+        prod *= __ddiv_rn(__dmul_rn(S.pi[c * S.nb + b], (double)S.nb), __dsub_rn(I.hi[c], I.lo[c]));
     }
-    return out;
+    return log(prod);
 }
 
 template <int D>
@@ -41,15 +41,19 @@ __device__ __forceinline__ double ln_pdf_av(const IntegDev& I, const SamplerDev&
 }
 
 // Per-component constants of a GMM member, computed once per block into shared memory instead of once per
-// sample: gc[c] = sum_i ln L_c[i][i] (same order as the per-sample loop had), gc[16 + c] = ln omega_c.
-// The densities below are bit-identical to evaluating these logarithms in place.
-#define GMM_GC 32
+// sample: gc[c] = sum_i ln L_c[i][i], gc[16 + c] = ln omega_c, gc[32 + 8 c + i] = 1 / L_c[i][i] (the forward
+// substitution multiplies by it; same constants as the EM kernel's, integ_update.cu).
+#define GMM_GC (32 + 16 * 8)
+#define LN_TWO_PI 1.8378770664093453
 __device__ __forceinline__ void gmm_consts(const IntegDev& I, const double* g, double* gc, int t, int nt) {
     const int d = I.gd, C = I.n_gmm;
     const double* L = g + C + C * d + C * d * d;
     for (int c = t; c < C; c += nt) {
         double lndet = 0.0;
-        for (int i = 0; i < d; i++) lndet = lndet + log(L[c * d * d + i * d + i]);
+        for (int i = 0; i < d; i++) {
+            lndet = lndet + log(L[c * d * d + i * d + i]);
+            gc[32 + 8 * c + i] = 1.0 / L[c * d * d + i * d + i];
+        }
         gc[c] = lndet;
         gc[16 + c] = log(g[c]);
     }
@@ -87,6 +91,7 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
         }
     double e[16];
     double mx = neg_inf();
+    const double cst = -0.5 * d * LN_TWO_PI;
     for (int c = 0; c < C; c++) {
         const double* Lc = L + c * d * d;
         double y[D];
@@ -97,10 +102,10 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
                 double s = zg[i] - mu[c * d + i];
 #pragma unroll
                 for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
-                y[i] = s / Lc[i * d + i];
+                y[i] = s * gc[32 + 8 * c + i];
                 quad = quad + y[i] * y[i];
             }
-        e[c] = -0.5 * quad - gc[c] - 0.5 * d * log(TWO_PI) + gc[16 + c];
+        e[c] = -0.5 * quad - gc[c] + cst + gc[16 + c];
         mx = fmax(mx, e[c]);
     }
     double sum = 0.0;

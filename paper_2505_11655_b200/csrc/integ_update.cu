@@ -472,8 +472,23 @@ __global__ void av_commit_kernel(IntegDev I, int a, UpdScratch* us) {
 // ---------------------------------------------------------------- GMM (one weighted EM step)
 #define GMM_NACC 36                                         // 1 + d + d(d+1)/2 at d = 7; d = 8 needs 45
 #define GMM_NACC_MAX 48
-// gc: per-component constants in shared memory (gc[c] = sum_i ln L_c[i][i], gc[16 + c] = ln omega_c), computed
-// once per block; bit-identical to evaluating the logarithms per sample
+// gc: per-component constants in shared memory, computed once per block: gc[c] = sum_i ln L_c[i][i],
+// gc[16 + c] = ln omega_c, gc[32 + 8 c + i] = 1 / L_c[i][i] (the forward substitution multiplies by it)
+#define GMM_GCN (32 + 16 * 8)
+#define LN_TWO_PI 1.8378770664093453
+__device__ __forceinline__ void gmm_block_consts(const IntegDev& I, const double* g, double* gc) {
+    const int d = I.gd, C = I.n_gmm;
+    const double* L = g + C + C * d + C * d * d;
+    for (int c = threadIdx.x; c < C; c += blockDim.x) {
+        double lndet = 0.0;
+        for (int i = 0; i < d; i++) {
+            lndet = lndet + log(L[c * d * d + i * d + i]);
+            gc[32 + 8 * c + i] = 1.0 / L[c * d * d + i * d + i];
+        }
+        gc[c] = lndet;
+        gc[16 + c] = log(g[c]);
+    }
+}
 template <int D>
 __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g, const double* zg, double* e, const double* gc) {
     const int d = I.gd;                      // modelled dimensions (zg: their coordinates, in the mixture's order)
@@ -481,6 +496,7 @@ __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g
     const double* omega = g;
     const double* mu = omega + C;
     const double* L = mu + C * d + C * d * d;
+    const double cst = -0.5 * d * LN_TWO_PI;
     double mx = neg_inf();
     for (int c = 0; c < C; c++) {
         const double* Lc = L + c * d * d;
@@ -492,95 +508,113 @@ __device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g
                 double s = zg[i] - mu[c * d + i];
 #pragma unroll
                 for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
-                y[i] = s / Lc[i * d + i];
+                y[i] = s * gc[32 + 8 * c + i];
                 quad = quad + y[i] * y[i];
             }
-        e[c] = -0.5 * quad - gc[c] - 0.5 * d * log(6.283185307179586) + gc[16 + c];
+        e[c] = -0.5 * quad - gc[c] + cst + gc[16 + c];
         mx = fmax(mx, e[c]);
     }
     return mx;
 }
 
-// E step: a[c][i] = responsibility of component c for sample i times its importance weight
-// (0 for samples outside the box or with a non-finite weight); one evaluation of the mixture per sample
+// One weighted EM step's sums in one pass (E step + M-step moments).  Per round of 256 samples: thread t evaluates the
+// mixture at its sample and leaves the responsibilities x importance weight R[t][c] (0 outside the box or for a
+// non-finite weight) and the modelled coordinates Z[t][.] in shared memory; then thread (slice, component c, moment q)
+// adds its slice of the round to its moment about the component's old mean: q = 0: sum R, 1 + r: sum R dz_r,
+// 1 + D + r (r + 1) / 2 + s: sum R dz_r dz_s (layout by the total dimension D; entries past gd stay 0).  Column D of Z is
+// the constant 1 with mean 0, so every moment is sum R (Z[ia] - mu[ia]) (Z[ib] - mu[ib]) for an index pair (ia, ib).
+#define GMM_SLOTS 3                                          // moment slots per thread: 16 components x 45 moments / 256
 template <int D>
-__global__ void __launch_bounds__(256) gmm_resp_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ lnw,
-                                                       const UpdScratch* __restrict__ us, double* __restrict__ aw) {
+__global__ void __launch_bounds__(256) gmm_em_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ lnw,
+                                                     const UpdScratch* __restrict__ us, double* __restrict__ part) {
     if (us->abort || us->n_valid == 0) return;
-    const int d = I.gd;
-    const int C = I.n_gmm;
+    constexpr int NACC = 1 + D + D * (D + 1) / 2, ZP = D + 1 + ((D + 1) & 1 ? 0 : 1);      // odd row strides: no bank conflicts
+    const int d = I.gd, C = I.n_gmm, CP = C | 1, t = threadIdx.x;
     const double* g = I.mem[a].gmm;
-    __shared__ double gc[32];
-    if (threadIdx.x < C) {
-        const double* L = g + C + C * d + C * d * d;
-        double lndet = 0.0;
-        for (int i = 0; i < d; i++) lndet = lndet + log(L[threadIdx.x * d * d + i * d + i]);
-        gc[threadIdx.x] = lndet;
-        gc[16 + threadIdx.x] = log(g[threadIdx.x]);
+    __shared__ double gc[GMM_GCN];
+    extern __shared__ double em_sh[];
+    double* R = em_sh;                       // [256][CP]
+    double* Z = R + 256 * CP;                // [256][ZP]
+    double* mu_s = Z + 256 * ZP;             // [C][D + 1]
+    gmm_block_consts(I, g, gc);
+    for (int q = t; q < C * (D + 1); q += 256) {
+        const int c = q / (D + 1), r = q - c * (D + 1);
+        mu_s[q] = r < d ? g[C + c * d + r] : 0.0;
+    }
+    // the moments this thread accumulates
+    const int NP = C * NACC, SL = NP >= 256 ? 1 : 256 / NP, per = (256 + SL - 1) / SL;
+    int sc[GMM_SLOTS], sia[GMM_SLOTS], sib[GMM_SLOTS], s0[GMM_SLOTS], s1[GMM_SLOTS];
+    double acc[GMM_SLOTS];
+#pragma unroll
+    for (int k = 0; k < GMM_SLOTS; k++) {
+        const int item = t + 256 * k;
+        acc[k] = 0.0;
+        sc[k] = sia[k] = sib[k] = s0[k] = s1[k] = 0;
+        if (item < NP * SL) {
+            const int pair = item % NP, sl = item / NP;
+            const int c = pair / NACC, q = pair - c * NACC;
+            int ia = D, ib = D;
+            if (q >= 1 && q <= D) ia = q - 1;
+            else if (q > D) {
+                int r = 0;
+                while (1 + D + (r + 1) * (r + 2) / 2 <= q) r++;
+                ia = r;
+                ib = q - (1 + D + r * (r + 1) / 2);
+            }
+            sc[k] = c; sia[k] = ia; sib[k] = ib;
+            s0[k] = sl * per;
+            s1[k] = min(256, s0[k] + per);
+        }
     }
     __syncthreads();
     const double m = double_from_ord(us->m_ord);
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
-        const double w = lnw[i];
-        const bool ok = is_finite_d(w) && in_box_dev(I, z, N, i);
+    for (long long base = (long long)blockIdx.x * 256; base < N; base += (long long)gridDim.x * 256) {
+        const long long i = base + t;
+        double w = neg_inf();
+        bool ok = false;
+        if (i < N) {
+            w = lnw[i];
+            ok = is_finite_d(w) && in_box_dev(I, z, N, i);
+        }
         double zz[D], e[16];
 #pragma unroll
-        for (int c = 0; c < D; c++)
-            if (c < d) zz[c] = z[(long long)I.gdim[c] * N + i];
+        for (int c = 0; c < D; c++) zz[c] = (c < d && i < N) ? z[(long long)I.gdim[c] * N + i] : 0.0;
         double mx = 0.0, sum = 1.0;
         if (ok) {
             mx = ln_comp_all<D>(I, g, zz, e, gc);
             sum = 0.0;
-            for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
+            for (int c = 0; c < C; c++) {
+                e[c] = exp(e[c] - mx);
+                sum += e[c];
+            }
         }
-        const double wt = ok ? exp(w - m) : 0.0;
-        for (int c = 0; c < C; c++) aw[(long long)c * N + i] = ok ? exp(e[c] - mx) / sum * wt : 0.0;
-    }
-}
-
-// M-step moments of component blockIdx.y about its old mean: s0, s1[D], s2[D(D+1)/2] (registers)
-template <int D>
-__global__ void __launch_bounds__(256) gmm_moments_kernel(IntegDev I, int a, int N, const double* __restrict__ z, const double* __restrict__ aw,
-                                                          const UpdScratch* __restrict__ us, double* __restrict__ part) {
-    if (us->abort || us->n_valid == 0) return;
-    constexpr int NACC = 1 + D + D * (D + 1) / 2;
-    const int C = I.n_gmm, comp = blockIdx.y, gd = I.gd;
-    const double* mu = I.mem[a].gmm + C + comp * gd;
-    double mu_r[D];
+        const double wt = ok ? exp(w - m) / sum : 0.0;
+        for (int c = 0; c < C; c++) R[t * CP + c] = ok ? e[c] * wt : 0.0;
 #pragma unroll
-    for (int r = 0; r < D; r++) mu_r[r] = r < gd ? mu[r] : 0.0;
-    double acc[NACC];
+        for (int c = 0; c < D; c++) Z[t * ZP + c] = zz[c];
+        Z[t * ZP + D] = 1.0;
+        __syncthreads();
 #pragma unroll
-    for (int q = 0; q < NACC; q++) acc[q] = 0.0;
-    const double* awc = aw + (long long)comp * N;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
-        const double wgt = awc[i];
-        if (wgt == 0.0) continue;
-        double dz[D];
-#pragma unroll
-        for (int r = 0; r < D; r++) dz[r] = r < gd ? z[(long long)I.gdim[r] * N + i] - mu_r[r] : 0.0;
-        acc[0] += wgt;
-        int q = 1 + D;                      // accumulator layout by the total dimension D (static indices); entries past gd stay 0
-#pragma unroll
-        for (int r = 0; r < D; r++) {
-            const double t = wgt * dz[r];
-            acc[1 + r] += t;
-#pragma unroll
-            for (int s2 = 0; s2 <= r; s2++) acc[q++] += t * dz[s2];
+        for (int k = 0; k < GMM_SLOTS; k++) {
+            const double ma = mu_s[sc[k] * (D + 1) + sia[k]], mb = mu_s[sc[k] * (D + 1) + sib[k]];
+            double v = acc[k];
+#pragma unroll 4
+            for (int sm = s0[k]; sm < s1[k]; sm++) v = fma(R[sm * CP + sc[k]], (Z[sm * ZP + sia[k]] - ma) * (Z[sm * ZP + sib[k]] - mb), v);
+            acc[k] = v;
         }
+        __syncthreads();
     }
-    __shared__ double sh[8][GMM_NACC_MAX];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    // slices of a moment meet in shared memory; one partial per (component, block, moment)
+    double* red = R;
 #pragma unroll
-    for (int q = 0; q < NACC; q++) {
-        const double v = warp_sum(acc[q]);
-        if (lane == 0) sh[w][q] = v;
-    }
+    for (int k = 0; k < GMM_SLOTS; k++)
+        if (t + 256 * k < NP * SL) red[t + 256 * k] = acc[k];
     __syncthreads();
-    if (threadIdx.x < NACC) {
+    for (int pair = t; pair < NP; pair += 256) {
         double v = 0.0;
-        for (int ww = 0; ww < 8; ww++) v += sh[ww][threadIdx.x];
-        part[((size_t)comp * gridDim.x + blockIdx.x) * GMM_NACC_MAX + threadIdx.x] = v;
+        for (int sl = 0; sl < SL; sl++) v += red[sl * NP + pair];
+        const int c = pair / NACC, q = pair - c * NACC;
+        part[((size_t)c * gridDim.x + blockIdx.x) * GMM_NACC_MAX + q] = v;
     }
 }
 
@@ -691,24 +725,28 @@ __global__ void __launch_bounds__(256) port_ness_kernel(IntegDev I, const double
 }
 
 __global__ void port_weights_kernel(IntegDev I, const double* __restrict__ part, int blocks) {
-    if (threadIdx.x || blockIdx.x) return;
+    // one warp: the lanes share the per-block partials of a member, lane 0 then sets the weights
     PortState* P = I.port;
-    const int Ns = I.n_members;
+    const int Ns = I.n_members, lane = threadIdx.x;
     double ness[ILE_MAX_MEMBERS], tot = 0.0;
     for (int a = 0; a < Ns; a++) {
         double bm = neg_inf();
-        for (int b = 0; b < blocks; b++) bm = fmax(bm, part[((size_t)a * blocks + b) * 3]);
+        for (int b = lane; b < blocks; b += 32) bm = fmax(bm, part[((size_t)a * blocks + b) * 3]);
+        bm = warp_max(bm);
         double t1 = 0.0, t2 = 0.0;
-        for (int b = 0; b < blocks; b++) {
+        for (int b = lane; b < blocks; b += 32) {
             const double* o = part + ((size_t)a * blocks + b) * 3;
             if (o[0] == neg_inf()) continue;
             const double e = exp(o[0] - bm);
             t1 += o[1] * e;
             t2 += o[2] * e * e;
         }
+        t1 = warp_sum(t1);
+        t2 = warp_sum(t2);
         ness[a] = (bm == neg_inf() || !(t2 > 0.0)) ? 0.0 : t1 * t1 / t2;
         tot += ness[a];
     }
+    if (lane) return;
     // members that are not activated are never trained; silent ones always are
     int n_con = 0;
     for (int a = 0; a < Ns; a++) {
@@ -803,15 +841,13 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
             ILE_LAUNCH_CHECK(ctx);
             mask_max_kernel<<<grid, 256, 0, st>>>(I, N, z, lnw, nullptr, MASK_BOX, it->us);
             ILE_LAUNCH_CHECK(ctx);
+            const size_t em_smem = ((size_t)256 * ((I.n_gmm | 1) + 10) + (size_t)I.n_gmm * 9 + 16) * sizeof(double);
             switch (I.d) {
-#define GMM_RESP(D) case D: gmm_resp_kernel<D><<<grid, 256, 0, st>>>(I, a, N, z, lnw, it->us, it->gmm_aw); break;
-                GMM_RESP(1) GMM_RESP(2) GMM_RESP(3) GMM_RESP(4) GMM_RESP(5) GMM_RESP(6) GMM_RESP(7) GMM_RESP(8)
-#undef GMM_RESP
-            }
-            ILE_LAUNCH_CHECK(ctx);
-            dim3 g(it->gmm_blocks, I.n_gmm);
-            switch (I.d) {
-#define GMM_CASE(D) case D: gmm_moments_kernel<D><<<g, 256, 0, st>>>(I, a, N, z, it->gmm_aw, it->us, it->gmm_part); break;
+#define GMM_CASE(D)                                                                                                        \
+    case D:                                                                                                                \
+        ILE_CUDA(ctx, cudaFuncSetAttribute(gmm_em_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)em_smem)); \
+        gmm_em_kernel<D><<<it->gmm_blocks, 256, em_smem, st>>>(I, a, N, z, lnw, it->us, it->gmm_part);                     \
+        break;
                 GMM_CASE(1) GMM_CASE(2) GMM_CASE(3) GMM_CASE(4) GMM_CASE(5) GMM_CASE(6) GMM_CASE(7) GMM_CASE(8)
 #undef GMM_CASE
             }

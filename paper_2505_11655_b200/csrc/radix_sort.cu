@@ -1,6 +1,7 @@
 // libile: device-resident stable LSD radix sort (see radix_sort.cuh).  Three kernels per 8-bit
-// pass: per-block digit histogram, one-block exclusive scan of the [digit][block] table, and a
-// stable scatter that ranks keys inside a warp with __match_any_sync.
+// pass: per-block digit histogram into a [digit][block] table, an exclusive scan of every digit's row
+// (one block per digit, row totals aside), and a stable scatter that ranks keys inside a warp with
+// __match_any_sync and adds the scan of the 256 row totals itself.
 #include "radix_sort.cuh"
 
 __device__ __forceinline__ int rs_passes(int bits) { return bits <= 0 ? 0 : (bits + 7) >> 3; }
@@ -30,40 +31,38 @@ __global__ void __launch_bounds__(RS_THREADS) rs_hist_kernel(int p, const long l
         if (act && (threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&sh[dg], (uint32_t)__popc(m));
     }
     __syncthreads();
-    hist[(size_t)blockIdx.x * 256 + threadIdx.x] = sh[threadIdx.x];      // [block][digit]: coalesced
+    hist[(size_t)threadIdx.x * max_blocks + blockIdx.x] = sh[threadIdx.x];      // [digit][block]
 }
 
-// exclusive scan of the counts in (digit, block) order; stored as hist[block][digit]
-__global__ void __launch_bounds__(1024) rs_scan_kernel(int p, const long long* __restrict__ n_dev, const int* __restrict__ bits_dev,
-                                                       uint32_t* __restrict__ hist, int max_blocks) {
+// exclusive scan of digit blockIdx.x's counts over the blocks, in place; the row total goes to hist[256 max_blocks + digit]
+__global__ void __launch_bounds__(256) rs_scan_kernel(int p, const long long* __restrict__ n_dev, const int* __restrict__ bits_dev,
+                                                      uint32_t* __restrict__ hist, int max_blocks) {
     const int npass = rs_passes(*bits_dev);
     if (p >= npass) return;
     const long long n = *n_dev;
     const int nblocks = (int)((n + RS_TILE - 1) / RS_TILE);
-    __shared__ uint32_t part[1024];
-    // thread (qd, dg): digit dg, quarter qd of the blocks; consecutive threads read consecutive digits
-    const int t = threadIdx.x, dg = t & 255, qd = t >> 8;
-    const int per = (nblocks + 3) >> 2;
-    const int b0 = min(qd * per, nblocks), b1 = min(b0 + per, nblocks);
+    uint32_t* row = hist + (size_t)blockIdx.x * max_blocks;
+    __shared__ uint32_t part[256];
+    const int t = threadIdx.x;
+    const int per = (nblocks + 255) >> 8;
+    const int b0 = min(t * per, nblocks), b1 = min(b0 + per, nblocks);
     uint32_t s = 0;
-#pragma unroll 8
-    for (int b = b0; b < b1; b++) s += hist[(size_t)b * 256 + dg];
-    part[dg * 4 + qd] = s;                       // digit-major order of the scan
+    for (int b = b0; b < b1; b++) s += row[b];
+    part[t] = s;
     __syncthreads();
-    // block-wide exclusive scan of part[] (1024 entries)
-    const int o_idx = dg * 4 + qd;
-    for (int o = 1; o < 1024; o <<= 1) {
-        uint32_t add = (t >= o) ? part[t - o] : 0;
+    for (int o = 1; o < 256; o <<= 1) {
+        const uint32_t add = (t >= o) ? part[t - o] : 0;
         __syncthreads();
         part[t] += add;
         __syncthreads();
     }
-    uint32_t run = part[o_idx] - s;
+    uint32_t run = part[t] - s;
     for (int b = b0; b < b1; b++) {
-        uint32_t c = hist[(size_t)b * 256 + dg];
-        hist[(size_t)b * 256 + dg] = run;
+        const uint32_t c = row[b];
+        row[b] = run;
         run += c;
     }
+    if (t == 255) hist[(size_t)256 * max_blocks + blockIdx.x] = part[255];
 }
 
 template <bool HAS_VAL>
@@ -98,10 +97,20 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(int p, const lon
         __syncwarp();
     }
     __syncthreads();
-    // phase B: turn the counts into start offsets (global base of (digit, block) + earlier warps)
+    // phase B: turn the counts into start offsets (digits below + this digit in earlier blocks + earlier warps)
     {
+        __shared__ uint32_t dsum[256];
         const int dg = threadIdx.x;
-        uint32_t run = hist[(size_t)blockIdx.x * 256 + dg];
+        const uint32_t tot = hist[(size_t)256 * max_blocks + dg];
+        dsum[dg] = tot;
+        __syncthreads();
+        for (int o = 1; o < 256; o <<= 1) {
+            const uint32_t add = (dg >= o) ? dsum[dg - o] : 0;
+            __syncthreads();
+            dsum[dg] += add;
+            __syncthreads();
+        }
+        uint32_t run = dsum[dg] - tot + hist[(size_t)dg * max_blocks + blockIdx.x];
         for (int ww = 0; ww < RS_THREADS / 32; ww++) {
             uint32_t c = wh[ww][dg];
             wh[ww][dg] = run;
@@ -145,7 +154,7 @@ __global__ void rs_finish_kernel(const long long* __restrict__ n_dev, const int*
 size_t radix_sort_scratch_bytes(int max_n) {
     size_t blocks = ((size_t)max_n + RS_TILE - 1) / RS_TILE;
     if (blocks < 1) blocks = 1;
-    return 256 * blocks * sizeof(uint32_t);
+    return (256 * blocks + 256) * sizeof(uint32_t);
 }
 
 int radix_sort_device(ile_ctx* ctx, int max_n, const long long* n_dev, const int* bits_dev, uint64_t* k0, uint32_t* v0, uint64_t* k1,
@@ -158,7 +167,7 @@ int radix_sort_device(ile_ctx* ctx, int max_n, const long long* n_dev, const int
     for (int p = 0; p < max_passes; p++) {
         rs_hist_kernel<<<blocks, RS_THREADS, 0, ctx->stream>>>(p, n_dev, bits_dev, k0, k1, hist, blocks);
         ILE_LAUNCH_CHECK(ctx);
-        rs_scan_kernel<<<1, 1024, 0, ctx->stream>>>(p, n_dev, bits_dev, hist, blocks);
+        rs_scan_kernel<<<256, 256, 0, ctx->stream>>>(p, n_dev, bits_dev, hist, blocks);
         ILE_LAUNCH_CHECK(ctx);
         if (has_val) rs_scatter_kernel<true><<<blocks, RS_THREADS, 0, ctx->stream>>>(p, n_dev, bits_dev, k0, v0, k1, v1, hist, blocks);
         else rs_scatter_kernel<false><<<blocks, RS_THREADS, 0, ctx->stream>>>(p, n_dev, bits_dev, k0, v0, k1, v1, hist, blocks);

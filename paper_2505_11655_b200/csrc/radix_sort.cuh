@@ -13,7 +13,7 @@
 struct RadixSortPlan {
     int max_n;                // capacity the buffers were sized for
     int max_blocks;           // ceil(max_n / RS_TILE)
-    uint32_t* hist;           // [256][max_blocks] per pass (reused), digit-major
+    uint32_t* hist;           // [256][max_blocks] per pass (reused), digit-major, + 256 row totals
     size_t bytes;             // scratch bytes behind hist
 };
 
