@@ -193,6 +193,64 @@ __device__ __forceinline__ unsigned long long av_key_dev(const IntegDev& I, cons
     return key;
 }
 
+// ---------------------------------------------------------------- GMM member in shared memory
+// One copy per block of what every density evaluation reads, at fixed strides (so that the unrolled forward
+// substitution addresses it with immediates): lndet[c] = sum_i ln L_c[i][i], lnom[c] = ln omega_c,
+// inv[c][i] = 1 / L_c[i][i], mu[c][i], L[c][i][k]; 16 components x 8 dimensions.
+#define GMS_LNDET 0
+#define GMS_LNOM 16
+#define GMS_INV 32
+#define GMS_MU (32 + 128)
+#define GMS_L (32 + 256)
+#define GMS_DOUBLES (32 + 256 + 1024)
+#define LN_TWO_PI 1.8378770664093453
+__device__ __forceinline__ void gmm_load_shared(const IntegDev& I, const double* __restrict__ g, double* __restrict__ gs) {
+    const int d = I.gd, C = I.n_gmm;
+    const double* mu = g + C;
+    const double* L = mu + C * d + C * d * d;
+    for (int c = threadIdx.x; c < C; c += blockDim.x) {
+        double lndet = 0.0;
+        for (int i = 0; i < d; i++) {
+            lndet = lndet + log(L[c * d * d + i * d + i]);
+            gs[GMS_INV + 8 * c + i] = 1.0 / L[c * d * d + i * d + i];
+        }
+        gs[GMS_LNDET + c] = lndet;
+        gs[GMS_LNOM + c] = log(g[c]);
+    }
+    for (int q = threadIdx.x; q < C * 64; q += blockDim.x) {
+        const int c = q >> 6, i = (q >> 3) & 7, k = q & 7;
+        gs[GMS_L + q] = (i < d && k < d) ? L[c * d * d + i * d + k] : 0.0;
+        if (k == 0) gs[GMS_MU + 8 * c + i] = i < d ? mu[c * d + i] : 0.0;
+    }
+}
+// e[c] = ln omega_c + ln N(zg; mu_c, Sigma_c) for every component (zg: the modelled coordinates, in the mixture's
+// order); returns the largest
+template <int D>
+__device__ __forceinline__ double gmm_ln_comps(const IntegDev& I, const double* __restrict__ gs, const double* zg, double* e) {
+    const int d = I.gd, C = I.n_gmm;
+    const double cst = -0.5 * d * LN_TWO_PI;
+    double mx = neg_inf();
+    for (int c = 0; c < C; c++) {
+        const double* Lc = gs + GMS_L + 64 * c;
+        const double* mc = gs + GMS_MU + 8 * c;
+        const double* ic = gs + GMS_INV + 8 * c;
+        double y[D];
+        double quad = 0.0;
+#pragma unroll
+        for (int i = 0; i < D; i++)
+            if (i < d) {
+                double s = zg[i] - mc[i];
+#pragma unroll
+                for (int k = 0; k < i; k++) s = s - Lc[i * 8 + k] * y[k];
+                y[i] = s * ic[i];
+                quad = quad + y[i] * y[i];
+            }
+        e[c] = -0.5 * quad - gs[GMS_LNDET + c] + cst + gs[GMS_LNOM + c];
+        mx = fmax(mx, e[c]);
+    }
+    return mx;
+}
+
 // ---------------------------------------------------------------- cross-file entry points
 int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, double* ln_ps);
 int integ_launch_ln_pdf(ile_integrator* it, int N, const double* z, double* ln_ps);

@@ -7,6 +7,7 @@
 //             p_s = sum_a W_a p_{s,a}
 // Counter-based generator: Philox4x32-10, counter (sample index, iteration, stream).
 #include "integ.cuh"
+#include <algorithm>
 
 #define TWO_PI 6.283185307179586
 
@@ -40,23 +41,14 @@ __device__ __forceinline__ double ln_pdf_av(const IntegDev& I, const SamplerDev&
     return (lo < av.C && S.keys[lo] == key) ? av.ln_ps : neg_inf();
 }
 
-// Per-component constants of a GMM member, computed once per block into shared memory instead of once per
-// sample: gc[c] = sum_i ln L_c[i][i], gc[16 + c] = ln omega_c, gc[32 + 8 c + i] = 1 / L_c[i][i] (the forward
-// substitution multiplies by it; same constants as the EM kernel's, integ_update.cu).
-#define GMM_GC (32 + 16 * 8)
-#define LN_TWO_PI 1.8378770664093453
-__device__ __forceinline__ void gmm_consts(const IntegDev& I, const double* g, double* gc, int t, int nt) {
-    const int d = I.gd, C = I.n_gmm;
-    const double* L = g + C + C * d + C * d * d;
-    for (int c = t; c < C; c += nt) {
-        double lndet = 0.0;
-        for (int i = 0; i < d; i++) {
-            lndet = lndet + log(L[c * d * d + i * d + i]);
-            gc[32 + 8 * c + i] = 1.0 / L[c * d * d + i * d + i];
-        }
-        gc[c] = lndet;
-        gc[16 + c] = log(g[c]);
-    }
+// Block-shared constants (dynamic shared memory): ln W_a of the members, then one GMM block (integ.cuh, GMS_*) per
+// GMM member in member order.
+#define DRAW_LNW 0
+#define DRAW_GMS ILE_MAX_MEMBERS
+__device__ __forceinline__ const double* member_gms(const IntegDev& I, int a, const double* sh) {
+    int slot = 0;
+    for (int b = 0; b < a; b++) slot += I.mem[b].kind == ILE_KIND_GMM;
+    return sh + DRAW_GMS + slot * GMS_DOUBLES;
 }
 
 // ln N(z; mu_c, Sigma_c) + ln omega_c for every component; returns the log-sum-exp
@@ -73,12 +65,9 @@ __device__ __forceinline__ void gmm_gather(const IntegDev& I, const double* zz, 
 }
 
 template <int D>
-__device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev& S, const double* zz, double* e_out, const double* gc) {
+__device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const double* zz, const double* gs) {
     const int d = I.gd;
     const int C = I.n_gmm;
-    const double* omega = S.gmm;
-    const double* mu = omega + C;
-    const double* L = mu + C * d + C * d * d;
     double zg[D];
     gmm_gather<D>(I, zz, zg);
     bool uok = true;                       // the dimensions the mixture leaves alone: uniform over the box, zero outside
@@ -90,57 +79,38 @@ __device__ __forceinline__ double ln_pdf_gmm(const IntegDev& I, const SamplerDev
                 if (I.udim[q] == c) uok = uok && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
         }
     double e[16];
-    double mx = neg_inf();
-    const double cst = -0.5 * d * LN_TWO_PI;
-    for (int c = 0; c < C; c++) {
-        const double* Lc = L + c * d * d;
-        double y[D];
-        double quad = 0.0;
-#pragma unroll
-        for (int i = 0; i < D; i++)
-            if (i < d) {
-                double s = zg[i] - mu[c * d + i];
-#pragma unroll
-                for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
-                y[i] = s * gc[32 + 8 * c + i];
-                quad = quad + y[i] * y[i];
-            }
-        e[c] = -0.5 * quad - gc[c] + cst + gc[16 + c];
-        mx = fmax(mx, e[c]);
-    }
+    const double mx = gmm_ln_comps<D>(I, gs, zg, e);
     double sum = 0.0;
     for (int c = 0; c < C; c++) sum += exp(e[c] - mx);
-    if (e_out)
-        for (int c = 0; c < C; c++) e_out[c] = e[c];
     const double out = mx + log(sum);
     if (d == D) return out;
     return uok ? out - I.ln_uvol : neg_inf();
 }
 
 template <int D>
-__device__ __forceinline__ double member_ln_pdf(const IntegDev& I, int a, const double* zz, bool inbox, const double* gc_all) {
+__device__ __forceinline__ double member_ln_pdf(const IntegDev& I, int a, const double* zz, bool inbox, const double* sh) {
     const SamplerDev& S = I.mem[a];
     switch (S.kind) {
         case ILE_KIND_UNIFORM: return inbox ? -log(I.V0) : neg_inf();
         case ILE_KIND_AC: return inbox ? ln_pdf_ac<D>(I, S, zz) : neg_inf();
         case ILE_KIND_AV: return inbox ? ln_pdf_av<D>(I, S, zz) : neg_inf();
-        case ILE_KIND_GMM: return ln_pdf_gmm<D>(I, S, zz, nullptr, gc_all + a * GMM_GC);
+        case ILE_KIND_GMM: return ln_pdf_gmm<D>(I, zz, member_gms(I, a, sh));
     }
     return neg_inf();
 }
 
 template <int D>
-__device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double* zz, const double* gc_all) {
+__device__ __forceinline__ double mixture_ln_pdf(const IntegDev& I, const double* zz, const double* sh) {
     bool inbox = true;
 #pragma unroll
     for (int c = 0; c < D; c++) inbox = inbox && (zz[c] >= I.lo[c]) && (zz[c] < I.hi[c]);
-    if (I.n_members == 1) return member_ln_pdf<D>(I, 0, zz, inbox, gc_all);
+    if (I.n_members == 1) return member_ln_pdf<D>(I, 0, zz, inbox, sh);
     double e[ILE_MAX_MEMBERS];
     double mx = neg_inf();
     for (int a = 0; a < I.n_members; a++) {
         // members that are not activated yet or contribute silently have weight 0 (ln W = -inf): no term
-        const double lw = gc_all[ILE_MAX_MEMBERS * GMM_GC + a];
-        e[a] = lw == neg_inf() ? neg_inf() : lw + member_ln_pdf<D>(I, a, zz, inbox, gc_all);
+        const double lw = sh[DRAW_LNW + a];
+        e[a] = lw == neg_inf() ? neg_inf() : lw + member_ln_pdf<D>(I, a, zz, inbox, sh);
         mx = fmax(mx, e[a]);
     }
     if (!is_finite_d(mx)) return neg_inf();
@@ -204,24 +174,26 @@ __global__ void alloc_kernel(IntegDev I, long long N, unsigned int g) {
 }
 
 // ---------------------------------------------------------------- draw
-// every GMM member's per-component constants and the members' ln W_a, once per block
-__device__ __forceinline__ void block_gmm_consts(const IntegDev& I, double* gc_all) {
-    bool any = I.n_members > 1;
-    if (I.n_members > 1 && threadIdx.x < I.n_members) gc_all[ILE_MAX_MEMBERS * GMM_GC + threadIdx.x] = I.port->W[threadIdx.x] > 0.0 ? log(I.port->W[threadIdx.x]) : neg_inf();   // ln W_a
+// every GMM member's constants and the members' ln W_a, once per block
+__device__ __forceinline__ void block_consts(const IntegDev& I, double* sh) {
+    if (I.n_members > 1 && threadIdx.x < I.n_members) sh[DRAW_LNW + threadIdx.x] = I.port->W[threadIdx.x] > 0.0 ? log(I.port->W[threadIdx.x]) : neg_inf();
+    int slot = 0;
     for (int a = 0; a < I.n_members; a++)
-        if (I.mem[a].kind == ILE_KIND_GMM) {
-            gmm_consts(I, I.mem[a].gmm, gc_all + a * GMM_GC, threadIdx.x, blockDim.x);
-            any = true;
-        }
-    if (any) __syncthreads();
+        if (I.mem[a].kind == ILE_KIND_GMM) gmm_load_shared(I, I.mem[a].gmm, sh + DRAW_GMS + (slot++) * GMS_DOUBLES);
+    __syncthreads();
+}
+static size_t draw_smem_bytes(const IntegDev& I) {
+    int n = 0;
+    for (int a = 0; a < I.n_members; a++) n += I.mem[a].kind == ILE_KIND_GMM;
+    return ((size_t)ILE_MAX_MEMBERS + (size_t)n * GMS_DOUBLES) * sizeof(double);
 }
 
 template <int D>
 __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned int g, double* __restrict__ z, double* __restrict__ ln_ps) {
-    __shared__ double gc_all[ILE_MAX_MEMBERS * GMM_GC + ILE_MAX_MEMBERS];
-    block_gmm_consts(I, gc_all);
-    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    extern __shared__ double draw_sh[];
+    block_consts(I, draw_sh);
+    // grid-stride: a block builds the shared constants once for all its samples
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
     int a = 0;
     while (a + 1 < I.n_members && i >= I.port->offset[a + 1]) a++;
     const SamplerDev& S = I.mem[a];
@@ -326,27 +298,34 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
 #pragma unroll
     for (int c = 0; c < d; c++) z[(long long)c * N + i] = zz[c];
     // a standalone AV draws inside its own cells: p_s is the constant 1 / (v V0)
-    ln_ps[i] = (I.n_members == 1 && S.kind == ILE_KIND_AV) ? S.av->ln_ps : mixture_ln_pdf<D>(I, zz, gc_all);
+    ln_ps[i] = (I.n_members == 1 && S.kind == ILE_KIND_AV) ? S.av->ln_ps : mixture_ln_pdf<D>(I, zz, draw_sh);
+    }
 }
 
 template <int D>
 __global__ void __launch_bounds__(128) ln_pdf_kernel(IntegDev I, int N, const double* __restrict__ z, double* __restrict__ ln_ps) {
-    __shared__ double gc_all[ILE_MAX_MEMBERS * GMM_GC + ILE_MAX_MEMBERS];
-    block_gmm_consts(I, gc_all);
-    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    double zz[D];
+    extern __shared__ double draw_sh[];
+    block_consts(I, draw_sh);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        double zz[D];
 #pragma unroll
-    for (int c = 0; c < D; c++) zz[c] = z[(long long)c * N + i];
-    ln_ps[i] = mixture_ln_pdf<D>(I, zz, gc_all);
+        for (int c = 0; c < D; c++) zz[c] = z[(long long)c * N + i];
+        ln_ps[i] = mixture_ln_pdf<D>(I, zz, draw_sh);
+    }
 }
 
 int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, double* ln_ps) {
     ile_ctx* ctx = it->ctx;
     alloc_kernel<<<1, 32, 0, ctx->stream>>>(it->I, (long long)N, g);
     ILE_LAUNCH_CHECK(ctx);
+    const size_t smem = draw_smem_bytes(it->I);
+    const int grid = (int)std::min<long long>(((long long)N + 127) / 128, (long long)ctx->sm_count * 32);
     switch (it->I.d) {
-#define DRAW_CASE(D_) case D_: draw_kernel<D_><<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, g, z, ln_ps); break;
+#define DRAW_CASE(D_)                                                                                                  \
+    case D_:                                                                                                           \
+        ILE_CUDA(ctx, cudaFuncSetAttribute(draw_kernel<D_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        draw_kernel<D_><<<grid, 128, smem, ctx->stream>>>(it->I, N, g, z, ln_ps);                                      \
+        break;
         DRAW_CASE(1) DRAW_CASE(2) DRAW_CASE(3) DRAW_CASE(4) DRAW_CASE(5) DRAW_CASE(6) DRAW_CASE(7) DRAW_CASE(8)
 #undef DRAW_CASE
         default: return ile_fail(ctx, ILE_EINVAL, "draw: d = %d", it->I.d);
@@ -357,8 +336,14 @@ int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, doub
 
 int integ_launch_ln_pdf(ile_integrator* it, int N, const double* z, double* ln_ps) {
     ile_ctx* ctx = it->ctx;
+    const size_t smem = draw_smem_bytes(it->I);
+    const int grid = (int)std::min<long long>(((long long)N + 127) / 128, (long long)ctx->sm_count * 32);
     switch (it->I.d) {
-#define PDF_CASE(D_) case D_: ln_pdf_kernel<D_><<<(N + 127) / 128, 128, 0, ctx->stream>>>(it->I, N, z, ln_ps); break;
+#define PDF_CASE(D_)                                                                                                     \
+    case D_:                                                                                                             \
+        ILE_CUDA(ctx, cudaFuncSetAttribute(ln_pdf_kernel<D_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        ln_pdf_kernel<D_><<<grid, 128, smem, ctx->stream>>>(it->I, N, z, ln_ps);                                         \
+        break;
         PDF_CASE(1) PDF_CASE(2) PDF_CASE(3) PDF_CASE(4) PDF_CASE(5) PDF_CASE(6) PDF_CASE(7) PDF_CASE(8)
 #undef PDF_CASE
         default: return ile_fail(ctx, ILE_EINVAL, "ln_pdf: d = %d", it->I.d);

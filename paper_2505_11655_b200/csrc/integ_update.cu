@@ -472,51 +472,6 @@ __global__ void av_commit_kernel(IntegDev I, int a, UpdScratch* us) {
 // ---------------------------------------------------------------- GMM (one weighted EM step)
 #define GMM_NACC 36                                         // 1 + d + d(d+1)/2 at d = 7; d = 8 needs 45
 #define GMM_NACC_MAX 48
-// gc: per-component constants in shared memory, computed once per block: gc[c] = sum_i ln L_c[i][i],
-// gc[16 + c] = ln omega_c, gc[32 + 8 c + i] = 1 / L_c[i][i] (the forward substitution multiplies by it)
-#define GMM_GCN (32 + 16 * 8)
-#define LN_TWO_PI 1.8378770664093453
-__device__ __forceinline__ void gmm_block_consts(const IntegDev& I, const double* g, double* gc) {
-    const int d = I.gd, C = I.n_gmm;
-    const double* L = g + C + C * d + C * d * d;
-    for (int c = threadIdx.x; c < C; c += blockDim.x) {
-        double lndet = 0.0;
-        for (int i = 0; i < d; i++) {
-            lndet = lndet + log(L[c * d * d + i * d + i]);
-            gc[32 + 8 * c + i] = 1.0 / L[c * d * d + i * d + i];
-        }
-        gc[c] = lndet;
-        gc[16 + c] = log(g[c]);
-    }
-}
-template <int D>
-__device__ __forceinline__ double ln_comp_all(const IntegDev& I, const double* g, const double* zg, double* e, const double* gc) {
-    const int d = I.gd;                      // modelled dimensions (zg: their coordinates, in the mixture's order)
-    const int C = I.n_gmm;
-    const double* omega = g;
-    const double* mu = omega + C;
-    const double* L = mu + C * d + C * d * d;
-    const double cst = -0.5 * d * LN_TWO_PI;
-    double mx = neg_inf();
-    for (int c = 0; c < C; c++) {
-        const double* Lc = L + c * d * d;
-        double y[D];
-        double quad = 0.0;
-#pragma unroll
-        for (int i = 0; i < D; i++)
-            if (i < d) {
-                double s = zg[i] - mu[c * d + i];
-#pragma unroll
-                for (int k = 0; k < i; k++) s = s - Lc[i * d + k] * y[k];
-                y[i] = s * gc[32 + 8 * c + i];
-                quad = quad + y[i] * y[i];
-            }
-        e[c] = -0.5 * quad - gc[c] + cst + gc[16 + c];
-        mx = fmax(mx, e[c]);
-    }
-    return mx;
-}
-
 // One weighted EM step's sums in one pass (E step + M-step moments).  Per round of 256 samples: thread t evaluates the
 // mixture at its sample and leaves the responsibilities x importance weight R[t][c] (0 outside the box or for a
 // non-finite weight) and the modelled coordinates Z[t][.] in shared memory; then thread (slice, component c, moment q)
@@ -529,29 +484,33 @@ __global__ void __launch_bounds__(256) gmm_em_kernel(IntegDev I, int a, int N, c
                                                      const UpdScratch* __restrict__ us, double* __restrict__ part) {
     if (us->abort || us->n_valid == 0) return;
     constexpr int NACC = 1 + D + D * (D + 1) / 2, ZP = D + 1 + ((D + 1) & 1 ? 0 : 1);      // odd row strides: no bank conflicts
-    const int d = I.gd, C = I.n_gmm, CP = C | 1, t = threadIdx.x;
+    constexpr int CP = 17;                   // row stride of R (16 components)
+    const int d = I.gd, C = I.n_gmm, t = threadIdx.x;
     const double* g = I.mem[a].gmm;
-    __shared__ double gc[GMM_GCN];
     extern __shared__ double em_sh[];
-    double* R = em_sh;                       // [256][CP]
+    double* gs = em_sh;                      // the member's constants
+    double* R = gs + GMS_DOUBLES;            // [256][CP]
     double* Z = R + 256 * CP;                // [256][ZP]
     double* mu_s = Z + 256 * ZP;             // [C][D + 1]
-    gmm_block_consts(I, g, gc);
+    gmm_load_shared(I, g, gs);
     for (int q = t; q < C * (D + 1); q += 256) {
         const int c = q / (D + 1), r = q - c * (D + 1);
         mu_s[q] = r < d ? g[C + c * d + r] : 0.0;
     }
     // the moments this thread accumulates
-    const int NP = C * NACC, SL = NP >= 256 ? 1 : 256 / NP, per = (256 + SL - 1) / SL;
-    int sc[GMM_SLOTS], sia[GMM_SLOTS], sib[GMM_SLOTS], s0[GMM_SLOTS], s1[GMM_SLOTS];
+    const int NP = C * NACC, SL = NP >= 256 ? 1 : 256 / NP;
+    int sc[GMM_SLOTS], sia[GMM_SLOTS], sib[GMM_SLOTS], sl[GMM_SLOTS];
+    bool used[GMM_SLOTS];
     double acc[GMM_SLOTS];
 #pragma unroll
     for (int k = 0; k < GMM_SLOTS; k++) {
         const int item = t + 256 * k;
         acc[k] = 0.0;
-        sc[k] = sia[k] = sib[k] = s0[k] = s1[k] = 0;
-        if (item < NP * SL) {
-            const int pair = item % NP, sl = item / NP;
+        sc[k] = sia[k] = sib[k] = sl[k] = 0;
+        used[k] = item < NP * SL;
+        if (used[k]) {
+            const int pair = item % NP;
+            sl[k] = item / NP;
             const int c = pair / NACC, q = pair - c * NACC;
             int ia = D, ib = D;
             if (q >= 1 && q <= D) ia = q - 1;
@@ -562,44 +521,73 @@ __global__ void __launch_bounds__(256) gmm_em_kernel(IntegDev I, int a, int N, c
                 ib = q - (1 + D + r * (r + 1) / 2);
             }
             sc[k] = c; sia[k] = ia; sib[k] = ib;
-            s0[k] = sl * per;
-            s1[k] = min(256, s0[k] + per);
         }
     }
     __syncthreads();
     const double m = double_from_ord(us->m_ord);
+    __shared__ int wcnt[8];
+    const int lane = t & 31, wid = t >> 5;
     for (long long base = (long long)blockIdx.x * 256; base < N; base += (long long)gridDim.x * 256) {
         const long long i = base + t;
-        double w = neg_inf();
-        bool ok = false;
+        // samples whose weight exp(ln w - max) underflows to 0 (most of a batch, PAPER.md:107 weights are peaked) add
+        // exactly nothing to any sum: they skip the mixture evaluation and are left out of the round's list
+        double wt = 0.0;
         if (i < N) {
-            w = lnw[i];
-            ok = is_finite_d(w) && in_box_dev(I, z, N, i);
+            const double w = lnw[i];
+            if (is_finite_d(w) && in_box_dev(I, z, N, i)) wt = exp(w - m);
         }
-        double zz[D], e[16];
+        const bool ok = wt > 0.0;
+        const unsigned bal = __ballot_sync(0xffffffffu, ok);
+        if (lane == 0) wcnt[wid] = __popc(bal);
+        __syncthreads();
+        int pos = __popc(bal & ((1u << lane) - 1u)), nround = 0;
 #pragma unroll
-        for (int c = 0; c < D; c++) zz[c] = (c < d && i < N) ? z[(long long)I.gdim[c] * N + i] : 0.0;
-        double mx = 0.0, sum = 1.0;
+        for (int q = 0; q < 8; q++) {
+            pos += q < wid ? wcnt[q] : 0;
+            nround += wcnt[q];
+        }
         if (ok) {
-            mx = ln_comp_all<D>(I, g, zz, e, gc);
-            sum = 0.0;
+            double zz[D], e[16];
+#pragma unroll
+            for (int c = 0; c < D; c++) zz[c] = c < d ? z[(long long)I.gdim[c] * N + i] : 0.0;
+            const double mx = gmm_ln_comps<D>(I, gs, zz, e);
+            double sum = 0.0;
             for (int c = 0; c < C; c++) {
                 e[c] = exp(e[c] - mx);
                 sum += e[c];
             }
-        }
-        const double wt = ok ? exp(w - m) / sum : 0.0;
-        for (int c = 0; c < C; c++) R[t * CP + c] = ok ? e[c] * wt : 0.0;
+            wt = wt / sum;
+            for (int c = 0; c < C; c++) R[pos * CP + c] = e[c] * wt;
 #pragma unroll
-        for (int c = 0; c < D; c++) Z[t * ZP + c] = zz[c];
-        Z[t * ZP + D] = 1.0;
+            for (int c = 0; c < D; c++) Z[pos * ZP + c] = zz[c];
+            Z[pos * ZP + D] = 1.0;
+        }
         __syncthreads();
+        const int per = (nround + SL - 1) / SL;
 #pragma unroll
         for (int k = 0; k < GMM_SLOTS; k++) {
+            if (!used[k]) continue;
+            const int b0 = min(nround, sl[k] * per), b1 = min(nround, b0 + per);
+            if (b1 <= b0) continue;
             const double ma = mu_s[sc[k] * (D + 1) + sia[k]], mb = mu_s[sc[k] * (D + 1) + sib[k]];
+            const double* pr = R + b0 * CP + sc[k];
+            const double* pa = Z + b0 * ZP + sia[k];
+            const double* pb = Z + b0 * ZP + sib[k];
             double v = acc[k];
-#pragma unroll 4
-            for (int sm = s0[k]; sm < s1[k]; sm++) v = fma(R[sm * CP + sc[k]], (Z[sm * ZP + sia[k]] - ma) * (Z[sm * ZP + sib[k]] - mb), v);
+            int n = b1 - b0;
+            for (; n >= 4; n -= 4) {
+#pragma unroll
+                for (int u = 0; u < 4; u++) v = fma(pr[u * CP], (pa[u * ZP] - ma) * (pb[u * ZP] - mb), v);
+                pr += 4 * CP;
+                pa += 4 * ZP;
+                pb += 4 * ZP;
+            }
+            for (; n > 0; n--) {
+                v = fma(pr[0], (pa[0] - ma) * (pb[0] - mb), v);
+                pr += CP;
+                pa += ZP;
+                pb += ZP;
+            }
             acc[k] = v;
         }
         __syncthreads();
@@ -612,7 +600,7 @@ __global__ void __launch_bounds__(256) gmm_em_kernel(IntegDev I, int a, int N, c
     __syncthreads();
     for (int pair = t; pair < NP; pair += 256) {
         double v = 0.0;
-        for (int sl = 0; sl < SL; sl++) v += red[sl * NP + pair];
+        for (int q = 0; q < SL; q++) v += red[q * NP + pair];
         const int c = pair / NACC, q = pair - c * NACC;
         part[((size_t)c * gridDim.x + blockIdx.x) * GMM_NACC_MAX + q] = v;
     }
@@ -841,7 +829,7 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
             ILE_LAUNCH_CHECK(ctx);
             mask_max_kernel<<<grid, 256, 0, st>>>(I, N, z, lnw, nullptr, MASK_BOX, it->us);
             ILE_LAUNCH_CHECK(ctx);
-            const size_t em_smem = ((size_t)256 * ((I.n_gmm | 1) + 10) + (size_t)I.n_gmm * 9 + 16) * sizeof(double);
+            const size_t em_smem = ((size_t)GMS_DOUBLES + 256 * (17 + 10) + (size_t)I.n_gmm * 9 + 16) * sizeof(double);
             switch (I.d) {
 #define GMM_CASE(D)                                                                                                        \
     case D:                                                                                                                \
