@@ -62,7 +62,7 @@ int ile_timing_drain(ile_ctx* ctx) {
 }
 extern "C" int ile_kernel_timing(ile_ctx* ctx, int on) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     int rc = ile_timing_drain(ctx);
     if (rc) return rc;
     if (on && !ctx->tev) {
@@ -77,7 +77,7 @@ extern "C" int ile_kernel_timing(ile_ctx* ctx, int on) {
 }
 extern "C" int ile_kernel_time(ile_ctx* ctx, double* total_ms, uint64_t* launches) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     int rc = ile_timing_drain(ctx);
     if (rc) return rc;
     if (total_ms) *total_ms = ctx->t_ms_total;
@@ -114,7 +114,7 @@ extern "C" int ile_create(ile_ctx** out, int device, void* cuda_stream) {
 
 extern "C" int ile_destroy(ile_ctx* ctx) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->d_ylm);
@@ -144,7 +144,7 @@ extern "C" const char* ile_last_error(const ile_ctx* ctx) { return ctx ? ctx->er
 
 extern "C" int ile_sync(ile_ctx* ctx) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     ILE_CUDA(ctx, cudaGetLastError());
     return ILE_OK;
@@ -160,7 +160,7 @@ extern "C" int ile_set_lnL_variant(ile_ctx* ctx, int variant) {
 
 extern "C" int ile_set_network(ile_ctx* ctx, int K, const double* D, const double* pos_m, double gmst) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (K < 1 || K > ILE_MAX_K || !D || !pos_m) return ile_fail(ctx, ILE_EINVAL, "set_network: K in 1..%d", ILE_MAX_K);
     for (int k = 0; k < K; k++)
         for (int a = 0; a < 3; a++)
@@ -199,7 +199,7 @@ static long double binom_ld(int n, int k) {
 // (Goldberg et al. 1967 closed form with s = -2).
 extern "C" int ile_set_modes(ile_ctx* ctx, int M, const int* ell, const int* m) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (M < 1 || M > ILE_MAX_M || !ell || !m) return ile_fail(ctx, ILE_EINVAL, "set_modes: M in 1..%d", ILE_MAX_M);
     if (ctx->have_quv && M != ctx->M) return ile_fail(ctx, ILE_ESTATE, "set_modes: M differs from the loaded Q/U/V");
     YlmTable& T = ctx->h_ylm;
@@ -292,8 +292,10 @@ __global__ void pack_uv_kernel(const double* __restrict__ U, const double* __res
     }
 }
 
-extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U,
-                            const double* V, double D_ref, int src_is_device) {
+// trusted: U and V were made by ile_precompute_quv, whose last kernel writes the lower triangle from the upper by
+// Eq. 17-18 - the symmetry check (and its copy to the host) is skipped
+int ile_load_quv_impl(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U, const double* V, double D_ref,
+                      int src_is_device, bool trusted) {
     if (!ctx) return ILE_EINVAL;
     cudaSetDevice(ctx->device);
     if (!ctx->have_net || !ctx->have_modes) return ile_fail(ctx, ILE_ESTATE, "load_quv: set_network and set_modes first");
@@ -305,7 +307,7 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     // symmetry check (Eq. 17-18) on the host
     std::vector<double> hU, hV;
     const double *pU = U, *pV = V;
-    if (src_is_device) {
+    if (src_is_device && !trusted) {
         hU.resize(nU);
         hV.resize(nU);
         ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));      // producers of U, V on the context's (possibly non-blocking) stream
@@ -314,7 +316,7 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
         pU = hU.data();
         pV = hV.data();
     }
-    for (size_t pk = 0; pk < (size_t)P * K; pk++) {
+    for (size_t pk = 0; pk < (trusted ? 0 : (size_t)P * K); pk++) {
         const double* u = pU + pk * M * M * 2;
         const double* v = pV + pk * M * M * 2;
         double scale = 0.0;
@@ -374,9 +376,14 @@ extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0
     return ILE_OK;
 }
 
+extern "C" int ile_load_quv(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U,
+                            const double* V, double D_ref, int src_is_device) {
+    return ile_load_quv_impl(ctx, P, N_Q, fs, t_Q0, Q, U, V, D_ref, src_is_device, false);
+}
+
 extern "C" int ile_set_time_grid(ile_ctx* ctx, double t_lo, double dt, int N_t, int interp) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (!ctx->have_quv) return ile_fail(ctx, ILE_ESTATE, "set_time_grid: load_quv first");
     if (N_t < 1 || !(dt > 0) || (interp != 0 && interp != 1)) return ile_fail(ctx, ILE_EINVAL, "set_time_grid: bad argument");
     double s = dt * ctx->fs;
@@ -394,7 +401,7 @@ extern "C" int ile_set_time_grid(ile_ctx* ctx, double t_lo, double dt, int N_t, 
 
 extern "C" int ile_set_prior(ile_ctx* ctx, double D_min, double D_max) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (!(D_min > 0) || !(D_max > D_min)) return ile_fail(ctx, ILE_EINVAL, "set_prior: need 0 < D_min < D_max");
     ctx->D_min = D_min; ctx->D_max = D_max; ctx->have_prior = true;
     return ILE_OK;

@@ -162,3 +162,5 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 __device__ __forceinline__ double neg_inf() { return __longlong_as_double(0xfff0000000000000LL); }
 __device__ __forceinline__ double pos_inf() { return __longlong_as_double(0x7ff0000000000000LL); }
+int ile_load_quv_impl(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U, const double* V, double D_ref,
+                      int src_is_device, bool trusted);

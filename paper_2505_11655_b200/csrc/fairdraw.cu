@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(256) fd_draw_kernel(int N, int M, unsigned lon
 // mode 0 = systematic resampling, 1 = independent draws.  Asynchronous on the context's stream.
 extern "C" int ile_fair_draw(ile_ctx* ctx, int N, const double* lnw, int M, uint64_t seed, uint64_t iter, int mode, int64_t* idx) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (N < 1 || M < 1 || !lnw || !idx || mode < 0 || mode > 1) return ile_fail(ctx, ILE_EINVAL, "fair_draw: bad argument");
     const int nblocks = (N + FD_TILE - 1) / FD_TILE;
     void* scratch = nullptr;

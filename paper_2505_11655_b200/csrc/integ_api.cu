@@ -222,7 +222,7 @@ extern "C" int ile_integrator_reset(ile_integrator* it);
 
 extern "C" int ile_integrator_create(ile_ctx* ctx, const ile_integrator_opts* o, ile_integrator** out) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (!o || !out) return ile_fail(ctx, ILE_EINVAL, "integrator_create: null argument");
     *out = nullptr;
     // max_batch: the fixed-point sums (q <= 2^40 per sample, uint64) cannot overflow up to 2^24 samples with flat weights

@@ -102,7 +102,7 @@ extern "C" int ile_antenna(ile_ctx* ctx, int N, const double* ra, const double* 
 
 extern "C" int ile_ylm(ile_ctx* ctx, int N, const double* incl, const double* phi, double* Y) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (!ctx->have_modes) return ile_fail(ctx, ILE_ESTATE, "ylm: set_modes first");
     if (N < 0 || (N > 0 && (!incl || !phi || !Y))) return ile_fail(ctx, ILE_EINVAL, "ylm: bad argument");
     if (N == 0) return ILE_OK;
@@ -145,6 +145,6 @@ int ile_launch_lnL_z(ile_ctx* ctx, int p, int N, int d, const double* z, const i
 
 extern "C" int ile_lnL_z(ile_ctx* ctx, int p, int N, int d, const double* z, double* lnL, double* ln_prior) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     return ile_launch_lnL_z(ctx, p, N, d, z, nullptr, lnL, ln_prior);
 }

@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(256) dmma_chain_kernel(int iters, double seed,
 // instruction).  Runs on the context's stream, synchronises, returns TFLOP/s of the best of 3 runs.
 extern "C" int ile_fp64_peak(ile_ctx* ctx, int mode, double* tflops) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     if (!tflops || mode < 0 || mode > 1) return ile_fail(ctx, ILE_EINVAL, "fp64_peak: mode 0 (DFMA) or 1 (DMMA)");
     const int blocks = ctx->sm_count * 8, threads = 256, iters = mode == 0 ? 4096 : 2048;
     void* scratch = nullptr;

@@ -126,6 +126,6 @@ int ile_launch_reduce(ile_ctx* ctx, int N, const double* lnw, ile_result* out_de
 
 extern "C" int ile_reduce(ile_ctx* ctx, int N, const double* lnw, ile_result* out_dev) {
     if (!ctx) return ILE_EINVAL;
-    cudaSetDevice(ctx->device);   // every entry runs on the context\'s device, whatever the caller\'s current one
+    cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     return ile_launch_reduce(ctx, N, lnw, out_dev, 0);
 }

@@ -12,7 +12,7 @@ def _close(got, ref, rel):
     assert np.all(np.abs(got - ref) <= rel * np.abs(ref).max()), np.abs(got - ref).max() / np.abs(ref).max()
 
 
-# 2048, 1024: one shared-memory FFT; 16384, 65536: four-step with N2 = 4, 16; 1536: not a power of two, by the definition
+# window of 300 bins -> 512-point transforms of the spectrum decimated by 4, 2, 32, 128 and 1; 1536: not a power of two, by the definition
 @pytest.mark.parametrize("lmax,K,N_f,P", [(2, 2, 2048, 2), (3, 3, 1024, 1), (2, 2, 16384, 2), (2, 1, 65536, 1), (2, 2, 1536, 1)])
 def test_precompute_parity_and_lnL_from_it(lmax, K, N_f, P):
     import torch
