@@ -441,9 +441,26 @@ def run_precompute(args):
     for _ in range(args.steps):
         call()                                               # returns after the tables are installed (synchronous)
     ms = (time.perf_counter() - t0) * 1e3 / args.steps
+    # roofline of the call (FP64 ALU bound): algorithmic flops of Eq. 6a-c as the kernels evaluate them:
+    # U, V: two complex products and 4 K real multiply-adds per (bin, pair a <= b); Q: the product w conj(h) d, N_f / Mq
+    # transforms of Mq = 2^ceil(log2 N_Q) points (5 Mq log2 Mq flops each) and one twiddled sum per stored bin
+    M = len(ell)
+    n_pairs = M * (M + 1) // 2
+    Mq = 1 << int(np.ceil(np.log2(N_Q)))
+    L = N_f // Mq
+    flops_uv = P * N_f * n_pairs * (12 + 8 * K)
+    flops_q = P * K * M * (L * 5 * Mq * int(np.log2(Mq)) + 8 * L * N_Q + 6 * N_f)
+    peak_dfma = ile.fp64_peak(0)
+    achieved = (flops_uv + flops_q) / (ms * 1e-3) / 1e12
+    hbm_bytes = 2 * P * M * N_f * 16 + P * K * M * N_Q * 16          # h read by both kernels, Q written
     print(json.dumps({"metric": "Q/U/V precompute (Eq. 6a-c)", "value": P / (ms * 1e-3), "unit": "intrinsic points/s", "ms_per_step": ms,
                       "steps": args.steps, "warmup": args.warmup, "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": f"P={P} points, K={K}, M={len(ell)}, N_f={N_f}, N_Q={N_Q}, spectra resident in HBM"}}))
+                      "config": {"workload": f"P={P} points, K={K}, M={M}, N_f={N_f}, N_Q={N_Q}, spectra resident in HBM"},
+                      "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_dfma, "unit": "TFLOP/s", "frac": achieved / peak_dfma,
+                                   "traffic": None, "flops_uv": flops_uv, "flops_q": flops_q,
+                                   "peak_source": "FP64 FMA rate measured by ile_fp64_peak(0) in this run",
+                                   "hbm_GBps": hbm_bytes / (ms * 1e-3) / 1e9,
+                                   "note": "whole call (weights, U/V, Q, install with digit image, final synchronisation), wall clock"}}))
 
 
 def main():

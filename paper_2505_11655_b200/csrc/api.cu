@@ -292,6 +292,35 @@ __global__ void pack_uv_kernel(const double* __restrict__ U, const double* __res
     }
 }
 
+// Device arrays of a Q/U/V set of P points and N_Q stored bins; a set of the same shape (the next intrinsic point of a
+// run) reuses the allocations.  The resident set is invalid from here until the load completes.
+int ile_quv_alloc(ile_ctx* ctx, int P, int N_Q) {
+    const int K = ctx->K, M = ctx->M;
+    const size_t nU = (size_t)P * K * M * M * 2, nQ = (size_t)P * K * M * N_Q * 2;
+    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    const int N_Qpad = ((N_Q + 1) & ~1) + 256;
+    size_t nQt = (size_t)P * K * N_Qpad * ILE_QT_ROW;
+    // same shapes as the resident set (the next intrinsic point of a run): reuse the allocations
+    const bool reuse = ctx->have_quv && ctx->P == P && ctx->N_Q == N_Q && ctx->quv_K == K && ctx->quv_M == M;
+    ctx->have_quv = false;
+    if (!reuse) {
+        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qf); cudaFree(ctx->d_U); cudaFree(ctx->d_V); cudaFree(ctx->d_UVp);
+        cudaFree(ctx->d_Qs); cudaFree(ctx->d_qeb); cudaFree(ctx->d_qhi); free(ctx->h_qeb);
+        ctx->d_Qc = ctx->d_Qf = ctx->d_U = ctx->d_V = ctx->d_UVp = nullptr;
+        ctx->d_Qs = nullptr; ctx->d_qeb = nullptr; ctx->d_qhi = nullptr;
+        ctx->h_qeb = (int*)malloc((size_t)P * K * sizeof(int));
+        if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qf, nQt * 8) != cudaSuccess ||
+            cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess ||
+            cudaMalloc(&ctx->d_UVp, (size_t)P * ctx->n_pairs * K * 4 * 8) != cudaSuccess ||
+            cudaMalloc(&ctx->d_Qs, ile_split_qs_bytes(P, K, N_Q)) != cudaSuccess || cudaMalloc(&ctx->d_qeb, (size_t)P * K * sizeof(int)) != cudaSuccess ||
+            cudaMalloc(&ctx->d_qhi, (size_t)P * K * sizeof(int)) != cudaSuccess || !ctx->h_qeb) {
+            cudaGetLastError();
+            return ile_fail(ctx, ILE_ENOMEM, "load_quv: device allocation failed");
+        }
+    }
+    return ILE_OK;
+}
+
 // trusted: U and V were made by ile_precompute_quv, whose last kernel writes the lower triangle from the upper by
 // Eq. 17-18 - the symmetry check (and its copy to the host) is skipped
 int ile_load_quv_impl(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U, const double* V, double D_ref,
@@ -334,33 +363,16 @@ int ile_load_quv_impl(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, cons
                     return ile_fail(ctx, ILE_EINVAL, "load_quv: V[%zu] is not symmetric at (%d,%d) (Eq. 18)", pk, a, b);
             }
     }
-    ILE_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    int N_Qpad = ((N_Q + 1) & ~1) + 256;
-    size_t nQt = (size_t)P * K * N_Qpad * ILE_QT_ROW;
-    // same shapes as the resident set (the next intrinsic point of a run): reuse the allocations
-    const bool reuse = ctx->have_quv && ctx->P == P && ctx->N_Q == N_Q && ctx->quv_K == K && ctx->quv_M == M;
-    ctx->have_quv = false;
-    if (!reuse) {
-        cudaFree(ctx->d_Qc); cudaFree(ctx->d_Qf); cudaFree(ctx->d_U); cudaFree(ctx->d_V); cudaFree(ctx->d_UVp);
-        cudaFree(ctx->d_Qs); cudaFree(ctx->d_qeb); cudaFree(ctx->d_qhi); free(ctx->h_qeb);
-        ctx->d_Qc = ctx->d_Qf = ctx->d_U = ctx->d_V = ctx->d_UVp = nullptr;
-        ctx->d_Qs = nullptr; ctx->d_qeb = nullptr; ctx->d_qhi = nullptr;
-        ctx->h_qeb = (int*)malloc((size_t)P * K * sizeof(int));
-        if (cudaMalloc(&ctx->d_Qc, nQ * 8) != cudaSuccess || cudaMalloc(&ctx->d_Qf, nQt * 8) != cudaSuccess ||
-            cudaMalloc(&ctx->d_U, nU * 8) != cudaSuccess || cudaMalloc(&ctx->d_V, nU * 8) != cudaSuccess ||
-            cudaMalloc(&ctx->d_UVp, (size_t)P * ctx->n_pairs * K * 4 * 8) != cudaSuccess ||
-            cudaMalloc(&ctx->d_Qs, ile_split_qs_bytes(P, K, N_Q)) != cudaSuccess || cudaMalloc(&ctx->d_qeb, (size_t)P * K * sizeof(int)) != cudaSuccess ||
-            cudaMalloc(&ctx->d_qhi, (size_t)P * K * sizeof(int)) != cudaSuccess || !ctx->h_qeb) {
-            cudaGetLastError();
-            return ile_fail(ctx, ILE_ENOMEM, "load_quv: device allocation failed");
-        }
+    if (Q != ctx->d_Qc) {                       // ile_precompute_quv has allocated and written the arrays themselves
+        const int rc_alloc = ile_quv_alloc(ctx, P, N_Q);
+        if (rc_alloc) return rc_alloc;
     }
+    const int N_Qpad = ((N_Q + 1) & ~1) + 256;
     cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-    ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_Qc, Q, nQ * 8, kind, ctx->stream));
-    ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_U, U, nU * 8, kind, ctx->stream));
-    ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, V, nU * 8, kind, ctx->stream));
-    repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qf, P * K, M, N_Q, N_Qpad);
-    ILE_LAUNCH_CHECK(ctx);
+    if (Q != ctx->d_Qc) ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_Qc, Q, nQ * 8, kind, ctx->stream));
+    if (U != ctx->d_U) ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_U, U, nU * 8, kind, ctx->stream));
+    if (V != ctx->d_V) ILE_CUDA(ctx, cudaMemcpyAsync(ctx->d_V, V, nU * 8, kind, ctx->stream));
+    ctx->qf_valid = 0;                          // the DMMA kernel's copy of Q is made when that kernel first runs (ile_ensure_qf)
     pack_uv_kernel<<<ctx->sm_count * 2, 256, 0, ctx->stream>>>(ctx->d_U, ctx->d_V, ctx->d_pairs, ctx->d_UVp, P, K, M, ctx->n_pairs);
     ILE_LAUNCH_CHECK(ctx);
     if (K <= 3 && M <= 24) {
@@ -373,6 +385,16 @@ int ile_load_quv_impl(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, cons
     ctx->P = P; ctx->N_Q = N_Q; ctx->N_Qpad = N_Qpad; ctx->quv_K = K; ctx->quv_M = M; ctx->fs = fs; ctx->t_Q0 = t_Q0; ctx->D_ref = D_ref;
     ctx->have_quv = true;
     ctx->have_grid = false;
+    return ILE_OK;
+}
+
+// The row-pair layout of Q that the DMMA kernel (lnl_fused2.cu) reads: built on first use, the default tcgen05 kernel
+// reads the digit image instead.
+int ile_ensure_qf(ile_ctx* ctx) {
+    if (ctx->qf_valid) return ILE_OK;
+    repack_q_kernel<<<ctx->sm_count * 8, 256, 0, ctx->stream>>>(ctx->d_Qc, ctx->d_Qf, ctx->P * ctx->quv_K, ctx->quv_M, ctx->N_Q, ctx->N_Qpad);
+    ILE_LAUNCH_CHECK(ctx);
+    ctx->qf_valid = 1;
     return ILE_OK;
 }
 

@@ -94,6 +94,8 @@ struct ile_ctx {
     int ylm_max_pow, ylm_max_abs_m;   // sizes of the harmonics' power and phase tables (shared-memory scratch of the prep kernel)
     void* pc_buf;                 // scratch of ile_precompute_quv (grow-only, freed at destroy)
     size_t pc_bytes;
+    int pc_W_nf;                 // N_f of the twiddle table held in pc_buf (0: none)
+    int qf_valid;                 // d_Qf matches d_Qc
     int lnl_split;                // 1 (default): tcgen05 integer-digit fused kernel (lnl_split.cu) where the shape allows
     int sky_sort;                 // 1 (default): order samples by delay cell before the fused kernel
     int sm_count;
@@ -164,3 +166,5 @@ __device__ __forceinline__ double neg_inf() { return __longlong_as_double(0xfff0
 __device__ __forceinline__ double pos_inf() { return __longlong_as_double(0x7ff0000000000000LL); }
 int ile_load_quv_impl(ile_ctx* ctx, int P, int N_Q, double fs, double t_Q0, const double* Q, const double* U, const double* V, double D_ref,
                       int src_is_device, bool trusted);
+int ile_quv_alloc(ile_ctx* ctx, int P, int N_Q);
+int ile_ensure_qf(ile_ctx* ctx);

@@ -177,6 +177,8 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         int* tstart = (int*)(tb + (size_t)sp_tiles * 32);
         return ile_launch_split(ctx, P, N, sp_bits, k0, z, uk, perm, lnL, ln_prior, tstart, tl, ntiles_dev);
     }
+    rc = ile_ensure_qf(ctx);
+    if (rc) return rc;
     // shared-memory scratch of the harmonics: (2 (max_pow + 1) + 2 (max_abs_m + 1)) doubles per thread
     // ... and a copy of the mode table
     const int scr_d = (2 * (ctx->ylm_max_pow + 1) + 2 * (ctx->ylm_max_abs_m + 1)) * 128;

@@ -397,7 +397,7 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     int Mq = 4, log2Mq = 2;
     while (Mq < N_Q) { Mq <<= 1; log2Mq++; }
     const bool pruned = (N_f & (N_f - 1)) == 0 && Mq <= 2048 && Mq <= N_f;
-    const size_t nQ = (size_t)P * K * M * N_Q, nU = (size_t)P * K * M * M, nX = pruned ? 0 : (size_t)P * K * M * N_f;
+    const size_t nX = pruned ? 0 : (size_t)P * K * M * N_f;
     // frequency slices per point: two CTAs per SM in all, at least one chunk each; UV_SUB partial sums per slice
     const int chunks = (N_f + UV_CH - 1) / UV_CH;
     int slices = 2 * ctx->sm_count / P;
@@ -407,15 +407,21 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     slices = (chunks + cpb - 1) / cpb;
     const int nsl = slices;
     const size_t nPart = (size_t)P * nsl * n_pairs * K * 4;
-    // one grow-only scratch allocation: w | W | w d | x | Q | U | V | part  (256-byte aligned pieces)
+    // the results go straight into the context's arrays
+    {
+        const int rc = ile_quv_alloc(ctx, P, N_Q);
+        if (rc) return rc;
+    }
+    // one grow-only scratch allocation: W | w | w d | x | part  (256-byte aligned pieces)
     auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
-    const size_t o_w = 0, o_W = o_w + al((size_t)K * N_f * 8), o_dw = o_W + al((size_t)N_f * 16), o_x = o_dw + al((size_t)K * N_f * 16), o_Q = o_x + al(nX * 16),
-                 o_U = o_Q + al(nQ * 16), o_V = o_U + al(nU * 16), o_p = o_V + al(nU * 16), total = o_p + al(nPart * 8);
+    const size_t o_W = 0, o_w = o_W + al((size_t)N_f * 16), o_dw = o_w + al((size_t)K * N_f * 8), o_x = o_dw + al((size_t)K * N_f * 16), o_p = o_x + al(nX * 16),
+                 total = o_p + al(nPart * 8);
     if (total > ctx->pc_bytes) {
         cudaStreamSynchronize(ctx->stream);
         cudaFree(ctx->pc_buf);
         ctx->pc_buf = nullptr;
         ctx->pc_bytes = 0;
+        ctx->pc_W_nf = 0;
         if (cudaMalloc(&ctx->pc_buf, total) != cudaSuccess) {
             cudaGetLastError();
             return ile_fail(ctx, ILE_ENOMEM, "precompute_quv: device allocation of %zu bytes failed", total);
@@ -424,13 +430,15 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     }
     char* buf = (char*)ctx->pc_buf;
     double* w = (double*)(buf + o_w);
-    double2 *W = (double2*)(buf + o_W), *x = (double2*)(buf + o_x), *Q = (double2*)(buf + o_Q), *U = (double2*)(buf + o_U),
-            *V = (double2*)(buf + o_V);
+    double2 *W = (double2*)(buf + o_W), *x = (double2*)(buf + o_x), *Q = (double2*)ctx->d_Qc, *U = (double2*)ctx->d_U, *V = (double2*)ctx->d_V;
     double* part = (double*)(buf + o_p);
     double2* dwp = (double2*)(buf + o_dw);
     cudaStream_t st = ctx->stream;
     pc_weight_kernel<<<dim3((N_f + 255) / 256, K), 256, 0, st>>>(K, N_f, df, f_low, S, (const double2*)d, w, dwp);
-    pc_twiddle_kernel<<<(N_f + 255) / 256, 256, 0, st>>>(N_f, W);
+    if (ctx->pc_W_nf != N_f) {                                             // the table survives in the scratch between calls
+        pc_twiddle_kernel<<<(N_f + 255) / 256, 256, 0, st>>>(N_f, W);
+        ctx->pc_W_nf = N_f;
+    }
     {
         const int MB = (M + 1) / 2, uv_threads = (MB * (MB + 1) / 2 * UV_SUB + 31) / 32 * 32;
         const size_t uv_stage = (size_t)4 * MB * UV_SB * sizeof(double2) + (size_t)2 * K * UV_CH * sizeof(double);
