@@ -208,3 +208,45 @@ def test_lnL_other_shapes(torch_mod, K, lmax):
         ile.set_lnL_variant(variant)
         got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
         assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
+
+
+def test_two_contexts_in_one_process(torch_mod):
+    """Two contexts alive at once (different networks, mode sets and time grids), calls interleaved: each answers as it
+    does alone.  The kernels' shared-memory opt-in and every other piece of launch state is per call, not per process."""
+    from oracle import likelihood as lk
+    torch = torch_mod
+    probs = [make_problem(1), make_problem(2)]
+    iles = [_ile(p) for p in probs]
+    zs = [uniform_box_samples(p.lo, p.hi, 900 + 37 * i, seed=500 + i) for i, p in enumerate(probs)]
+    refs = [lk.lnL_z(p.D, p.pos, p.gmst, p.ell, p.m, p.Q[0], p.U[0], p.V[0], p.D_ref, p.fs, p.t_Q0, p.t_lo, p.dt, p.N_t, z)
+            for p, z in zip(probs, zs)]
+    for variant in FUSED:
+        for ile in iles:
+            ile.set_lnL_variant(variant)
+        for rnd in range(2):
+            outs = [ile.lnL_z(0, _dev(torch, z)) for ile, z in zip(iles, zs)]           # both queued before either is read
+            for out, ref in zip(outs, refs):
+                got = out.cpu().numpy()
+                assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, rnd, np.abs(got - ref).max())
+    # an integrator on each, stepped alternately (same kernel as the solo runs: the default)
+    for ile in iles:
+        ile.set_lnL_variant(0)
+    from paper_2505_11655_b200 import Integrator
+    from paper_2505_11655_b200.binding import result_from_device
+
+    def make(ile, p, i):
+        return Integrator(ile, "AC", p.d, p.lo, p.hi, seed=9 + i, max_batch=4096)
+
+    def step(it, g):
+        return float(result_from_device(it.step(0, 4096, g))["ln_integral"][0])
+
+    solo = []
+    for i, p in enumerate(probs):
+        it = make(_ile(p), p, i)
+        solo.append([step(it, g) for g in range(3)])
+    its = [make(ile, p, i) for i, (ile, p) in enumerate(zip(iles, probs))]
+    both = [[], []]
+    for g in range(3):
+        for i, it in enumerate(its):
+            both[i].append(step(it, g))
+    assert both == solo
