@@ -189,7 +189,7 @@ static size_t draw_smem_bytes(const IntegDev& I) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned int g, double* __restrict__ z, double* __restrict__ ln_ps) {
+__global__ void __launch_bounds__(128, 6) draw_kernel(IntegDev I, int N, unsigned int g, double* __restrict__ z, double* __restrict__ ln_ps) {
     extern __shared__ double draw_sh[];
     block_consts(I, draw_sh);
     // grid-stride: a block builds the shared constants once for all its samples
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(128) draw_kernel(IntegDev I, int N, unsigned i
 }
 
 template <int D>
-__global__ void __launch_bounds__(128) ln_pdf_kernel(IntegDev I, int N, const double* __restrict__ z, double* __restrict__ ln_ps) {
+__global__ void __launch_bounds__(128, 6) ln_pdf_kernel(IntegDev I, int N, const double* __restrict__ z, double* __restrict__ ln_ps) {
     extern __shared__ double draw_sh[];
     block_consts(I, draw_sh);
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
