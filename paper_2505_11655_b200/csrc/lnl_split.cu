@@ -14,15 +14,18 @@
 //   operand A (coefficients): [c_0 | c_1 | ... | c_5], 48 bytes per digit block (2M <= 42 used), written to tensor
 //              memory by the thread that owns the sample (tcgen05.st); stationary for the whole tile
 //   operand B (Q digits): per stored bin 304 bytes [q_5 | q_4 | ... | q_0 | 16 zero bytes], built once per intrinsic
-//              point at ile_load_quv in the K-major no-swizzle core-matrix layout, so that a 16-bin chunk is one
-//              contiguous 4864-byte TMA bulk copy; sum s reads the view that starts at block 5 - s, which pairs
+//              point at ile_load_quv in the K-major no-swizzle core-matrix layout, so that a 32-bin chunk is one
+//              contiguous 9728-byte TMA bulk copy; sum s reads the view that starts at block 5 - s, which pairs
 //              c_a with q_{s-a} (descriptor start addresses move in 16-byte steps)
-//   tile       128 samples of one delay cell (16 stored bins per detector) = the 128 lanes of tensor memory
-//   work item  (16-bin chunk, detector): 33 MMAs of 128 x 16 x 32 into one of two accumulator sets
-//   warps      0-3: one thread per sample: coefficients and digits, the U/V quadratic term (step 4), then per item
-//              accumulators -> FP64, interpolation weights, accumulation of A_j = sum_k S_k(t_j + tau_k) into a
-//              thread-private column of a shared-memory ring (the per-sample delay shift is an address offset),
-//              and the streaming log-sum-exp over complete time bins (step 6);  warp 4: TMA producer + MMA issuer
+//   tile       up to 128 samples of one delay cell (16 stored bins per detector) = the 128 lanes of tensor memory
+//   work item  (32-bin chunk, detector): 33 MMAs of 128 x 32 x 32 into one set of six accumulators (192 columns), freed
+//              as soon as the math warps have loaded it
+//   warps      0-15: four threads per sample (group = warp / 4, lane quarter = warp % 4 = the tensor-memory lanes the warp
+//              can reach): steps 1-2, harmonics, coefficients and digits (by detector), the U/V quadratic term (step 4, by
+//              rows of the triangle); then per item accumulators -> 64-bit integer -> FP64 (8 bins per thread), interpolation
+//              weights, accumulation of A_j = sum_k S_k(t_j + tau_k) into a thread-private column of a 64-row shared-memory
+//              ring (the per-sample delay shift is an address offset), and the streaming log-sum-exp over complete time
+//              bins (step 6, rows split over the four threads);  warp 16: TMA producer + MMA issuer
 #include "common.cuh"
 #include "likelihood_dev.cuh"
 #include "radix_sort.cuh"

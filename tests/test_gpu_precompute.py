@@ -84,6 +84,32 @@ def test_precompute_parity_at_the_bench_shape():
             rQ = precompute_q(h[p], d, S, df, f_low, (n0 + first) / fs, 32)
             assert np.all(np.abs(Q[:, :, first:first + 32] - rQ) <= 1e-11 * scale), np.abs(Q[:, :, first:first + 32] - rQ).max() / scale
 
+@pytest.mark.parametrize("N_f,N_Q,n0", [(4096, 200, -100), (2048, 1024, -700), (4096, 1500, 3000), (8192, 2048, -1024), (8192, 2500, -10)])
+def test_precompute_q_window_shapes(N_f, N_Q, n0):
+    """The transform sizes the pruned FFT instantiates (windows of 200 -> 256 points: the register tail, one output per
+    thread; 1024 points with a spectrum decimated by 2 only: half-empty groups; 1500 and 2048 -> 2048 points: odd log2, eight
+    outputs per thread), windows that wrap around the segment (n0 > 0 near the end), and a window above 2048 bins, which the
+    definition kernel takes.  Q in full against the oracle's definition; K = 1, l = 2."""
+    import torch
+    from paper_2505_11655_b200 import Ile
+    from oracle.precompute import precompute_q, precompute_uv
+    fs, K = 4096.0, 1
+    ell, m = make_modes(2)
+    M = len(ell)
+    D, pos = make_network(K, np.random.Generator(np.random.Philox(99)))
+    h, d, S, df = make_spectra(K, ell, m, N_f, fs, seed=31 + N_Q, P=1)
+    ile = Ile(0)
+    ile.set_network(D, pos, 0.0)
+    ile.set_modes(ell, m)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    ile.precompute_quv(dev(h), dev(d), dev(S), df, 20.0, n0 / fs, N_Q, D_ref=500.0)
+    Q, U, V = ile.get_quv(0, K, M, N_Q)
+    rQ = precompute_q(h[0], d, S, df, 20.0, n0 / fs, N_Q)
+    rU, rV = precompute_uv(h[0], S, df, 20.0)
+    _close(Q, rQ, 1e-11)
+    _close(U, rU, 1e-12)
+    _close(V, rV, 1e-12)
+
 
 def test_precompute_argument_errors():
     import torch
