@@ -157,7 +157,9 @@ int ile_load_quv(ile_ctx *ctx, int P, int N_Q, double fs, double t_Q0,
  * result like ile_load_quv (synchronises).  The inputs stay the caller's; scratch is one grow-only
  * device allocation owned by the context (freed by ile_destroy).  Errors: ILE_ESTATE before
  * set_network/set_modes, ILE_EINVAL for bad sizes, N_Q > N_f, t_Q0 off the sample grid or more
- * than 22 modes (the resident Q/U/V stay as they were), ILE_ENOMEM, ILE_ECUDA.
+ * than 24 modes (the resident Q/U/V stay as they were), ILE_ENOMEM (of the scratch: the resident set
+ * stays; of the result arrays: nothing is resident afterwards), ILE_ECUDA.  U and V come out Hermitian and
+ * symmetric by construction (Eq. 17-18), so the install skips ile_load_quv's check.
  * ile_get_quv copies point p back to host arrays in ile_load_quv's layout (any of Q, U, V may be NULL). */
 int ile_precompute_quv(ile_ctx *ctx, int P, int N_f, double df, double f_low, const double *h, const double *d,
                        const double *S, double t_Q0, int N_Q, double D_ref);

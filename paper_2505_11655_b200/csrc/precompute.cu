@@ -407,11 +407,6 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     slices = (chunks + cpb - 1) / cpb;
     const int nsl = slices;
     const size_t nPart = (size_t)P * nsl * n_pairs * K * 4;
-    // the results go straight into the context's arrays
-    {
-        const int rc = ile_quv_alloc(ctx, P, N_Q);
-        if (rc) return rc;
-    }
     // one grow-only scratch allocation: W | w | w d | x | part  (256-byte aligned pieces)
     auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
     const size_t o_W = 0, o_w = o_W + al((size_t)N_f * 16), o_dw = o_w + al((size_t)K * N_f * 8), o_x = o_dw + al((size_t)K * N_f * 16), o_p = o_x + al(nX * 16),
@@ -427,6 +422,11 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
             return ile_fail(ctx, ILE_ENOMEM, "precompute_quv: device allocation of %zu bytes failed", total);
         }
         ctx->pc_bytes = total;
+    }
+    // the results go straight into the context's arrays
+    {
+        const int rc = ile_quv_alloc(ctx, P, N_Q);
+        if (rc) return rc;
     }
     char* buf = (char*)ctx->pc_buf;
     double* w = (double*)(buf + o_w);
