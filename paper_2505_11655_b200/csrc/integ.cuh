@@ -68,7 +68,8 @@ struct SamplerDev {
 };
 
 struct IntegDev {
-    int kind, d, n_members, nb, n_gmm, pad;
+    int kind, d, n_members, nb, n_gmm;
+    int box_trusted;          // 1: the batch was drawn by this integrator without a GMM member, so every sample lies in the box (no test, no read of z for it)
     double lo[ILE_MAX_D], hi[ILE_MAX_D], below_hi[ILE_MAX_D];
     double V0;
     unsigned long long seed;
@@ -169,6 +170,7 @@ __device__ __forceinline__ long long bin_index_dev(double z, double lo, double h
 }
 
 __device__ __forceinline__ bool in_box_dev(const IntegDev& I, const double* __restrict__ z, long long N, long long i) {
+    if (I.box_trusted) return true;
     bool ok = true;
     for (int c = 0; c < I.d; c++) {
         const double v = z[(long long)c * N + i];

@@ -422,6 +422,12 @@ extern "C" int ile_integrator_update(ile_integrator* it, int N, const double* z,
     return integ_launch_update(it, N, z, lnw, ln_ps);
 }
 
+static int draws_stay_in_box(const IntegDev& I) {
+    for (int a = 0; a < I.n_members; a++)
+        if (I.mem[a].kind == ILE_KIND_GMM) return 0;
+    return 1;
+}
+
 // samples of the contributing members in a batch of N at iteration g (alloc_kernel's N_c): silent
 // activated members take N / N_active each and sit after the contributing ones
 static int contributing_samples(const IntegDev& I, int N, uint64_t g) {
@@ -452,7 +458,9 @@ static int step_internal(ile_integrator* it, int p, int N, uint64_t iter, ile_re
     ILE_LAUNCH_CHECK(ctx);
     // a standalone AV samples uniformly inside its cells: V_{g+1} = V_g N_min / N
     const double* lp = (I.n_members == 1 && I.mem[0].kind == ILE_KIND_AV) ? nullptr : it->ln_ps;
+    it->I.box_trusted = draws_stay_in_box(it->I);          // UNIFORM, AC and AV draws lie in [lo, hi) by construction; Gaussian tails do not
     rc = integ_launch_update(it, N, it->z, it->lnw, lp);
+    it->I.box_trusted = 0;
     if (rc) return rc;
     annotate_kernel<<<1, 32, 0, ctx->stream>>>(I, it->res, 0);
     ILE_LAUNCH_CHECK(ctx);
@@ -523,7 +531,9 @@ extern "C" int ile_integrator_step_integrand(ile_integrator* it, const ile_integ
     annotate_kernel<<<1, 32, 0, ctx->stream>>>(I, it->res, 1);
     ILE_LAUNCH_CHECK(ctx);
     const double* lp = (I.n_members == 1 && I.mem[0].kind == ILE_KIND_AV) ? nullptr : it->ln_ps;
+    it->I.box_trusted = draws_stay_in_box(it->I);          // UNIFORM, AC and AV draws lie in [lo, hi) by construction; Gaussian tails do not
     rc = integ_launch_update(it, N, it->z, it->lnw, lp);
+    it->I.box_trusted = 0;
     if (rc) return rc;
     annotate_kernel<<<1, 32, 0, ctx->stream>>>(I, it->res, 0);
     ILE_LAUNCH_CHECK(ctx);
