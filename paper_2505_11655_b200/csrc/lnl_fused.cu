@@ -175,7 +175,7 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         char* tb = base + rec_bytes + y_bytes + uk_bytes + 2 * key_bytes + 2 * val_bytes + sort_bytes + 256;
         SpTile* tl = (SpTile*)tb;
         int* tstart = (int*)(tb + (size_t)sp_tiles * 32);
-        return ile_launch_split(ctx, P, N, sp_bits, k0, z, uk, perm, lnL, ln_prior, tstart, tl, ntiles_dev);
+        return ile_launch_split(ctx, P, N, n_min, sp_bits, k0, z, uk, perm, lnL, ln_prior, tstart, tl, ntiles_dev);
     }
     rc = ile_ensure_qf(ctx);
     if (rc) return rc;

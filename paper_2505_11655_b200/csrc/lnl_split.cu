@@ -206,46 +206,39 @@ __global__ void __launch_bounds__(256) sp_run_tiles_kernel(int N, const unsigned
     }
 }
 
-// one warp per tile: extent, window base per detector, largest offset
-__global__ void __launch_bounds__(256) sp_tile_info_kernel(LnlParams P, int N, int invalid_shift, const unsigned long long* __restrict__ key,
-                                                           const int* __restrict__ tstart, const int* __restrict__ ntiles_dev,
-                                                           const double* __restrict__ uk, const int* __restrict__ perm, SpTile* __restrict__ tiles) {
+// one warp per tile: extent; the window base per detector is the tile's delay cell (read off the key), so that every
+// offset above it is at most 15 + 7 (cells of 16 bins on an 8-aligned grid) and no sample has to be looked at
+__global__ void __launch_bounds__(256) sp_tile_info_kernel(LnlParams P, int N, int n_min, int cell_bits, const unsigned long long* __restrict__ key,
+                                                           const int* __restrict__ tstart, const int* __restrict__ ntiles_dev, SpTile* __restrict__ tiles) {
     const int id = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (id >= *ntiles_dev) return;
     const int start = tstart[id];
     const unsigned long long k0 = key[start];
-    int cnt = 0, nmin[3] = {0x7fffffff, 0x7fffffff, 0x7fffffff}, nmax[3] = {0, 0, 0};
+    int cnt = 0;
     bool open = true;
     for (int q = 0; q < SP_TS / 32; q++) {
         const int pos = start + 32 * q + lane;
         const bool mem = open && pos < N && key[pos] == k0;
         const unsigned b = __ballot_sync(0xffffffffu, mem);
         const int lead = b == 0xffffffffu ? 32 : __ffs(~b) - 1;      // members are a prefix
-        if (lane < lead && !(k0 >> invalid_shift)) {
-            const size_t sidx = (size_t)perm[pos];
-#pragma unroll
-            for (int k = 0; k < 3; k++)
-                if (k < P.K) {
-                    const int nk = (int)floor(uk[sidx * 4 + k]);
-                    nmin[k] = min(nmin[k], nk);
-                    nmax[k] = max(nmax[k], nk);
-                }
-        }
         cnt += lead;
         if (lead < 32) open = false;
     }
     SpTile t;
     t.start = start;
     t.cnt = cnt;
-    t.flags = (k0 >> invalid_shift) ? 1 : 0;
+    t.flags = (k0 >> (cell_bits * P.K)) ? 1 : 0;
     t.cap = 0;
 #pragma unroll
     for (int k = 0; k < 3; k++) {
-        const int lo = __reduce_min_sync(0xffffffffu, nmin[k]), hi = __reduce_max_sync(0xffffffffu, nmax[k]);
-        t.base[k] = k < P.K ? (max(lo, 0) & ~7) : 0;
-        if (k < P.K) t.cap = max(t.cap, hi - t.base[k]);
+        t.base[k] = 0;
+        if (k < P.K) {
+            const int cell = (int)((k0 >> (cell_bits * (P.K - 1 - k))) & ((1ull << cell_bits) - 1ull));
+            const int first = n_min + (cell << SP_CELL_SHIFT);          // first bin of the cell (n_min is a multiple of 8)
+            t.base[k] = max(first, 0);
+            t.cap = max(t.cap, first + (1 << SP_CELL_SHIFT) - 1 - t.base[k]);
+        }
     }
-    if (t.flags == 0 && t.cap > SP_CAPMAX) t.flags = 2;
     t.nchunk = t.flags ? 0 : (P.N_t + 1 + t.cap + SP_NB - 1) / SP_NB;
     if (lane == 0) tiles[id] = t;
 }
@@ -452,6 +445,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
             //      values the tile's window was built from).  Coordinates are gathered through the sort permutation.
             double fr[K], fi[K], w0[K], w1[K], x;
             int off[K];
+            bool off_bad = false;
             {
                 const size_t sidx = member ? (size_t)perm[pos] : 0;
                 double* const shr = &sm.lse[0][0][i];                     // rows 0..2 Re F_k, 3..5 Im F_k, 6 x
@@ -522,6 +516,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                     w1[k] = u - fl;
                     w0[k] = 1.0 - w1[k];
                     off[k] = min(max((int)fl - ti.base[k], 0), SP_CAPMAX);
+                    off_bad = off_bad || ((int)fl - ti.base[k] != off[k]);      // outside the tile's window: cannot happen for a sample of this cell
                 }
                 // ---- harmonics (Eq. 4): group g evaluates modes g, g + 4, ... from the tables
                 const int M = sm.ytab.M;
@@ -808,7 +803,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                 double tot = 0.0;
 #pragma unroll
                 for (int gg = 0; gg < SP_G; gg++) tot += sm.lse[gg][1][i] * exp(sm.lse[gg][0][i] - mx);
-                lnL[perm[pos]] = mx + log(tot) - P.ln_Nt;
+                lnL[perm[pos]] = off_bad ? __longlong_as_double(0x7ff8000000000000LL) : mx + log(tot) - P.ln_Nt;
             }
             qbar();                                                     // the next tile's prologue reuses sm.lse
         }
@@ -854,7 +849,7 @@ int ile_launch_split_keys(ile_ctx* ctx, const LnlParams& P, int N, const double*
 }
 
 // z [d][N] in the caller's order; key / perm = the sorted keys of sp_key_kernel and the sort permutation; uk = its u_k [N][4]
-int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int cell_bits, const unsigned long long* key, const double* z, const double* uk,
+int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int n_min, int cell_bits, const unsigned long long* key, const double* z, const double* uk,
                      const int* perm, double* lnL, double* ln_prior, int* tstart, SpTile* tiles, int* ntiles_dev) {
     const int max_tiles = ile_split_max_tiles(N, cell_bits, P.K);
     int* runs = tstart + max_tiles;                     // run starts; their count sits behind the tile count
@@ -863,7 +858,7 @@ int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int cell_bits, con
     ILE_LAUNCH_CHECK(ctx);
     sp_run_tiles_kernel<<<ctx->sm_count * 2, 256, 0, ctx->stream>>>(N, key, runs, nruns_dev, tstart, ntiles_dev);
     ILE_LAUNCH_CHECK(ctx);
-    sp_tile_info_kernel<<<(max_tiles * 32 + 255) / 256, 256, 0, ctx->stream>>>(P, N, cell_bits * P.K, key, tstart, ntiles_dev, uk, perm, tiles);
+    sp_tile_info_kernel<<<(max_tiles * 32 + 255) / 256, 256, 0, ctx->stream>>>(P, N, n_min, cell_bits, key, tstart, ntiles_dev, tiles);
     ILE_LAUNCH_CHECK(ctx);
     const bool tb = P.use_table != 0;
 #define SP_LAUNCH(K_, T_) launch_split_t<K_, T_>(ctx, P, N, z, uk, perm, lnL, ln_prior, tiles, ntiles_dev)

@@ -22,11 +22,16 @@ __global__ void __launch_bounds__(RS_THREADS) rs_hist_kernel(int p, const long l
     __syncthreads();
     const uint64_t* src = rs_src(p, npass) ? k1 : k0;
     const int shift = 8 * p;
-#pragma unroll 4
+    uint64_t keys[RS_TILE / RS_THREADS];
+#pragma unroll
     for (int r = 0; r < RS_TILE / RS_THREADS; r++) {
         const long long i = base + r * RS_THREADS + threadIdx.x;
-        const bool act = i < n;
-        const int dg = act ? (int)((src[i] >> shift) & 0xffu) : 256;
+        keys[r] = i < n ? src[i] : 0ull;
+    }
+#pragma unroll
+    for (int r = 0; r < RS_TILE / RS_THREADS; r++) {
+        const bool act = base + r * RS_THREADS + threadIdx.x < n;
+        const int dg = act ? (int)((keys[r] >> shift) & 0xffu) : 256;
         const unsigned m = __match_any_sync(0xffffffffu, dg);
         if (act && (threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&sh[dg], (uint32_t)__popc(m));
     }
@@ -85,13 +90,22 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(int p, const lon
     const uint32_t* vsrc = s ? v1 : v0;
     uint32_t* vdst = s ? v0 : v1;
     const int shift = 8 * p;
-    const int ROUNDS = RS_TILE / RS_THREADS;          // rounds per warp; warp w owns keys [w*ROUNDS*32, ...)
+    constexpr int ROUNDS = RS_TILE / RS_THREADS;      // rounds per warp; warp w owns keys [w*ROUNDS*32, ...)
     const long long wbase = base + (long long)w * ROUNDS * 32;
-    // phase A: per-warp digit counts
+    // the warp's keys (and payloads) are read once, all loads in flight together, and stay in registers for both phases
+    uint64_t keys[ROUNDS];
+    uint32_t vals[ROUNDS];
+#pragma unroll
     for (int r = 0; r < ROUNDS; r++) {
         const long long i = wbase + r * 32 + lane;
-        const bool act = i < n;
-        const int dg = act ? (int)((ksrc[i] >> shift) & 0xffu) : 256;
+        keys[r] = i < n ? ksrc[i] : 0ull;
+        if (HAS_VAL) vals[r] = i < n ? vsrc[i] : 0u;
+    }
+    // phase A: per-warp digit counts
+#pragma unroll
+    for (int r = 0; r < ROUNDS; r++) {
+        const bool act = wbase + r * 32 + lane < n;
+        const int dg = act ? (int)((keys[r] >> shift) & 0xffu) : 256;
         const unsigned m = __match_any_sync(0xffffffffu, dg);
         if (lane == __ffs(m) - 1) wh[w][dg] += (uint32_t)__popc(m);
         __syncwarp();
@@ -119,11 +133,10 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(int p, const lon
     }
     __syncthreads();
     // phase C: stable rank and scatter
+#pragma unroll
     for (int r = 0; r < ROUNDS; r++) {
-        const long long i = wbase + r * 32 + lane;
-        const bool act = i < n;
-        uint64_t key = 0;
-        if (act) key = ksrc[i];
+        const bool act = wbase + r * 32 + lane < n;
+        const uint64_t key = keys[r];
         const int dg = act ? (int)((key >> shift) & 0xffu) : 256;
         const unsigned m = __match_any_sync(0xffffffffu, dg);
         const uint32_t pos = wh[w][dg] + (uint32_t)__popc(m & ((1u << lane) - 1u));
@@ -132,7 +145,7 @@ __global__ void __launch_bounds__(RS_THREADS) rs_scatter_kernel(int p, const lon
         __syncwarp();
         if (act) {
             kdst[pos] = key;
-            if (HAS_VAL) vdst[pos] = vsrc[i];
+            if (HAS_VAL) vdst[pos] = vals[r];
         }
     }
 }
