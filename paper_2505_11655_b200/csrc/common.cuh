@@ -34,6 +34,7 @@ struct YlmTable {
 // ---------------------------------------------------------------- kernel parameter block (by value)
 struct LnlParams {
     int K, M, N_Q, N_t, stride, interp, d, use_table;
+    int box_trusted;              // 1: every sample of the batch lies in the prior box (the integrator drew it inside a box within it): no test
     int N_Qpad;                   // bins allocated per (p,k) in the tiled layout
     double fs, t_Q0, t_lo, dt, D_ref, gmst;
     double D[ILE_MAX_K][9];
@@ -96,6 +97,8 @@ struct ile_ctx {
     size_t pc_bytes;
     int pc_W_nf;                 // N_f of the twiddle table held in pc_buf (0: none)
     int qf_valid;                 // d_Qf matches d_Qc
+    int zbox_hint;                // set by the integrator around its own lnL call: the batch lies in [zbox_lo, zbox_hi)
+    double zbox_lo[8], zbox_hi[8];
     int lnl_split;                // 1 (default): tcgen05 integer-digit fused kernel (lnl_split.cu) where the shape allows
     int sky_sort;                 // 1 (default): order samples by delay cell before the fused kernel
     int sm_count;

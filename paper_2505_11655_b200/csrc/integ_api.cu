@@ -448,7 +448,12 @@ static int step_internal(ile_integrator* it, int p, int N, uint64_t iter, ile_re
     if (rc) return rc;
     it->drew = true;
     it->last_N = N;
+    if (draws_stay_in_box(I)) {
+        ctx->zbox_hint = 1;
+        for (int c = 0; c < I.d; c++) { ctx->zbox_lo[c] = I.lo[c]; ctx->zbox_hi[c] = I.hi[c]; }
+    }
     rc = ile_launch_lnL_z(ctx, p, N, I.d, it->z, nullptr, it->lnL, it->ln_prior);
+    ctx->zbox_hint = 0;
     if (rc) return rc;
     lnw_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(N, it->lnL, it->ln_prior, it->ln_ps, it->lnw);
     ILE_LAUNCH_CHECK(ctx);

@@ -139,6 +139,11 @@ int ile_launch_lnL_z(ile_ctx* ctx, int p, int N, int d, const double* z, const i
     if (rc) return rc;
     if (N < 0 || (N > 0 && (!z || !lnL))) return ile_fail(ctx, ILE_EINVAL, "lnL_z: bad argument");
     if (N == 0) return ILE_OK;
+    if (ctx->zbox_hint) {                        // a batch drawn inside a box that lies within the prior box needs no box test
+        bool inside = true;
+        for (int c = 0; c < d; c++) inside = inside && ctx->zbox_lo[c] >= P.lo[c] && ctx->zbox_hi[c] <= P.hi[c];
+        P.box_trusted = inside ? 1 : 0;
+    }
     if (ctx->variant == 1) return ile_launch_lnL_plain_z(ctx, P, N, z, lnL, ln_prior);
     return ile_launch_lnL_fused(ctx, P, N, z, perm, lnL, ln_prior);
 }

@@ -151,10 +151,11 @@ __global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const d
     if (i >= N) return;
     const double ra = z[i], sd = z[(size_t)N + i];
     bool ok = true;
-    for (int c = 0; c < P.d; c++) {
-        const double v = z[(size_t)c * N + i];
-        ok = ok && (v >= P.lo[c]) && (v < P.hi[c]);
-    }
+    if (!P.box_trusted)
+        for (int c = 0; c < P.d; c++) {
+            const double v = z[(size_t)c * N + i];
+            ok = ok && (v >= P.lo[c]) && (v < P.hi[c]);
+        }
     unsigned long long k = 1ull << (cell_bits * P.K);      // out-of-box samples last
     if (ok) {
         const double cd = sqrt(fmax((1.0 - sd) * (1.0 + sd), 0.0));
