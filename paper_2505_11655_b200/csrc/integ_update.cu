@@ -770,7 +770,7 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
     const IntegDev& I = it->I;
     const SamplerDev& S = I.mem[a];
     cudaStream_t st = ctx->stream;
-    const int grid = ctx->sm_count * 4;
+    const int grid = ctx->sm_count * 8;
     switch (S.kind) {
         case ILE_KIND_UNIFORM:
             return ILE_OK;
