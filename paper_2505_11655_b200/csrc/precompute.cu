@@ -33,13 +33,14 @@ __global__ void pc_twiddle_kernel(int N_f, double2* __restrict__ W) {
     W[m] = make_double2(c, s);
 }
 
-// U and V, upper triangle.  CTA (slice, p): the frequency slice of point p in chunks of UV_CH bins, double-buffered in
+// U and V, upper triangle.  CTA (slice, p): the frequency slice of point p in chunks of UV_CH bins, triple-buffered in
 // shared memory by asynchronous copies (h_m[j] and h_m[-j] for all modes, w_k[j]).  Thread = (2 x 2 tile of mode pairs,
 // one of UV_SUB interleaved sub-slices of the chunk): 6 shared-memory loads feed 4 pairs x (8 + 12 K / 3) FP64 operations,
 // 16 K running sums in registers.  The sub-slices are added in shared memory, the per-CTA partial sums part[p][slice][pair][k][4]
 // in slice order by pc_uv_finish_kernel (deterministic), which also fills the lower triangle by Eq. 17-18.
 #define UV_CH 64
 #define UV_SUB 5
+#define UV_NBUF 3
 #define UV_SB (2 * UV_CH + 1)                  // stride of a mode pair's rows in 16-byte units (odd: no bank conflicts)
 #define UV_MAXTHREADS(BIG) ((BIG) ? 416 : 352)  // 78 tiles (24 modes) or 66 (22 modes) x 5 sub-slices: 13 or 11 warps, close to even over 4 sub-partitions
 template <int KK, bool BIG>
@@ -47,9 +48,9 @@ __global__ void __launch_bounds__(UV_MAXTHREADS(BIG), 1) pc_uv_kernel(int M, int
                                                                  double* __restrict__ part) {
     extern __shared__ double2 uv_sm[];
     const int MB = (M + 1) >> 1, n_tiles = MB * (MB + 1) / 2;
-    double2* hs = uv_sm;                                   // [2][MB][UV_CH][2]  (+1 per mode pair)
-    double2* hm = hs + 2 * MB * UV_SB;                     // the same at -f
-    double* ws = reinterpret_cast<double*>(hm + 2 * MB * UV_SB);   // [2][KK][UV_CH]
+    double2* hs = uv_sm;                                   // [UV_NBUF][MB][UV_CH][2]  (+1 per mode pair)
+    double2* hm = hs + UV_NBUF * MB * UV_SB;               // the same at -f
+    double* ws = reinterpret_cast<double*>(hm + UV_NBUF * MB * UV_SB);   // [UV_NBUF][KK][UV_CH]
     const int p = blockIdx.y, tid = threadIdx.x, nthr = blockDim.x;
     const double2* hp = h + (size_t)p * M * N_f;
     const int tile = tid % n_tiles, sub = tid / n_tiles;
@@ -64,7 +65,7 @@ __global__ void __launch_bounds__(UV_MAXTHREADS(BIG), 1) pc_uv_kernel(int M, int
 #pragma unroll
     for (int e = 0; e < 16 * KK; e++) (&acc[0][0][0][0])[e] = 0.0;
     // rows of a padding mode (odd M) stay zero in both buffers
-    for (int q = tid; q < 2 * 2 * MB * UV_SB; q += nthr) hs[q] = make_double2(0.0, 0.0);
+    for (int q = tid; q < 2 * UV_NBUF * MB * UV_SB; q += nthr) hs[q] = make_double2(0.0, 0.0);
     __syncthreads();
     const int c_begin = blockIdx.x * chunks_per_block, c_end = min(c_begin + chunks_per_block, (N_f + UV_CH - 1) / UV_CH);
     auto stage = [&](int c, int buf) {
@@ -89,12 +90,15 @@ __global__ void __launch_bounds__(UV_MAXTHREADS(BIG), 1) pc_uv_kernel(int M, int
         }
         __pipeline_commit();
     };
+    // three buffers: chunk c + 2 is requested right after the barrier of chunk c, into the buffer chunk c - 1 was read from
+    // (every thread is past it), so one barrier per chunk suffices
     if (c_begin < c_end) stage(c_begin, 0);
+    if (c_begin + 1 < c_end) stage(c_begin + 1, 1);
     for (int c = c_begin; c < c_end; c++) {
-        const int buf = (c - c_begin) & 1;
-        if (c + 1 < c_end) stage(c + 1, buf ^ 1);
+        const int buf = (c - c_begin) % UV_NBUF;
         if (c + 1 < c_end) __pipeline_wait_prior(1); else __pipeline_wait_prior(0);
         __syncthreads();
+        if (c + 2 < c_end) stage(c + 2, (c + 2 - c_begin) % UV_NBUF);
         if (act) {
             const double2* xa = hs + (buf * MB + ta) * UV_SB;
             const double2* xm = hm + (buf * MB + ta) * UV_SB;
@@ -123,8 +127,8 @@ __global__ void __launch_bounds__(UV_MAXTHREADS(BIG), 1) pc_uv_kernel(int M, int
                     }
             }
         }
-        __syncthreads();                                              // the chunk is consumed before its buffer is refilled
     }
+    __syncthreads();                                                  // the staging buffers are free
     // the sub-slices of a tile meet in shared memory (sub-slice order), one partial per (slice, pair)
     double* red = reinterpret_cast<double*>(uv_sm);                  // [UV_SUB][n_tiles][16 KK], the staging buffers are idle
     if (act) {
@@ -441,7 +445,7 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     }
     {
         const int MB = (M + 1) / 2, uv_threads = (MB * (MB + 1) / 2 * UV_SUB + 31) / 32 * 32;
-        const size_t uv_stage = (size_t)4 * MB * UV_SB * sizeof(double2) + (size_t)2 * K * UV_CH * sizeof(double);
+        const size_t uv_stage = (size_t)2 * UV_NBUF * MB * UV_SB * sizeof(double2) + (size_t)UV_NBUF * K * UV_CH * sizeof(double);
         const size_t uv_red = (size_t)UV_SUB * (MB * (MB + 1) / 2) * 16 * K * sizeof(double);
         const size_t uv_smem = uv_stage > uv_red ? uv_stage : uv_red;
         const double2* hh = (const double2*)h;
