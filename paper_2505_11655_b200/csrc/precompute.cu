@@ -271,6 +271,54 @@ __global__ void __launch_bounds__(PQ_THREADS, NOUT <= 4 ? 2 : 1) pc_q_pruned_ker
         }
         __syncthreads();
         int H = Mq >> 1, ts = 1, stages = log2Mq;
+        if (tail16 && stages >= 8) {
+            // the first four stages (quarters Mq/4 and Mq/16) on 16 elements Mq/16 apart in registers: thread = (transform, offset)
+            const int q2 = Mq >> 4;
+            for (int it = tid; it < q2 * PQ_BG; it += PQ_THREADS) {
+                const int i0 = it % q2;
+                double2* sm = xs + (it / q2) * MqP;
+                double2 v[16];
+#pragma unroll
+                for (int m = 0; m < 16; m++) v[m] = sm[pq_pad(i0 + q2 * m)];
+#pragma unroll
+                for (int c = 0; c < 4; c++) {                 // quarter Mq/4: elements c, c + 4, c + 8, c + 12
+                    const int pos = i0 + q2 * c;
+                    const double2 w1 = tw[pos], w2 = tw[2 * pos];
+                    const double2 x0 = v[c], x1 = v[c + 4], x2 = v[c + 8], x3 = v[c + 12];
+                    const double2 y0 = make_double2(x0.x + x2.x, x0.y + x2.y), y1 = make_double2(x1.x + x3.x, x1.y + x3.y);
+                    const double ar = x0.x - x2.x, ai = x0.y - x2.y, br = x1.x - x3.x, bi = x1.y - x3.y;
+                    const double2 y2 = make_double2(ar * w1.x - ai * w1.y, ar * w1.y + ai * w1.x);
+                    const double2 y3 = make_double2(-(br * w1.y + bi * w1.x), br * w1.x - bi * w1.y);
+                    const double cr = y0.x - y1.x, ci = y0.y - y1.y, dr = y2.x - y3.x, di = y2.y - y3.y;
+                    v[c] = make_double2(y0.x + y1.x, y0.y + y1.y);
+                    v[c + 4] = make_double2(cr * w2.x - ci * w2.y, cr * w2.y + ci * w2.x);
+                    v[c + 8] = make_double2(y2.x + y3.x, y2.y + y3.y);
+                    v[c + 12] = make_double2(dr * w2.x - di * w2.y, dr * w2.y + di * w2.x);
+                }
+                {
+                    const double2 w1 = tw[4 * i0], w2 = tw[8 * i0];   // quarter Mq/16: elements 4 r .. 4 r + 3, one twiddle pair
+#pragma unroll
+                    for (int r = 0; r < 4; r++) {
+                        const double2 x0 = v[4 * r], x1 = v[4 * r + 1], x2 = v[4 * r + 2], x3 = v[4 * r + 3];
+                        const double2 y0 = make_double2(x0.x + x2.x, x0.y + x2.y), y1 = make_double2(x1.x + x3.x, x1.y + x3.y);
+                        const double ar = x0.x - x2.x, ai = x0.y - x2.y, br = x1.x - x3.x, bi = x1.y - x3.y;
+                        const double2 y2 = make_double2(ar * w1.x - ai * w1.y, ar * w1.y + ai * w1.x);
+                        const double2 y3 = make_double2(-(br * w1.y + bi * w1.x), br * w1.x - bi * w1.y);
+                        const double cr = y0.x - y1.x, ci = y0.y - y1.y, dr = y2.x - y3.x, di = y2.y - y3.y;
+                        v[4 * r] = make_double2(y0.x + y1.x, y0.y + y1.y);
+                        v[4 * r + 1] = make_double2(cr * w2.x - ci * w2.y, cr * w2.y + ci * w2.x);
+                        v[4 * r + 2] = make_double2(y2.x + y3.x, y2.y + y3.y);
+                        v[4 * r + 3] = make_double2(dr * w2.x - di * w2.y, dr * w2.y + di * w2.x);
+                    }
+                }
+#pragma unroll
+                for (int m = 0; m < 16; m++) sm[pq_pad(i0 + q2 * m)] = v[m];
+            }
+            __syncthreads();
+            H >>= 4;
+            ts <<= 4;
+            stages -= 4;
+        }
         while (stages >= 2 && !(tail16 && stages == 4)) {
             const int q = H >> 1;
             for (int t = tid; t < (Mq >> 2); t += PQ_THREADS) {
