@@ -265,11 +265,13 @@ __global__ void __launch_bounds__(128, 6) draw_kernel(IntegDev I, int N, unsigne
             if (cell > av.C - 1) cell = av.C - 1;
             key = S.keys[cell];
         }
-        double ua = 0.0, ub = 0.0;
+        // all the uniforms first: the Philox calls are independent chains the scheduler can interleave
+        double uc[D + 1];
+#pragma unroll
+        for (int pq = 0; pq < (D + 1) / 2; pq++) philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + pq), &uc[2 * pq], &uc[2 * pq + 1]);
 #pragma unroll
         for (int c = 0; c < d; c++) {
-            if ((c & 1) == 0) philox_pair(I.seed, (unsigned long long)i, g, (unsigned int)(1 + (c >> 1)), &ua, &ub);
-            const double u = (c & 1) ? ub : ua;
+            const double u = uc[c];
             const double lo = I.lo[c], hi = I.hi[c];
             double zc;
             if (S.kind == ILE_KIND_UNIFORM) {
