@@ -105,26 +105,42 @@ __global__ void __launch_bounds__(256) ac_hist_kernel(IntegDev I, int a, int N, 
         if (sh_h[q]) atomicAdd(&H[q], sh_h[q]);
 }
 
-// pi_c[b] = (1 - eps) H_c[b] / sum H_c + eps / n_b; cdf = left-to-right running sum
-__global__ void ac_finish_kernel(IntegDev I, int a, const UpdScratch* __restrict__ us) {
+// pi_c[b] = (1 - eps) H_c[b] / sum H_c + eps / n_b; cdf = left-to-right running sum.  One block per dimension: the
+// integer total and the bins' divisions in parallel, the running sum by one thread in bin order (the oracle's order)
+__global__ void __launch_bounds__(256) ac_finish_kernel(IntegDev I, int a, const UpdScratch* __restrict__ us) {
     if (us->abort) return;
-    const int c = threadIdx.x;
-    if (c >= I.d) return;
+    const int c = blockIdx.x, t = threadIdx.x;
     const int nb = I.mem[a].nb;
     const unsigned long long* H = I.mem[a].H + c * nb;
     double* pi = I.mem[a].pi + c * nb;
     double* cdf = I.mem[a].cdf + c * (nb + 1);
-    unsigned long long tot = 0;
-    for (int b = 0; b < nb; b++) tot += H[b];
+    __shared__ unsigned long long part[8];
+    __shared__ unsigned long long tot_sh;
+    unsigned long long s = 0;
+    for (int b = t; b < nb; b += blockDim.x) s += H[b];
+    s = warp_sum_u64(s);
+    if ((t & 31) == 0) part[t >> 5] = s;
+    __syncthreads();
+    if (t == 0) {
+        unsigned long long tot = 0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) tot += part[w];
+        tot_sh = tot;
+    }
+    __syncthreads();
+    const unsigned long long tot = tot_sh;
     if (tot == 0) return;                         // keep the old marginal
-    double acc = 0.0;
-    cdf[0] = 0.0;
-    for (int b = 0; b < nb; b++) {
+    for (int b = t; b < nb; b += blockDim.x) {
         const double frac = __ddiv_rn(__ull2double_rn(H[b]), __ull2double_rn(tot));
-        const double p = __dadd_rn(__dmul_rn(__dsub_rn(1.0, I.eps), frac), __ddiv_rn(I.eps, (double)nb));
-        pi[b] = p;
-        acc = __dadd_rn(acc, p);
-        cdf[b + 1] = acc;
+        pi[b] = __dadd_rn(__dmul_rn(__dsub_rn(1.0, I.eps), frac), __ddiv_rn(I.eps, (double)nb));
+    }
+    __syncthreads();
+    if (t == 0) {
+        double acc = 0.0;
+        cdf[0] = 0.0;
+        for (int b = 0; b < nb; b++) {
+            acc = __dadd_rn(acc, pi[b]);
+            cdf[b + 1] = acc;
+        }
     }
 }
 
@@ -781,7 +797,7 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
             ILE_LAUNCH_CHECK(ctx);
             ac_hist_kernel<<<grid, 256, (size_t)I.d * S.nb * 8, st>>>(I, a, N, z, lnw, it->us);
             ILE_LAUNCH_CHECK(ctx);
-            ac_finish_kernel<<<1, 32, 0, st>>>(I, a, it->us);
+            ac_finish_kernel<<<I.d, 256, 0, st>>>(I, a, it->us);
             ILE_LAUNCH_CHECK(ctx);
             return ILE_OK;
         }
