@@ -201,6 +201,16 @@ int ile_lnL_z(ile_ctx *ctx, int p, int N, int d, const double *z /*[d][N]*/, dou
 int ile_set_lnL_variant(ile_ctx *ctx, int variant);
 /* Step 7 (Eq. 8, 9, 16): reduce N log-weights into *out_dev (device; cumulative fields reset). */
 int ile_reduce(ile_ctx *ctx, int N, const double *lnw, ile_result *out_dev);
+/* The same reduction for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): calls no cudaMalloc, cudaFree or allocating library routine.  Its per-block partial sums live in a
+ * 64 KB file-scope device array (2048 partials of 32 bytes) that every GPU loading the library holds until exit.
+ * N <= ILE_REDUCE_NOALLOC_MAX_N, else ILE_EINVAL with a message (ile_last_error) and nothing launched.  lnw [N] and
+ * out_dev are device pointers owned by the caller, as for ile_reduce; the work is queued on the context's stream.  All
+ * calls on a device share the array: calls that overlap on the GPU (two contexts, two streams) race; calls on one stream
+ * are ordered and safe.  Nothing in the array has to start at zero: a call reads only what it wrote.  Results are
+ * bit-identical to ile_reduce's (same kernels, same grid). */
+#define ILE_REDUCE_NOALLOC_MAX_N (1 << 24)
+int ile_reduce_noalloc(ile_ctx *ctx, int N, const double *lnw, ile_result *out_dev);
 
 /* ------------------------------------------------------------------ integrators (steps 8-11) */
 int ile_integrator_opts_default(ile_integrator_opts *opts, int kind, int d);

@@ -270,6 +270,13 @@ class Ile:
         self._ck(self.lib.ile_reduce(self.ctx, C.c_int(lnw.numel()), _ptr(lnw), _ptr(res)))
         return result_from_device(res)[0]
 
+    def reduce_noalloc(self, lnw, out=None):
+        """ile_reduce_noalloc: the same reduction with its scratch in a static device array (no allocation in the library;
+        pass `out` to allocate nothing here either).  Returns the decoded result (synchronises)."""
+        res = self.torch.zeros(C.sizeof(Result), dtype=self.torch.uint8, device=f"cuda:{self.device}") if out is None else out
+        self._ck(self.lib.ile_reduce_noalloc(self.ctx, C.c_int(lnw.numel()), _ptr(lnw), _ptr(res)))
+        return result_from_device(res)[0]
+
 
 def result_from_device(buf):
     """uint8 CUDA tensor holding ile_result structs -> numpy structured array (synchronises)."""

@@ -129,3 +129,51 @@ extern "C" int ile_reduce(ile_ctx* ctx, int N, const double* lnw, ile_result* ou
     cudaSetDevice(ctx->device);   // every entry runs on the context's device, whatever the caller's current one
     return ile_launch_reduce(ctx, N, lnw, out_dev, 0);
 }
+
+// ---------------------------------------------------------------- ile_reduce without allocation
+// For callers that must not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the
+// per-block partials live in a file-scope device array instead of the context's grow-only scratch.  Every GPU that
+// loads the library holds the array (64 KB) until exit.  All calls on a device share it: calls that overlap on the GPU
+// (two contexts, or two streams) race; calls on one stream do not.  Every partial a call reads was written by that
+// call (block b writes entry b, the final kernel reads entries 0 .. nblocks - 1), so nothing has to start at zero and the
+// contents the last call left behind are never seen.
+#define RED_NOALLOC_MAX_BLOCKS 2048
+#define RED_NOALLOC_MAX_DEVICES 64
+static __device__ __align__(256) RedPart red_noalloc_part[RED_NOALLOC_MAX_BLOCKS];
+
+// device address of the array on the current device; looked up once per device, with that device current
+static int red_noalloc_address(ile_ctx* ctx, RedPart** out) {
+    static RedPart* addr[RED_NOALLOC_MAX_DEVICES];            // zero-initialised: not looked up yet
+    const int dev = ctx->device;
+    if (dev < 0 || dev >= RED_NOALLOC_MAX_DEVICES) return ile_fail(ctx, ILE_EINVAL, "reduce_noalloc: device %d beyond %d", dev, RED_NOALLOC_MAX_DEVICES);
+    if (!addr[dev]) {
+        RedPart* p = nullptr;
+        ILE_CUDA(ctx, cudaGetSymbolAddress((void**)&p, red_noalloc_part));     // the symbol's name is not a device address in host code
+        if (!p) return ile_fail(ctx, ILE_ECUDA, "reduce_noalloc: no device address for the static scratch");
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return ILE_OK;
+}
+
+extern "C" int ile_reduce_noalloc(ile_ctx* ctx, int N, const double* lnw, ile_result* out_dev) {
+    if (!ctx) return ILE_EINVAL;
+    cudaSetDevice(ctx->device);
+    if (N < 1 || !lnw || !out_dev) return ile_fail(ctx, ILE_EINVAL, "reduce_noalloc: bad argument");
+    if (N > ILE_REDUCE_NOALLOC_MAX_N)
+        return ile_fail(ctx, ILE_EINVAL, "reduce_noalloc: N = %d exceeds the maximum %d of the allocation-free path (use ile_reduce)", N,
+                        ILE_REDUCE_NOALLOC_MAX_N);
+    RedPart* part = nullptr;
+    int rc = red_noalloc_address(ctx, &part);
+    if (rc) return rc;
+    // the same grid as ile_reduce, capped by the array
+    int nblocks = (N + 256 * 8 - 1) / (256 * 8);
+    if (nblocks > ctx->sm_count * 8) nblocks = ctx->sm_count * 8;
+    if (nblocks > RED_NOALLOC_MAX_BLOCKS) nblocks = RED_NOALLOC_MAX_BLOCKS;
+    ILE_CUDA(ctx, cudaMemsetAsync(out_dev, 0, sizeof(ile_result), ctx->stream));
+    reduce_partial_kernel<<<nblocks, 256, 0, ctx->stream>>>(N, lnw, part);
+    ILE_LAUNCH_CHECK(ctx);
+    reduce_final_kernel<<<1, 256, 0, ctx->stream>>>(nblocks, part, N, out_dev, 0);
+    ILE_LAUNCH_CHECK(ctx);
+    return ILE_OK;
+}
