@@ -131,8 +131,9 @@ int ile_split_cell_bits(int n_min, int n_max);
 int ile_split_max_tiles(int N, int cell_bits, int K);
 size_t ile_split_tile_bytes(int max_tiles);
 int ile_launch_split_keys(ile_ctx* ctx, const LnlParams& P, int N, const double* z, int n_min, int cell_bits, unsigned long long* key,
-                          unsigned int* val, double* uk, long long* n_dev, int* bits_dev, int* ntiles_dev);
-int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int n_min, int cell_bits, const unsigned long long* key, const double* z, const double* uk,
+                          unsigned int* val, double* rec, long long* n_dev, int* bits_dev, int* ntiles_dev);
+size_t ile_split_rec_bytes(int N);
+int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int n_min, int cell_bits, const unsigned long long* key, const double* rec,
                      const int* perm, double* lnL, double* ln_prior, int* tstart, SpTile* tiles, int* ntiles_dev);
 int ile_timing_begin(ile_ctx* ctx);            // returns a slot (or -1 when timing is off)
 void ile_timing_end(ile_ctx* ctx, int slot);

@@ -128,7 +128,7 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
     const int tiles = (N + 63) / 64 * 2;                       // 32-sample sub-tiles, padded to whole 64-sample tiles
     const size_t rec_bytes = split ? 0 : ((size_t)tiles * FT_TS * FT_REC * sizeof(double) + 255) / 256 * 256;
     const size_t y_bytes = split ? 0 : ((size_t)tiles * FT_YM * FT_TS * sizeof(double2) + 255) / 256 * 256;
-    const size_t uk_bytes = split ? ((size_t)N * 32 + 255) / 256 * 256 : 0;
+    const size_t uk_bytes = split ? (ile_split_rec_bytes(N) + 255) / 256 * 256 : 0;      // sample records of the tcgen05 path (coordinates + u_k)
     const size_t key_bytes = ((size_t)N * 8 + 255) / 256 * 256, val_bytes = ((size_t)N * 4 + 255) / 256 * 256;
     const size_t sort_bytes = (radix_sort_scratch_bytes(N) + 255) / 256 * 256;
     const bool sort = perm == nullptr && (split || (ctx->sky_sort && N > FT_TS));
@@ -175,7 +175,7 @@ int ile_launch_lnL_fused(ile_ctx* ctx, const LnlParams& P, int N, const double* 
         char* tb = base + rec_bytes + y_bytes + uk_bytes + 2 * key_bytes + 2 * val_bytes + sort_bytes + 256;
         SpTile* tl = (SpTile*)tb;
         int* tstart = (int*)(tb + (size_t)sp_tiles * 32);
-        return ile_launch_split(ctx, P, N, n_min, sp_bits, k0, z, uk, perm, lnL, ln_prior, tstart, tl, ntiles_dev);
+        return ile_launch_split(ctx, P, N, n_min, sp_bits, k0, uk, perm, lnL, ln_prior, tstart, tl, ntiles_dev);
     }
     rc = ile_ensure_qf(ctx);
     if (rc) return rc;

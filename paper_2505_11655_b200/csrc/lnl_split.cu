@@ -48,6 +48,7 @@
 #define SP_G 4                // threads per sample (warp groups): digits by detector, bins, triangle rows, log-sum-exp rows
 #define SP_MATH (SP_G * SP_TS)
 #define SP_RAISE_HI 0x40800000   // high word of 512.0: the streaming log-sum-exp raises its reference beyond e^512
+#define SP_REC 12               // doubles per sample record: z[0..5] (RA, sin Dec, psi, phi_ref, cos incl, D), u_k[0..2], padding
 #define SP_THREADS (SP_MATH + 32)
 #define SP_UVMAX (300 * 3 * 2)
 #define SP_MAGIC 6755399441055744.0   // 1.5 * 2^52
@@ -139,7 +140,7 @@ int ile_split_build_q(ile_ctx* ctx, int P, int K, int M, int N_Q, const double* 
 
 // ---------------------------------------------------------------- delay-cell keys and tiles
 __global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const double* __restrict__ z, int n_min, int cell_bits,
-                                                     unsigned long long* __restrict__ key, unsigned int* __restrict__ val, double* __restrict__ uk,
+                                                     unsigned long long* __restrict__ key, unsigned int* __restrict__ val, double* __restrict__ rec,
                                                      long long* n_dev, int* bits_dev, int* ntiles_dev) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) {
@@ -148,33 +149,53 @@ __global__ void __launch_bounds__(256) sp_key_kernel(LnlParams P, int N, const d
         ntiles_dev[0] = 0;                                 // tile count, run count
         ntiles_dev[1] = 0;
     }
-    if (i >= N) return;
-    const double ra = z[i], sd = z[(size_t)N + i];
-    bool ok = true;
-    if (!P.box_trusted)
-        for (int c = 0; c < P.d; c++) {
-            const double v = z[(size_t)c * N + i];
-            ok = ok && (v >= P.lo[c]) && (v < P.hi[c]);
+    __shared__ double srec[256 * (SP_REC + 1)];
+    if (i < N) {
+        // the sample's record: coordinates (coalesced reads, one array per coordinate) and below its u_k, 96 bytes = three
+        // whole 32-byte sectors, so that the fused kernel's gather through the sort permutation fetches nothing it does not use
+        double zc[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 1.0}, uo[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+        for (int c = 0; c < 6; c++)
+            if (c < P.d) zc[c] = z[(size_t)c * N + i];          // six independent loads in flight
+        const double ra = zc[0], sd = zc[1];
+        bool ok = true;
+        if (!P.box_trusted) {
+#pragma unroll
+            for (int c = 0; c < 6; c++)
+                if (c < P.d) ok = ok && (zc[c] >= P.lo[c]) && (zc[c] < P.hi[c]);
         }
-    unsigned long long k = 1ull << (cell_bits * P.K);      // out-of-box samples last
-    if (ok) {
-        const double cd = sqrt(fmax((1.0 - sd) * (1.0 + sd), 0.0));
-        double sg, cg;
-        sincos(P.gmst - ra, &sg, &cg);
-        const double n0 = cd * cg, n1 = -cd * sg, n2 = sd;
-        k = 0;
-        for (int kk = 0; kk < P.K; kk++) {
-            const double tau = -(P.pos[kk][0] * n0 + P.pos[kk][1] * n1 + P.pos[kk][2] * n2) / ILE_C_LIGHT;
-            double u = (P.t_lo + tau - P.t_Q0) * P.fs;
-            if (!P.interp) u = floor(u + 0.5);
-            uk[(size_t)i * 4 + kk] = u;                      // the fused kernel and the tile builder use this very value
-            int cell = ((int)floor(u) - n_min) >> SP_CELL_SHIFT;
-            cell = max(0, min(cell, (1 << cell_bits) - 1));
-            k = (k << cell_bits) | (unsigned long long)cell;
+        unsigned long long k = 1ull << (cell_bits * P.K);      // out-of-box samples last
+        if (ok) {
+            const double cd = sqrt(fmax((1.0 - sd) * (1.0 + sd), 0.0));
+            double sg, cg;
+            sincos(P.gmst - ra, &sg, &cg);
+            const double n0 = cd * cg, n1 = -cd * sg, n2 = sd;
+            k = 0;
+            for (int kk = 0; kk < P.K; kk++) {
+                const double tau = -(P.pos[kk][0] * n0 + P.pos[kk][1] * n1 + P.pos[kk][2] * n2) / ILE_C_LIGHT;
+                double u = (P.t_lo + tau - P.t_Q0) * P.fs;
+                if (!P.interp) u = floor(u + 0.5);
+                if (kk < 3) uo[kk] = u;                          // the fused kernel uses this very value
+                int cell = ((int)floor(u) - n_min) >> SP_CELL_SHIFT;
+                cell = max(0, min(cell, (1 << cell_bits) - 1));
+                k = (k << cell_bits) | (unsigned long long)cell;
+            }
+        }
+        key[i] = k;
+        val[i] = (unsigned int)i;
+        {
+            double* r = &srec[threadIdx.x * (SP_REC + 1)];     // odd stride: conflict-free
+    #pragma unroll
+            for (int c = 0; c < 6; c++) r[c] = zc[c];
+            r[6] = uo[0]; r[7] = uo[1]; r[8] = uo[2];
+            r[9] = r[10] = r[11] = 0.0;
         }
     }
-    key[i] = k;
-    val[i] = (unsigned int)i;
+    // the block's records are contiguous in global memory: consecutive threads write consecutive doubles
+    __syncthreads();
+    const size_t first = (size_t)blockIdx.x * blockDim.x;
+    const int nrec = (int)min((size_t)blockDim.x, (size_t)N - first);
+    for (int q = threadIdx.x; q < nrec * SP_REC; q += blockDim.x) rec[first * SP_REC + q] = srec[(q / SP_REC) * (SP_REC + 1) + q % SP_REC];
 }
 
 // Tiles: the sorted order is cut at every cell change (run start) and every 128 samples after it.
@@ -334,7 +355,7 @@ __device__ __forceinline__ void sp_cursor_next(SpCursor& cu, const SpTile* __res
 
 template <int K, bool TABLE>
 __global__ void __launch_bounds__(SP_THREADS, 1)
-lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double* __restrict__ uk, const int* __restrict__ perm,
+lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* __restrict__ perm,
                  double* __restrict__ lnL, double* __restrict__ ln_prior, const SpTile* __restrict__ tiles, const int* __restrict__ ntiles_dev) {
     extern __shared__ __align__(1024) unsigned char sp_smem_raw[];
     SplitSmem& sm = *reinterpret_cast<SplitSmem*>(sp_smem_raw);
@@ -461,9 +482,10 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                     SampleIn sp;
                     sp.ra = 0.0; sp.sd = 0.0; sp.cd = 1.0; sp.psi = 0.0; sp.phi_ref = 0.0; sp.ch = 1.0; sp.sh = 0.0; sp.dist = 1.0; sp.valid = member;
                     if (member) {
-                        sp.ra = __ldg(z + sidx);
-                        sp.sd = __ldg(z + (size_t)N + sidx);
-                        sp.psi = __ldg(z + 2 * (size_t)N + sidx);
+                        const double2 r0 = __ldg(reinterpret_cast<const double2*>(rec + sidx * SP_REC));
+                        sp.ra = r0.x;
+                        sp.sd = r0.y;
+                        sp.psi = __ldg(rec + sidx * SP_REC + 2);
                         sp.cd = sqrt(fmax((1.0 - sp.sd) * (1.0 + sp.sd), 0.0));
                     }
                     double Fp[ILE_MAX_K], Fx[ILE_MAX_K], tau[ILE_MAX_K];
@@ -474,7 +496,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                         shr[(3 + k) * SP_TS] = -Fx[k];
                     }
                 } else if (g == 1) {
-                    const double ci = member ? __ldg(z + 4 * (size_t)N + sidx) : 1.0;
+                    const double ci = member ? __ldg(rec + sidx * SP_REC + 4) : 1.0;
                     const double ch = sqrt(fmax(0.5 * (1.0 + ci), 0.0)), sh = sqrt(fmax(0.5 * (1.0 - ci), 0.0));
                     double a = 1.0, b = 1.0;
                     pc[0] = 1.0;
@@ -486,7 +508,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                         ps[q * SP_TS] = b;
                     }
                 } else if (g == 2) {
-                    const double phi = member ? -__ldg(z + 3 * (size_t)N + sidx) : 0.0;   // -2Y_lm(iota, -phi_ref) (reading G7)
+                    const double phi = member ? -__ldg(rec + sidx * SP_REC + 3) : 0.0;   // -2Y_lm(iota, -phi_ref) (reading G7)
                     cm[0] = 1.0;
                     sn[0] = 0.0;
                     for (int q = 1; q <= mm; q++) {
@@ -499,13 +521,13 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                     double xs = 0.0;
                     if (member) {
                         SampleIn sp;
-                        sp.dist = P.d > 5 ? __ldg(z + 5 * (size_t)N + sidx) : 1.0;
+                        sp.dist = P.d > 5 ? __ldg(rec + sidx * SP_REC + 5) : 1.0;
                         xs = TABLE ? 1.0 : P.D_ref / sp.dist;
                         if (ln_prior) ln_prior[sidx] = ln_prior_dev(P, sp);
                     }
                     shr[6 * SP_TS] = xs;
 #pragma unroll
-                    for (int k = 0; k < K; k++) shu[k * SP_TS] = member ? __ldg(uk + sidx * 4 + k) : (double)ti.base[k];
+                    for (int k = 0; k < K; k++) shu[k * SP_TS] = member ? __ldg(rec + sidx * SP_REC + 6 + k) : (double)ti.base[k];
                 }
                 qbar();
                 x = shr[6 * SP_TS];
@@ -535,17 +557,14 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
                 }
             }
             qbar();
-            // ---- the next tile's coordinates are gathered through the sort permutation (scattered 8-byte reads): ask for
+            // ---- the next tile's records are gathered through the sort permutation (scattered 96-byte reads): ask for
             //      them now, so that its prologue finds them in L2 instead of waiting two dependent DRAM round trips
             if (t + (int)gridDim.x < ntiles) {
                 const SpTile tn = tiles[t + gridDim.x];
                 if (tn.nchunk > 0 && i < tn.cnt) {
                     const size_t sn_ = (size_t)perm[tn.start + i];
                     auto pf = [](const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); };
-                    if (g == 0) { pf(z + sn_); pf(z + (size_t)N + sn_); pf(z + 2 * (size_t)N + sn_); }
-                    else if (g == 1) pf(z + 4 * (size_t)N + sn_);
-                    else if (g == 2) pf(z + 3 * (size_t)N + sn_);
-                    else { if (P.d > 5) pf(z + 5 * (size_t)N + sn_); pf(uk + sn_ * 4); }
+                    if (g < 3) pf(rec + sn_ * SP_REC + 4 * g);           // the record's three sectors
                 }
             }
             // ---- step 3 (group k does detector k): coefficients x F_k Y_m -> six signed 8-bit digits -> tensor memory (operand A)
@@ -816,12 +835,12 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ z, const double*
 
 // ---------------------------------------------------------------- launch
 template <int K, bool TABLE>
-static int launch_split_t(ile_ctx* ctx, const LnlParams& P, int N, const double* z, const double* uk, const int* perm, double* lnL,
+static int launch_split_t(ile_ctx* ctx, const LnlParams& P, int N, const double* rec, const int* perm, double* lnL,
                           double* ln_prior, const SpTile* tiles, const int* ntiles_dev) {
     const int smem = (int)sizeof(SplitSmem) + 1024;
     ILE_CUDA(ctx, cudaFuncSetAttribute(lnl_split_kernel<K, TABLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     const int slot = ile_timing_begin(ctx);
-    lnl_split_kernel<K, TABLE><<<ctx->sm_count, SP_THREADS, smem, ctx->stream>>>(P, N, z, uk, perm, lnL, ln_prior, tiles, ntiles_dev);
+    lnl_split_kernel<K, TABLE><<<ctx->sm_count, SP_THREADS, smem, ctx->stream>>>(P, N, rec, perm, lnL, ln_prior, tiles, ntiles_dev);
     ile_timing_end(ctx, slot);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
@@ -836,6 +855,8 @@ int ile_split_max_tiles(int N, int cell_bits, int K) {
     return (int)t;
 }
 size_t ile_split_tile_bytes(int max_tiles) { return ((size_t)max_tiles * (sizeof(SpTile) + 2 * sizeof(int)) + 255) / 256 * 256; }   // tiles, tile starts, run starts
+size_t ile_split_rec_bytes(int N) { return (size_t)N * SP_REC * sizeof(double); }
+
 int ile_split_cell_bits(int n_min, int n_max) {
     int cell_bits = 1;
     while ((1 << cell_bits) <= ((n_max - n_min) >> SP_CELL_SHIFT)) cell_bits++;
@@ -843,14 +864,14 @@ int ile_split_cell_bits(int n_min, int n_max) {
 }
 
 int ile_launch_split_keys(ile_ctx* ctx, const LnlParams& P, int N, const double* z, int n_min, int cell_bits, unsigned long long* key,
-                          unsigned int* val, double* uk, long long* n_dev, int* bits_dev, int* ntiles_dev) {
-    sp_key_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(P, N, z, n_min, cell_bits, key, val, uk, n_dev, bits_dev, ntiles_dev);
+                          unsigned int* val, double* rec, long long* n_dev, int* bits_dev, int* ntiles_dev) {
+    sp_key_kernel<<<(N + 255) / 256, 256, 0, ctx->stream>>>(P, N, z, n_min, cell_bits, key, val, rec, n_dev, bits_dev, ntiles_dev);
     ILE_LAUNCH_CHECK(ctx);
     return ILE_OK;
 }
 
-// z [d][N] in the caller's order; key / perm = the sorted keys of sp_key_kernel and the sort permutation; uk = its u_k [N][4]
-int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int n_min, int cell_bits, const unsigned long long* key, const double* z, const double* uk,
+// key / perm = the sorted keys of sp_key_kernel and the sort permutation; rec = its sample records [N][SP_REC] (caller's order)
+int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int n_min, int cell_bits, const unsigned long long* key, const double* rec,
                      const int* perm, double* lnL, double* ln_prior, int* tstart, SpTile* tiles, int* ntiles_dev) {
     const int max_tiles = ile_split_max_tiles(N, cell_bits, P.K);
     int* runs = tstart + max_tiles;                     // run starts; their count sits behind the tile count
@@ -862,7 +883,7 @@ int ile_launch_split(ile_ctx* ctx, const LnlParams& P, int N, int n_min, int cel
     sp_tile_info_kernel<<<(max_tiles * 32 + 255) / 256, 256, 0, ctx->stream>>>(P, N, n_min, cell_bits, key, tstart, ntiles_dev, tiles);
     ILE_LAUNCH_CHECK(ctx);
     const bool tb = P.use_table != 0;
-#define SP_LAUNCH(K_, T_) launch_split_t<K_, T_>(ctx, P, N, z, uk, perm, lnL, ln_prior, tiles, ntiles_dev)
+#define SP_LAUNCH(K_, T_) launch_split_t<K_, T_>(ctx, P, N, rec, perm, lnL, ln_prior, tiles, ntiles_dev)
     if (P.K == 3) return tb ? SP_LAUNCH(3, true) : SP_LAUNCH(3, false);
     if (P.K == 2) return tb ? SP_LAUNCH(2, true) : SP_LAUNCH(2, false);
     return tb ? SP_LAUNCH(1, true) : SP_LAUNCH(1, false);
