@@ -321,11 +321,13 @@ int integ_launch_draw(ile_integrator* it, int N, unsigned int g, double* z, doub
     alloc_kernel<<<1, 32, 0, ctx->stream>>>(it->I, (long long)N, g);
     ILE_LAUNCH_CHECK(ctx);
     const size_t smem = draw_smem_bytes(it->I);
-    const int grid = (int)std::min<long long>(((long long)N + 127) / 128, (long long)ctx->sm_count * 32);
+    int grid = (int)std::min<long long>(((long long)N + 127) / 128, (long long)ctx->sm_count * 32), per_sm = 1;
     switch (it->I.d) {
 #define DRAW_CASE(D_)                                                                                                  \
     case D_:                                                                                                           \
         ILE_CUDA(ctx, cudaFuncSetAttribute(draw_kernel<D_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        ILE_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, draw_kernel<D_>, 128, smem));             \
+        grid = (int)std::min<long long>(grid, (long long)std::max(1, per_sm) * ctx->sm_count * 2);   /* two full waves */ \
         draw_kernel<D_><<<grid, 128, smem, ctx->stream>>>(it->I, N, g, z, ln_ps);                                      \
         break;
         DRAW_CASE(1) DRAW_CASE(2) DRAW_CASE(3) DRAW_CASE(4) DRAW_CASE(5) DRAW_CASE(6) DRAW_CASE(7) DRAW_CASE(8)

@@ -7,6 +7,7 @@
 // Every decision (N_min, n_bins, frozen members, "nothing to train on") is taken on the device;
 // the kernels that follow read it from UpdScratch, so an iteration needs no host round-trip.
 #include "integ.cuh"
+#include <algorithm>
 #include "radix_sort.cuh"
 
 enum { MASK_BOX = 1, MASK_LNPS = 2 };
@@ -846,17 +847,20 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
             mask_max_kernel<<<grid, 256, 0, st>>>(I, N, z, lnw, nullptr, MASK_BOX, it->us);
             ILE_LAUNCH_CHECK(ctx);
             const size_t em_smem = ((size_t)GMS_DOUBLES + 256 * (17 + 10) + (size_t)I.n_gmm * 9 + 16) * sizeof(double);
+            int per_sm = 1, em_blocks = it->gmm_blocks;
             switch (I.d) {
 #define GMM_CASE(D)                                                                                                        \
     case D:                                                                                                                \
         ILE_CUDA(ctx, cudaFuncSetAttribute(gmm_em_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)em_smem)); \
-        gmm_em_kernel<D><<<it->gmm_blocks, 256, em_smem, st>>>(I, a, N, z, lnw, it->us, it->gmm_part);                     \
+        ILE_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gmm_em_kernel<D>, 256, em_smem));             \
+        em_blocks = std::max(1, std::min(it->gmm_blocks, per_sm * ctx->sm_count));        /* one full wave, grid-stride */ \
+        gmm_em_kernel<D><<<em_blocks, 256, em_smem, st>>>(I, a, N, z, lnw, it->us, it->gmm_part);                          \
         break;
                 GMM_CASE(1) GMM_CASE(2) GMM_CASE(3) GMM_CASE(4) GMM_CASE(5) GMM_CASE(6) GMM_CASE(7) GMM_CASE(8)
 #undef GMM_CASE
             }
             ILE_LAUNCH_CHECK(ctx);
-            gmm_finish_kernel<<<1, 256, 0, st>>>(I, a, it->us, it->gmm_part, it->gmm_blocks);
+            gmm_finish_kernel<<<1, 256, 0, st>>>(I, a, it->us, it->gmm_part, em_blocks);
             ILE_LAUNCH_CHECK(ctx);
             return ILE_OK;
         }
