@@ -208,7 +208,8 @@ int ile_reduce(ile_ctx *ctx, int N, const double *lnw, ile_result *out_dev);
  * out_dev are device pointers owned by the caller, as for ile_reduce; the work is queued on the context's stream.  All
  * calls on a device share the array: calls that overlap on the GPU (two contexts, two streams) race; calls on one stream
  * are ordered and safe.  Nothing in the array has to start at zero: a call reads only what it wrote.  Results are
- * bit-identical to ile_reduce's (same kernels, same grid). */
+ * bit-identical to ile_reduce's (same kernels, same grid).  The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress, no allocation) and caches it per process: make that first call from one host thread. */
 #define ILE_REDUCE_NOALLOC_MAX_N (1 << 24)
 int ile_reduce_noalloc(ile_ctx *ctx, int N, const double *lnw, ile_result *out_dev);
 
