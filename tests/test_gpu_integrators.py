@@ -159,11 +159,13 @@ def test_av_member_update_with_nonuniform_ps(env):
         assert np.array_equal(st["keys"], o.keys)
 
 
-def test_gmm_parity(env):
+# (5, 8): config 5's member; (6, 16): the most moments per component the tests' box allows (448 sums: every thread of the EM
+# kernel carries two); (2, 3): 18 sums, fourteen slices of a round per sum
+@pytest.mark.parametrize("d,n_gmm,N", [(5, 8, 30011), (6, 16, 20003), (2, 3, 7001)])
+def test_gmm_parity(env, d, n_gmm, N):
     torch, ile, _ = env
-    N, d = 30011, 5
-    g = _make(ile, "GMM", d, N, n_gmm=8)
-    o = _oracle("GMM", d, n_gmm=8)
+    g = _make(ile, "GMM", d, N, n_gmm=n_gmm)
+    o = _oracle("GMM", d, n_gmm=n_gmm)
     lo, hi = LO6[:d], HI6[:d]
     st = g.get_state()
     assert np.array_equal(st["mu"], o.mu) and np.array_equal(st["L"], o.L)      # seeded initial state
