@@ -52,6 +52,7 @@
 #define SP_THREADS (SP_MATH + 32)
 #define SP_UVMAX (300 * 3 * 2)
 #define SP_MAGIC 6755399441055744.0   // 1.5 * 2^52
+#define SP_HOT 32               // distance table: first cells of a sample's row pair kept (blended over B) in shared memory
 
 struct SpTile {
     int start, cnt;           // sorted positions [start, start + cnt)
@@ -670,6 +671,13 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
             // per-sample constants of the time marginalisation
             double init = -(x * x * Bq), tb_f = 0.0;
             const double* tb_row = nullptr;
+            // the sample's hot part of the table: R[q] = T(A_q, B) for the first nhot nodes q of its row pair, blended over B
+            // once per sample (the B fraction is a constant of the sample), in the columns of sm.Y (idle from here to the
+            // next tile's harmonics; column i belongs to the four threads of sample i).  A_j is noise outside the few bins
+            // around the arrival time, so most lookups fall below node nhot - 1 and take two shared-memory loads instead of
+            // a 32-byte gather whose L1 misses stall the whole batch for an L2 round trip.
+            double* const hot = reinterpret_cast<double*>(&sm.Y[0][0]) + i;
+            const int nhot = min(SP_HOT, P.nA - 1);
             if (TABLE) {
                 double b = (Bq - P.B_lo) / (P.B_hi - P.B_lo) * (double)(P.nB - 1);
                 b = fmin(fmax(b, 0.0), (double)(P.nB - 1));
@@ -677,6 +685,16 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                 tb_f = b - ib;
                 tb_row = P.lnT4 + (size_t)ib * (P.nA - 1) * 4;
                 init = 0.0;
+                double T0[SP_HOT / SP_G], T1[SP_HOT / SP_G];                                      // T[ib][q], T[ib + 1][q]: all loads in flight together
+#pragma unroll
+                for (int qq = 0; qq < SP_HOT / SP_G; qq++) {
+                    const int q = min(g + SP_G * qq, nhot - 1);
+                    T0[qq] = __ldg(tb_row + 4 * q);
+                    T1[qq] = __ldg(tb_row + 4 * q + 2);
+                }
+#pragma unroll
+                for (int qq = 0; qq < SP_HOT / SP_G; qq++)
+                    if (g + SP_G * qq < nhot) hot[(g + SP_G * qq) * SP_TS] = fma(tb_f, T1[qq] - T0[qq], T0[qq]);
             }
             qbar();                                              // partial sums read by everybody before the ring is initialised
 #pragma unroll 4
@@ -705,19 +723,50 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                     if (FULL || j0 + SP_G * e < jend) *pr[e] = init;
                 bool need = false;
                 double dl[4];
+                if (TABLE) {
+                    // node index and fraction of the four rows; a < 0 is clamped on the high word (to a denormal above 0:
+                    // node 0, fraction 0 to rounding), the conversion saturates
+                    int ia[4];
+                    double fa[4];
+                    bool cold = false;
+#pragma unroll
+                    for (int e = 0; e < 4; e++) {
+                        double a = fma(v[e], tabA_s, tabA_o);
+                        a = __hiloint2double(max(__double2hiint(a), 0), __double2loint(a));
+                        ia[e] = min(__double2int_rz(a), P.nA - 2);
+                        fa[e] = a - (double)ia[e];
+                        cold = cold || ia[e] >= nhot - 1;
+                    }
+                    if (!__any_sync(0xffffffffu, cold)) {
+                        // every lane's four rows below node nhot - 1: the sample's blended row in shared memory
+                        double R0[4], R1[4];
+#pragma unroll
+                        for (int e = 0; e < 4; e++) {
+                            R0[e] = hot[ia[e] * SP_TS];
+                            R1[e] = hot[(ia[e] + 1) * SP_TS];
+                        }
+#pragma unroll
+                        for (int e = 0; e < 4; e++) v[e] = fma(fa[e], R1[e] - R0[e], R0[e]);
+                    } else {
+                        double2 lo2[4], hi2[4];
+#pragma unroll
+                        for (int e = 0; e < 4; e++) {
+                            const double2* T0 = reinterpret_cast<const double2*>(tb_row + 4 * ia[e]);    // one 32-byte cell
+                            lo2[e] = __ldg(T0);
+                            hi2[e] = __ldg(T0 + 1);
+                        }
+#pragma unroll
+                        for (int e = 0; e < 4; e++) {
+                            // beyond the last node (ia = nA - 2, fraction above 1): clamped to the edge
+                            const double f = __double2hiint(fa[e]) >= 0x3ff00000 ? 1.0 : fa[e];
+                            const double t0 = fma(f, lo2[e].y - lo2[e].x, lo2[e].x), t1 = fma(f, hi2[e].y - hi2[e].x, hi2[e].x);
+                            v[e] = fma(tb_f, t1 - t0, t0);
+                        }
+                    }
+                }
 #pragma unroll
                 for (int e = 0; e < 4; e++) {
-                    double A = v[e];
-                    if (TABLE) {
-                        double a = fma(A, tabA_s, tabA_o);
-                        a = fmin(fmax(a, 0.0), (double)(P.nA - 1));
-                        const int ia = min((int)a, P.nA - 2);
-                        const double fa = a - (double)ia;
-                        const double2* T0 = reinterpret_cast<const double2*>(tb_row + 4 * ia);       // one 32-byte cell
-                        const double2 lo2 = __ldg(T0), hi2 = __ldg(T0 + 1);
-                        const double t0 = fma(fa, lo2.y - lo2.x, lo2.x), t1 = fma(fa, hi2.y - hi2.x, hi2.x);
-                        A = fma(tb_f, t1 - t0, t0);
-                    }
+                    const double A = v[e];
                     v[e] = (FULL || j0 + SP_G * e < jend) ? A : neg_inf();
                     dl[e] = v[e] - run_m;
                     need = need || (__double2hiint(dl[e]) >= SP_RAISE_HI);   // dl >= 512 (or NaN): test on the high word

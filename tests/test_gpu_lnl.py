@@ -127,6 +127,37 @@ def test_lnL_nearest_bin_and_table(torch_mod):
         assert np.all(np.abs(got0 - ref0) <= _tol(ref0)), (variant, np.abs(got0 - ref0).max())
 
 
+@pytest.mark.parametrize("nA,nB,a_lo,a_hi", [(256, 256, 0.05, 0.2), (40, 7, -0.1, 0.5), (5, 3, 0.0, 1.3), (2, 2, 0.0, 0.1), (33, 2, 0.0, 0.02)])
+def test_lnL_table_edges(torch_mod, nA, nB, a_lo, a_hi):
+    """Distance tables whose A range is left on both sides (lookups clamped to the edges, G28) and whose rows are shorter
+    than, equal to and longer than the part of a row the fused kernel keeps in shared memory; B range narrower than the
+    samples' B."""
+    from oracle import likelihood as lk
+    from synth.workloads import make_distance_table, D0_MPC
+    torch = torch_mod
+    prob = make_problem(5, N=1)
+    x0 = prob.D_ref / D0_MPC
+    A_pk, B_pk = prob.rho2 / x0, prob.rho2 / (2.0 * x0 * x0)
+    table = make_distance_table(prob.D_ref, prob.D_min, prob.D_max, a_lo * A_pk, a_hi * A_pk, 0.4 * B_pk, 0.9 * B_pk, nA=nA, nB=nB, nodes=257)
+    ile = _ile(prob)
+    ile.load_distance_table(table)
+    N = 1301
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=21)
+    # a few samples at the injected parameters' neighbourhood, so that rows near the arrival time reach the top of the table
+    th = prob.inj[0]["theta0"]
+    inj = np.array([th["ra"], math.sin(th["dec"]), th["psi"], th["phi_ref"], math.cos(th["incl"])])[: z.shape[0]]
+    z[:, :64] = inj[:, None] + 1e-3 * (z[:, :64] - inj[:, None])
+    z = np.minimum(np.maximum(z, np.asarray(prob.lo)[:, None]), np.nextafter(np.asarray(prob.hi), -np.inf)[:, None])
+    args = (prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+            prob.t_Q0, prob.t_lo, prob.dt, prob.N_t)
+    ref = lk.lnL_z(*args, z, table=table)
+    zd = _dev(torch, z)
+    for variant in FUSED:
+        ile.set_lnL_variant(variant)
+        got = ile.lnL_z(0, zd).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
+
+
 def test_reduce_parity(torch_mod):
     from oracle.reduce import reduce_lnw
     torch = torch_mod
