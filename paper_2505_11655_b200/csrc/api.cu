@@ -495,6 +495,18 @@ int ile_fill_params(ile_ctx* ctx, int p, int d, LnlParams* L) {
         L->NG8 = ile_split_ng8(ctx->N_Q);
         L->Qs = ctx->d_Qs + (size_t)p * K * L->NG8 * 2432;
         for (int k = 0; k < K; k++) L->qeb[k] = ctx->h_qeb[p * K + k];
+        // rows of the triangle (row a has M - a pairs) to the four thread groups of a sample, longest row first to the
+        // group with the least work so far; groups 0..K-1 start with the digit cutting of one detector, which costs about
+        // as much as `head` pairs (measured: the kernel time is flat around these values)
+        const int head = K == 1 ? 36 : K == 2 ? 26 : 20;
+        int load[4] = {head, K > 1 ? head : 0, K > 2 ? head : 0, 0};
+        for (int a = 0; a < M; a++) {
+            int gmin = 0;
+            for (int g = 1; g < 4; g++)
+                if (load[g] < load[gmin]) gmin = g;
+            L->tri_group[a] = (unsigned char)gmin;
+            load[gmin] += M - a;
+        }
     }
     return ILE_OK;
 }

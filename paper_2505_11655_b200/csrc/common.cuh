@@ -64,6 +64,9 @@ struct LnlParams {
     const unsigned char* Qs;
     int NG8;
     int qeb[ILE_MAX_K];
+    // step 4 in the tcgen05 kernel: the thread group (0..3) of a sample that walks row a of the upper triangle.  Groups
+    // 0..K-1 also cut one detector's coefficients into digits, so they get fewer pairs (ile_fill_params balances the two)
+    unsigned char tri_group[24];
 };
 
 struct ile_ctx {

@@ -42,7 +42,7 @@ struct UpdScratch {           // per-update scalars
     unsigned long long n_valid;
     unsigned long long total_q;
     int abort;                    // nothing to train on: leave the state unchanged
-    int pad;
+    unsigned int ticket;          // blocks of a select pass that have added their histogram (the last one fixes the digit)
     SelPath path[2];              // 0: weight-mass target (P_thr), 1: count target (N_min*)
     int use_path;                 // threshold path chosen: 0, 1, or 2 = keep every valid sample
     int n_bits;                   // significant bits of the new cell keys

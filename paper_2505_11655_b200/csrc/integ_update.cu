@@ -208,11 +208,51 @@ __device__ __forceinline__ int sel_digit(int nd, unsigned long long k, unsigned 
     return nd < 8 ? (int)((k >> (56 - 8 * nd)) & 0xffull) : (int)((idx >> (24 - 8 * (nd - 8))) & 0xffu);
 }
 
+// Fix the next digit of each live path and clear the histogram for the next pass: one block of 256 threads, thread b = bin b.
+// The digit is the first bin at which the running metric reaches the target; the running sums are exact integers, so the
+// block scan gives what a bin-by-bin walk gives.
+__device__ void sel_pick_block(UpdScratch* us, unsigned long long* hist) {
+    __shared__ unsigned long long wtot[2][8];
+    __shared__ int dg_sh;
+    const int b = threadIdx.x, lane = b & 31, wp = b >> 5;
+    for (int p = 0; p < 2; p++) {
+        SelPath P = us->path[p];
+        if (P.done || P.fail) continue;                      // the same for every thread
+        const unsigned long long cnt = __ldcg(hist + (p * 2 + 0) * 256 + b), met = __ldcg(hist + (p * 2 + 1) * 256 + b);
+        unsigned long long sm = met, sc = cnt;                // inclusive sums over the warp's bins
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long tm = __shfl_up_sync(0xffffffffu, sm, o), tc = __shfl_up_sync(0xffffffffu, sc, o);
+            if (lane >= o) { sm += tm; sc += tc; }
+        }
+        if (lane == 31) { wtot[0][wp] = sm; wtot[1][wp] = sc; }
+        if (b == 0) dg_sh = 256;
+        __syncthreads();
+        unsigned long long om = P.cum_metric, oc = P.cum_count;
+        for (int w2 = 0; w2 < wp; w2++) { om += wtot[0][w2]; oc += wtot[1][w2]; }
+        if (om + sm >= P.target) atomicMin(&dg_sh, b);
+        __syncthreads();
+        const int dg = dg_sh;
+        if (dg == 256) {
+            if (b == 0) { P.fail = 1; us->path[p] = P; }
+        } else if (b == dg) {
+            P.cum_metric = om + sm - met;
+            P.cum_count = oc + sc - cnt;
+            if (P.ndig < 8) P.prefix_key |= (unsigned long long)dg << (56 - 8 * P.ndig);
+            else P.prefix_idx |= (unsigned int)dg << (24 - 8 * (P.ndig - 8));
+            P.ndig++;
+            if (cnt == 1 || P.ndig == AV_SEL_PASSES) P.done = 1;
+            us->path[p] = P;
+        }
+        __syncthreads();
+    }
+    for (int q = b; q < 1024; q += 256) hist[q] = 0ull;
+}
+
 // histogram of the next digit among the elements matching each path's prefix
 // hist layout: [path][0 = count, 1 = metric][256]
 __global__ void __launch_bounds__(256) av_sel_hist_kernel(int N, const unsigned long long* __restrict__ skey,
-                                                          const unsigned long long* __restrict__ qv, const UpdScratch* __restrict__ us,
-                                                          unsigned long long* __restrict__ hist) {
+                                                          const unsigned long long* __restrict__ qv, UpdScratch* us,
+                                                          unsigned long long* hist) {
     if (us->abort) return;
     __shared__ unsigned long long sh[2][2][256];
     __shared__ SelPath P[2];
@@ -252,39 +292,16 @@ __global__ void __launch_bounds__(256) av_sel_hist_kernel(int N, const unsigned 
         const unsigned long long v = (&sh[0][0][0])[q];
         if (v) atomicAdd(&hist[q], v);
     }
-}
-
-// fix the next digit of each live path; clears the histogram for the next pass
-__global__ void av_sel_pick_kernel(UpdScratch* us, unsigned long long* hist) {
-    if (us->abort) return;
-    const int p = threadIdx.x;
-    if (p < 2) {
-        SelPath P = us->path[p];
-        if (!P.done && !P.fail) {
-            const unsigned long long* cnt = hist + (p * 2 + 0) * 256;
-            const unsigned long long* met = hist + (p * 2 + 1) * 256;
-            unsigned long long run = P.cum_metric, rc = P.cum_count;
-            int dg = -1;
-            for (int b = 0; b < 256; b++) {
-                if (run + met[b] >= P.target) { dg = b; break; }
-                run += met[b];
-                rc += cnt[b];
-            }
-            if (dg < 0) {
-                P.fail = 1;
-            } else {
-                P.cum_metric = run;
-                P.cum_count = rc;
-                if (P.ndig < 8) P.prefix_key |= (unsigned long long)dg << (56 - 8 * P.ndig);
-                else P.prefix_idx |= (unsigned int)dg << (24 - 8 * (P.ndig - 8));
-                P.ndig++;
-                if (cnt[dg] == 1 || P.ndig == AV_SEL_PASSES) P.done = 1;
-            }
-            us->path[p] = P;
-        }
-    }
+    // the last block to get here sees every block's sums and fixes the digit (no second launch per pass)
+    __shared__ bool last;
+    __threadfence();
     __syncthreads();
-    for (int q = threadIdx.x; q < 1024; q += blockDim.x) hist[q] = 0ull;
+    if (threadIdx.x == 0) last = atomicAdd(&us->ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    sel_pick_block(us, hist);
+    if (threadIdx.x == 0) us->ticket = 0u;
 }
 
 __device__ __forceinline__ bool av_kept(const UpdScratch& U, const SelPath& P, unsigned long long k, unsigned int idx) {
@@ -813,8 +830,6 @@ static int member_update(ile_integrator* it, int a, int N, const double* z, cons
             ILE_LAUNCH_CHECK(ctx);
             for (int p = 0; p < AV_SEL_PASSES; p++) {
                 av_sel_hist_kernel<<<grid, 256, 0, st>>>(N, it->skey, it->q, it->us, it->sel_hist);
-                ILE_LAUNCH_CHECK(ctx);
-                av_sel_pick_kernel<<<1, 256, 0, st>>>(it->us, it->sel_hist);
                 ILE_LAUNCH_CHECK(ctx);
             }
             av_decide_kernel<<<1, 32, 0, st>>>(I, N, it->us);

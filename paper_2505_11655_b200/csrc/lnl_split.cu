@@ -608,7 +608,8 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
             tc_fence_before();
             mbar_arrive(&sm.a_full);
             // ---- step 4: B = 1/4 sum_k [ |F_k|^2 Re(y^H U_k y) + Re(F_k^2 y^T V_k y) ] over the upper triangle (Eq. 17-18).
-            //      Group g walks the rows a with a % 8 == g or 7 - g (equal pair counts); the partial sums meet in the ring's memory.
+            //      Group g walks the rows P.tri_group gives it (fewer pairs for the groups that cut digits above); the partial
+            //      sums meet in the ring's memory.
             double* const qpart = &sm.ring[0][0];                // [SP_G][3 K][128], the ring is idle until the first work item
             {
                 double uu[K], vr[K], vi[K];
@@ -627,7 +628,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                     }
                 };
                 for (int a = 0; a < M; a++) {
-                    if ((a & 7) != g && (a & 7) != 7 - g) continue;
+                    if (P.tri_group[a] != g) continue;
                     const double2 ya = sm.Y[a][i];
                     const double2* uv = sm.uv + (size_t)(a * M - (a * (a - 1)) / 2) * 2 * K;
                     int b = a;
