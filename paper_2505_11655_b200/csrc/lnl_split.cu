@@ -52,7 +52,7 @@
 #define SP_THREADS (SP_MATH + 32)
 #define SP_UVMAX (300 * 3 * 2)
 #define SP_MAGIC 6755399441055744.0   // 1.5 * 2^52
-#define SP_HOT 32               // distance table: first cells of a sample's row pair kept (blended over B) in shared memory
+#define SP_HOT 24               // distance table: first nodes of a sample's row pair kept (blended over B) in shared memory, one per row of sm.Y
 
 struct SpTile {
     int start, cnt;           // sorted positions [start, start + cnt)
@@ -672,13 +672,14 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
             // per-sample constants of the time marginalisation
             double init = -(x * x * Bq), tb_f = 0.0;
             const double* tb_row = nullptr;
-            // the sample's hot part of the table: R[q] = T(A_q, B) for the first nhot nodes q of its row pair, blended over B
-            // once per sample (the B fraction is a constant of the sample), in the columns of sm.Y (idle from here to the
-            // next tile's harmonics; column i belongs to the four threads of sample i).  A_j is noise outside the few bins
-            // around the arrival time, so most lookups fall below node nhot - 1 and take two shared-memory loads instead of
-            // a 32-byte gather whose L1 misses stall the whole batch for an L2 round trip.
-            double* const hot = reinterpret_cast<double*>(&sm.Y[0][0]) + i;
-            const int nhot = min(SP_HOT, P.nA - 1);
+            // the sample's hot part of the table: for the first nhot nodes q of its row pair, R_q = T(A_q, B) blended over B once
+            // per sample (the B fraction is a constant of the sample) and the step to the next node, in sm.Y[q][i] - idle from
+            // here to the next tile's harmonics, and entry [q][i] is touched by the four threads of sample i only (the quartets
+            // of a tile are not in step with each other).  A_j is noise outside the few bins around the arrival time, so most
+            // lookups fall below node nhot and take one shared-memory load instead of a 32-byte gather whose L1 misses stall
+            // the whole batch for an L2 round trip.
+            double2* const hot = &sm.Y[0][i];
+            const int nhot = min(SP_HOT, P.nA - 2);              // not the last cell: a lookup there may lie past the table's edge (clamped in the other branch)
             if (TABLE) {
                 double b = (Bq - P.B_lo) / (P.B_hi - P.B_lo) * (double)(P.nB - 1);
                 b = fmin(fmax(b, 0.0), (double)(P.nB - 1));
@@ -686,16 +687,18 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                 tb_f = b - ib;
                 tb_row = P.lnT4 + (size_t)ib * (P.nA - 1) * 4;
                 init = 0.0;
-                double T0[SP_HOT / SP_G], T1[SP_HOT / SP_G];                                      // T[ib][q], T[ib + 1][q]: all loads in flight together
+                double2 lo2[SP_HOT / SP_G], hi2[SP_HOT / SP_G];                                   // cell q = (T[ib][q], T[ib][q+1]), (T[ib+1][q], T[ib+1][q+1]): all loads in flight together
 #pragma unroll
                 for (int qq = 0; qq < SP_HOT / SP_G; qq++) {
-                    const int q = min(g + SP_G * qq, nhot - 1);
-                    T0[qq] = __ldg(tb_row + 4 * q);
-                    T1[qq] = __ldg(tb_row + 4 * q + 2);
+                    const double2* c = reinterpret_cast<const double2*>(tb_row + 4 * max(min(g + SP_G * qq, nhot - 1), 0));
+                    lo2[qq] = __ldg(c);
+                    hi2[qq] = __ldg(c + 1);
                 }
 #pragma unroll
-                for (int qq = 0; qq < SP_HOT / SP_G; qq++)
-                    if (g + SP_G * qq < nhot) hot[(g + SP_G * qq) * SP_TS] = fma(tb_f, T1[qq] - T0[qq], T0[qq]);
+                for (int qq = 0; qq < SP_HOT / SP_G; qq++) {
+                    const double R0 = fma(tb_f, hi2[qq].x - lo2[qq].x, lo2[qq].x), R1 = fma(tb_f, hi2[qq].y - lo2[qq].y, lo2[qq].y);
+                    if (g + SP_G * qq < nhot) hot[(g + SP_G * qq) * SP_TS] = make_double2(R0, R1 - R0);
+                }
             }
             qbar();                                              // partial sums read by everybody before the ring is initialised
 #pragma unroll 4
@@ -736,18 +739,15 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                         a = __hiloint2double(max(__double2hiint(a), 0), __double2loint(a));
                         ia[e] = min(__double2int_rz(a), P.nA - 2);
                         fa[e] = a - (double)ia[e];
-                        cold = cold || ia[e] >= nhot - 1;
+                        cold = cold || ia[e] >= nhot;
                     }
                     if (!__any_sync(0xffffffffu, cold)) {
-                        // every lane's four rows below node nhot - 1: the sample's blended row in shared memory
-                        double R0[4], R1[4];
+                        // every lane's four rows below node nhot: the sample's blended row in shared memory
+                        double2 R[4];
 #pragma unroll
-                        for (int e = 0; e < 4; e++) {
-                            R0[e] = hot[ia[e] * SP_TS];
-                            R1[e] = hot[(ia[e] + 1) * SP_TS];
-                        }
+                        for (int e = 0; e < 4; e++) R[e] = hot[ia[e] * SP_TS];
 #pragma unroll
-                        for (int e = 0; e < 4; e++) v[e] = fma(fa[e], R1[e] - R0[e], R0[e]);
+                        for (int e = 0; e < 4; e++) v[e] = fma(fa[e], R[e].y, R[e].x);
                     } else {
                         double2 lo2[4], hi2[4];
 #pragma unroll

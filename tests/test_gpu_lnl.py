@@ -158,6 +158,35 @@ def test_lnL_table_edges(torch_mod, nA, nB, a_lo, a_hi):
         assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
 
 
+@pytest.mark.parametrize("cfg", [1, 2, 4, 5])
+def test_lnL_repeatable(torch_mod, cfg):
+    """The fused kernels on the same batch again and again: bit-identical results.  Nothing in them depends on the order in
+    which warps run, so any difference is a race (the quartets of a tile are not in step with each other, and shared-memory
+    arrays are reused between the phases); the first call is compared with the oracle on a subset."""
+    from oracle import likelihood as lk
+    torch = torch_mod
+    prob = make_problem(cfg, N=1) if cfg in (4, 5) else make_problem(cfg)
+    ile = _ile(prob)
+    N = 60013
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=101 + cfg)
+    th = prob.inj[0]["theta0"]
+    inj = np.array([th["ra"], math.sin(th["dec"]), th["psi"], th["phi_ref"], math.cos(th["incl"]), th["dist"]])[: z.shape[0]]
+    half = N // 2                                                     # half of the batch around the injected parameters
+    z[:, :half] = inj[:, None] + 0.05 * (z[:, :half] - inj[:, None])
+    z = np.minimum(np.maximum(z, np.asarray(prob.lo)[:, None]), np.nextafter(np.asarray(prob.hi), -np.inf)[:, None])
+    zd = _dev(torch, z)
+    for variant in FUSED:
+        ile.set_lnL_variant(variant)
+        first = ile.lnL_z(0, zd).cpu().numpy()
+        for rep in range(6):
+            again = ile.lnL_z(0, zd).cpu().numpy()
+            assert np.array_equal(first, again, equal_nan=True), (variant, rep, np.nanmax(np.abs(first - again)))
+        sub = np.r_[0:96, half - 48:half + 48, N - 96:N]
+        ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                       prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z[:, sub], table=prob.table)
+        assert np.all(np.abs(first[sub] - ref) <= _tol(ref)), (variant, np.abs(first[sub] - ref).max())
+
+
 def test_reduce_parity(torch_mod):
     from oracle.reduce import reduce_lnw
     torch = torch_mod
