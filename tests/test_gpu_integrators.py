@@ -355,6 +355,46 @@ def test_step_parity_with_oracle(env, cfg, N, n_iter):
         assert abs(res["W"][:3].sum() - 1.0) < 1e-12
 
 
+def _assert_same_state(a, b, where):
+    if isinstance(a, dict):
+        assert a.keys() == b.keys(), where
+        for k in a:
+            _assert_same_state(a[k], b[k], where + (k,))
+    elif isinstance(a, (list, tuple)):
+        assert len(a) == len(b), where
+        for q, (x, y) in enumerate(zip(a, b)):
+            _assert_same_state(x, y, where + (q,))
+    elif isinstance(a, np.ndarray):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8)), where
+    else:
+        assert a == b or (a != a and b != b), where
+
+
+@pytest.mark.parametrize("cfg,N,n_iter", [(2, 40000, 4), (3, 50000, 5), (5, 30000, 5)])
+def test_run_repeatable(env, cfg, N, n_iter):
+    """ile_integrator_run from the reset state, again and again: every ile_result field and the final sampler state bit for
+    bit the same.  The update kernels take their decisions in integers (histograms, threshold select, cell keys) and fix the
+    order of every floating-point sum, so a difference is a race (e.g. in the select pass whose last block fixes the digit)."""
+    torch, _, _ = env
+    from paper_2505_11655_b200 import Ile, Integrator
+    prob = make_problem(cfg, N=N, n_iter=n_iter)
+    ile = Ile(0)
+    ile.load_problem(prob)
+    g = Integrator.from_problem(ile, prob, max_batch=N)
+    first, first_state = None, None
+    for rep in range(4):
+        g.reset()
+        res = g.run(0, 1, n_iter, N)
+        torch.cuda.synchronize()
+        raw = res.cpu().numpy().copy().view(np.uint8)
+        st = g.get_state()
+        if first is None:
+            first, first_state = raw, st
+            continue
+        assert np.array_equal(first, raw), (cfg, rep)
+        _assert_same_state(st, first_state, (cfg, rep))
+
+
 def test_run_matches_steps_and_resets_between_points(env):
     torch, _, _ = env
     from paper_2505_11655_b200 import Ile, Integrator, result_from_device
