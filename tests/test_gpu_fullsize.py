@@ -82,6 +82,10 @@ def test_full_batch_sampled_parity(cfg, P, n_iter):
             assert abs(res["n_ess"] - red["n_ess"]) <= 1e-7 * max(1.0, red["n_ess"])
             assert 1.0 - 1e-9 <= res["n_eff"] <= res["n_ess"] * (1 + 1e-12) <= N * (1 + 1e-12)
             assert res["n_samples"] == N and res["cum_n_samples"] == N * (it + 1)
+            # the whole batch once more through the public entry point: the fused kernel's result does not depend on how
+            # its warps interleave, so every one of the N values must come out bit for bit the same (a race would show)
+            again = ile.lnL_z(p, z)
+            assert torch.equal(again.view(torch.int64), lnL.view(torch.int64))
     if prob.kind == "AV":
         assert res["n_bins"] > 1 and 1 <= res["n_cells"] <= N and res["N_min"] >= 4096
         keys = g.get_state()["keys"]
