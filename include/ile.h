@@ -144,7 +144,8 @@ int ile_set_network(ile_ctx *ctx, int K, const double *D /*[K][3][3]*/, const do
 int ile_set_modes(ile_ctx *ctx, int M, const int *ell, const int *m);
 /* PAPER.md:78-87 (Eq. 6a-c): Q_{k,lm}(t) on N_Q bins at rate fs starting at t_Q0 (geocentric
  * seconds), U, V mode-mode matrices, for P intrinsic points; D_ref in the distance unit of the
- * prior.  U = U^H and V = V^T are verified to 1e-12 relative (Eq. 17-18) -> ILE_EINVAL.
+ * prior.  U = U^H and V = V^T are verified to 1e-12 relative (Eq. 17-18) -> ILE_EINVAL.  At most 22 modes
+ * (l <= 4 gives 21; the packed Q layouts hold 24 complex columns, two of them padding) -> ILE_EINVAL.
  * src_is_device != 0: Q/U/V are device pointers (copied device-to-device). */
 int ile_load_quv(ile_ctx *ctx, int P, int N_Q, double fs, double t_Q0,
                  const double *Q /*[P][K][M][N_Q][2]*/, const double *U /*[P][K][M][M][2]*/,
@@ -157,7 +158,7 @@ int ile_load_quv(ile_ctx *ctx, int P, int N_Q, double fs, double t_Q0,
  * result like ile_load_quv (synchronises).  The inputs stay the caller's; scratch is one grow-only
  * device allocation owned by the context (freed by ile_destroy).  Errors: ILE_ESTATE before
  * set_network/set_modes, ILE_EINVAL for bad sizes, N_Q > N_f, t_Q0 off the sample grid or more
- * than 24 modes (the resident Q/U/V stay as they were), ILE_ENOMEM (of the scratch: the resident set
+ * than 22 modes (the resident Q/U/V stay as they were), ILE_ENOMEM (of the scratch: the resident set
  * stays; of the result arrays: nothing is resident afterwards), ILE_ECUDA.  U and V come out Hermitian and
  * symmetric by construction (Eq. 17-18), so the install skips ile_load_quv's check.
  * ile_get_quv copies point p back to host arrays in ile_load_quv's layout (any of Q, U, V may be NULL). */

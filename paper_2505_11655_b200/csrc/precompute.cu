@@ -445,7 +445,8 @@ extern "C" int ile_precompute_quv(ile_ctx* ctx, int P, int N_f, double df, doubl
     const long long n0 = llrint(n0d);
     if (fabs(n0d - (double)n0) > 1e-6) return ile_fail(ctx, ILE_EINVAL, "precompute_quv: t_Q0 * fs = %.9g is not an integer", n0d);
     const int K = ctx->K, M = ctx->M, n_pairs = ctx->n_pairs;
-    if (M > 24 || K > 4) return ile_fail(ctx, ILE_EINVAL, "precompute_quv: at most 24 modes and 4 detectors");
+    if (M > ILE_QT_ROW / 2 - 2 || K > 4)                       // the limit of ile_load_quv, which installs the result
+        return ile_fail(ctx, ILE_EINVAL, "precompute_quv: at most %d modes and 4 detectors", ILE_QT_ROW / 2 - 2);
     int Mq = 4, log2Mq = 2;
     while (Mq < N_Q) { Mq <<= 1; log2Mq++; }
     const bool pruned = (N_f & (N_f - 1)) == 0 && Mq <= 2048 && Mq <= N_f;

@@ -304,13 +304,16 @@ def make_problem(cfg: int, P: int | None = None, N: int | None = None, n_iter: i
                    n_iter=n_iter, opts=opts, table=table, inj=inj)
 
 
-def make_custom_problem(K: int, lmax: int, snr: float, seed: int, N_Q: int = 820, N_t: int = 300) -> Problem:
+def make_custom_problem(K: int, lmax: int, snr: float, seed: int, N_Q: int = 820, N_t: int = 300, modes=None) -> Problem:
     """A one-point problem with a detector / mode count outside the five configs (parity of the kernels' other
     shapes).  The template's mode coefficients are seeded random numbers with the usual amplitude law, not a
     physical signal (no injection fixture is needed): Q = q0 A_m(t - tau_k) + coloured noise as in make_q."""
     rng = _rng(SEED_BASE + 900000 + seed)
     D, pos = make_network(K, rng)
     ell, m = make_modes(lmax)
+    if modes is not None:                                   # an explicit (l, m) list instead of all modes up to lmax
+        ell = np.array([lm[0] for lm in modes], dtype=ell.dtype)
+        m = np.array([lm[1] for lm in modes], dtype=m.dtype)
     M = len(ell)
     t_Q0 = -(N_Q // 2) / FS
     U, V, G = make_uv(K, ell, m, rng, profile=0)

@@ -270,6 +270,43 @@ def test_lnL_other_shapes(torch_mod, K, lmax):
         assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
 
 
+_L4 = [(l, mm) for l in (2, 3, 4) for mm in range(-l, l + 1)]
+
+
+@pytest.mark.parametrize("K,modes", [(3, _L4 + [(5, 5)]),                                         # M = 22: the most ile_load_quv takes
+                                     (2, [lm for lm in _L4 if lm[1] != 0]),                       # M = 18: even row lengths in step 4
+                                     (3, [(2, 2), (2, -2), (3, 3), (3, -3), (4, 4), (4, -4), (2, 1)]),   # M = 7
+                                     (1, [(2, 2)])])                                              # one mode
+def test_lnL_mode_lists(torch_mod, K, modes):
+    """Mode sets that are not 'all modes up to l_max': the largest the library takes, an even count, a short odd list and a
+    single mode (step 4's rows are dealt to the thread groups per (M, K); digits are cut in groups of four reals)."""
+    from oracle import likelihood as lk
+    from synth.workloads import make_custom_problem
+    torch = torch_mod
+    prob = make_custom_problem(K=K, lmax=2, snr=30.0, seed=70 + len(modes), modes=modes)
+    ile = _ile(prob)
+    N = 900
+    z = uniform_box_samples(prob.lo, prob.hi, N, seed=11)
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z)
+    for variant in FUSED:
+        ile.set_lnL_variant(variant)
+        got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
+
+
+def test_too_many_modes_rejected(torch_mod):
+    from paper_2505_11655_b200 import Ile
+    from paper_2505_11655_b200.binding import IleError
+    from synth.workloads import make_custom_problem
+    prob = make_custom_problem(K=2, lmax=2, snr=30.0, seed=99, modes=_L4 + [(5, 5), (5, -5)])           # M = 23
+    ile = Ile(0)
+    ile.set_network(prob.D, prob.pos, prob.gmst)
+    ile.set_modes(prob.ell, prob.m)
+    with pytest.raises(IleError, match="at most 22 modes"):
+        ile.load_quv(prob.Q, prob.U, prob.V, prob.fs, prob.t_Q0, prob.D_ref)
+
+
 def test_two_contexts_in_one_process(torch_mod):
     """Two contexts alive at once (different networks, mode sets and time grids), calls interleaved: each answers as it
     does alone.  The kernels' shared-memory opt-in and every other piece of launch state is per call, not per process."""
