@@ -295,6 +295,29 @@ def test_lnL_mode_lists(torch_mod, K, modes):
         assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
 
 
+@pytest.mark.parametrize("K,lmax", [(1, 2), (2, 3), (2, 4)])
+def test_lnL_table_other_shapes(torch_mod, K, lmax):
+    """Distance marginalisation through the table with one and two detectors (the fused kernels are instantiated per detector
+    count and table mode; config 5 covers three detectors only)."""
+    from oracle import likelihood as lk
+    from synth.workloads import make_custom_problem, make_distance_table, D0_MPC
+    torch = torch_mod
+    prob = make_custom_problem(K=K, lmax=lmax, snr=25.0, seed=300 + 10 * K + lmax)
+    x0 = prob.D_ref / D0_MPC
+    A_pk, B_pk = prob.rho2 / x0, prob.rho2 / (2.0 * x0 * x0)
+    table = make_distance_table(prob.D_ref, prob.D_min, prob.D_max, 0.0, 1.3 * A_pk, 0.02 * B_pk, 3.0 * B_pk, nA=96, nB=64, nodes=513)
+    ile = _ile(prob)
+    ile.load_distance_table(table)
+    N = 1100
+    z = uniform_box_samples(prob.lo[:5], prob.hi[:5], N, seed=17)
+    ref = lk.lnL_z(prob.D, prob.pos, prob.gmst, prob.ell, prob.m, prob.Q[0], prob.U[0], prob.V[0], prob.D_ref, prob.fs,
+                   prob.t_Q0, prob.t_lo, prob.dt, prob.N_t, z, table=table)
+    for variant in FUSED:
+        ile.set_lnL_variant(variant)
+        got = ile.lnL_z(0, _dev(torch, z)).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= _tol(ref)), (variant, np.abs(got - ref).max())
+
+
 def test_too_many_modes_rejected(torch_mod):
     from paper_2505_11655_b200 import Ile
     from paper_2505_11655_b200.binding import IleError
