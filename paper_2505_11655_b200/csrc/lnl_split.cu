@@ -794,6 +794,17 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                 run_s += part;
             };
             auto lse_rows = [&](const int jend) {
+                if (TABLE) {
+                    // rows above the kept nodes (around the arrival time): ask for their cells now, so that the batches below
+                    // find them in L1 instead of each waiting an L2 round trip
+                    for (int j = jdone + g; j < jend; j += SP_G) {
+                        const int ia = __double2int_rz(fma(rcol[(j & (SP_RING - 1)) * SP_TS], tabA_s, tabA_o));
+                        if (ia >= nhot) {
+                            unsigned dummy;
+                            asm volatile("ld.global.nc.b32 %0, [%1];" : "=r"(dummy) : "l"(tb_row + 4 * min(ia, P.nA - 2)));
+                        }
+                    }
+                }
                 int j0 = jdone + g;
                 for (; j0 + 3 * SP_G < jend; j0 += 4 * SP_G) lse_batch(j0, jend, std::true_type{});
                 if (j0 < jend) lse_batch(j0, jend, std::false_type{});
