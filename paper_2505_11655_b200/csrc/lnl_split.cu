@@ -276,6 +276,8 @@ struct SplitSmem {
     double xch[2][3][SP_TS];                  // last bin of a chunk, from group 3 to group 0 of the next chunk (slot = chunk parity)
     double lse[SP_G][2][SP_TS];               // partial (reference, sum) of the four threads of a sample
     int eb[3][SP_TS];                         // biased exponent of max |coefficient| per detector
+    double wgt[2][3][SP_TS];                  // interpolation weights of the sample's window per detector (scaled: unit of the integer contraction)
+    int offs[3][SP_TS];                       // first stored bin of the sample's window above the tile's base, per detector
     YlmTable ytab;                            // term table of the harmonics (Eq. 4), copied once per CTA
     uint64_t a_full, d_full, d_empty, b_full[SP_NSTAGE], b_empty[SP_NSTAGE];
     uint32_t tmem_base;
@@ -445,6 +447,8 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
         const int i = 32 * qd + lane;
         const uint32_t tlane = tmem + ((uint32_t)(32 * qd) << 16);
         double* const rcol = &sm.ring[0][i];
+        const double* const fx_col = &sm.lse[0][0][i];           // prologue: rows 0..2 Re F_k, 3..5 Im F_k, 6 x of sample i
+        const double* const u_col = &sm.xch[0][0][i];            // prologue: rows 0..2 u_k
         const double* const etab = &sm.etab[0][lane & 15];
         const double tabA_s = TABLE ? (double)(P.nA - 1) / (P.A_hi - P.A_lo) : 0.0, tabA_o = -P.A_lo * tabA_s;
         auto qbar = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + qd), "r"(32 * SP_G) : "memory"); };
@@ -531,17 +535,6 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                     for (int k = 0; k < K; k++) shu[k * SP_TS] = member ? __ldg(rec + sidx * SP_REC + 6 + k) : (double)ti.base[k];
                 }
                 qbar();
-                x = shr[6 * SP_TS];
-#pragma unroll
-                for (int k = 0; k < K; k++) {
-                    fr[k] = shr[k * SP_TS];
-                    fi[k] = shr[(3 + k) * SP_TS];
-                    const double u = shu[k * SP_TS], fl = floor(u);
-                    w1[k] = u - fl;
-                    w0[k] = 1.0 - w1[k];
-                    off[k] = min(max((int)fl - ti.base[k], 0), SP_CAPMAX);
-                    off_bad = off_bad || ((int)fl - ti.base[k] != off[k]);      // outside the tile's window: cannot happen for a sample of this cell
-                }
                 // ---- harmonics (Eq. 4): group g evaluates modes g, g + 4, ... from the tables
                 const int M = sm.ytab.M;
                 for (int m = g; m < 24; m += SP_G) {
@@ -572,7 +565,8 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
 #pragma unroll
             for (int k = 0; k < K; k++) {
                 if (k != g) continue;
-                const double xr = x * fr[k], xi = x * fi[k];
+                const double xk = fx_col[6 * SP_TS];                               // x, F_k from step 1 (read again after step 4: registers)
+                const double xr = xk * fx_col[k * SP_TS], xi = xk * fx_col[(3 + k) * SP_TS];
                 int mh = 0;
 #pragma unroll 4
                 for (int m = 0; m < 24; m++) {
@@ -652,6 +646,18 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                 }
             }
             qbar();
+            // the sample's F_k, x and window offsets are picked up only now: step 4 above has the registers for its loads
+            x = fx_col[6 * SP_TS];
+#pragma unroll
+            for (int k = 0; k < K; k++) {
+                fr[k] = fx_col[k * SP_TS];
+                fi[k] = fx_col[(3 + k) * SP_TS];
+                const double u = u_col[k * SP_TS], fl = floor(u);
+                w1[k] = u - fl;
+                w0[k] = 1.0 - w1[k];
+                off[k] = min(max((int)fl - ti.base[k], 0), SP_CAPMAX);
+                off_bad = off_bad || ((int)fl - ti.base[k] != off[k]);      // outside the tile's window: cannot happen for a sample of this cell
+            }
             double Bq = 0.0;
 #pragma unroll
             for (int k = 0; k < K; k++) {
@@ -667,6 +673,11 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                 const double un = __hiloint2double(min(max(sm.eb[k][i] + P.qeb[k] - 1023 - 50, 1), 2046) << 20, 0);
                 w0[k] *= un;
                 w1[k] *= un;
+                if (g == 0) {                                   // read back item by item: fifteen registers less across the work items
+                    sm.wgt[0][k][i] = w0[k];
+                    sm.wgt[1][k][i] = w1[k];
+                    sm.offs[k][i] = off[k];
+                }
             }
             Bq *= 0.25;
             // per-sample constants of the time marginalisation
@@ -817,6 +828,8 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                 const bool guard = !(SP_NB * c - 1 - ti.cap >= 0 && SP_NB * c + SP_NB - 2 < N_t);
 #pragma unroll
                 for (int k = 0; k < K; k++) {
+                    const double w0k = sm.wgt[0][k][i], w1k = sm.wgt[1][k][i];
+                    const int offk = sm.offs[k][i];
                     mbar_wait(&sm.d_full, im & 1);
                     tc_fence_after();
                     uint32_t acc[6][8], accp[6];
@@ -838,7 +851,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
 #pragma unroll
                     for (int e = 0; e < 8; e++) V[e + 1] = sp_recombine(acc[0][e], acc[1][e], acc[2][e], acc[3][e], acc[4][e], acc[5][e]);
                     if (g == SP_G - 1) sm.xch[c & 1][k][i] = V[8];
-                    const int j0 = SP_NB * c + 8 * g - 1 - off[k];      // time bin of the pair (V[0], V[1])
+                    const int j0 = SP_NB * c + 8 * g - 1 - offk;        // time bin of the pair (V[0], V[1])
                     if (guard) {
                         double rv[8];
                         double* pr[8];
@@ -850,7 +863,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                             rv[e] = ok[e] ? *pr[e] : 0.0;
                         }
 #pragma unroll
-                        for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e + 1], fma(w0[k], V[e], rv[e]));
+                        for (int e = 0; e < 8; e++) rv[e] = fma(w1k, V[e + 1], fma(w0k, V[e], rv[e]));
 #pragma unroll
                         for (int e = 0; e < 8; e++)
                             if (ok[e]) *pr[e] = rv[e];
@@ -863,7 +876,7 @@ lnl_split_kernel(LnlParams P, int N, const double* __restrict__ rec, const int* 
                             rv[e] = *pr[e];
                         }
 #pragma unroll
-                        for (int e = 0; e < 8; e++) rv[e] = fma(w1[k], V[e + 1], fma(w0[k], V[e], rv[e]));
+                        for (int e = 0; e < 8; e++) rv[e] = fma(w1k, V[e + 1], fma(w0k, V[e], rv[e]));
 #pragma unroll
                         for (int e = 0; e < 8; e++) *pr[e] = rv[e];
                     }
